@@ -1,0 +1,200 @@
+/*
+ * nanobte.h -- C ABI of the B200-native NanoBTE hot path (arxiv/paper_2607_03226).
+ *
+ * What the library computes (citations: /root/reference/PAPER.md line numbers; "Rn" are the readings
+ * listed in DESIGN.md where the paper is silent):
+ *
+ *   steady, non-gray phonon BTE under the relaxation-time approximation, energy form (PAPER.md:41-55,
+ *   Eq. 1-4), linearised equilibrium e0_b = C_b T_L / W (Eq. 11), discrete ordinates
+ *   (PAPER.md:51, 57), first-order-upwind finite volumes (R1).  For every (band b, direction i) the
+ *   transport system (I/tau_b + v_b K_i) e = e0_b/tau_b + S_b (Eq. 13) is lower
+ *   triangular in upwind order and is solved as a wavefront sweep, fused with the wall closures
+ *   (thermalizing / diffuse / specular / mixed-p; R6-R9), followed by the
+ *   band x direction reduction to T_L (Eq. 5), T and q (Eq. 7), wrapped in
+ *   plain source iteration (Eq. 6) or the synthetic, diffusion-accelerated iteration
+ *   (Eq. 8-12; R14) whose macroscopic solve is a GPU conjugate gradient.
+ *
+ * Conventions
+ *   - everything is fp64; variables are deviational about T_ref (R2): eps = e - C_b T_ref / W.
+ *   - structured cell id = i + nx*(j + ny*k); side codes 0..5 = -x,+x,-y,+y,-z,+z; nz == 1 means 2-D
+ *     (unit depth, only sides 0..3, s_z ignored).
+ *   - direction table s is [D][3] unit vectors, weights w [D] > 0, W = sum w (Eq. 11).
+ *   - tag types: 0 thermalizing (T_wall used), 1 diffuse, 2 specular, 3 mixed (per-face p in bf_p).
+ *   - canonical e export layout is [band][direction][cell] over ALL n_cells (inactive cells read 0).
+ *
+ * Pointers: every pointer in the create_* argument structs is a HOST pointer, read during the call and
+ * never retained.  Getters take `dst_is_device`: 0 = host pointer (the call synchronises the stream),
+ * 1 = device pointer (copy is enqueued on the solver's stream, no synchronisation).
+ * Device memory: if options.workspace is non-NULL it must be a device allocation of at least
+ * nanobte_workspace_bytes_*() bytes, 256-byte aligned, owned by the caller (e.g. a torch tensor) and
+ * alive until nanobte_destroy; otherwise the library allocates with cudaMalloc and frees at destroy.
+ * All kernels are enqueued on options.stream (a cudaStream_t; NULL = legacy default stream).
+ *
+ * Errors: int return; 0 OK; NANOBTE_NOT_CONVERGED (1) = state valid, max_iter reached; < 0 error.  No
+ * exceptions cross the ABI, no global state; nanobte_last_error(h) gives the message.  There is NO CPU
+ * fallback: without a CUDA device of compute capability 10.x every create_* fails with NANOBTE_E_ARCH.
+ * A solver handle is not thread-safe.
+ */
+#ifndef NANOBTE_H
+#define NANOBTE_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nanobte_solver nanobte_solver;
+
+enum {
+  NANOBTE_OK = 0,
+  NANOBTE_NOT_CONVERGED = 1,
+  NANOBTE_E_INVALID = -1,      /* bad argument (message says which)                               */
+  NANOBTE_E_ALLOC = -2,        /* host or device allocation failed / workspace too small          */
+  NANOBTE_E_CUDA = -3,         /* a CUDA runtime call failed (message carries cudaGetErrorString) */
+  NANOBTE_E_ARCH = -4,         /* no CUDA device, or device is not sm_100                          */
+  NANOBTE_E_UNTAGGED = -5,     /* an exposed face of an active cell has no boundary tag           */
+  NANOBTE_E_SPECULAR = -6,     /* mirror image of an incoming direction is not in the quadrature  */
+  NANOBTE_E_CYCLE = -7,        /* upwind graph of a direction is cyclic (unstructured, R16)       */
+  NANOBTE_E_QUADRATURE = -8,   /* non-unit direction, non-positive weight, or sum w s != 0        */
+  NANOBTE_E_SINGULAR = -9,     /* synthetic mode without any thermalizing face                    */
+  NANOBTE_E_NONFINITE = -10,   /* max|dT| is NaN/Inf                                              */
+  NANOBTE_E_UNSUPPORTED = -11  /* problem shape outside what the kernels support (message)        */
+};
+
+enum { NANOBTE_THERMALIZING = 0, NANOBTE_DIFFUSE = 1, NANOBTE_SPECULAR = 2, NANOBTE_MIXED = 3 };
+enum { NANOBTE_MODE_PLAIN = 0, NANOBTE_MODE_SYNTHETIC = 1 };
+
+/* Band table: C_b [J/m^3K], v_b [m/s], tau_b [s]; src_share NULL -> C_b/sum C (R5). */
+typedef struct {
+  int32_t B;
+  const double *C, *v, *tau;
+  const double *src_share;
+} nanobte_bands;
+
+/* Angular quadrature. */
+typedef struct {
+  int32_t D;
+  const double *s; /* [D][3] */
+  const double *w; /* [D]    */
+} nanobte_quadrature;
+
+/* Boundary tag table entry. */
+typedef struct {
+  int32_t type;   /* NANOBTE_THERMALIZING ... NANOBTE_MIXED */
+  double T_wall;  /* thermalizing only */
+} nanobte_tag;
+
+/* Structured (optionally masked) grid. */
+typedef struct {
+  int32_t nx, ny, nz;
+  const double *hx, *hy, *hz;   /* [nx], [ny], [nz] cell sizes in metres (hz unused when nz == 1) */
+  const uint8_t *active;        /* [nx*ny*nz] or NULL = all active */
+  int32_t n_bfaces;
+  const int32_t *bf_cell;       /* [n_bfaces] owner cell id        */
+  const uint8_t *bf_side;       /* [n_bfaces] side code 0..5       */
+  const int32_t *bf_tag;        /* [n_bfaces] index into tags      */
+  const double *bf_p;           /* [n_bfaces] specularity of mixed faces, or NULL */
+} nanobte_structured_mesh;
+
+/* Unstructured 2-D polygon mesh (counter-clockwise cells, CSR). */
+typedef struct {
+  int32_t n_nodes, n_cells;
+  const double *xy;             /* [n_nodes][2] */
+  const int32_t *cell_ptr;      /* [n_cells+1]  */
+  const int32_t *cell_nodes;    /* [cell_ptr[n_cells]] */
+  int32_t n_bfaces;
+  const int32_t *bf_nodes;      /* [n_bfaces][2] */
+  const int32_t *bf_tag;
+  const double *bf_p;
+} nanobte_unstructured_mesh;
+
+typedef struct {
+  double T_ref;                 /* reference temperature of the deviational variables (R2)        */
+  const double *T_init;         /* [n_cells] host, or NULL -> T_ref (R12)                          */
+  void *stream;                 /* cudaStream_t                                                    */
+  void *workspace;              /* device memory or NULL                                           */
+  size_t workspace_bytes;
+  double cg_rtol;               /* <= 0 -> 1e-12 (R14e)                                            */
+  int32_t cg_max_iter;          /* <= 0 -> 100000                                                  */
+  int32_t sweep_G;              /* tuning: systems per thread in the structured sweep (1,2,4); 0 = auto */
+  int32_t sweep_threads;        /* tuning: threads per thread group; 0 = auto                      */
+  int32_t sweep_groups;         /* tuning: thread groups (each with its own systems) per CTA; 0 = auto */
+} nanobte_options;
+
+/* Layout / schedule facts of a created solver (for reporting and roofline arithmetic). */
+typedef struct {
+  int32_t dim, n_cells, n_active, B, D, n_bfaces;
+  int32_t n_octants;            /* direction classes in use (structured) / D (unstructured)       */
+  int32_t n_planes;             /* hyperplanes per octant (structured) / max levels per direction */
+  int32_t n_tasks;              /* CTAs per sweep launch                                           */
+  int32_t sweep_G, sweep_threads, sweep_groups, sweep_rmax, pencil_axis;
+  int64_t n_pos;                /* e slots per (band,direction) incl. holes and padding            */
+  int64_t n_inflow;             /* sum over directions of boundary-inflow values per band          */
+  size_t device_bytes;          /* total device memory in use by the solver                        */
+  size_t sweep_smem_bytes;
+} nanobte_info;
+
+/* Bytes of device workspace create_* would need for this problem (same validation as create). */
+int nanobte_workspace_bytes_structured(const nanobte_structured_mesh *, const nanobte_bands *,
+                                       const nanobte_quadrature *, const nanobte_tag *tags, int32_t n_tags,
+                                       const nanobte_options *, size_t *bytes_out);
+int nanobte_workspace_bytes_unstructured(const nanobte_unstructured_mesh *, const nanobte_bands *,
+                                         const nanobte_quadrature *, const nanobte_tag *tags, int32_t n_tags,
+                                         const nanobte_options *, size_t *bytes_out);
+
+/* (a1) one-time setup: schedules, coefficients, reflection maps, boundary caches.
+ * Qdot: [n_cells] W/m^3 host pointer or NULL.  On failure *out is still a valid handle
+ * (if allocation of the handle itself succeeded) whose only use is nanobte_last_error / nanobte_destroy. */
+int nanobte_create_structured(const nanobte_structured_mesh *, const nanobte_bands *, const nanobte_quadrature *,
+                              const nanobte_tag *tags, int32_t n_tags, const double *Qdot,
+                              const nanobte_options *, nanobte_solver **out);
+int nanobte_create_unstructured(const nanobte_unstructured_mesh *, const nanobte_bands *,
+                                const nanobte_quadrature *, const nanobte_tag *tags, int32_t n_tags,
+                                const double *Qdot, const nanobte_options *, nanobte_solver **out);
+void nanobte_destroy(nanobte_solver *);
+
+/* (a2)-(a5) one transport sweep: eps <- (I/tau + vK)^-1 (e0(T)/tau + S + boundary inflow), PAPER.md:55, 104,
+ * 110.  Boundary inflow values are the ones cached by the previous nanobte_update_temperature (R9: lagged);
+ * before the first update they are the thermalizing constants and zero elsewhere (R12).  Asynchronous. */
+int nanobte_sweep(nanobte_solver *);
+
+/* (a6) moments + closure refresh + plain update: T_SI (Eq. 5), T_energy (R13), q (Eq. 7), diffuse averages G
+ * and the boundary inflow cache for the next sweep (R6-R8), T <- T_SI (Eq. 6).  max_dT (host pointer or
+ * NULL) receives max_c |T_new - T_old|; the call synchronises the stream iff max_dT != NULL. */
+int nanobte_update_temperature(nanobte_solver *, double *max_dT);
+
+/* (a7) synthetic correction after update_temperature: CG on the two-point-flux diffusion operator,
+ * T <- T_SI + delta (R14).  cg_iters/max_dT host pointers or NULL; synchronises. */
+int nanobte_diffusion_correct(nanobte_solver *, int32_t *cg_iters, double *max_dT);
+
+/* (a8) outer loop until max|dT| < tol or max_iter sweeps (R11).  Synchronises once per iteration
+ * (one double device->host). */
+int nanobte_solve(nanobte_solver *, double tol, int32_t max_iter, int32_t mode, int32_t *iters_out,
+                  double *last_dT_out);
+
+int nanobte_set_T(nanobte_solver *, const double *T /* [n_cells] absolute */, int32_t src_is_device);
+int nanobte_get_T(nanobte_solver *, int32_t which /* 0 T_L, 1 T_energy, 2 T_SI */, double *dst /* [n_cells] */,
+                  int32_t dst_is_device);
+int nanobte_get_q(nanobte_solver *, double *dst /* [n_cells][dim] */, int32_t dst_is_device);
+/* dst [nb][nd][n_cells]; deviational != 0 -> eps, else e = eps + C_b T_ref / W. */
+int nanobte_get_e(nanobte_solver *, int32_t b0, int32_t nb, int32_t d0, int32_t nd, double *dst,
+                  int32_t deviational, int32_t dst_is_device);
+int nanobte_get_G(nanobte_solver *, double *dst /* [n_bfaces][B] deviational diffuse averages */,
+                  int32_t dst_is_device);
+/* Heat leaving through the faces of each tag [W, or W/m in 2-D], outward positive (O8), for the last
+ * sweep + update pair.  per_tag is a host pointer [n_tags]; synchronises. */
+int nanobte_get_boundary_heat(nanobte_solver *, double *per_tag);
+/* History of the last nanobte_solve: returns the number of iterations recorded, fills up to cap entries. */
+int nanobte_get_history(nanobte_solver *, double *dT, int32_t *cg_iters, int32_t cap);
+int nanobte_get_info(const nanobte_solver *, nanobte_info *out);
+/* Number of kernels the library has launched on behalf of this solver since create. */
+int64_t nanobte_launch_count(const nanobte_solver *);
+double nanobte_kappa(const nanobte_solver *); /* kappa_bulk of R14d */
+
+const char *nanobte_strerror(int code);
+const char *nanobte_last_error(const nanobte_solver *);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NANOBTE_H */

@@ -1,0 +1,353 @@
+// api.cu -- the C-ABI entry points of libnanobte that do not depend on the mesh kind, plus the host-side
+// validation and the upload of the tables both kinds share.  See include/nanobte.h for the contract.
+#include <algorithm>
+
+#include "host_util.h"
+
+int nb_fail(nanobte_solver *h, int code, const char *fmt, ...) {
+  if (h) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    h->err = buf;
+  }
+  return code;
+}
+
+extern "C" const char *nanobte_strerror(int code) {
+  switch (code) {
+    case NANOBTE_OK: return "OK";
+    case NANOBTE_NOT_CONVERGED: return "NOT_CONVERGED";
+    case NANOBTE_E_INVALID: return "INVALID";
+    case NANOBTE_E_ALLOC: return "ALLOC";
+    case NANOBTE_E_CUDA: return "CUDA";
+    case NANOBTE_E_ARCH: return "ARCH";
+    case NANOBTE_E_UNTAGGED: return "UNTAGGED";
+    case NANOBTE_E_SPECULAR: return "SPECULAR";
+    case NANOBTE_E_CYCLE: return "CYCLE";
+    case NANOBTE_E_QUADRATURE: return "QUADRATURE";
+    case NANOBTE_E_SINGULAR: return "SINGULAR";
+    case NANOBTE_E_NONFINITE: return "NONFINITE";
+    case NANOBTE_E_UNSUPPORTED: return "UNSUPPORTED";
+  }
+  return "?";
+}
+
+extern "C" const char *nanobte_last_error(const nanobte_solver *h) { return h ? h->err.c_str() : "null handle"; }
+
+int nb_check_device(nanobte_solver *h) {
+  int n = 0;
+  cudaError_t e = cudaGetDeviceCount(&n);
+  if (e != cudaSuccess || n == 0)
+    return nb_fail(h, NANOBTE_E_ARCH, "no CUDA device (%s); libnanobte has no CPU fallback",
+                   e == cudaSuccess ? "count 0" : cudaGetErrorString(e));
+  int dev = 0;
+  cudaDeviceProp p;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&p, dev) != cudaSuccess)
+    return nb_fail(h, NANOBTE_E_ARCH, "cannot query the CUDA device");
+  if (p.major != 10) return nb_fail(h, NANOBTE_E_ARCH, "device is sm_%d%d; libnanobte is built for sm_100a only", p.major, p.minor);
+  h->n_sm = p.multiProcessorCount;
+  return 0;
+}
+
+int nb_validate_common(nanobte_solver *h, int dim, const nanobte_bands *bands, const nanobte_quadrature *quad,
+                       const nanobte_tag *tags, int n_tags, Common &c) {
+  if (!bands || !quad || (n_tags > 0 && !tags)) return nb_fail(h, NANOBTE_E_INVALID, "null argument");
+  const int B = bands->B, D = quad->D;
+  if (B < 1 || D < 1 || n_tags < 0) return nb_fail(h, NANOBTE_E_INVALID, "B, D must be >= 1");
+  if (!bands->C || !bands->v || !bands->tau || !quad->s || !quad->w) return nb_fail(h, NANOBTE_E_INVALID, "null table");
+  c.B = B; c.D = D; c.dim = dim; c.n_tags = n_tags;
+  c.C.assign(bands->C, bands->C + B);
+  c.v.assign(bands->v, bands->v + B);
+  c.tau.assign(bands->tau, bands->tau + B);
+  c.share.resize(B);
+  c.Csum = 0; c.beta = 0;
+  for (int b = 0; b < B; ++b) {
+    if (!(c.C[b] > 0) || !(c.v[b] > 0) || !(c.tau[b] > 0))
+      return nb_fail(h, NANOBTE_E_INVALID, "band %d: C, v, tau must be > 0", b);
+    c.Csum += c.C[b];
+    c.beta += c.C[b] / c.tau[b];  // denominator of Eq. 5
+  }
+  for (int b = 0; b < B; ++b) c.share[b] = bands->src_share ? bands->src_share[b] : c.C[b] / c.Csum;
+  c.s.assign(quad->s, quad->s + 3 * (size_t)D);
+  c.w.assign(quad->w, quad->w + D);
+  c.W = 0;  // W_Omega, Eq. 11
+  double ws[3] = {0, 0, 0}, sxx = 0;
+  for (int i = 0; i < D; ++i) {
+    if (!(c.w[i] > 0)) return nb_fail(h, NANOBTE_E_QUADRATURE, "weight %d not positive", i);
+    const double *s = &c.s[3 * i];
+    double nn = std::sqrt(s[0] * s[0] + s[1] * s[1] + s[2] * s[2]);
+    if (std::fabs(nn - 1.0) > 1e-12) return nb_fail(h, NANOBTE_E_QUADRATURE, "direction %d is not a unit vector", i);
+    for (int k = 0; k < 3; ++k) ws[k] += c.w[i] * s[k];
+    c.W += c.w[i];
+    sxx += c.w[i] * s[0] * s[0];
+  }
+  for (int k = 0; k < dim; ++k)
+    if (std::fabs(ws[k]) > 1e-12 * c.W)
+      return nb_fail(h, NANOBTE_E_QUADRATURE, "sum_i w_i s_i != 0 (component %d: %g)", k, ws[k]);
+  c.kappa = 0;  // R14d
+  for (int b = 0; b < B; ++b) c.kappa += c.C[b] * c.v[b] * c.v[b] * c.tau[b];
+  c.kappa *= sxx / c.W;
+  c.tag_type.resize(n_tags);
+  c.tag_T.resize(n_tags);
+  for (int t = 0; t < n_tags; ++t) {
+    if (tags[t].type < 0 || tags[t].type > 3) return nb_fail(h, NANOBTE_E_INVALID, "tag %d: unknown type %d", t, tags[t].type);
+    c.tag_type[t] = tags[t].type;
+    c.tag_T[t] = tags[t].T_wall;
+  }
+  return 0;
+}
+
+int nb_find_mirror(const Common &c, int d, const double n[3]) {
+  const double *s = &c.s[3 * d];
+  const double sn = s[0] * n[0] + s[1] * n[1] + s[2] * n[2];
+  const double r[3] = {s[0] - 2 * sn * n[0], s[1] - 2 * sn * n[1], s[2] - 2 * sn * n[2]};
+  for (int j = 0; j < c.D; ++j) {
+    const double d0 = c.s[3 * j] - r[0], d1 = c.s[3 * j + 1] - r[1], d2 = c.s[3 * j + 2] - r[2];
+    if (d0 * d0 + d1 * d1 + d2 * d2 < 1e-18) return j;
+  }
+  return -1;
+}
+
+int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTables &g) {
+  const size_t na = g.act2cell.size(), nbf = g.bf_act.size();
+  h->B = c.B; h->D = c.D; h->dim = c.dim; h->n_tags = c.n_tags;
+  h->W = c.W; h->beta = c.beta; h->Csum = c.Csum; h->kappa = c.kappa;
+  h->n_act = (int)na; h->n_bf = (int)nbf;
+  h->h_C = c.C;
+  BoundaryArgs &bd = h->bd;
+  bd.n_bf = (int)nbf; bd.B = c.B; bd.D = c.D;
+  bd.bf_act = A.put(g.bf_act);
+  bd.bf_type = A.put(g.bf_type);
+  bd.bf_p = A.put(g.bf_p);
+  bd.bf_den = A.put(g.bf_den);
+  bd.bf_area = A.put(g.bf_area);
+  bd.bf_eps_w = A.put(g.bf_eps_w);
+  bd.bf_sn = A.put(g.bf_sn);
+  bd.bf_mirror = A.put(g.bf_mirror);
+  bd.bf_inidx = A.put(g.bf_inidx);
+  bd.bf_opos = A.put(g.bf_opos);
+  bd.w = A.put(c.w);
+  bd.C = A.put(c.C);
+  bd.v = A.put(c.v);
+  bd.dir_bin = A.put(g.dir_bin);
+  bd.dir_nin = A.put(g.dir_nin);
+  bd.bin = A.zeros<double>((size_t)g.bin_total);
+  bd.G = A.zeros<double>(nbf * c.B);
+  bd.faceflux = A.zeros<double>(nbf * c.B);
+  h->n_inflow = 0;
+  for (int d = 0; d < c.D; ++d) h->n_inflow += g.dir_nin[d];
+  h->any_therm = false;
+  for (size_t f = 0; f < nbf; ++f)
+    if (g.bf_type[f] == NANOBTE_THERMALIZING) h->any_therm = true;
+  h->mcoef = A.put(g.mcoef);
+  h->act2cell = A.put(g.act2cell);
+  h->cell2act = A.put(g.cell2act);
+  h->vol = A.put(g.vol);
+  h->Qdot = A.put(g.Qdot_act);
+  h->theta = A.put(g.theta0);
+  h->theta_prev = A.zeros<double>(na);
+  h->theta_SI = A.zeros<double>(na);
+  h->theta_en = A.zeros<double>(na);
+  h->q = A.zeros<double>(na * 3);
+  h->d_maxdT = A.zeros<unsigned long long>(4);
+  // CG
+  h->cg_nf = g.cg_nf;
+  h->cg_nbr = A.put(g.cg_nbr);
+  h->cg_coef = A.put(g.cg_coef);
+  h->cg_diag = A.put(g.cg_diag);
+  h->cellbf_ptr = A.put(g.cellbf_ptr);
+  h->cellbf = A.put(g.cellbf);
+  h->cg_x = A.zeros<double>(na);
+  h->cg_r = A.zeros<double>(na);
+  h->cg_p0 = A.zeros<double>(na);
+  h->cg_p1 = A.zeros<double>(na);
+  h->cg_rhs = A.zeros<double>(na);
+  h->cg_scal = A.zeros<double>(16);
+  h->cg_partial = A.zeros<double>(4 * 2048);
+  h->tagface_ptr = A.put(g.tagface_ptr);
+  h->tagface = A.put(g.tagface);
+  h->d_tagheat = A.zeros<double>((size_t)std::max(1, c.n_tags));
+  return A.rc;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" void nanobte_destroy(nanobte_solver *h) {
+  if (!h) return;
+  if (h->stream || h->arena) cudaStreamSynchronize(h->stream);
+  nb_free_unstructured(h);
+  if (h->arena && h->arena_owned) cudaFree(h->arena);
+  if (h->h_pinned) cudaFreeHost(h->h_pinned);
+  delete h;
+}
+
+extern "C" int nanobte_sweep(nanobte_solver *h) {
+  if (!h || !h->arena) return NANOBTE_E_INVALID;
+  return h->kind == 0 ? nb_launch_sweep_structured(h) : nb_launch_sweep_unstructured(h);
+}
+
+static int read_maxdT(nanobte_solver *h, double *out) {
+  // d_maxdT[0] = bit pattern of max|dT| (non-negative double), d_maxdT[1] = CG iteration count of the last solve
+  NB_CUDA(h, cudaMemcpyAsync(h->h_pinned, h->d_maxdT, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  NB_CUDA(h, cudaStreamSynchronize(h->stream));
+  *out = h->h_pinned[0];
+  return std::isfinite(*out) ? 0 : nb_fail(h, NANOBTE_E_NONFINITE, "max|dT| is not finite");
+}
+
+extern "C" int nanobte_update_temperature(nanobte_solver *h, double *max_dT) {
+  if (!h || !h->arena) return NANOBTE_E_INVALID;
+  int rc;
+  if ((rc = nb_launch_boundary(h)) < 0) return rc;  // G, face fluxes, inflow cache for the next sweep (O3)
+  if ((rc = nb_launch_moments(h)) < 0) return rc;   // O4
+  if ((rc = nb_launch_update(h, 0)) < 0) return rc; // O5
+  if (max_dT) return read_maxdT(h, max_dT);
+  return 0;
+}
+
+extern "C" int nanobte_diffusion_correct(nanobte_solver *h, int32_t *cg_iters, double *max_dT) {
+  if (!h || !h->arena) return NANOBTE_E_INVALID;
+  if (!h->any_therm) return nb_fail(h, NANOBTE_E_SINGULAR, "synthetic mode needs at least one thermalizing face");
+  int rc;
+  if ((rc = nb_cg_solve(h, nullptr)) < 0) return rc;
+  if ((rc = nb_launch_update(h, 1)) < 0) return rc;
+  double d = 0;
+  if ((rc = read_maxdT(h, &d)) < 0) return rc;
+  if (cg_iters) {
+    unsigned long long it;
+    memcpy(&it, h->h_pinned + 1, sizeof(it));
+    *cg_iters = (int32_t)it;
+  }
+  if (max_dT) *max_dT = d;
+  return 0;
+}
+
+extern "C" int nanobte_solve(nanobte_solver *h, double tol, int32_t max_iter, int32_t mode, int32_t *iters_out,
+                             double *last_dT_out) {
+  if (!h || !h->arena) return NANOBTE_E_INVALID;
+  if (mode != 0 && mode != 1) return nb_fail(h, NANOBTE_E_INVALID, "mode must be 0 (plain) or 1 (synthetic)");
+  if (mode == 1 && !h->any_therm) return nb_fail(h, NANOBTE_E_SINGULAR, "synthetic mode needs at least one thermalizing face");
+  h->hist_dT.clear();
+  h->hist_cg.clear();
+  double dT = INFINITY;
+  int n = 0, rc = NANOBTE_NOT_CONVERGED, r;
+  while (n < max_iter) {
+    int cg = 0;
+    if ((r = nanobte_sweep(h)) < 0) return r;
+    if (mode == 0) {
+      if ((r = nanobte_update_temperature(h, &dT)) < 0) return r;
+    } else {
+      if ((r = nanobte_update_temperature(h, nullptr)) < 0) return r;
+      if ((r = nanobte_diffusion_correct(h, &cg, &dT)) < 0) return r;
+    }
+    ++n;
+    h->hist_dT.push_back(dT);
+    h->hist_cg.push_back(cg);
+    if (dT < tol) {
+      rc = NANOBTE_OK;
+      break;
+    }
+  }
+  if (iters_out) *iters_out = n;
+  if (last_dT_out) *last_dT_out = dT;
+  return rc;
+}
+
+// ---- getters / setters ---------------------------------------------------------------------------------------
+// Device scratch for getters that need a host round trip: the part[] buffer (>= 5 * e_stride doubles) is free
+// between update_temperature calls; it always holds at least 3 * n_cells doubles (checked at create).
+static int copy_out(nanobte_solver *h, const double *dev_src, double *dst, size_t n, int dst_is_device) {
+  if (dst_is_device) {
+    NB_CUDA(h, cudaMemcpyAsync(dst, dev_src, n * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+  } else {
+    NB_CUDA(h, cudaMemcpyAsync(dst, dev_src, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    NB_CUDA(h, cudaStreamSynchronize(h->stream));
+  }
+  return 0;
+}
+
+extern "C" int nanobte_set_T(nanobte_solver *h, const double *T, int32_t src_is_device) {
+  if (!h || !h->arena || !T) return NANOBTE_E_INVALID;
+  const double *src = T;
+  if (!src_is_device) {
+    NB_CUDA(h, cudaMemcpyAsync(h->part, T, (size_t)h->n_cells * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    src = h->part;
+  }
+  int rc = nb_launch_set_theta(h, src);
+  if (rc < 0) return rc;
+  if (!src_is_device) NB_CUDA(h, cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+extern "C" int nanobte_get_T(nanobte_solver *h, int32_t which, double *dst, int32_t dst_is_device) {
+  if (!h || !h->arena || !dst) return NANOBTE_E_INVALID;
+  const double *src = which == 0 ? h->theta : which == 1 ? h->theta_en : which == 2 ? h->theta_SI : nullptr;
+  if (!src) return nb_fail(h, NANOBTE_E_INVALID, "which must be 0, 1 or 2");
+  double *stage = dst_is_device ? dst : h->part;
+  int rc = nb_launch_scatter_cells(h, src, stage, 1, h->T_ref);
+  if (rc < 0) return rc;
+  if (!dst_is_device) return copy_out(h, stage, dst, (size_t)h->n_cells, 0);
+  return 0;
+}
+
+extern "C" int nanobte_get_q(nanobte_solver *h, double *dst, int32_t dst_is_device) {
+  if (!h || !h->arena || !dst) return NANOBTE_E_INVALID;
+  double *stage = dst_is_device ? dst : h->part;
+  int rc = nb_launch_scatter_cells(h, h->q, stage, h->dim, 0.0);
+  if (rc < 0) return rc;
+  if (!dst_is_device) return copy_out(h, stage, dst, (size_t)h->n_cells * h->dim, 0);
+  return 0;
+}
+
+extern "C" int nanobte_get_e(nanobte_solver *h, int32_t b0, int32_t nb, int32_t d0, int32_t nd, double *dst,
+                             int32_t deviational, int32_t dst_is_device) {
+  if (!h || !h->arena || !dst) return NANOBTE_E_INVALID;
+  if (b0 < 0 || nb < 0 || b0 + nb > h->B || d0 < 0 || nd < 0 || d0 + nd > h->D)
+    return nb_fail(h, NANOBTE_E_INVALID, "band/direction range");
+  if (dst_is_device) return nb_launch_get_e(h, b0, nb, d0, nd, dst, deviational);
+  // host destination: one (band, direction) row at a time through the part[] scratch
+  for (int b = 0; b < nb; ++b)
+    for (int d = 0; d < nd; ++d) {
+      int rc = nb_launch_get_e(h, b0 + b, 1, d0 + d, 1, h->part, deviational);
+      if (rc < 0) return rc;
+      rc = copy_out(h, h->part, dst + ((size_t)b * nd + d) * h->n_cells, (size_t)h->n_cells, 0);
+      if (rc < 0) return rc;
+    }
+  return 0;
+}
+
+extern "C" int nanobte_get_G(nanobte_solver *h, double *dst, int32_t dst_is_device) {
+  if (!h || !h->arena || !dst) return NANOBTE_E_INVALID;
+  return copy_out(h, h->bd.G, dst, (size_t)h->n_bf * h->B, dst_is_device);
+}
+
+extern "C" int nanobte_get_boundary_heat(nanobte_solver *h, double *per_tag) {
+  if (!h || !h->arena || !per_tag) return NANOBTE_E_INVALID;
+  if (h->n_tags == 0) return 0;
+  int rc = nb_launch_tagheat(h);
+  if (rc < 0) return rc;
+  return copy_out(h, h->d_tagheat, per_tag, (size_t)h->n_tags, 0);
+}
+
+extern "C" int nanobte_get_history(nanobte_solver *h, double *dT, int32_t *cg_iters, int32_t cap) {
+  if (!h) return NANOBTE_E_INVALID;
+  const int n = std::min<int>((int)h->hist_dT.size(), cap);
+  for (int k = 0; k < n; ++k) {
+    if (dT) dT[k] = h->hist_dT[k];
+    if (cg_iters) cg_iters[k] = h->hist_cg[k];
+  }
+  return (int)h->hist_dT.size();
+}
+
+extern "C" int nanobte_get_info(const nanobte_solver *h, nanobte_info *o) {
+  if (!h || !o) return NANOBTE_E_INVALID;
+  o->dim = h->dim; o->n_cells = h->n_cells; o->n_active = h->n_act; o->B = h->B; o->D = h->D; o->n_bfaces = h->n_bf;
+  o->n_octants = h->n_cls; o->n_planes = h->n_planes; o->n_tasks = h->n_tasks; o->sweep_G = h->sweep_G;
+  o->sweep_threads = h->sweep_threads; o->sweep_groups = h->sweep_groups; o->sweep_rmax = h->sweep_rmax; o->pencil_axis = h->pencil_axis; o->n_pos = h->n_pos;
+  o->n_inflow = h->n_inflow; o->device_bytes = h->arena_bytes; o->sweep_smem_bytes = h->sweep_smem;
+  return 0;
+}
+
+extern "C" int64_t nanobte_launch_count(const nanobte_solver *h) { return h ? h->launches : 0; }
+extern "C" double nanobte_kappa(const nanobte_solver *h) { return h ? h->kappa : 0.0; }

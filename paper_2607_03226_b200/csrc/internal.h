@@ -1,0 +1,151 @@
+// internal.h -- private declarations of libnanobte (CUDA, sm_100a).  Not part of the ABI (include/nanobte.h).
+//
+// Data layout in HBM:
+//   e      [D][B][n_pos]         one contiguous row per (direction, band) system, cells in the sweep order of
+//                                the direction's class (octant hyperplane order / per-direction level order)
+//   bin    per direction d: [B][n_in(class(d))]   boundary inflow values consumed by the sweep (R9: lagged)
+//   thetaP/QP [class][n_pos]     deviational temperature / heat source permuted into each class's sweep order
+//   part   [class][5][n_pos]     per-class partial moments (A1, A2, qx, qy, qz)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/nanobte.h"
+
+#define NB_MAX_CLASSES 8  // structured: octants (quadrants in 2-D)
+
+// ---- per-octant tables of the structured sweep -------------------------------------------------------------
+struct OctTab {
+  const uint32_t *pen;       // [n_pen]  slot | (m << 16), pencils sorted by (m = v'+w', w')
+  const int32_t *plane_off;  // [H]      pos = plane_off[h] + pencil index
+  const uint32_t *cellinfo;  // [n_pos]  bit0..2: u/v/w upwind value is a boundary inflow, bit3: hole, bits 4..: first inflow idx
+  const double2 *tq;         // [n_pos]  (theta, Qdot) in sweep order
+  const double *rhu, *rhv, *rhw;  // reciprocal spacings in primed coordinates (non-uniform path)
+  int32_t n_pen, H, n_pos, n_in;
+};
+
+struct SweepArgs {
+  const int32_t *task_oct;   // [n_tasks]
+  const int32_t *task_sys;   // [n_tasks][G]  global system id d*B+b, or -1 (padding)
+  const double *coef;        // [D*B][8]   uniform: k_theta,k_Q,c_u,c_v,c_w ; general: A,S,1/tau,v|s_u|,v|s_v|,v|s_w|
+  const int64_t *sys_bin;    // [D*B]      offset of the system's inflow row in bin
+  const double *bin;
+  double *e;
+  int64_t e_stride;          // n_pos padded
+  int32_t nu, pitch, slots;  // pencil length, slot pitch, slots per system (pitch * nw)
+};
+
+// ---- boundary-closure kernel ----------------------------------------------------------------------------------
+struct BoundaryArgs {
+  int32_t n_bf, B, D, n_cls;
+  const int32_t *bf_act;      // [n_bf] owner (active index)
+  const int32_t *bf_type;     // [n_bf]
+  const double *bf_p, *bf_den, *bf_area, *bf_eps_w;  // bf_eps_w = (T_w - T_ref)/W for thermalizing faces
+  const double *bf_sn;        // [n_bf][D]  s_d . n_f
+  const int32_t *bf_mirror;   // [n_bf][D]  mirrored direction for incoming d (specular/mixed) or -1
+  const int32_t *bf_inidx;    // [n_bf][D]  index of this face in direction d's inflow row, -1 if not incoming
+  const int32_t *bf_opos;     // [n_bf][D]  position of the owner cell in direction d's e row (outgoing d), else -1
+  const double *w, *C, *v;
+  const int64_t *dir_bin;     // [D] base offset of direction d in bin
+  const int32_t *dir_nin;     // [D] inflow row length of direction d
+  const double *e;
+  int64_t e_stride;
+  double *bin, *G, *faceflux; // G [n_bf][B], faceflux [n_bf][B] = v_b sum_i w_i (s_i.n) eps_face
+};
+
+struct nanobte_solver {
+  int kind = 0;  // 0 structured, 1 unstructured
+  int dim = 0, n_cells = 0, n_act = 0, B = 0, D = 0, n_bf = 0, n_tags = 0, n_cls = 0;
+  double T_ref = 0, W = 0, beta = 0, Csum = 0, kappa = 0, cg_rtol = 1e-12;
+  int cg_max_iter = 100000;
+  bool any_therm = false;
+  cudaStream_t stream = nullptr;
+  int n_sm = 148;
+
+  // device arena
+  char *arena = nullptr;
+  size_t arena_bytes = 0;
+  bool arena_owned = false;
+
+  // host copies needed at run time
+  std::vector<int32_t> h_bf_tag;
+  std::vector<double> h_C;
+
+  // structured sweep
+  SweepArgs sw{};
+  int sweep_G = 1, sweep_threads = 0, sweep_rmax = 1, sweep_groups = 1, n_tasks = 0, pencil_axis = 0, n_planes = 0;
+  bool uniform = true, has_w = true, sweep_attr_set = false;
+  const OctTab *d_octs = nullptr;
+  size_t sweep_smem = 0;
+  int64_t n_pos = 0, n_inflow = 0, e_stride = 0;
+
+  // unstructured sweep (see sweep_unstructured.cu)
+  struct UnsArgs *uns = nullptr;
+
+  BoundaryArgs bd{};
+
+  // moments / update
+  int32_t *cls_npos_h = nullptr;
+  int32_t cls_npos[NB_MAX_CLASSES] = {0};
+  const int32_t *cls_sys = nullptr;      // [n_cls][max systems] system ids per class
+  int32_t cls_nsys[NB_MAX_CLASSES] = {0};
+  int32_t cls_sys_off[NB_MAX_CLASSES] = {0};
+  const double *mcoef = nullptr;         // [D*B][5]  w/tau, w, v w sx, v w sy, v w sz
+  double *part = nullptr;                // [n_cls][5][e_stride]
+  const int32_t *a2pos = nullptr;        // [n_cls][n_act]
+  const int32_t *dir_cls = nullptr;      // [D] class of each direction
+  double2 *tq[NB_MAX_CLASSES] = {nullptr};
+  double *theta = nullptr, *theta_prev = nullptr, *theta_SI = nullptr, *theta_en = nullptr, *q = nullptr;  // [n_act]
+  const double *Qdot = nullptr;          // [n_act]
+  const int32_t *act2cell = nullptr, *cell2act = nullptr;
+  unsigned long long *d_maxdT = nullptr; // bit pattern of a non-negative double
+  double *h_pinned = nullptr;            // pinned host scratch (8 doubles)
+
+  // diffusion / CG
+  const int32_t *cg_nbr = nullptr;       // [6 or maxf][n_act]
+  const double *cg_coef = nullptr;       // [nf][n_act]
+  const double *cg_diag = nullptr, *vol = nullptr;
+  const int32_t *cellbf_ptr = nullptr, *cellbf = nullptr;  // CSR: reflecting boundary faces of each active cell
+  int cg_nf = 0;
+  double *cg_x = nullptr, *cg_r = nullptr, *cg_p0 = nullptr, *cg_p1 = nullptr, *cg_rhs = nullptr, *cg_scal = nullptr;
+  double *cg_partial = nullptr;
+  int cg_blocks = 0;
+
+  // boundary heat
+  const int32_t *tagface_ptr = nullptr, *tagface = nullptr;  // CSR faces per tag
+  double *d_tagheat = nullptr;
+
+  std::vector<double> hist_dT;
+  std::vector<int32_t> hist_cg;
+  int64_t launches = 0;
+  std::string err;
+};
+
+// error helpers ------------------------------------------------------------------------------------------------
+int nb_fail(nanobte_solver *h, int code, const char *fmt, ...);
+#define NB_CUDA(h, call)                                                                              \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess) return nb_fail((h), NANOBTE_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+// kernels_common.cu
+int nb_launch_boundary(nanobte_solver *h);
+int nb_launch_moments(nanobte_solver *h);
+int nb_launch_update(nanobte_solver *h, int mode /*0: theta<-theta_SI, 1: theta<-theta_SI+x*/);
+int nb_launch_get_e(nanobte_solver *h, int b0, int nb, int d0, int nd, double *dst_dev, int deviational);
+int nb_launch_scatter_cells(nanobte_solver *h, const double *src_act, double *dst_cells, int ncomp, double add);
+int nb_launch_set_theta(nanobte_solver *h, const double *T_cells_dev);
+int nb_launch_tagheat(nanobte_solver *h);
+int nb_cg_solve(nanobte_solver *h, int *iters);
+int nb_cg_blocks(nanobte_solver *h);
+// sweep_structured.cu
+int nb_launch_sweep_structured(nanobte_solver *h);
+int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int slots, int want_G, int want_threads, int want_groups,
+                               int n_sys_min_class);
+// sweep_unstructured.cu
+int nb_launch_sweep_unstructured(nanobte_solver *h);
+void nb_free_unstructured(nanobte_solver *h);

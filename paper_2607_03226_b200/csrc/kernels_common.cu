@@ -1,0 +1,358 @@
+// kernels_common.cu -- kernels shared by both mesh kinds: boundary closures (a3), moment reduction (a6),
+// temperature update (a8), exports, and the conjugate-gradient diffusion correction (a7).
+// Everything is fp64, deterministic (no floating-point atomics; fixed reduction trees).
+#include <cooperative_groups.h>
+
+#include "internal.h"
+namespace cg = cooperative_groups;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double nanmax(double a, double b) { return !(b <= a) ? b : a; }  // NaN wins
+__device__ __forceinline__ double warp_nanmax(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = nanmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// =================================================================================================================
+// (a3) boundary closures, one warp per boundary face, lanes over directions, loop over bands.
+//   G_bf   = sum_{s.n>0} w (s.n) eps_{b,s,c} / sum_{s.n<0} w |s.n|                     (R7)
+//   inflow = thermalizing C_b (T_w - T_ref)/W (R6) | G (diffuse) | eps_{b,r(s),c} (specular) | p spec + (1-p) G (R8)
+//   faceflux_bf,b = v_b [ sum_out w (s.n) eps^{n+1} + sum_in w (s.n) inflow^{n} ]       (O8; inflow^n = what the
+//                   sweep that produced eps^{n+1} consumed -- read before it is overwritten)
+// =================================================================================================================
+struct BoundaryRun {
+  BoundaryArgs a;
+  double W;
+  int unstructured;  // e layout [D][n_pos][B] instead of [D][B][n_pos]
+};
+
+__global__ void __launch_bounds__(256) boundary_kernel(BoundaryRun R) {
+  extern __shared__ double sm[];
+  const BoundaryArgs &a = R.a;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int bf = blockIdx.x * (blockDim.x >> 5) + wib;
+  if (bf >= a.n_bf) return;
+  double *eo = sm + (size_t)wib * a.D;
+  const int type = a.bf_type[bf];
+  const double p = a.bf_p[bf], den = a.bf_den[bf], dTw = a.bf_eps_w[bf];
+  const size_t row = (size_t)bf * a.D;
+  for (int b = 0; b < a.B; ++b) {
+    double gnum = 0.0;
+    for (int d = lane; d < a.D; d += 32) {
+      const double sn = a.bf_sn[row + d];
+      if (sn > 0.0) {
+        const int64_t pos = a.bf_opos[row + d];
+        const double val = R.unstructured ? a.e[((int64_t)d * a.e_stride + pos) * a.B + b]
+                                          : a.e[((int64_t)d * a.B + b) * a.e_stride + pos];
+        eo[d] = val;
+        gnum += a.w[d] * sn * val;
+      }
+    }
+    gnum = warp_sum(gnum);
+    __syncwarp();
+    const double Gb = den > 0.0 ? gnum / den : 0.0;
+    double fin = 0.0;
+    for (int d = lane; d < a.D; d += 32) {
+      const double sn = a.bf_sn[row + d];
+      if (sn < 0.0) {
+        const int64_t addr = a.dir_bin[d] + (int64_t)b * a.dir_nin[d] + a.bf_inidx[row + d];
+        fin += a.w[d] * sn * a.bin[addr];
+        double nv;
+        if (type == NANOBTE_THERMALIZING) nv = a.C[b] * dTw / R.W;
+        else if (type == NANOBTE_DIFFUSE) nv = Gb;
+        else {
+          const double spec = eo[a.bf_mirror[row + d]];
+          nv = (type == NANOBTE_SPECULAR) ? spec : p * spec + (1.0 - p) * Gb;
+        }
+        a.bin[addr] = nv;
+      }
+    }
+    fin = warp_sum(fin);
+    if (lane == 0) {
+      a.G[(size_t)bf * a.B + b] = Gb;
+      a.faceflux[(size_t)bf * a.B + b] = a.v[b] * (gnum + fin);
+    }
+    __syncwarp();
+  }
+}
+
+int nb_launch_boundary(nanobte_solver *h) {
+  if (h->n_bf == 0) return 0;
+  BoundaryRun R;
+  R.a = h->bd;
+  R.W = h->W;
+  R.unstructured = h->kind;
+  const int wpb = 8;
+  const size_t smem = (size_t)wpb * h->D * sizeof(double);
+  boundary_kernel<<<(h->n_bf + wpb - 1) / wpb, wpb * 32, smem, h->stream>>>(R);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+// =================================================================================================================
+// (a6) moments, structured layout.  One thread per pair of positions of one class (octant); streams every e row
+// of the class exactly once (8 B per update) and writes the class's partial sums
+//   part[c][0] = sum w/tau eps   part[c][1] = sum w eps   part[c][2..4] = sum v w s eps      (Eq. 5, R13, Eq. 7)
+// =================================================================================================================
+struct MomentsArgs {
+  const double *e;
+  const double *mcoef;
+  const int32_t *cls_sys;
+  double *part;
+  int64_t e_stride;
+  int32_t cls_nsys[NB_MAX_CLASSES], cls_sys_off[NB_MAX_CLASSES], cls_npos[NB_MAX_CLASSES];
+};
+
+__global__ void __launch_bounds__(256) moments_structured_kernel(MomentsArgs a) {
+  extern __shared__ double smc[];  // [nsys][5]
+  const int c = blockIdx.y;
+  const int nsys = a.cls_nsys[c];
+  const int32_t *sysl = a.cls_sys + a.cls_sys_off[c];
+  for (int k = threadIdx.x; k < nsys * 5; k += blockDim.x) smc[k] = a.mcoef[(size_t)sysl[k / 5] * 5 + (k % 5)];
+  __syncthreads();
+  const int64_t pos = 2 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
+  if (pos >= a.cls_npos[c]) return;
+  double2 m0 = {0, 0}, m1 = {0, 0}, m2 = {0, 0}, m3 = {0, 0}, m4 = {0, 0};
+  const double *base = a.e + pos;
+  int k = 0;
+  for (; k + 4 <= nsys; k += 4) {
+    double2 v[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) v[j] = __ldcs(reinterpret_cast<const double2 *>(base + (int64_t)sysl[k + j] * a.e_stride));
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const double *cf = smc + (k + j) * 5;
+      m0.x += cf[0] * v[j].x; m0.y += cf[0] * v[j].y;
+      m1.x += cf[1] * v[j].x; m1.y += cf[1] * v[j].y;
+      m2.x += cf[2] * v[j].x; m2.y += cf[2] * v[j].y;
+      m3.x += cf[3] * v[j].x; m3.y += cf[3] * v[j].y;
+      m4.x += cf[4] * v[j].x; m4.y += cf[4] * v[j].y;
+    }
+  }
+  for (; k < nsys; ++k) {
+    const double2 v = __ldcs(reinterpret_cast<const double2 *>(base + (int64_t)sysl[k] * a.e_stride));
+    const double *cf = smc + k * 5;
+    m0.x += cf[0] * v.x; m0.y += cf[0] * v.y;
+    m1.x += cf[1] * v.x; m1.y += cf[1] * v.y;
+    m2.x += cf[2] * v.x; m2.y += cf[2] * v.y;
+    m3.x += cf[3] * v.x; m3.y += cf[3] * v.y;
+    m4.x += cf[4] * v.x; m4.y += cf[4] * v.y;
+  }
+  double *p = a.part + (size_t)c * 5 * a.e_stride + pos;
+  *reinterpret_cast<double2 *>(p) = m0;
+  *reinterpret_cast<double2 *>(p + a.e_stride) = m1;
+  *reinterpret_cast<double2 *>(p + 2 * a.e_stride) = m2;
+  *reinterpret_cast<double2 *>(p + 3 * a.e_stride) = m3;
+  *reinterpret_cast<double2 *>(p + 4 * a.e_stride) = m4;
+}
+
+int nb_launch_moments_unstructured(nanobte_solver *h);
+
+int nb_launch_moments(nanobte_solver *h) {
+  if (h->kind == 1) return nb_launch_moments_unstructured(h);
+  MomentsArgs a;
+  a.e = h->sw.e;
+  a.mcoef = h->mcoef;
+  a.cls_sys = h->cls_sys;
+  a.part = h->part;
+  a.e_stride = h->e_stride;
+  int maxpos = 0, maxsys = 0;
+  for (int c = 0; c < NB_MAX_CLASSES; ++c) {
+    a.cls_nsys[c] = h->cls_nsys[c];
+    a.cls_sys_off[c] = h->cls_sys_off[c];
+    a.cls_npos[c] = h->cls_npos[c];
+    maxpos = max(maxpos, h->cls_npos[c]);
+    maxsys = max(maxsys, h->cls_nsys[c]);
+  }
+  dim3 grid((maxpos + 511) / 512, h->n_cls);
+  const size_t smem = (size_t)maxsys * 5 * sizeof(double);
+  if (smem > 48 * 1024)
+    NB_CUDA(h, cudaFuncSetAttribute(moments_structured_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  moments_structured_kernel<<<grid, 256, smem, h->stream>>>(a);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+// =================================================================================================================
+// (a6)/(a8) combine the class partials per cell (fixed class order), update T, track max |dT|, and refresh the
+// sweep-order copies of theta.
+// =================================================================================================================
+struct UpdateArgs {
+  int32_t n_act, n_cls, mode, dim;
+  const double *part;
+  int64_t e_stride;
+  const int32_t *a2pos;  // [n_cls][n_act]
+  double2 *tq[NB_MAX_CLASSES];
+  double *theta, *theta_prev, *theta_SI, *theta_en, *q;
+  const double *x;       // CG solution (mode 1)
+  double beta, Csum;
+  unsigned long long *maxdT;
+  double *uns_theta;     // unstructured: nothing to permute (theta is read by cell id)
+};
+
+__global__ void __launch_bounds__(256) update_kernel(UpdateArgs u) {
+  __shared__ double red[8];
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  double d = 0.0;
+  if (a < u.n_act) {
+    double th;
+    if (u.mode == 0) {
+      double m[5] = {0, 0, 0, 0, 0};
+      for (int c = 0; c < u.n_cls; ++c) {
+        const int64_t pos = u.a2pos[(size_t)c * u.n_act + a];
+        const double *p = u.part + (size_t)c * 5 * u.e_stride + pos;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) m[k] += p[(size_t)k * u.e_stride];
+      }
+      th = m[0] / u.beta;               // Eq. 5
+      u.theta_SI[a] = th;
+      u.theta_en[a] = m[1] / u.Csum;    // R13
+      u.q[3 * (size_t)a] = m[2];        // Eq. 7
+      u.q[3 * (size_t)a + 1] = m[3];
+      u.q[3 * (size_t)a + 2] = m[4];
+      u.theta_prev[a] = u.theta[a];
+    } else {
+      th = u.theta_SI[a] + u.x[a];      // R14a
+    }
+    u.theta[a] = th;                    // Eq. 6
+    d = fabs(th - u.theta_prev[a]);
+    for (int c = 0; c < u.n_cls; ++c) u.tq[c][u.a2pos[(size_t)c * u.n_act + a]].x = th;
+  }
+  d = warp_nanmax(d);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = d;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    d = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+    d = warp_nanmax(d);
+    if (threadIdx.x == 0) atomicMax(u.maxdT, (unsigned long long)__double_as_longlong(d));
+  }
+}
+
+int nb_launch_update_unstructured(nanobte_solver *h, int mode);
+
+int nb_launch_update(nanobte_solver *h, int mode) {
+  NB_CUDA(h, cudaMemsetAsync(h->d_maxdT, 0, sizeof(unsigned long long), h->stream));
+  if (h->kind == 1) return nb_launch_update_unstructured(h, mode);
+  UpdateArgs u;
+  u.n_act = h->n_act; u.n_cls = h->n_cls; u.mode = mode; u.dim = h->dim;
+  u.part = h->part; u.e_stride = h->e_stride; u.a2pos = h->a2pos;
+  for (int c = 0; c < NB_MAX_CLASSES; ++c) u.tq[c] = h->tq[c];
+  u.theta = h->theta; u.theta_prev = h->theta_prev; u.theta_SI = h->theta_SI; u.theta_en = h->theta_en; u.q = h->q;
+  u.x = h->cg_x; u.beta = h->beta; u.Csum = h->Csum; u.maxdT = h->d_maxdT; u.uns_theta = nullptr;
+  update_kernel<<<(h->n_act + 255) / 256, 256, 0, h->stream>>>(u);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+// ---- set_T: theta <- T - T_ref (cells -> active), refresh sweep-order copies --------------------------------------
+__global__ void set_theta_kernel(int n_act, int n_cls, const int32_t *act2cell, const double *T, double T_ref,
+                                 double *theta, const int32_t *a2pos, UpdateArgs u) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= n_act) return;
+  const double th = T[act2cell[a]] - T_ref;
+  theta[a] = th;
+  for (int c = 0; c < n_cls; ++c) u.tq[c][a2pos[(size_t)c * n_act + a]].x = th;
+}
+
+int nb_launch_set_theta(nanobte_solver *h, const double *T_cells_dev) {
+  UpdateArgs u{};
+  for (int c = 0; c < NB_MAX_CLASSES; ++c) u.tq[c] = h->tq[c];
+  const int ncls = h->kind == 0 ? h->n_cls : 0;
+  set_theta_kernel<<<(h->n_act + 255) / 256, 256, 0, h->stream>>>(h->n_act, ncls, h->act2cell, T_cells_dev, h->T_ref,
+                                                                   h->theta, h->a2pos, u);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+// ---- exports ---------------------------------------------------------------------------------------------------------
+__global__ void scatter_cells_kernel(int n_cells, const int32_t *cell2act, const double *src, int src_stride,
+                                     double *dst, int ncomp, double add) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_cells) return;
+  const int a = cell2act[c];
+  for (int k = 0; k < ncomp; ++k) dst[(size_t)c * ncomp + k] = add + (a >= 0 ? src[(size_t)a * src_stride + k] : 0.0);
+}
+
+int nb_launch_scatter_cells(nanobte_solver *h, const double *src_act, double *dst_cells, int ncomp, double add) {
+  const int stride = (src_act == h->q) ? 3 : 1;
+  scatter_cells_kernel<<<(h->n_cells + 255) / 256, 256, 0, h->stream>>>(h->n_cells, h->cell2act, src_act, stride,
+                                                                       dst_cells, ncomp, add);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+struct GetEArgs {
+  int32_t n_cells, n_act, B, b0, nb, d0, nd, unstructured;
+  const int32_t *cell2act, *a2pos, *dir_cls;
+  const double *e, *C;
+  int64_t e_stride;
+  double off_scale;  // T_ref / W, or 0 for the deviational export
+  double *dst;
+};
+
+__global__ void get_e_kernel(GetEArgs g) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= g.n_cells) return;
+  const int bi = blockIdx.y / g.nd, di = blockIdx.y % g.nd;
+  const int b = g.b0 + bi, d = g.d0 + di;
+  const int a = g.cell2act[c];
+  double val = 0.0;
+  if (a >= 0) {
+    const int64_t pos = g.a2pos[(size_t)g.dir_cls[d] * g.n_act + a];
+    val = g.unstructured ? g.e[((int64_t)d * g.e_stride + pos) * g.B + b] : g.e[((int64_t)d * g.B + b) * g.e_stride + pos];
+    val += g.C[b] * g.off_scale;
+  }
+  g.dst[((size_t)bi * g.nd + di) * g.n_cells + c] = val;
+}
+
+int nb_launch_get_e(nanobte_solver *h, int b0, int nb, int d0, int nd, double *dst_dev, int deviational) {
+  if (nb == 0 || nd == 0) return 0;
+  GetEArgs g;
+  g.n_cells = h->n_cells; g.n_act = h->n_act; g.B = h->B; g.b0 = b0; g.nb = nb; g.d0 = d0; g.nd = nd;
+  g.unstructured = h->kind;
+  g.cell2act = h->cell2act; g.a2pos = h->a2pos; g.dir_cls = h->dir_cls; g.e = h->bd.e; g.C = h->bd.C;
+  g.e_stride = h->e_stride; g.off_scale = deviational ? 0.0 : h->T_ref / h->W; g.dst = dst_dev;
+  dim3 grid((h->n_cells + 255) / 256, nb * nd);
+  get_e_kernel<<<grid, 256, 0, h->stream>>>(g);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+// ---- boundary heat per tag (O8): one block per tag, fixed-order tree -----------------------------------------------------
+__global__ void __launch_bounds__(256) tagheat_kernel(const int32_t *tagface_ptr, const int32_t *tagface, const double *faceflux,
+                                                      const double *bf_area, int B, double *out) {
+  __shared__ double red[256];
+  const int t = blockIdx.x;
+  double acc = 0.0;
+  for (int k = tagface_ptr[t] + threadIdx.x; k < tagface_ptr[t + 1]; k += blockDim.x) {
+    const int bf = tagface[k];
+    double F = 0.0;
+    for (int b = 0; b < B; ++b) F += faceflux[(size_t)bf * B + b];
+    acc += bf_area[bf] * F;
+  }
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[t] = red[0];
+}
+
+int nb_launch_tagheat(nanobte_solver *h) {
+  tagheat_kernel<<<h->n_tags, 256, 0, h->stream>>>(h->tagface_ptr, h->tagface, h->bd.faceflux, h->bd.bf_area, h->B, h->d_tagheat);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}

@@ -1,0 +1,100 @@
+"""CPU-side checks of the C-ABI library: it builds, loads without a GPU, exports every symbol include/nanobte.h
+declares, its host-side setup (validation, schedules, workspace sizing) runs, and it fails loudly -- never falls
+back -- when no CUDA device is present."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2607_03226_b200 import workloads as wl
+from paper_2607_03226_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load()
+
+
+def test_exports_every_declared_symbol(lib):
+    hdr = open(os.path.join(ROOT, "include", "nanobte.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(nanobte_[a-z_A-Z0-9]+)\s*\(", hdr))
+    assert declared, "no declarations parsed"
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_struct_layouts_match_header(lib):
+    # sizes the C compiler gives the ABI structs (LP64): a drifted ctypes mirror would corrupt every call
+    assert C.sizeof(binding.Bands) == 40 and C.sizeof(binding.Quadrature) == 24 and C.sizeof(binding.Tag) == 16
+    assert C.sizeof(binding.StructuredMesh) == 88 and C.sizeof(binding.UnstructuredMesh) == 64
+    assert C.sizeof(binding.Options) == 64
+    assert C.sizeof(binding.Info) == 88
+
+
+def test_strerror(lib):
+    assert lib.nanobte_strerror(0) == b"OK" and lib.nanobte_strerror(-4) == b"ARCH" and lib.nanobte_strerror(-11) == b"UNSUPPORTED"
+
+
+@pytest.mark.parametrize("name,kw,nupd", [
+    ("gray_square", {}, 6400),
+    ("nongray_square", {}, 5242880),
+    ("cube", {"n": 16}, 16**3 * 20 * 128),
+    ("finfet", {"nx": 32, "ny": 16, "nz": 16}, None),
+])
+def test_workspace_bytes_and_host_setup(lib, name, kw, nupd):
+    pr = wl.CONFIGS[name](**kw)
+    nbytes = binding.workspace_bytes(pr)
+    n_e = wl.n_updates(pr) * 8
+    if nupd is not None:
+        assert wl.n_updates(pr) == nupd
+    assert nbytes > n_e  # the e array dominates; tables and caches come on top
+    assert nbytes < 3 * n_e + (64 << 20)
+
+
+def test_host_validation_errors(lib):
+    pr = wl.config_gray_square(n=6)
+    bad = dict(pr, quad={"s": pr["quad"]["s"] * 1.1, "w": pr["quad"]["w"], "dim": 2})
+    with pytest.raises(binding.NanoBTEError) as e:
+        binding.workspace_bytes(bad)
+    assert e.value.code == -8
+    m = dict(pr["mesh"])
+    m["bf_cell"], m["bf_side"], m["bf_tag"] = m["bf_cell"][1:], m["bf_side"][1:], m["bf_tag"][1:]
+    with pytest.raises(binding.NanoBTEError) as e:
+        binding.workspace_bytes(dict(pr, mesh=m))
+    assert e.value.code == -5
+    spec = wl.config_gray_square(n=6, wall=wl.SPECULAR)
+    q = wl.inplane_quadrature(16)
+    q["s"] = q["s"][:-2].copy()
+    q["w"] = q["w"][:-2].copy()
+    # a quadrature that is not closed under reflection: first failure is sum w s != 0
+    with pytest.raises(binding.NanoBTEError):
+        binding.workspace_bytes(dict(spec, quad=q))
+    b = dict(pr["bands"])
+    b["tau"] = np.array([-1.0])
+    with pytest.raises(binding.NanoBTEError) as e:
+        binding.workspace_bytes(dict(pr, bands=b))
+    assert e.value.code == -1
+
+
+def test_no_cpu_fallback(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA device present")
+    with pytest.raises(RuntimeError):
+        binding.Solver(wl.config_gray_square(n=4))
+    # straight through the C ABI: create must refuse with NANOBTE_E_ARCH
+    ms = binding._Marshalled(wl.config_gray_square(n=4))
+    opt = binding.Options(300.0, None, None, None, 0, 0.0, 0, 0, 0, 0)
+    h = C.c_void_p()
+    rc = lib.nanobte_create_structured(C.byref(ms.mesh), C.byref(ms.bands), C.byref(ms.quad), ms.tags, ms.n_tags, None,
+                                       C.byref(opt), C.byref(h))
+    assert rc == -4
+    assert b"no CPU fallback" in lib.nanobte_last_error(h) or b"CUDA" in lib.nanobte_last_error(h)
+    lib.nanobte_destroy(h)

@@ -1,0 +1,216 @@
+"""Parity of the CUDA library (through its C ABI) against the CPU oracle, element by element, on the same seeded
+inputs (`-m gpu`).  Bar (BASELINE.json north_star): per-sweep e_{b,s} and T within 1e-10 max-norm relative error
+(deviational variables, per band -- SURVEY.md 8(d)), converged T within 1e-8 K with an identical iteration count.
+"""
+import numpy as np
+import pytest
+
+from oracle.ref import RefSolver
+from paper_2607_03226_b200 import workloads as wl
+from test_oracle_pins import TINY, random_T, small_bands
+
+pytestmark = pytest.mark.gpu
+
+TOL_SWEEP = 1e-10  # max-norm relative, north_star
+TOL_T_CONVERGED = 1e-8  # K, north_star
+
+
+def gpu_solver(pr, **kw):
+    from paper_2607_03226_b200.binding import Solver
+    return Solver(pr, **kw)
+
+
+def rel(a, b):
+    s = np.abs(b).max()
+    return np.abs(a - b).max() / s if s > 0 else np.abs(a - b).max()
+
+
+def compare_state(g, r, pr, what=""):
+    eg, er = g.get_e(), r.get_e()
+    assert eg.shape == er.shape
+    for b in range(er.shape[0]):
+        assert rel(eg[b], er[b]) <= TOL_SWEEP, f"{what}: e band {b}: {rel(eg[b], er[b]):.3e}"
+
+
+def compare_fields(g, r, pr, what=""):
+    Tr = pr["T_ref"]
+    for which in (0, 1, 2):
+        a, b = g.get_T(which) - Tr, r.get_T(which) - Tr
+        assert rel(a, b) <= TOL_SWEEP, f"{what}: T[{which}] {rel(a, b):.3e}"
+    assert rel(g.get_q(), r.get_q()) <= TOL_SWEEP, f"{what}: q"
+    if r.n_bf:
+        assert rel(g.get_G(), r.get_G()) <= TOL_SWEEP, f"{what}: G"
+
+
+def step_parity(pr, n_steps=3, T_init=None, mode="plain", **kw):
+    r = RefSolver(pr, T_init=T_init)
+    g = gpu_solver(pr, T_init=T_init, **kw)
+    assert g.n_active == r.n_active and abs(g.kappa - r.kappa) <= 1e-14 * abs(r.kappa)
+    for n in range(n_steps):
+        r.sweep()
+        g.sweep()
+        compare_state(g, r, pr, f"sweep {n}")
+        dr = r.update_temperature()
+        dg = g.update_temperature()
+        compare_fields(g, r, pr, f"update {n}")
+        assert abs(dg - dr) <= 1e-9 * max(abs(dr), 1e-300) + 1e-13
+        Hg, Hr = g.get_boundary_heat(), r.get_boundary_heat()
+        assert np.abs(Hg - Hr).max() <= 1e-9 * max(np.abs(Hr).max(), 1e-300)
+        if mode == "synthetic":
+            (ir, d2r), (ig, d2g) = r.diffusion_correct(), g.diffusion_correct()
+            a, b = g.get_T(0) - pr["T_ref"], r.get_T(0) - pr["T_ref"]
+            assert rel(a, b) <= 1e-9, f"synthetic step {n}: {rel(a, b):.3e}"
+            assert abs(ig - ir) <= max(2, ir // 20)
+    g.close()
+    r.close()
+
+
+# ---- tiny meshes: every closure type, non-uniform spacing, a masked L-shape ------------------------------------------
+@pytest.mark.parametrize("name", [k for k in TINY if TINY[k]["kind"] == "structured"])
+def test_tiny_steps(name):
+    pr = TINY[name]
+    step_parity(pr, 4, T_init=random_T(pr, 5))
+
+
+@pytest.mark.parametrize("name", [k for k in TINY if TINY[k]["kind"] == "structured"])
+def test_tiny_synthetic_steps(name):
+    pr = dict(TINY[name])
+    pr["bands"] = small_bands(len(pr["bands"]["C"]), 21, lo=-11.3)
+    step_parity(pr, 3, T_init=random_T(pr, 6), mode="synthetic")
+
+
+@pytest.mark.parametrize("name", [k for k in TINY if TINY[k]["kind"] == "structured"])
+@pytest.mark.parametrize("mode", ["plain", "synthetic"])
+def test_tiny_solve(name, mode):
+    pr = dict(TINY[name])
+    if mode == "synthetic":
+        pr["bands"] = small_bands(len(pr["bands"]["C"]), 21, lo=-11.3)
+    r, g = RefSolver(pr), gpu_solver(pr)
+    rr, rg = r.solve(1e-11, 20000, mode), g.solve(1e-11, 20000, mode)
+    assert rr["converged"] and rg["converged"]
+    assert rg["iters"] == rr["iters"]
+    assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+    hg, hr = g.get_history()[0], r.get_history()[0]
+    np.testing.assert_allclose(hg, hr, rtol=1e-6, atol=1e-14)
+
+
+# ---- BASELINE.json configs[0] (full size) and configs[1] (full size), several launch shapes --------------------------------
+def test_config0_gray_square_full():
+    pr = wl.config_gray_square()
+    step_parity(pr, 3)
+    r, g = RefSolver(pr), gpu_solver(pr)
+    rr, rg = r.solve(pr["tol"], pr["max_iter"]), g.solve(pr["tol"], pr["max_iter"])
+    assert rr["iters"] == rg["iters"] == 35
+    assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+    assert np.abs(g.get_T(1) - r.get_T(1)).max() <= TOL_T_CONVERGED
+    assert rel(g.get_q(), r.get_q()) <= 1e-8
+
+
+@pytest.mark.parametrize("kw", [{}, {"sweep_G": 1}, {"sweep_G": 2, "sweep_threads": 64}, {"sweep_G": 4},
+                                {"sweep_G": 1, "sweep_groups": 4}])
+def test_config1_nongray_square_full(kw):
+    pr = wl.config_nongray_square()
+    step_parity(pr, 2, **kw)
+
+
+def test_config1_solve():
+    pr = wl.config_nongray_square(n=48)
+    r, g = RefSolver(pr), gpu_solver(pr)
+    rr, rg = r.solve(pr["tol"], pr["max_iter"]), g.solve(pr["tol"], pr["max_iter"])
+    assert rr["converged"] and rg["converged"] and rr["iters"] == rg["iters"]
+    assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+
+
+# ---- cuts of configs[2] (cube) and configs[3] (finfet): several tiles and ragged tails ---------------------------------------
+@pytest.mark.parametrize("n,kw", [(12, {}), (20, {"sweep_G": 1}), (20, {"sweep_G": 2}), (20, {"sweep_G": 4, "sweep_threads": 128}),
+                                  (33, {"sweep_G": 2, "sweep_threads": 160}), (24, {"sweep_G": 1, "sweep_groups": 3})])
+def test_cube_cut_steps(n, kw):
+    pr = wl.config_cube(n=n, B=3, n_polar=4, n_azim=8)
+    step_parity(pr, 3, T_init=random_T(pr, 9), **kw)
+
+
+def test_cube_cut_solve_both_modes():
+    pr = wl.config_cube(n=10, B=4, n_polar=2, n_azim=8)
+    Ts = {}
+    for mode in ("plain", "synthetic"):
+        r, g = RefSolver(pr), gpu_solver(pr)
+        rr, rg = r.solve(1e-9, 3000, mode), g.solve(1e-9, 3000, mode)
+        assert rr["converged"] and rg["converged"], (rr, rg)
+        assert rr["iters"] == rg["iters"], (mode, rr, rg)
+        assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+        Ts[mode] = g.get_T(0)
+    assert np.abs(Ts["plain"] - Ts["synthetic"]).max() < 1e-6  # P6 on the GPU side
+
+
+@pytest.mark.parametrize("shape,kw", [((16, 8, 8), {}), ((32, 16, 16), {"sweep_G": 2}), ((24, 12, 12), {"sweep_G": 1})])
+def test_finfet_cut_steps(shape, kw):
+    nx, ny, nz = shape
+    pr = wl.config_finfet(nx=nx, ny=ny, nz=nz, B=3, n_polar=2, n_azim=8)
+    step_parity(pr, 3, T_init=random_T(pr, 10), mode="synthetic", **kw)
+
+
+def test_finfet_cut_solve():
+    pr = wl.config_finfet(nx=16, ny=8, nz=8, B=3, n_polar=2, n_azim=8)
+    for mode in ("plain", "synthetic"):
+        r, g = RefSolver(pr), gpu_solver(pr)
+        rr, rg = r.solve(1e-9, 5000, mode), g.solve(1e-9, 5000, mode)
+        assert rr["converged"] and rg["converged"], (rr, rg)
+        assert rr["iters"] == rg["iters"], (mode, rr, rg)
+        assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+
+
+# ---- degenerate shapes ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape", [(1, 1, 1), (7, 1, 1), (1, 9, 1), (5, 1, 3), (1, 1, 6), (2, 3, 1)])
+def test_degenerate_shapes(shape):
+    nx, ny, nz = shape
+    tags = [(wl.THERMALIZING, 302.0), (wl.THERMALIZING, 297.0), (wl.DIFFUSE, 0.0), (wl.SPECULAR, 0.0)]
+    quad = wl.product_quadrature(2, 4) if nz > 1 else wl.inplane_quadrature(8)
+    pr = wl.make_structured_problem(nx, ny, nz, 7e-9, 9e-9, 11e-9, small_bands(2, 3), quad, tags, [0, 1, 2, 2, 3, 3],
+                                    Qdot=np.full(nx * ny * nz, 3e16))
+    step_parity(pr, 3)
+
+
+def test_isothermal_stays_isothermal():
+    pr = wl.config_cube(n=8, B=2, n_polar=2, n_azim=4, src=0.0)
+    pr["mesh"]["tags"] = [(wl.THERMALIZING, 305.0), (wl.THERMALIZING, 305.0), (wl.DIFFUSE, 0.0), (wl.SPECULAR, 0.0)]
+    g = gpu_solver(pr)
+    res = g.solve(1e-12, 10)
+    assert res["iters"] == 1 and res["last_dT"] == 0.0
+    assert np.abs(g.get_e()).max() == 0.0
+
+
+def test_bitwise_reproducible():
+    pr = wl.config_cube(n=16, B=2, n_polar=2, n_azim=8)
+    outs = []
+    for _ in range(2):
+        g = gpu_solver(pr)
+        g.solve(1e-9, 6, "synthetic")
+        outs.append((g.get_T(0).copy(), g.get_e(0, 1, 0, 4).copy()))
+        g.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+def test_set_T_and_device_getters():
+    import torch
+    pr = wl.config_cube(n=8, B=2, n_polar=2, n_azim=4)
+    T0 = random_T(pr, 3)
+    r, g = RefSolver(pr), gpu_solver(pr)
+    r.set_T(T0)
+    g.set_T(torch.as_tensor(T0, device="cuda"))
+    r.sweep(); g.sweep()
+    compare_state(g, r, pr)
+    ed = g.get_e(device=True)
+    assert ed.is_cuda and np.array_equal(ed.cpu().numpy(), g.get_e())
+    assert rel(g.get_e(deviational=False), r.get_e(deviational=False)) <= 1e-12
+    Td = g.get_T(0, device=True)
+    assert np.array_equal(Td.cpu().numpy(), g.get_T(0))
+
+
+def test_errors_on_gpu():
+    from paper_2607_03226_b200.binding import NanoBTEError
+    pr = wl.config_cube(n=6, B=2, n_polar=2, n_azim=4)
+    pr["mesh"]["tags"] = [(wl.DIFFUSE, 0.0)] * 4
+    g = gpu_solver(pr)
+    with pytest.raises(NanoBTEError) as e:
+        g.solve(1e-9, 5, "synthetic")
+    assert e.value.code == -9
