@@ -1,0 +1,352 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's measurement contract for the NanoBTE hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload finfet|cube|nongray_square|gray_square|triangles]
+                    [--mode plain|synthetic] [--impl reference] [--no-cpu-baseline]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: transport sweep (a2-a5), closures +
+moments + temperature update (a3, a6, a8) and, in synthetic mode, the CG diffusion correction (a7).  The default
+workload is BASELINE.json configs[3] (FinFET-like masked grid, 844 M cell.band.direction updates per sweep, the
+"largest structured config" the north_star's roofline bar is set on), in the mode that config names (synthetic).
+Prints ONE JSON line (rank 0).  Multi-GPU: the path is single-GPU by the north_star, so --gpus N runs N independent
+replicas (one per rank under torchrun), no data-path collective; value is the whole-job aggregate.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell-band-direction updates/s through one source iteration (sweep + closures + moments [+ CG]), fp64"
+UNIT = "updates/s"
+SMI_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="finfet")
+    ap.add_argument("--mode", default=None, help="plain | synthetic (default: the config's own)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample-bands", type=int, default=0, help="bands in the oracle's sample (0 = auto)")
+    ap.add_argument("--sweep-G", type=int, default=0)
+    ap.add_argument("--sweep-threads", type=int, default=0)
+    ap.add_argument("--sweep-groups", type=int, default=0)
+    return ap.parse_args()
+
+
+def make_problem(name):
+    from paper_2607_03226_b200 import workloads as wl
+    return wl.CONFIGS[name]()
+
+
+def workload_config(pr, mode, extra=None):
+    from paper_2607_03226_b200 import workloads as wl
+    m = pr["mesh"]
+    grid = f"{m['nx']}x{m['ny']}x{m['nz']}" if pr["kind"] == "structured" else f"{m['n_cells']} triangles"
+    cfg = {"workload": pr["name"], "grid": grid, "active_cells": wl.n_active(pr), "bands": len(pr["bands"]["C"]),
+           "directions": len(pr["quad"]["w"]), "updates_per_sweep": wl.n_updates(pr), "mode": mode,
+           "l2_policy": "inputs larger than L2 (e array >> 126 MB); no flush needed" if wl.n_updates(pr) * 8 > 4 * 126e6
+           else "e array fits L2: numbers are L2-resident, no roofline claim"}
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# clocks
+# ---------------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi polled every 100 ms during the timed region (B200_PROFILING.md 'clocks' line)."""
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={SMI_QUERY}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[5 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        try:
+            os.unlink(self.path)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # samples under load = the upper half (the sampler also sees the idle edges of the region)
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline / --impl reference)
+# ---------------------------------------------------------------------------------------------------------------------
+def oracle_sample_problem(pr, n_bands):
+    """Same mesh, quadrature, tags and source; the first n_bands bands of the table.  (band, direction) systems are
+    independent, so the cost per update is the workload's own."""
+    B = len(pr["bands"]["C"])
+    n_bands = max(1, min(B, n_bands))
+    sub = dict(pr)
+    sub["bands"] = {k: np.ascontiguousarray(v[:n_bands]) for k, v in pr["bands"].items()}
+    return sub, n_bands
+
+
+def auto_sample_bands(pr, target_updates=1.0e8):
+    from paper_2607_03226_b200 import workloads as wl
+    per_band = wl.n_active(pr) * len(pr["quad"]["w"])
+    return int(max(1, min(len(pr["bands"]["C"]), round(target_updates / per_band))))
+
+
+def run_oracle(pr, mode, steps, warmup, n_bands):
+    """Times `steps` oracle source iterations on the sample; returns (updates/s, seconds per step, cores, sample text)."""
+    from oracle.ref import RefSolver
+    from paper_2607_03226_b200 import workloads as wl
+    sub, nb = oracle_sample_problem(pr, n_bands)
+    cores = len(os.sched_getaffinity(0))
+    r = RefSolver(sub, threads=cores)
+    cores = r.threads
+
+    def step():
+        r.sweep()
+        r.update_temperature()
+        if mode == "synthetic":
+            r.diffusion_correct()
+
+    for _ in range(warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step()
+    dt = (time.perf_counter() - t0) / max(1, steps)
+    upd = wl.n_updates(sub)
+    r.close()
+    sample = (f"{pr['name']}: same mesh/quadrature/walls/source, first {nb} of {len(pr['bands']['C'])} bands "
+              f"({upd} updates per step), {steps} timed steps after {warmup} warm-up, mode {mode}")
+    return upd / dt, dt, cores, sample
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    pr = make_problem(args.workload)
+    mode = args.mode or pr["mode"]
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        nb = args.cpu_sample_bands or auto_sample_bands(pr, 4.0e7)
+        steps, warmup = max(1, min(args.steps, 5)), max(1, min(args.warmup, 1))
+        val, dt, cores, sample = run_oracle(pr, mode, steps, warmup, nb)
+        out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+               "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+               "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+               "config": workload_config(pr, mode, {"note": "CPU oracle on a bounded sample; ms_per_step is per sample step"}),
+               "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+               "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+               "gpu_launches": 0}
+        print(json.dumps(out))
+        return 0
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libnanobte has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2607_03226_b200 import build as nb_build
+    from paper_2607_03226_b200 import workloads as wl
+    if rank == 0:
+        nb_build.build()
+    if dist:
+        dist.barrier()
+    from paper_2607_03226_b200.binding import Solver
+
+    t_c0 = time.perf_counter()
+    g = Solver(pr, sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_groups=args.sweep_groups)
+    torch.cuda.synchronize()
+    create_s = time.perf_counter() - t_c0
+    upd = wl.n_updates(pr)
+    synthetic = mode == "synthetic"
+
+    def step(ev=None):
+        if ev is not None:
+            ev[0].record()
+        g.sweep()
+        if ev is not None:
+            ev[1].record()
+        if synthetic:
+            g.update_temperature(sync=False)
+            if ev is not None:
+                ev[2].record()
+            g.diffusion_correct()
+        else:
+            g.update_temperature(sync=True)
+            if ev is not None:
+                ev[2].record()
+        if ev is not None:
+            ev[3].record()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident arm -------------------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        step()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local)
+    l0 = g.launches
+    barrier()
+    sampler.start()
+    for k in range(args.steps):
+        step(evs[k])
+    barrier()
+    clocks = sampler.stop()
+    launches = g.launches - l0
+    total_ms = evs[0][0].elapsed_time(evs[-1][3])
+    sweep_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    update_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    cg_ms = float(np.mean([e[2].elapsed_time(e[3]) for e in evs])) if synthetic else 0.0
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if dist:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * upd / (ms_per_step * 1e-3)
+
+    # ---- end-to-end arm: host buffers through the C ABI, copies inside the timed region ------------------------------
+    T_host = torch.empty(g.n_cells, dtype=torch.float64).pin_memory()
+    T_host.copy_(torch.as_tensor(g.get_T(0)))
+    T_np = T_host.numpy()
+    e2e_steps = args.steps
+
+    def e2e_step():
+        g.set_T(T_np)                       # H2D: n_cells doubles from pinned host memory
+        g.sweep()
+        if synthetic:
+            g.update_temperature(sync=False)
+            g.diffusion_correct()           # D2H: max|dT|, CG iterations
+        else:
+            g.update_temperature(sync=True)
+        T_np[:] = g.get_T(0)                # D2H: n_cells doubles
+
+    for _ in range(min(2, args.warmup)):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if dist:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t.item())
+    e2e = {"value": world * upd / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(g.n_cells * 8),
+           "d2h_bytes_per_step": int(g.n_cells * 8 + 16), "ms_per_step": e2e_s * 1e3}
+
+    # ---- roofline of the dominant kernel (the sweep): 8 algorithmic bytes per update ----------
+    peak, peak_src = measured_peaks()
+    alg_bytes = 8.0 * upd
+    achieved = alg_bytes / (sweep_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "sweep_structured_kernel" if pr["kind"] == "structured" else "sweep_unstructured_kernel",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
+                "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": sweep_ms,
+                "moments_pass": {"achieved": alg_bytes / (update_ms * 1e-3) / 1e9, "launch_ms": update_ms,
+                                 "note": "closures + moments + update; 8 B/update read"}}
+    tr = os.path.join(ROOT, "profiles", "traffic.json")  # written by hand from the ncu --set full capture
+    if os.path.exists(tr):
+        try:
+            roofline["traffic"] = json.load(open(tr)).get(pr["name"], {}).get("sweep_dram_bytes_per_launch")
+        except Exception:
+            pass
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": workload_config(pr, mode, {"parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                                                "sweep": {k: g.info[k] for k in ("sweep_G", "sweep_threads", "sweep_groups",
+                                                                               "sweep_rmax", "n_tasks", "n_planes",
+                                                                               "sweep_smem_bytes", "pencil_axis")},
+                                                "device_bytes": g.info["device_bytes"]}),
+           "sweep_updates_per_s": world * upd / (sweep_ms * 1e-3), "s_per_iteration": ms_per_step * 1e-3,
+           "breakdown_ms": {"sweep": sweep_ms, "closures_moments_update": update_ms, "cg": cg_ms},
+           "create_s": create_s, "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+    g.close()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nb = args.cpu_sample_bands or auto_sample_bands(pr)
+        val, dt, cores, sample = run_oracle(pr, mode, 2, 1, nb)
+        out["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                               "s_per_sample_step": dt}
+    if rank == 0:
+        print(json.dumps(out))
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
