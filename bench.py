@@ -48,7 +48,6 @@ def parse_args():
     ap.add_argument("--cpu-sample-bands", type=int, default=0, help="bands in the oracle's sample (0 = auto)")
     ap.add_argument("--sweep-G", type=int, default=0)
     ap.add_argument("--sweep-threads", type=int, default=0)
-    ap.add_argument("--sweep-groups", type=int, default=0)
     return ap.parse_args()
 
 
@@ -221,7 +220,7 @@ def main():
     from paper_2607_03226_b200.binding import Solver
 
     t_c0 = time.perf_counter()
-    g = Solver(pr, sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_groups=args.sweep_groups)
+    g = Solver(pr, sweep_G=args.sweep_G, sweep_threads=args.sweep_threads)
     torch.cuda.synchronize()
     create_s = time.perf_counter() - t_c0
     upd = wl.n_updates(pr)
@@ -327,8 +326,7 @@ def main():
            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
            "config": workload_config(pr, mode, {"parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-                                                "sweep": {k: g.info[k] for k in ("sweep_G", "sweep_threads", "sweep_groups",
-                                                                               "sweep_rmax", "n_tasks", "n_planes",
+                                                "sweep": {k: g.info[k] for k in ("sweep_G", "sweep_threads", "sweep_rmax", "n_tasks", "n_planes",
                                                                                "sweep_smem_bytes", "pencil_axis")},
                                                 "device_bytes": g.info["device_bytes"]}),
            "sweep_updates_per_s": world * upd / (sweep_ms * 1e-3), "s_per_iteration": ms_per_step * 1e-3,

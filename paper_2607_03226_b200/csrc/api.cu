@@ -134,6 +134,7 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
   bd.v = A.put(c.v);
   bd.dir_bin = A.put(g.dir_bin);
   bd.dir_nin = A.put(g.dir_nin);
+  bd.dir_row0 = A.put(g.dir_row0);
   bd.bin = A.zeros<double>((size_t)g.bin_total);
   bd.G = A.zeros<double>(nbf * c.B);
   bd.faceflux = A.zeros<double>(nbf * c.B);
@@ -344,7 +345,7 @@ extern "C" int nanobte_get_info(const nanobte_solver *h, nanobte_info *o) {
   if (!h || !o) return NANOBTE_E_INVALID;
   o->dim = h->dim; o->n_cells = h->n_cells; o->n_active = h->n_act; o->B = h->B; o->D = h->D; o->n_bfaces = h->n_bf;
   o->n_octants = h->n_cls; o->n_planes = h->n_planes; o->n_tasks = h->n_tasks; o->sweep_G = h->sweep_G;
-  o->sweep_threads = h->sweep_threads; o->sweep_groups = h->sweep_groups; o->sweep_rmax = h->sweep_rmax; o->pencil_axis = h->pencil_axis; o->n_pos = h->n_pos;
+  o->sweep_threads = h->sweep_threads; o->sweep_rmax = h->sweep_rmax; o->pencil_axis = h->pencil_axis; o->n_pos = h->n_pos;
   o->n_inflow = h->n_inflow; o->device_bytes = h->arena_bytes; o->sweep_smem_bytes = h->sweep_smem;
   return 0;
 }

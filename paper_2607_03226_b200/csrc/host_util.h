@@ -68,7 +68,7 @@ struct GenericTables {
   std::vector<int32_t> bf_mirror, bf_inidx, bf_opos;
   // per direction
   std::vector<int64_t> dir_bin;
-  std::vector<int32_t> dir_nin;
+  std::vector<int32_t> dir_nin, dir_row0;
   // moments
   std::vector<double> mcoef;
   // cells

@@ -18,24 +18,29 @@
 #define NB_MAX_CLASSES 8  // structured: octants (quadrants in 2-D)
 
 // ---- per-octant tables of the structured sweep -------------------------------------------------------------
+// Pencils (lines of cells along the sweep axis u) of a class are sorted by (m = v'+w', w'); the pencil index p is
+// also the pencil's slot in the shared-memory wavefront state.  Hyperplane h = u'+v'+w' holds the contiguous pencil
+// range [lo, lo+cnt) and lives at positions start + (p - lo) of every e row of the class; start is a multiple of 16
+// cells so that the per-plane table segments can be fetched with 1-D bulk TMA and every warp stores whole lines.
 struct OctTab {
-  const uint32_t *pen;       // [n_pen]  slot | (m << 16), pencils sorted by (m = v'+w', w')
-  const int32_t *plane_off;  // [H]      pos = plane_off[h] + pencil index
-  const uint32_t *cellinfo;  // [n_pos]  bit0..2: u/v/w upwind value is a boundary inflow, bit3: hole, bits 4..: first inflow idx
-  const double2 *tq;         // [n_pos]  (theta, Qdot) in sweep order
-  const double *rhu, *rhv, *rhw;  // reciprocal spacings in primed coordinates (non-uniform path)
-  int32_t n_pen, H, n_pos, n_in;
+  const uint2 *pen;          // [n_pen]   .x = m, .y = pencil index of the v-upwind pencil | w-upwind pencil << 16 (n_pen = none)
+  const int4 *plane;         // [H]       {lo, cnt, start, 0}
+  const uint32_t *cellinfo;  // [n_pos+16] bit0..2: u/v/w upwind value is a boundary inflow, bit3: hole, bits 4..: first inflow idx
+  const double2 *tq;         // [n_pos+16] (theta, Qdot) in sweep order
+  const double *rhu;         // [nu]      1/h_u in primed coordinates (non-uniform spacing only)
+  const double2 *pen_rh;     // [n_pen]   (1/h_v, 1/h_w) of the pencil (non-uniform spacing only)
+  int64_t bin_base;          // offset of the class's first inflow row in bin
+  int32_t n_pen, H, n_pos, n_in, row0, n_rows, p_max;
 };
 
 struct SweepArgs {
   const int32_t *task_oct;   // [n_tasks]
-  const int32_t *task_sys;   // [n_tasks][G]  global system id d*B+b, or -1 (padding)
-  const double *coef;        // [D*B][8]   uniform: k_theta,k_Q,c_u,c_v,c_w ; general: A,S,1/tau,v|s_u|,v|s_v|,v|s_w|
-  const int64_t *sys_bin;    // [D*B]      offset of the system's inflow row in bin
-  const double *bin;
-  double *e;
-  int64_t e_stride;          // n_pos padded
-  int32_t nu, pitch, slots;  // pencil length, slot pitch, slots per system (pitch * nw)
+  const int32_t *task_row;   // [n_tasks] first row of the task, relative to the class's row0
+  const double *coef;        // [rows][8]  uniform: k_theta,k_Q,c_u,c_v,c_w ; general: A,S,1/tau,v|s_u|,v|s_v|,v|s_w|
+  const double *bin;         // inflow rows: class c, local row k at bin_base[c] + k * n_in[c]
+  double *e;                 // [rows][e_stride]
+  int64_t e_stride;
+  int32_t nu, sp, pcap;      // pencil length, state pitch (>= n_pen + 1), stage capacity in cells (multiple of 4)
 };
 
 // ---- boundary-closure kernel ----------------------------------------------------------------------------------
@@ -48,6 +53,7 @@ struct BoundaryArgs {
   const int32_t *bf_mirror;   // [n_bf][D]  mirrored direction for incoming d (specular/mixed) or -1
   const int32_t *bf_inidx;    // [n_bf][D]  index of this face in direction d's inflow row, -1 if not incoming
   const int32_t *bf_opos;     // [n_bf][D]  position of the owner cell in direction d's e row (outgoing d), else -1
+  const int32_t *dir_row0;    // [D]        e row of (direction d, band 0); band b is row dir_row0[d] + b
   const double *w, *C, *v;
   const int64_t *dir_bin;     // [D] base offset of direction d in bin
   const int32_t *dir_nin;     // [D] inflow row length of direction d
@@ -76,8 +82,8 @@ struct nanobte_solver {
 
   // structured sweep
   SweepArgs sw{};
-  int sweep_G = 1, sweep_threads = 0, sweep_rmax = 1, sweep_groups = 1, n_tasks = 0, pencil_axis = 0, n_planes = 0;
-  bool uniform = true, has_w = true, sweep_attr_set = false;
+  int sweep_G = 1, sweep_threads = 0, sweep_rmax = 1, n_tasks = 0, pencil_axis = 0, n_planes = 0;
+  bool uniform = true, sweep_attr_set = false;
   const OctTab *d_octs = nullptr;
   size_t sweep_smem = 0;
   int64_t n_pos = 0, n_inflow = 0, e_stride = 0;
@@ -90,10 +96,9 @@ struct nanobte_solver {
   // moments / update
   int32_t *cls_npos_h = nullptr;
   int32_t cls_npos[NB_MAX_CLASSES] = {0};
-  const int32_t *cls_sys = nullptr;      // [n_cls][max systems] system ids per class
-  int32_t cls_nsys[NB_MAX_CLASSES] = {0};
-  int32_t cls_sys_off[NB_MAX_CLASSES] = {0};
-  const double *mcoef = nullptr;         // [D*B][5]  w/tau, w, v w sx, v w sy, v w sz
+  int32_t cls_nsys[NB_MAX_CLASSES] = {0};  // e rows of class c: [cls_row0[c], cls_row0[c] + cls_nsys[c])
+  int32_t cls_row0[NB_MAX_CLASSES] = {0};
+  const double *mcoef = nullptr;         // [rows][5]  w/tau, w, v w sx, v w sy, v w sz
   double *part = nullptr;                // [n_cls][5][e_stride]
   const int32_t *a2pos = nullptr;        // [n_cls][n_act]
   const int32_t *dir_cls = nullptr;      // [D] class of each direction
@@ -144,7 +149,7 @@ int nb_cg_solve(nanobte_solver *h, int *iters);
 int nb_cg_blocks(nanobte_solver *h);
 // sweep_structured.cu
 int nb_launch_sweep_structured(nanobte_solver *h);
-int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int slots, int want_G, int want_threads, int want_groups,
+int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int H, int want_G, int want_threads,
                                int n_sys_min_class);
 // sweep_unstructured.cu
 int nb_launch_sweep_unstructured(nanobte_solver *h);

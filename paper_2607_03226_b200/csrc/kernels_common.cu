@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256) boundary_kernel(BoundaryRun R) {
       if (sn > 0.0) {
         const int64_t pos = a.bf_opos[row + d];
         const double val = R.unstructured ? a.e[((int64_t)d * a.e_stride + pos) * a.B + b]
-                                          : a.e[((int64_t)d * a.B + b) * a.e_stride + pos];
+                                          : a.e[((int64_t)a.dir_row0[d] + b) * a.e_stride + pos];
         eo[d] = val;
         gnum += a.w[d] * sn * val;
       }
@@ -102,29 +102,28 @@ int nb_launch_boundary(nanobte_solver *h) {
 // =================================================================================================================
 struct MomentsArgs {
   const double *e;
-  const double *mcoef;
-  const int32_t *cls_sys;
+  const double *mcoef;  // [rows][5]
   double *part;
   int64_t e_stride;
-  int32_t cls_nsys[NB_MAX_CLASSES], cls_sys_off[NB_MAX_CLASSES], cls_npos[NB_MAX_CLASSES];
+  int32_t cls_nsys[NB_MAX_CLASSES], cls_row0[NB_MAX_CLASSES], cls_npos[NB_MAX_CLASSES];
 };
 
 __global__ void __launch_bounds__(256) moments_structured_kernel(MomentsArgs a) {
   extern __shared__ double smc[];  // [nsys][5]
   const int c = blockIdx.y;
   const int nsys = a.cls_nsys[c];
-  const int32_t *sysl = a.cls_sys + a.cls_sys_off[c];
-  for (int k = threadIdx.x; k < nsys * 5; k += blockDim.x) smc[k] = a.mcoef[(size_t)sysl[k / 5] * 5 + (k % 5)];
+  const int64_t row0 = a.cls_row0[c];
+  for (int k = threadIdx.x; k < nsys * 5; k += blockDim.x) smc[k] = a.mcoef[(size_t)row0 * 5 + k];
   __syncthreads();
   const int64_t pos = 2 * ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
   if (pos >= a.cls_npos[c]) return;
   double2 m0 = {0, 0}, m1 = {0, 0}, m2 = {0, 0}, m3 = {0, 0}, m4 = {0, 0};
-  const double *base = a.e + pos;
+  const double *base = a.e + row0 * a.e_stride + pos;
   int k = 0;
   for (; k + 4 <= nsys; k += 4) {
     double2 v[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) v[j] = __ldcs(reinterpret_cast<const double2 *>(base + (int64_t)sysl[k + j] * a.e_stride));
+    for (int j = 0; j < 4; ++j) v[j] = __ldcs(reinterpret_cast<const double2 *>(base + (int64_t)(k + j) * a.e_stride));
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       const double *cf = smc + (k + j) * 5;
@@ -136,7 +135,7 @@ __global__ void __launch_bounds__(256) moments_structured_kernel(MomentsArgs a) 
     }
   }
   for (; k < nsys; ++k) {
-    const double2 v = __ldcs(reinterpret_cast<const double2 *>(base + (int64_t)sysl[k] * a.e_stride));
+    const double2 v = __ldcs(reinterpret_cast<const double2 *>(base + (int64_t)k * a.e_stride));
     const double *cf = smc + k * 5;
     m0.x += cf[0] * v.x; m0.y += cf[0] * v.y;
     m1.x += cf[1] * v.x; m1.y += cf[1] * v.y;
@@ -159,13 +158,12 @@ int nb_launch_moments(nanobte_solver *h) {
   MomentsArgs a;
   a.e = h->sw.e;
   a.mcoef = h->mcoef;
-  a.cls_sys = h->cls_sys;
   a.part = h->part;
   a.e_stride = h->e_stride;
   int maxpos = 0, maxsys = 0;
   for (int c = 0; c < NB_MAX_CLASSES; ++c) {
     a.cls_nsys[c] = h->cls_nsys[c];
-    a.cls_sys_off[c] = h->cls_sys_off[c];
+    a.cls_row0[c] = h->cls_row0[c];
     a.cls_npos[c] = h->cls_npos[c];
     maxpos = max(maxpos, h->cls_npos[c]);
     maxsys = max(maxsys, h->cls_nsys[c]);
@@ -293,7 +291,7 @@ int nb_launch_scatter_cells(nanobte_solver *h, const double *src_act, double *ds
 
 struct GetEArgs {
   int32_t n_cells, n_act, B, b0, nb, d0, nd, unstructured;
-  const int32_t *cell2act, *a2pos, *dir_cls;
+  const int32_t *cell2act, *a2pos, *dir_cls, *dir_row0;
   const double *e, *C;
   int64_t e_stride;
   double off_scale;  // T_ref / W, or 0 for the deviational export
@@ -309,7 +307,7 @@ __global__ void get_e_kernel(GetEArgs g) {
   double val = 0.0;
   if (a >= 0) {
     const int64_t pos = g.a2pos[(size_t)g.dir_cls[d] * g.n_act + a];
-    val = g.unstructured ? g.e[((int64_t)d * g.e_stride + pos) * g.B + b] : g.e[((int64_t)d * g.B + b) * g.e_stride + pos];
+    val = g.unstructured ? g.e[((int64_t)d * g.e_stride + pos) * g.B + b] : g.e[((int64_t)g.dir_row0[d] + b) * g.e_stride + pos];
     val += g.C[b] * g.off_scale;
   }
   g.dst[((size_t)bi * g.nd + di) * g.n_cells + c] = val;
@@ -320,7 +318,7 @@ int nb_launch_get_e(nanobte_solver *h, int b0, int nb, int d0, int nd, double *d
   GetEArgs g;
   g.n_cells = h->n_cells; g.n_act = h->n_act; g.B = h->B; g.b0 = b0; g.nb = nb; g.d0 = d0; g.nd = nd;
   g.unstructured = h->kind;
-  g.cell2act = h->cell2act; g.a2pos = h->a2pos; g.dir_cls = h->dir_cls; g.e = h->bd.e; g.C = h->bd.C;
+  g.cell2act = h->cell2act; g.a2pos = h->a2pos; g.dir_cls = h->dir_cls; g.dir_row0 = h->bd.dir_row0; g.e = h->bd.e; g.C = h->bd.C;
   g.e_stride = h->e_stride; g.off_scale = deviational ? 0.0 : h->T_ref / h->W; g.dst = dst_dev;
   dim3 grid((h->n_cells + 255) / 256, nb * nd);
   get_e_kernel<<<grid, 256, 0, h->stream>>>(g);

@@ -22,15 +22,16 @@ struct Grid {
 struct OctHost {
   int sign[3];
   std::vector<int> dirs;
-  std::vector<uint32_t> pen;
-  std::vector<int32_t> plane_off;
+  std::vector<uint2> pen;
+  std::vector<int4> plane;
   std::vector<uint32_t> cellinfo;
   std::vector<double2> tq;
-  std::vector<double> rhu, rhv, rhw;
+  std::vector<double> rhu;
+  std::vector<double2> pen_rh;
   std::vector<int32_t> in_bf;      // inflow list: boundary face ids in consumption order
   std::vector<int32_t> bf_slot;    // [n_bf] index of the face in in_bf, or -1
   std::vector<int32_t> cell2pos;   // [n_cells]
-  int n_pen = 0, H = 0, n_pos = 0;
+  int n_pen = 0, H = 0, n_pos = 0, p_max = 0;
 };
 
 int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_bands *bands, const nanobte_quadrature *quad,
@@ -152,55 +153,63 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   const int va = pa == 0 ? 1 : 0, wa = pa == 2 ? 1 : 2;
   const int nu = g.n[pa], nv = g.n[va], nw = g.n[wa];
   const bool has_w = !(dim == 2);  // in 2-D the w axis is z (one layer, no faces)
-  const int pitch = nv + (nv & 1);
-  const int slots = pitch * nw;
-  if (slots > 65535 || nv + nw > 65000 || nu + nv + nw > 65000) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section too large for the 16-bit pencil encoding");
+  if ((int64_t)nv * nw >= 65535) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section too large for the 16-bit pencil encoding");
   const int H = nu + nv + nw - 2;
   bool uniform = true;
   for (int a = 0; a < dim; ++a)
     for (double v : g.hsz[a]) uniform &= (v == g.hsz[a][0]);
 
   // ---- per class: pencils, hyperplanes, cell info, inflow lists ----------------------------------------------------------
-  int n_pen_max = 0, n_pos_max = 0;
+  int n_pen_max = 0, n_pos_max = 0, p_max = 0;
   for (int ci = 0; ci < ncls; ++ci) {
     OctHost &o = oct[ci];
     auto phys = [&](int axis, int x) { return o.sign[axis] > 0 ? x : g.n[axis] - 1 - x; };
     auto cell_of = [&](int u, int v, int w) { int c[3]; c[pa] = phys(pa, u); c[va] = phys(va, v); c[wa] = phys(wa, w); return g.cell(c[0], c[1], c[2]); };
-    std::vector<int> pen_v, pen_w, first_of_m(nv + nw, 0);
+    std::vector<int> pen_v, pen_w, first_of_m(nv + nw, 0), pen_of((size_t)nv * nw, -1);
     for (int mm = 0; mm <= nv + nw - 2; ++mm) {
       first_of_m[mm] = (int)pen_v.size();
       for (int w = std::max(0, mm - nv + 1); w <= std::min(nw - 1, mm); ++w) {
         const int v = mm - w;
         bool any = false;
         for (int u = 0; u < nu && !any; ++u) any = g.act[cell_of(u, v, w)];
-        if (any) { pen_v.push_back(v); pen_w.push_back(w); }
+        if (any) { pen_of[(size_t)v + (size_t)nv * w] = (int)pen_v.size(); pen_v.push_back(v); pen_w.push_back(w); }
       }
     }
     first_of_m[nv + nw - 1] = (int)pen_v.size();
     o.n_pen = (int)pen_v.size();
     o.pen.resize(o.n_pen);
-    for (int p = 0; p < o.n_pen; ++p) o.pen[p] = (uint32_t)(pen_v[p] + pen_w[p] * pitch) | ((uint32_t)(pen_v[p] + pen_w[p]) << 16);
+    o.pen_rh.resize(o.n_pen);
+    for (int p = 0; p < o.n_pen; ++p) {
+      const int v = pen_v[p], w = pen_w[p];
+      int nbv = v > 0 ? pen_of[(size_t)(v - 1) + (size_t)nv * w] : -1, nbw = w > 0 ? pen_of[(size_t)v + (size_t)nv * (w - 1)] : -1;
+      if (nbv < 0) nbv = o.n_pen;  // the zero slot: such a cell always carries the boundary flag of that face
+      if (nbw < 0) nbw = o.n_pen;
+      o.pen[p] = make_uint2((uint32_t)(v + w), (uint32_t)nbv | ((uint32_t)nbw << 16));
+      o.pen_rh[p] = make_double2(1.0 / g.hsz[va][phys(va, v)], has_w ? 1.0 / g.hsz[wa][phys(wa, w)] : 0.0);
+    }
     o.H = H;
-    o.plane_off.resize(H);
-    std::vector<int> lo(H), hi(H);
+    o.plane.resize(H);
+    std::vector<int> lo(H), hi(H), start(H);
     int base = 0;
     for (int hh = 0; hh < H; ++hh) {
       const int mlo = std::max(0, hh - nu + 1), mhi = std::min(hh, nv + nw - 2);
       lo[hh] = first_of_m[mlo];
       hi[hh] = mhi >= mlo ? first_of_m[mhi + 1] : lo[hh];
-      o.plane_off[hh] = base - lo[hh];
-      base += hi[hh] - lo[hh];
+      start[hh] = (base + 15) / 16 * 16;  // 128-byte aligned e segments, 16-byte aligned table segments (bulk TMA)
+      base = start[hh] + (hi[hh] - lo[hh]);
+      o.plane[hh] = make_int4(lo[hh], hi[hh] - lo[hh], start[hh], 0);
+      o.p_max = std::max(o.p_max, hi[hh] - lo[hh]);
     }
     o.n_pos = base;
-    o.cellinfo.assign((size_t)o.n_pos + 2, 8u);
-    o.tq.assign((size_t)o.n_pos + 2, make_double2(0.0, 0.0));
+    o.cellinfo.assign((size_t)o.n_pos + 16, 8u);
+    o.tq.assign((size_t)o.n_pos + 16, make_double2(0.0, 0.0));
     o.cell2pos.assign(nc, -1);
     o.bf_slot.assign(nbf, -1);
     const int axes[3] = {pa, va, wa};
     for (int hh = 0; hh < H; ++hh)
       for (int p = lo[hh]; p < hi[hh]; ++p) {
         const int u = hh - (pen_v[p] + pen_w[p]);
-        const int pos = o.plane_off[hh] + p;
+        const int pos = start[hh] + (p - lo[hh]);
         const int c = cell_of(u, pen_v[p], pen_w[p]);
         if (!g.act[c]) continue;  // hole
         o.cell2pos[c] = pos;
@@ -225,12 +234,11 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
         const double th0 = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
         o.tq[pos] = make_double2(th0, Qdot ? Qdot[c] : 0.0);
       }
-    // reciprocal spacings in primed coordinates
-    o.rhu.resize(nu); o.rhv.resize(nv); o.rhw.resize(nw);
+    // reciprocal spacings along the sweep axis, in primed coordinates
+    o.rhu.resize(nu);
     for (int u = 0; u < nu; ++u) o.rhu[u] = 1.0 / g.hsz[pa][phys(pa, u)];
-    for (int v = 0; v < nv; ++v) o.rhv[v] = 1.0 / g.hsz[va][phys(va, v)];
-    for (int w = 0; w < nw; ++w) o.rhw[w] = has_w ? 1.0 / g.hsz[wa][phys(wa, w)] : 0.0;
     n_pen_max = std::max(n_pen_max, o.n_pen);
+    p_max = std::max(p_max, o.p_max);
     n_pos_max = std::max(n_pos_max, o.n_pos);
   }
   const int64_t e_stride = ((int64_t)n_pos_max + 31) / 32 * 32;
@@ -269,23 +277,32 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     }
     G.bf_den[f] = den;
   }
-  // inflow rows: direction d owns [B][n_in(class(d))]
-  G.dir_bin.resize(D); G.dir_nin.resize(D);
+  // e rows and inflow rows are class-contiguous: class c owns rows [row0[c], row0[c] + |dirs(c)|*B) in the order
+  // (direction within the class, band); its inflow rows [n_in(c)] follow the same order from bin_base[c].
+  G.dir_bin.resize(D); G.dir_nin.resize(D); G.dir_row0.resize(D);
+  std::vector<int32_t> cls_row0(ncls);
+  std::vector<int64_t> cls_bin(ncls);
   int64_t tot = 0;
-  for (int d = 0; d < D; ++d) {
-    G.dir_bin[d] = tot;
-    G.dir_nin[d] = (int32_t)oct[dir_cls[d]].in_bf.size();
-    tot += (int64_t)B * G.dir_nin[d];
+  int row = 0;
+  for (int ci = 0; ci < ncls; ++ci) {
+    cls_row0[ci] = row;
+    cls_bin[ci] = tot;
+    for (int d : oct[ci].dirs) {
+      G.dir_bin[d] = tot;
+      G.dir_nin[d] = (int32_t)oct[ci].in_bf.size();
+      G.dir_row0[d] = row;
+      tot += (int64_t)B * G.dir_nin[d];
+      row += B;
+    }
   }
   G.bin_total = tot;
 
-  // ---- per-system coefficient tables -----------------------------------------------------------------------------------------
+  // ---- per-row coefficient tables ----------------------------------------------------------------------------------------------
   std::vector<double> coef((size_t)D * B * 8, 0.0);
-  std::vector<int64_t> sys_bin((size_t)D * B);
   G.mcoef.resize((size_t)D * B * 5);
   for (int d = 0; d < D; ++d)
     for (int b = 0; b < B; ++b) {
-      const size_t sys = (size_t)d * B + b;
+      const size_t sys = (size_t)G.dir_row0[d] + b;
       const double A = cm.C[b] / (cm.W * cm.tau[b]), S = cm.share[b] / cm.W, it = 1.0 / cm.tau[b];
       const double su = std::fabs(cm.s[3 * d + pa]), sv = std::fabs(cm.s[3 * d + va]), sw = has_w ? std::fabs(cm.s[3 * d + wa]) : 0.0;
       double *cf = &coef[sys * 8];
@@ -296,7 +313,6 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       } else {
         cf[0] = A; cf[1] = S; cf[2] = it; cf[3] = cm.v[b] * su; cf[4] = cm.v[b] * sv; cf[5] = cm.v[b] * sw;
       }
-      sys_bin[sys] = G.dir_bin[d] + (int64_t)b * G.dir_nin[d];
       double *mc = &G.mcoef[sys * 5];
       mc[0] = cm.w[d] / cm.tau[b];
       mc[1] = cm.w[d];
@@ -349,29 +365,23 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   // ---- sweep launch shape, tasks ---------------------------------------------------------------------------------------------------
   int nsys_min = 1 << 30;
   for (auto &o : oct) nsys_min = std::min<int>(nsys_min, (int)o.dirs.size() * B);
-  rc = nb_sweep_structured_config(h, n_pen_max, slots, opt->sweep_G, opt->sweep_threads, opt->sweep_groups, nsys_min);
+  rc = nb_sweep_structured_config(h, n_pen_max, p_max, H, opt->sweep_G, opt->sweep_threads, nsys_min);
   if (rc) return rc;
-  const int per_task = h->sweep_G * h->sweep_groups;
-  std::vector<int32_t> task_oct, task_sys, cls_sys;
+  const int per_task = h->sweep_G;
+  std::vector<int32_t> task_oct, task_row;
   for (int ci = 0; ci < ncls; ++ci) {
-    h->cls_sys_off[ci] = (int)cls_sys.size();
-    for (int d : oct[ci].dirs)
-      for (int b = 0; b < B; ++b) cls_sys.push_back(d * B + b);
+    h->cls_row0[ci] = cls_row0[ci];
     h->cls_nsys[ci] = (int)oct[ci].dirs.size() * B;
     h->cls_npos[ci] = oct[ci].n_pos;
-    const int nt = (h->cls_nsys[ci] + per_task - 1) / per_task;
-    for (int t = 0; t < nt; ++t) {
+    for (int r0 = 0; r0 < h->cls_nsys[ci]; r0 += per_task) {
       task_oct.push_back(ci);
-      for (int k = 0; k < per_task; ++k) {
-        const int idx = t * per_task + k;
-        task_sys.push_back(idx < h->cls_nsys[ci] ? cls_sys[h->cls_sys_off[ci] + idx] : -1);
-      }
+      task_row.push_back(r0);
     }
   }
   h->n_tasks = (int)task_oct.size();
   h->n_cls = ncls; h->bd.n_cls = ncls;
   h->n_cells = nc; h->kind = 0; h->pencil_axis = pa; h->n_planes = H;
-  h->uniform = uniform; h->has_w = has_w;
+  h->uniform = uniform;
   h->n_pos = n_pos_max; h->e_stride = e_stride;
   h->T_ref = opt->T_ref;
   h->cg_rtol = opt->cg_rtol > 0 ? opt->cg_rtol : 1e-12;
@@ -392,20 +402,21 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       OctHost &o = oct[ci];
       OctTab &t = tabs[ci];
       t.pen = A.put(o.pen);
-      t.plane_off = A.put(o.plane_off);
+      t.plane = A.put(o.plane);
       t.cellinfo = A.put(o.cellinfo);
       double2 *tq = A.put(o.tq);
       t.tq = tq;
       h->tq[ci] = tq;
-      t.rhu = A.put(o.rhu); t.rhv = A.put(o.rhv); t.rhw = A.put(o.rhw);
+      t.rhu = A.put(o.rhu);
+      t.pen_rh = A.put(o.pen_rh);
+      t.bin_base = cls_bin[ci];
       t.n_pen = o.n_pen; t.H = o.H; t.n_pos = o.n_pos; t.n_in = (int)o.in_bf.size();
+      t.row0 = cls_row0[ci]; t.n_rows = h->cls_nsys[ci]; t.p_max = o.p_max;
     }
     h->d_octs = A.put(tabs);
     h->sw.task_oct = A.put(task_oct);
-    h->sw.task_sys = A.put(task_sys);
+    h->sw.task_row = A.put(task_row);
     h->sw.coef = A.put(coef);
-    h->sw.sys_bin = A.put(sys_bin);
-    h->cls_sys = A.put(cls_sys);
     h->a2pos = A.put(a2pos);
     h->dir_cls = A.put(dir_cls);
     const size_t part_n = std::max<size_t>((size_t)ncls * 5 * e_stride, (size_t)3 * nc + 64);
@@ -413,7 +424,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     double *e = A.zeros<double>((size_t)D * B * e_stride);
     h->sw.e = e; h->bd.e = e; h->bd.e_stride = e_stride;
     h->sw.bin = h->bd.bin;
-    h->sw.e_stride = e_stride; h->sw.nu = nu; h->sw.pitch = pitch; h->sw.slots = slots;
+    h->sw.e_stride = e_stride; h->sw.nu = nu;
     if (A.rc) return nb_fail(h, A.rc, "device upload failed");
     if (dry) {
       const size_t need = A.off + 256;

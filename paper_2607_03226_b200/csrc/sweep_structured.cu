@@ -6,209 +6,297 @@
 //
 // B200 design: the B*D systems are independent and each is a triangular solve whose
 // dependency is the hyperplane u'+v'+w' = h of the direction's octant.  Instead of one launch per hyperplane over
-// all systems (a chain of ~200 dependent launches with all upwind traffic through L2), ONE launch runs the whole
-// sweep: a CTA (or a thread group inside it) owns a few systems for the entire grid and walks the hyperplanes
-// itself.  The wavefront state -- one value per (v', w') pencil, i.e. the previous hyperplane -- lives in shared
-// memory, updated in place, so the three upwind reads never leave the SM and HBM sees exactly one coalesced
-// 8-byte store per update.  Threads own pencils (lines along the sweep axis u) sorted by v'+w', which makes the
-// set of active pencils of a hyperplane a contiguous thread range and the global store position
-// plane_off[h] + pencil index contiguous as well.
+// all systems (a chain of ~250 dependent launches with all upwind traffic through L2), ONE launch runs the whole
+// sweep: a CTA owns G systems of one octant for the entire grid and walks the hyperplanes itself.
+//   * The wavefront state -- one value per (v', w') pencil and system, i.e. the previous hyperplane -- lives in
+//     shared memory, so the v/w upwind reads never leave the SM; the u upwind value is the thread's own previous
+//     result and stays in a register.  HBM sees exactly one coalesced 8-byte streaming store per update.
+//   * Threads own pencils (lines along the sweep axis u) sorted by v'+w': the active pencils of a hyperplane are a
+//     contiguous thread range and the global store position start[h] + (p - lo[h]) is contiguous as well.
+//   * The per-cell tables of hyperplane h+1 (boundary flags / inflow index, theta, Qdot) are fetched by 1-D bulk TMA
+//     (cp.async.bulk + mbarrier complete_tx) into a two-stage shared-memory ring while hyperplane h is computed, so
+//     no global-memory round trip sits on the per-plane critical path except the (rare) boundary inflow values.
 #include <algorithm>
 
 #include "internal.h"
 
-__device__ __forceinline__ void group_barrier(int id, int count) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
+namespace {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// 1-D bulk TMA global -> shared, completion on an mbarrier (bytes: multiple of 16, both addresses 16-byte aligned)
+__device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
 }
 
-template <int GT, int RMAX, bool UNIFORM, bool HAS_W>
-__global__ void __launch_bounds__((GT * RMAX >= 8) ? 512 : 1024)
-    sweep_structured_kernel(const SweepArgs a, const OctTab *__restrict__ octs, const int tpg, const int ng) {
-  extern __shared__ double smem[];
-  const int grp = threadIdx.x / tpg, t = threadIdx.x - grp * tpg;
+// Shared-memory carve-up (all offsets multiples of 16 bytes).
+struct SmemLayout {
+  uint32_t tq, state, info, plane, bar, total;
+};
+__host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int H) {
+  SmemLayout L;
+  L.tq = 0;                                                  // [2][pcap] double2
+  L.state = L.tq + 2u * (uint32_t)pcap * 16u;                // [G][sp]   double
+  L.info = L.state + (uint32_t)G * (uint32_t)sp * 8u;        // [2][pcap] uint32
+  L.plane = L.info + 2u * (uint32_t)pcap * 4u;               // [H]       int4
+  L.bar = L.plane + (uint32_t)H * 16u;                       // [2]       mbarrier
+  L.total = L.bar + 16u;
+  return L;
+}
+
+template <int G, int R, bool UNIFORM>
+__global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a, const OctTab *__restrict__ octs) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int t = threadIdx.x, nt = blockDim.x;
   const int task = blockIdx.x;
   const OctTab T = octs[a.task_oct[task]];
-  const int nu = a.nu, pitch = a.pitch, slots = a.slots;
-  double *buf = smem + (size_t)grp * GT * slots;
+  const int nu = a.nu, sp = a.sp, pcap = a.pcap;
+  const SmemLayout L = smem_layout(G, sp, pcap, T.H);
+  double2 *tq_s = reinterpret_cast<double2 *>(smem + L.tq);
+  double *st = reinterpret_cast<double *>(smem + L.state);
+  uint32_t *info_s = reinterpret_cast<uint32_t *>(smem + L.info);
+  int4 *plane_s = reinterpret_cast<int4 *>(smem + L.plane);
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + L.bar);
 
-  int sys[GT];
-  bool live = false;
+  const int row_loc = a.task_row[task];
+  const int n_valid = min(G, T.n_rows - row_loc);  // rows past the class's end recompute the last row and store nothing
+  const int64_t row_g0 = (int64_t)T.row0 + row_loc;
+  double cf[G][UNIFORM ? 5 : 6];
 #pragma unroll
-  for (int g = 0; g < GT; ++g) {
-    sys[g] = a.task_sys[((size_t)task * ng + grp) * GT + g];
-    live |= sys[g] >= 0;
+  for (int g = 0; g < G; ++g) {
+    const int64_t row = row_g0 + min(g, n_valid - 1);
+#pragma unroll
+    for (int k = 0; k < (UNIFORM ? 5 : 6); ++k) cf[g][k] = a.coef[row * 8 + k];
   }
-  if (!live) return;  // padding group of the last task: uses its own named barrier, nobody waits for it
-  const double *binrow[GT];
-  double *erow[GT];
-  double cf[GT][UNIFORM ? 5 : 6];
-#pragma unroll
-  for (int g = 0; g < GT; ++g) {
-    const int s = sys[g] >= 0 ? sys[g] : sys[0];  // padded entries recompute system 0 and store nothing
-    binrow[g] = a.bin + a.sys_bin[s];
-    erow[g] = a.e + (int64_t)s * a.e_stride;
-#pragma unroll
-    for (int k = 0; k < (UNIFORM ? 5 : 6); ++k) cf[g][k] = a.coef[(size_t)s * 8 + k];
-  }
+  double *const e0 = a.e + row_g0 * a.e_stride;
+  const double *const bin0 = a.bin + T.bin_base + (int64_t)row_loc * T.n_in;
+  const int64_t e_stride = a.e_stride;
+  const int n_in = T.n_in;
 
-  uint32_t pk[RMAX];
-  double rv[UNIFORM ? 1 : RMAX], rw[UNIFORM ? 1 : RMAX];
+  // per-thread pencils
+  int pm[R];
+  uint32_t pnb[R];
+  double rv[UNIFORM ? 1 : R], rw[UNIFORM ? 1 : R];
 #pragma unroll
-  for (int r = 0; r < RMAX; ++r) {
-    const int p = t + r * tpg;
-    pk[r] = p < T.n_pen ? T.pen[p] : 0xffffffffu;  // m = 65535: never in range
-    if (!UNIFORM) {
-      const int slot = pk[r] & 0xffff;
-      rv[r] = p < T.n_pen ? T.rhv[slot % pitch] : 0.0;
-      rw[r] = (p < T.n_pen && HAS_W) ? T.rhw[slot / pitch] : 0.0;
+  for (int r = 0; r < R; ++r) {
+    const int p = t + r * nt;
+    if (p < T.n_pen) {
+      const uint2 q = T.pen[p];
+      pm[r] = (int)q.x;
+      pnb[r] = q.y;
+      if (!UNIFORM) {
+        const double2 rh = T.pen_rh[p];
+        rv[r] = rh.x;
+        rw[r] = rh.y;
+      }
+    } else {
+      pm[r] = 0x3fffffff;  // never active
+      pnb[r] = 0;
+      if (!UNIFORM) rv[r] = rw[r] = 0.0;
     }
   }
+  for (int k = t; k < T.H; k += nt) plane_s[k] = T.plane[k];
+  for (int k = t; k < G; k += nt) st[(size_t)k * sp + T.n_pen] = 0.0;  // the "no upwind pencil" slot
+  if (t == 0) {
+    mbar_init(bar, 1);
+    mbar_init(bar + 1, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  auto issue = [&](int h) {  // thread 0: fetch the tables of hyperplane h into stage h & 1
+    const int4 P = plane_s[h];
+    const int s = h & 1;
+    const uint32_t c4 = ((uint32_t)P.y + 3u) & ~3u;
+    mbar_expect_tx(bar + s, c4 * 20u);
+    if (c4) {
+      tma_load_1d(tq_s + (size_t)s * pcap, T.tq + P.z, c4 * 16u, bar + s);
+      tma_load_1d(info_s + (size_t)s * pcap, T.cellinfo + P.z, c4 * 4u, bar + s);
+    }
+  };
+  if (t == 0) issue(0);
+
+  double res[R][G];
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+#pragma unroll
+    for (int g = 0; g < G; ++g) res[r][g] = 0.0;
 
   for (int h = 0; h < T.H; ++h) {
-    const int poff = __ldg(T.plane_off + h);
-    double res[RMAX][GT];
+    const int s = h & 1;
+    mbar_wait(bar + s, (h >> 1) & 1);
+    if (t == 0 && h + 1 < T.H) issue(h + 1);  // stage s^1 was last read before the closing barrier of step h-1
+    const int4 P = plane_s[h];
+    const double2 *tqh = tq_s + (size_t)s * pcap - P.x;
+    const uint32_t *infoh = info_s + (size_t)s * pcap - P.x;
     unsigned act = 0;
 #pragma unroll
-    for (int r = 0; r < RMAX; ++r) {
-      const int u = h - (int)(pk[r] >> 16);
+    for (int r = 0; r < R; ++r) {
+      const int u = h - pm[r];
       if ((unsigned)u < (unsigned)nu) {
-        const int64_t pos = poff + t + r * tpg;
-        const uint32_t info = __ldg(T.cellinfo + pos);
+        const int p = t + r * nt;
+        const uint32_t info = infoh[p];
         if (!(info & 8u)) {
           act |= 1u << r;
-          const double2 tq = __ldg(T.tq + pos);
-          const int slot = pk[r] & 0xffff;
-          const int sv = (info & 2u) ? slot : slot - 1;
-          const int sw = (!HAS_W || (info & 4u)) ? slot : slot - pitch;
-          double au = 0, av = 0, aw = 0;
-          if (!UNIFORM) au = T.rhu[u];
+          const double2 tq = tqh[p];
+          const uint32_t nbv = pnb[r] & 0xffffu, nbw = pnb[r] >> 16;
+          double eu[G], ev[G], ew[G];
 #pragma unroll
-          for (int g = 0; g < GT; ++g) {
-            const double *b = buf + g * slots;
-            double eu = b[slot], ev = b[sv], ew = HAS_W ? b[sw] : 0.0;
-            if (info & 7u) {
-              int idx = info >> 4;
-              if (info & 1u) eu = __ldg(binrow[g] + idx++);
-              if (info & 2u) ev = __ldg(binrow[g] + idx++);
-              if (HAS_W && (info & 4u)) ew = __ldg(binrow[g] + idx);
+          for (int g = 0; g < G; ++g) {
+            eu[g] = res[r][g];
+            ev[g] = st[g * sp + nbv];
+            ew[g] = st[g * sp + nbw];
+          }
+          if (info & 7u) {
+            const double *b = bin0 + (info >> 4);
+            const int iv = (info & 1u), iw = iv + ((info >> 1) & 1u);
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+              const double *bg = b + (int64_t)min(g, n_valid - 1) * n_in;
+              if (info & 1u) eu[g] = __ldg(bg);
+              if (info & 2u) ev[g] = __ldg(bg + iv);
+              if (info & 4u) ew[g] = __ldg(bg + iw);
             }
-            double val;
-            if (UNIFORM) {
-              val = cf[g][0] * tq.x + cf[g][1] * tq.y + cf[g][2] * eu + cf[g][3] * ev;
-              if (HAS_W) val += cf[g][4] * ew;
-            } else {
-              const double gu = cf[g][3] * au, gv = cf[g][4] * rv[r], gw = HAS_W ? cf[g][5] * rw[r] : 0.0;
-              const double num = cf[g][0] * tq.x + cf[g][1] * tq.y + gu * eu + gv * ev + gw * ew;
-              val = num / (cf[g][2] + gu + gv + gw);
+          }
+          if (UNIFORM) {
+#pragma unroll
+            for (int g = 0; g < G; ++g)
+              res[r][g] = cf[g][0] * tq.x + cf[g][1] * tq.y + cf[g][2] * eu[g] + cf[g][3] * ev[g] + cf[g][4] * ew[g];
+          } else {
+            const double au = __ldg(T.rhu + u);
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+              const double gu = cf[g][3] * au, gv = cf[g][4] * rv[r], gw = cf[g][5] * rw[r];
+              const double num = cf[g][0] * tq.x + cf[g][1] * tq.y + gu * eu[g] + gv * ev[g] + gw * ew[g];
+              res[r][g] = num / (cf[g][2] + gu + gv + gw);
             }
-            res[r][g] = val;
           }
         }
       }
     }
-    group_barrier(grp + 1, tpg);  // every read of hyperplane h-1 is done
+    __syncthreads();  // every read of hyperplane h-1 (and of stage s) is done
+    const int64_t pbase = (int64_t)P.z - P.x;
 #pragma unroll
-    for (int r = 0; r < RMAX; ++r) {
+    for (int r = 0; r < R; ++r) {
       if (act & (1u << r)) {
-        const int64_t pos = poff + t + r * tpg;
-        const int slot = pk[r] & 0xffff;
+        const int p = t + r * nt;
+        double *ep = e0 + pbase + p;
 #pragma unroll
-        for (int g = 0; g < GT; ++g) {
-          buf[g * slots + slot] = res[r][g];
-          if (sys[g] >= 0) __stcs(erow[g] + pos, res[r][g]);
+        for (int g = 0; g < G; ++g) {
+          st[g * sp + p] = res[r][g];
+          if (g < n_valid) __stcs(ep + g * e_stride, res[r][g]);
         }
       }
     }
-    group_barrier(grp + 1, tpg);  // hyperplane h is visible
+    __syncthreads();  // hyperplane h is visible
   }
 }
 
 // ---- host side: variant table ---------------------------------------------------------------------------------------
-typedef void (*sweep_fn)(const SweepArgs, const OctTab *, const int, const int);
+typedef void (*sweep_fn)(const SweepArgs, const OctTab *);
 
-template <int GT, int RMAX>
-static sweep_fn pick_uw(bool uniform, bool has_w) {
-  if (uniform) return has_w ? sweep_structured_kernel<GT, RMAX, true, true> : sweep_structured_kernel<GT, RMAX, true, false>;
-  return has_w ? sweep_structured_kernel<GT, RMAX, false, true> : sweep_structured_kernel<GT, RMAX, false, false>;
+template <int G>
+sweep_fn pick_r(int r, bool uniform) {
+#define NB_CASE(RR) \
+  case RR: return uniform ? sweep_structured_kernel<G, RR, true> : sweep_structured_kernel<G, RR, false>;
+  switch (r) {
+    NB_CASE(1)
+    NB_CASE(2)
+    NB_CASE(3)
+    NB_CASE(4)
+    NB_CASE(5)
+    NB_CASE(6)
+    NB_CASE(8)
+  }
+#undef NB_CASE
+  return nullptr;
 }
-template <int GT>
-static sweep_fn pick_r(int rmax, bool uniform, bool has_w) {
-  switch (rmax) {
-    case 1: return pick_uw<GT, 1>(uniform, has_w);
-    case 2: return pick_uw<GT, 2>(uniform, has_w);
-    case 4: return pick_uw<GT, 4>(uniform, has_w);
-    case 8: return pick_uw<GT, 8>(uniform, has_w);
+sweep_fn pick(int g, int r, bool uniform) {
+  switch (g) {
+    case 1: return pick_r<1>(r, uniform);
+    case 2: return pick_r<2>(r, uniform);
+    case 4: return pick_r<4>(r, uniform);
   }
   return nullptr;
 }
-static sweep_fn pick(int gt, int rmax, bool uniform, bool has_w) {
-  switch (gt) {
-    case 1: return pick_r<1>(rmax, uniform, has_w);
-    case 2: return pick_r<2>(rmax, uniform, has_w);
-    case 4: return pick_r<4>(rmax, uniform, has_w);
-  }
-  return nullptr;
-}
-static int max_threads(int gt, int rmax) { return gt * rmax >= 8 ? 512 : 1024; }
+const int kR[7] = {1, 2, 3, 4, 5, 6, 8};
 
-// Chooses systems per thread (GT), pencils per thread (RMAX), threads per group and groups per CTA.
-// want_G / want_threads / want_groups: 0 = auto.
-int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int slots, int want_G, int want_threads, int want_groups,
+}  // namespace
+
+// Chooses systems per CTA (G), pencils per thread (R) and threads per CTA.  want_G / want_threads: 0 = auto.
+int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int H, int want_G, int want_threads,
                                int n_sys_min_class) {
   const size_t smem_cap = 227 * 1024;
-  int gt = want_G > 0 ? want_G : 2;
-  if (gt != 1 && gt != 2 && gt != 4) return nb_fail(h, NANOBTE_E_INVALID, "sweep_G must be 1, 2 or 4");
-  if (want_G <= 0 && n_sys_min_class < 2) gt = 1;
-  while (gt > 1 && (size_t)gt * slots * 8 > smem_cap) gt >>= 1;
-  if ((size_t)gt * slots * 8 > smem_cap)
-    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section of %d cells needs %zu B of shared memory per system (> %zu)",
-                   slots, (size_t)slots * 8, smem_cap);
-  int rmax = 0, tpg = 0;
+  if (want_G != 0 && want_G != 1 && want_G != 2 && want_G != 4) return nb_fail(h, NANOBTE_E_INVALID, "sweep_G must be 0, 1, 2 or 4");
+  if (n_pen_max > 8 * 512 || n_pen_max >= 65535)
+    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section has %d pencils; the sweep kernel supports up to %d", n_pen_max, 8 * 512);
+  int R = 0, T = 0;
   if (want_threads > 0) {
-    tpg = (want_threads + 31) / 32 * 32;
-    int r = (n_pen_max + tpg - 1) / tpg;
-    rmax = r <= 1 ? 1 : r <= 2 ? 2 : r <= 4 ? 4 : r <= 8 ? 8 : 0;
-    if (!rmax || tpg > max_threads(gt, rmax))
-      return nb_fail(h, NANOBTE_E_INVALID, "sweep_threads=%d cannot cover %d pencils", want_threads, n_pen_max);
+    T = std::min(512, (want_threads + 31) / 32 * 32);
+    for (int k = 0; k < 7 && !R; ++k)
+      if ((long)kR[k] * T >= n_pen_max) R = kR[k];
+    if (!R) return nb_fail(h, NANOBTE_E_INVALID, "sweep_threads=%d cannot cover %d pencils", want_threads, n_pen_max);
   } else {
-    const int pref[4] = {1, 2, 4, 8};
-    for (int k = 0; k < 4 && !rmax; ++k) {
-      int r = pref[k];
-      int tt = ((n_pen_max + r - 1) / r + 31) / 32 * 32;
-      // prefer at least ~4 pencils per thread on big cross-sections (fewer, fatter threads), 1 on small ones
-      if (tt <= max_threads(gt, r) && (tt <= 256 || r >= 4 || k == 3)) { rmax = r; tpg = tt; }
+    for (int k = 0; k < 7 && !R; ++k) {
+      const int tt = ((n_pen_max + kR[k] - 1) / kR[k] + 31) / 32 * 32;
+      if (tt <= 512) { R = kR[k]; T = tt; }
     }
-    if (!rmax) {
-      for (int k = 0; k < 4 && !rmax; ++k) {
-        int r = pref[k];
-        int tt = ((n_pen_max + r - 1) / r + 31) / 32 * 32;
-        if (tt <= max_threads(gt, r)) { rmax = r; tpg = tt; }
-      }
-    }
-    if (!rmax)
-      return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section has %d pencils; the sweep kernel supports up to %d", n_pen_max,
-                     8 * 512);
   }
-  int ng = want_groups > 0 ? want_groups : 1;
-  ng = std::min(ng, 15);
-  while (ng > 1 && (ng * tpg > max_threads(gt, rmax) || (size_t)ng * gt * slots * 8 > smem_cap)) --ng;
-  h->sweep_G = gt;
-  h->sweep_rmax = rmax;
-  h->sweep_threads = tpg;
-  h->sweep_groups = ng;
-  h->sweep_smem = (size_t)ng * gt * slots * 8;
+  const int sp = (n_pen_max + 1 + 1) & ~1;
+  const int pcap = (p_max + 3 + 4) & ~3;
+  int G = 0;
+  const int cand[3] = {4, 2, 1};
+  for (int k = 0; k < 3 && !G; ++k) {
+    const int g = cand[k];
+    if (want_G > 0 && g != want_G) continue;
+    if (smem_layout(g, sp, pcap, H).total > smem_cap) continue;
+    if (want_G <= 0 && (g * R > 20 || g > std::max(1, n_sys_min_class))) continue;  // registers: 2*G*R for the results
+    G = g;
+  }
+  if (!G) {
+    if (want_G > 0) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "sweep_G=%d needs %u B of shared memory (> %zu)", want_G,
+                                   smem_layout(want_G, sp, pcap, H).total, smem_cap);
+    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section of %d pencils needs %u B of shared memory (> %zu)", n_pen_max,
+                   smem_layout(1, sp, pcap, H).total, smem_cap);
+  }
+  h->sweep_G = G;
+  h->sweep_rmax = R;
+  h->sweep_threads = T;
+  h->sweep_smem = smem_layout(G, sp, pcap, H).total;
+  h->sw.sp = sp;
+  h->sw.pcap = pcap;
   return 0;
 }
 
 int nb_launch_sweep_structured(nanobte_solver *h) {
-  sweep_fn fn = pick(h->sweep_G, h->sweep_rmax, h->uniform, h->has_w);
+  sweep_fn fn = pick(h->sweep_G, h->sweep_rmax, h->uniform);
   if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "no sweep kernel variant for G=%d R=%d", h->sweep_G, h->sweep_rmax);
   if (!h->sweep_attr_set) {
     NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(h->sweep_smem, 1024)));
     h->sweep_attr_set = true;
   }
-  fn<<<h->n_tasks, h->sweep_groups * h->sweep_threads, h->sweep_smem, h->stream>>>(h->sw, h->d_octs, h->sweep_threads,
-                                                                                   h->sweep_groups);
+  fn<<<h->n_tasks, h->sweep_threads, h->sweep_smem, h->stream>>>(h->sw, h->d_octs);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
   return 0;

@@ -91,7 +91,7 @@ def test_no_cpu_fallback(lib):
         binding.Solver(wl.config_gray_square(n=4))
     # straight through the C ABI: create must refuse with NANOBTE_E_ARCH
     ms = binding._Marshalled(wl.config_gray_square(n=4))
-    opt = binding.Options(300.0, None, None, None, 0, 0.0, 0, 0, 0, 0)
+    opt = binding.Options(300.0, None, None, None, 0, 0.0, 0, 0, 0)
     h = C.c_void_p()
     rc = lib.nanobte_create_structured(C.byref(ms.mesh), C.byref(ms.bands), C.byref(ms.quad), ms.tags, ms.n_tags, None,
                                        C.byref(opt), C.byref(h))

@@ -107,7 +107,7 @@ def test_config0_gray_square_full():
 
 
 @pytest.mark.parametrize("kw", [{}, {"sweep_G": 1}, {"sweep_G": 2, "sweep_threads": 64}, {"sweep_G": 4},
-                                {"sweep_G": 1, "sweep_groups": 4}])
+                                {"sweep_G": 1, "sweep_threads": 32}])
 def test_config1_nongray_square_full(kw):
     pr = wl.config_nongray_square()
     step_parity(pr, 2, **kw)
@@ -123,7 +123,7 @@ def test_config1_solve():
 
 # ---- cuts of configs[2] (cube) and configs[3] (finfet): several tiles and ragged tails ---------------------------------------
 @pytest.mark.parametrize("n,kw", [(12, {}), (20, {"sweep_G": 1}), (20, {"sweep_G": 2}), (20, {"sweep_G": 4, "sweep_threads": 128}),
-                                  (33, {"sweep_G": 2, "sweep_threads": 160}), (24, {"sweep_G": 1, "sweep_groups": 3})])
+                                  (33, {"sweep_G": 2, "sweep_threads": 160}), (24, {"sweep_G": 1, "sweep_threads": 96})])
 def test_cube_cut_steps(n, kw):
     pr = wl.config_cube(n=n, B=3, n_polar=4, n_azim=8)
     step_parity(pr, 3, T_init=random_T(pr, 9), **kw)
