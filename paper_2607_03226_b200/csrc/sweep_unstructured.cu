@@ -1,20 +1,623 @@
-// sweep_unstructured.cu -- placeholder until the level-scheduled unstructured path lands.
+// sweep_unstructured.cu -- (a1)+(a2)+(a5)+(a6) for unstructured 2-D polygon meshes (BASELINE.json configs[4]):
+// one-time setup (geometry, per-direction level schedules, closure tables, diffusion stencil), the level-scheduled
+// transport sweep, and the band x direction moment reduction in the per-direction layout.
+//
+// What the sweep computes (Eq. 4, 91 Eq. 11, 104/110 transport system, 178 source split; R1 first-order upwind):
+//   eps_{b,i,c} = [ C_b th_c/(W tau_b) + share_b Qdot_c/W + v_b sum_{f: g<0} |g_cf,i| eps_up,f ] / [ 1/tau_b + v_b sum_{f: g>0} g_cf,i ]
+//   g_cf,i = A_cf (s_i . n_cf) / V_c                                                             (K_i)
+// with eps_up,f the neighbour's value (interior face) or the lagged closure value (boundary face, R9).
+//
+// B200 design: the upwind graph of every direction is levelled once on the host
+// (Kahn, R16: per DIRECTION -- the union graph of an octant is cyclic on the config-4 mesh); cells are stored in level
+// order, e is [direction][position][band] so that a cell's bands are one contiguous chunk.  ONE launch runs the
+// whole sweep: a CTA owns (direction, group of BG bands) and walks the levels itself with one CTA barrier per
+// level -- no dependent-launch chain (~1,500 levels), upwind chunks are re-read from L2 where the same CTA wrote
+// them one level earlier.  The per-(direction, position) geometry records are prefetched one pass ahead.
+#include <algorithm>
+#include <map>
+#include <numeric>
+
 #include "host_util.h"
 
-int nb_launch_sweep_unstructured(nanobte_solver *h) { return nb_fail(h, NANOBTE_E_UNSUPPORTED, "unstructured sweep not built yet"); }
-int nb_launch_moments_unstructured(nanobte_solver *h) { return nb_fail(h, NANOBTE_E_UNSUPPORTED, "unstructured moments not built yet"); }
-int nb_launch_update_unstructured(nanobte_solver *h, int) { return nb_fail(h, NANOBTE_E_UNSUPPORTED, "unstructured update not built yet"); }
-void nb_free_unstructured(nanobte_solver *) {}
+struct UnsArgs {
+  int32_t D, B, BG, NBG, MI, cpp;   // bands per CTA, band groups, max inflow faces per cell, cells per pass
+  int32_t n_act, l_max;
+  int64_t e_stride;                 // positions per direction (n_act rounded up)
+  const int32_t *n_lvl;             // [D]
+  const int32_t *lvl_ptr;           // [D][l_max+1] first position of each level
+  const int32_t *cell;              // [D][e_stride] active cell at a position
+  const int32_t *up;                // [MI][D][e_stride] position of the upwind cell, -1-k = inflow value k, INT_MIN = none
+  const double *gin;                // [MI][D][e_stride] |g| of the inflow face
+  const double *gout;               // [D][e_stride] sum of g over the outflow faces
+  const double *theta, *Qdot;       // [n_act]
+  const double *kA, *kS, *itau, *vb;  // [B] C_b/(W tau_b), share_b/W, 1/tau_b, v_b
+  const double *bin;
+  const int64_t *dir_bin;
+  const int32_t *dir_nin;
+  double *e;
+  // moments
+  const int32_t *a2pos;             // [D][n_act]
+  const double *w, *s;              // [D], [D][3]
+  double *theta_SI, *theta_en, *q;
+  double beta, Csum;
+};
 
-extern "C" int nanobte_workspace_bytes_unstructured(const nanobte_unstructured_mesh *, const nanobte_bands *,
-                                                    const nanobte_quadrature *, const nanobte_tag *, int32_t,
-                                                    const nanobte_options *, size_t *) {
-  return NANOBTE_E_UNSUPPORTED;
+namespace {
+
+constexpr int32_t kNone = INT32_MIN;
+
+// ---- (a5) the sweep -----------------------------------------------------------------------------------------------------
+template <int MI>
+__global__ void __launch_bounds__(1024) sweep_unstructured_kernel(const UnsArgs a) {
+  const int d = blockIdx.x / a.NBG, bg = blockIdx.x % a.NBG;
+  const int slot0 = threadIdx.x / a.BG, bl = threadIdx.x - slot0 * a.BG;
+  const int b = bg * a.BG + bl;
+  const bool live = b < a.B && slot0 < a.cpp;
+  const int bb = min(b, a.B - 1);
+  const double kA = a.kA[bb], kS = a.kS[bb], itau = a.itau[bb], vb = a.vb[bb];
+  const int64_t dbase = (int64_t)d * a.e_stride;
+  double *const ed = a.e + dbase * a.B + bb;             // + pos * B
+  const double *const bind = a.bin + a.dir_bin[d] + (int64_t)bb * a.dir_nin[d];
+  const int32_t *const cell = a.cell + dbase;
+  const double *const gout = a.gout + dbase;
+  const int32_t *const lp = a.lvl_ptr + (int64_t)d * (a.l_max + 1);
+  const int64_t kstride = (int64_t)a.D * a.e_stride;
+  const int n_lvl = a.n_lvl[d], cpp = a.cpp;
+
+  // record of the first position this thread will touch; afterwards always one pass ahead
+  int c_n = 0, up_n[MI];
+  double go_n = 0.0, gi_n[MI];
+  auto fetch = [&](int pos) {
+    c_n = __ldg(cell + pos);
+    go_n = __ldg(gout + pos);
+#pragma unroll
+    for (int k = 0; k < MI; ++k) {
+      up_n[k] = __ldg(a.up + k * kstride + dbase + pos);
+      gi_n[k] = __ldg(a.gin + k * kstride + dbase + pos);
+    }
+  };
+  int lo = lp[0], hi = n_lvl > 0 ? lp[1] : 0;
+  int pos = lo + slot0;
+  // the next position this thread handles, possibly in a later level
+  auto next_pos = [&](int p, int &l, int &l_lo, int &l_hi) {
+    p += cpp;
+    while (p >= l_hi && l + 1 < n_lvl) {
+      ++l;
+      l_lo = l_hi;
+      l_hi = lp[l + 1];
+      p = l_lo + slot0;
+    }
+    return p;
+  };
+  int l_f = 0, lo_f = lo, hi_f = hi;  // fetch cursor
+  int p_f = pos;
+  while (p_f >= hi_f && l_f + 1 < n_lvl) {
+    ++l_f;
+    lo_f = hi_f;
+    hi_f = lp[l_f + 1];
+    p_f = lo_f + slot0;
+  }
+  bool have = live && p_f < hi_f;
+  if (have) fetch(p_f);
+
+  for (int l = 0; l < n_lvl; ++l) {
+    lo = lp[l];
+    hi = lp[l + 1];
+    if (live) {
+      for (pos = lo + slot0; pos < hi; pos += cpp) {
+        // pos == p_f by construction: consume the prefetched record, start the next fetch
+        const int c = c_n;
+        const double go = go_n;
+        int up[MI];
+        double gi[MI];
+#pragma unroll
+        for (int k = 0; k < MI; ++k) {
+          up[k] = up_n[k];
+          gi[k] = gi_n[k];
+        }
+        p_f = next_pos(p_f, l_f, lo_f, hi_f);
+        if (p_f < hi_f) fetch(p_f);
+        double num = kA * a.theta[c] + kS * a.Qdot[c];
+        const double den = itau + vb * go;
+#pragma unroll
+        for (int k = 0; k < MI; ++k) {
+          if (up[k] != kNone) {
+            const double val = up[k] >= 0 ? ed[(int64_t)up[k] * a.B] : bind[-1 - up[k]];
+            num += vb * gi[k] * val;
+          }
+        }
+        ed[(int64_t)pos * a.B] = num / den;
+      }
+    }
+    __syncthreads();  // level l is visible to the whole CTA (it alone reads these rows)
+  }
 }
-extern "C" int nanobte_create_unstructured(const nanobte_unstructured_mesh *, const nanobte_bands *, const nanobte_quadrature *,
-                                           const nanobte_tag *, int32_t, const double *, const nanobte_options *, nanobte_solver **out) {
+
+// ---- (a6) moments in the per-direction layout: one warp per cell, lanes over bands, directions in order ---------------------
+__global__ void __launch_bounds__(256) moments_unstructured_kernel(const UnsArgs a) {
+  extern __shared__ double sm[];  // w[D], s[D][3]
+  for (int k = threadIdx.x; k < a.D; k += blockDim.x) sm[k] = a.w[k];
+  for (int k = threadIdx.x; k < 3 * a.D; k += blockDim.x) sm[a.D + k] = a.w[k / 3] * a.s[k];
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (c >= a.n_act) return;
+  double A1 = 0.0, A2 = 0.0, qx = 0.0, qy = 0.0, qz = 0.0;
+  for (int b0 = 0; b0 < a.B; b0 += 32) {
+    const int b = b0 + lane;
+    double E = 0.0, Fx = 0.0, Fy = 0.0, Fz = 0.0;
+    if (b < a.B) {
+      for (int d = 0; d < a.D; ++d) {
+        const int64_t pos = a.a2pos[(int64_t)d * a.n_act + c];
+        const double v = __ldcs(a.e + ((int64_t)d * a.e_stride + pos) * a.B + b);
+        E += sm[d] * v;
+        Fx += sm[a.D + 3 * d] * v;
+        Fy += sm[a.D + 3 * d + 1] * v;
+        Fz += sm[a.D + 3 * d + 2] * v;
+      }
+      const double it = a.itau[b], vb = a.vb[b];
+      A1 += E * it;  // Eq. 5 numerator
+      A2 += E;       // R13
+      qx += vb * Fx; // Eq. 7
+      qy += vb * Fy;
+      qz += vb * Fz;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    A1 += __shfl_xor_sync(0xffffffffu, A1, o);
+    A2 += __shfl_xor_sync(0xffffffffu, A2, o);
+    qx += __shfl_xor_sync(0xffffffffu, qx, o);
+    qy += __shfl_xor_sync(0xffffffffu, qy, o);
+    qz += __shfl_xor_sync(0xffffffffu, qz, o);
+  }
+  if (lane == 0) {
+    a.theta_SI[c] = A1 / a.beta;
+    a.theta_en[c] = A2 / a.Csum;
+    a.q[3 * (int64_t)c] = qx;
+    a.q[3 * (int64_t)c + 1] = qy;
+    a.q[3 * (int64_t)c + 2] = qz;
+  }
+}
+
+// ---- (a8) theta <- theta_SI (mode 0) or theta_SI + delta (mode 1), max |dT| -----------------------------------------------------
+__global__ void __launch_bounds__(256) update_unstructured_kernel(int n, int mode, const double *theta_SI, const double *x,
+                                                                  double *theta, double *theta_prev, unsigned long long *maxdT) {
+  __shared__ double red[8];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  double dlt = 0.0;
+  if (i < n) {
+    if (mode == 0) theta_prev[i] = theta[i];
+    const double th = mode == 0 ? theta_SI[i] : theta_SI[i] + x[i];
+    theta[i] = th;
+    dlt = fabs(th - theta_prev[i]);
+  }
+  auto nanmax = [](double p, double q) { return !(q <= p) ? q : p; };
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) dlt = nanmax(dlt, __shfl_xor_sync(0xffffffffu, dlt, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = dlt;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    dlt = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dlt = nanmax(dlt, __shfl_xor_sync(0xffffffffu, dlt, o));
+    if (threadIdx.x == 0) atomicMax(maxdT, (unsigned long long)__double_as_longlong(dlt));
+  }
+}
+
+typedef void (*uns_fn)(const UnsArgs);
+uns_fn pick_uns(int mi) {
+  switch (mi) {
+    case 1: return sweep_unstructured_kernel<1>;
+    case 2: return sweep_unstructured_kernel<2>;
+    case 3: return sweep_unstructured_kernel<3>;
+    case 4: return sweep_unstructured_kernel<4>;
+    case 5: return sweep_unstructured_kernel<5>;
+    case 6: return sweep_unstructured_kernel<6>;
+    case 7: return sweep_unstructured_kernel<7>;
+  }
+  return nullptr;
+}
+
+}  // namespace
+
+int nb_launch_sweep_unstructured(nanobte_solver *h) {
+  const UnsArgs &a = *h->uns;
+  uns_fn fn = pick_uns(a.MI);
+  if (!fn) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "cells with more than 7 inflow faces are not supported");
+  fn<<<a.D * a.NBG, h->sweep_threads, 0, h->stream>>>(a);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+int nb_launch_moments_unstructured(nanobte_solver *h) {
+  const UnsArgs &a = *h->uns;
+  const int wpb = 8;
+  moments_unstructured_kernel<<<(a.n_act + wpb - 1) / wpb, wpb * 32, (size_t)4 * a.D * sizeof(double), h->stream>>>(a);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+int nb_launch_update_unstructured(nanobte_solver *h, int mode) {
+  update_unstructured_kernel<<<(h->n_act + 255) / 256, 256, 0, h->stream>>>(h->n_act, mode, h->theta_SI, h->cg_x, h->theta,
+                                                                           h->theta_prev, h->d_maxdT);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+void nb_free_unstructured(nanobte_solver *h) {
+  delete h->uns;
+  h->uns = nullptr;
+}
+
+// =====================================================================================================================
+// (a1) host setup
+// =====================================================================================================================
+namespace {
+
+int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanobte_bands *bands, const nanobte_quadrature *quad,
+              const nanobte_tag *tags, int n_tags, const double *Qdot, const nanobte_options *opt, bool size_only,
+              size_t *bytes_out) {
+  if (!m || !opt) return nb_fail(h, NANOBTE_E_INVALID, "null argument");
+  const int nn = m->n_nodes, nc = m->n_cells;
+  if (nn < 3 || nc < 1 || !m->xy || !m->cell_ptr || !m->cell_nodes) return nb_fail(h, NANOBTE_E_INVALID, "bad mesh");
+  Common cm;
+  int rc = nb_validate_common(h, 2, bands, quad, tags, n_tags, cm);
+  if (rc) return rc;
+  const int B = cm.B, D = cm.D;
+  const int nf = m->cell_ptr[nc];
+  if (m->cell_ptr[0] != 0 || nf < 3 * nc) return nb_fail(h, NANOBTE_E_INVALID, "bad cell_ptr");
+
+  // ---- geometry: area, centroid, edge length / outward normal / centroid distance; edge matching ---------------------------
+  std::vector<double> vol(nc), cen(2 * (size_t)nc), flen(nf), fnx(nf), fny(nf), fdist(nf);
+  std::vector<int32_t> fnbr(nf, -1), fbf(nf, -1), fcell(nf);
+  std::map<std::pair<int, int>, int> open_edge;  // (lo, hi) -> face waiting for its partner
+  std::vector<char> matched(nf, 0);
+  for (int c = 0; c < nc; ++c) {
+    const int p0 = m->cell_ptr[c], np = m->cell_ptr[c + 1] - p0;
+    if (np < 3) return nb_fail(h, NANOBTE_E_INVALID, "cell %d has fewer than 3 nodes", c);
+    double a2 = 0, sx = 0, sy = 0;
+    for (int k = 0; k < np; ++k) {
+      const int n0 = m->cell_nodes[p0 + k], n1 = m->cell_nodes[p0 + (k + 1) % np];
+      if (n0 < 0 || n0 >= nn || n1 < 0 || n1 >= nn) return nb_fail(h, NANOBTE_E_INVALID, "cell %d: bad node id", c);
+      const double x0 = m->xy[2 * n0], y0 = m->xy[2 * n0 + 1], x1 = m->xy[2 * n1], y1 = m->xy[2 * n1 + 1];
+      const double cr = x0 * y1 - x1 * y0;
+      a2 += cr;
+      sx += (x0 + x1) * cr;
+      sy += (y0 + y1) * cr;
+    }
+    if (!(a2 > 0)) return nb_fail(h, NANOBTE_E_INVALID, "cell %d is not counter-clockwise (area %g)", c, 0.5 * a2);
+    vol[c] = 0.5 * a2;  // unit depth
+    cen[2 * c] = sx / (3.0 * a2);
+    cen[2 * c + 1] = sy / (3.0 * a2);
+    for (int k = 0; k < np; ++k) {
+      const int f = p0 + k, n0 = m->cell_nodes[p0 + k], n1 = m->cell_nodes[p0 + (k + 1) % np];
+      const double ex = m->xy[2 * n1] - m->xy[2 * n0], ey = m->xy[2 * n1 + 1] - m->xy[2 * n0 + 1];
+      const double len = std::sqrt(ex * ex + ey * ey);
+      if (!(len > 0)) return nb_fail(h, NANOBTE_E_INVALID, "cell %d has a zero-length edge", c);
+      flen[f] = len;
+      fnx[f] = ey / len;  // outward normal of a counter-clockwise polygon edge
+      fny[f] = -ex / len;
+      fcell[f] = c;
+      fdist[f] = (m->xy[2 * n0] - cen[2 * c]) * fnx[f] + (m->xy[2 * n0 + 1] - cen[2 * c + 1]) * fny[f];
+      const std::pair<int, int> key(std::min(n0, n1), std::max(n0, n1));
+      auto it = open_edge.find(key);
+      if (it == open_edge.end()) {
+        open_edge.emplace(key, f);
+      } else {
+        const int g = it->second;
+        if (matched[g]) return nb_fail(h, NANOBTE_E_INVALID, "edge (%d,%d) is shared by more than two cells", key.first, key.second);
+        matched[g] = matched[f] = 1;
+        fnbr[f] = fcell[g];
+        fnbr[g] = c;
+      }
+    }
+  }
+  for (int f = 0; f < nf; ++f)
+    if (fnbr[f] >= 0) {
+      const int c0 = fcell[f], c1 = fnbr[f];
+      const double dx = cen[2 * c1] - cen[2 * c0], dy = cen[2 * c1 + 1] - cen[2 * c0 + 1];
+      fdist[f] = std::sqrt(dx * dx + dy * dy);
+    }
+
+  // ---- boundary faces ------------------------------------------------------------------------------------------------------
+  const int nbf = m->n_bfaces;
+  if (nbf < 0 || (nbf > 0 && (!m->bf_nodes || !m->bf_tag))) return nb_fail(h, NANOBTE_E_INVALID, "bad boundary face arrays");
+  GenericTables G;
+  G.act2cell.resize(nc);
+  std::iota(G.act2cell.begin(), G.act2cell.end(), 0);
+  G.cell2act = G.act2cell;
+  G.bf_act.resize(nbf); G.bf_type.resize(nbf); G.bf_p.resize(nbf); G.bf_den.resize(nbf); G.bf_area.resize(nbf); G.bf_eps_w.resize(nbf);
+  std::vector<int32_t> bf_face(nbf);
+  h->h_bf_tag.assign(m->bf_tag, m->bf_tag + nbf);
+  for (int bf = 0; bf < nbf; ++bf) {
+    const int n0 = m->bf_nodes[2 * bf], n1 = m->bf_nodes[2 * bf + 1];
+    auto it = open_edge.find(std::make_pair(std::min(n0, n1), std::max(n0, n1)));
+    if (it == open_edge.end()) return nb_fail(h, NANOBTE_E_INVALID, "boundary face %d: no such edge", bf);
+    const int f = it->second;
+    if (matched[f]) return nb_fail(h, NANOBTE_E_INVALID, "boundary face %d is an interior edge", bf);
+    if (fbf[f] >= 0) return nb_fail(h, NANOBTE_E_INVALID, "boundary face %d listed twice", bf);
+    const int tg = m->bf_tag[bf];
+    if (tg < 0 || tg >= n_tags) return nb_fail(h, NANOBTE_E_INVALID, "boundary face %d: bad tag", bf);
+    const double p = m->bf_p ? m->bf_p[bf] : 0.0;
+    if (p < 0 || p > 1) return nb_fail(h, NANOBTE_E_INVALID, "boundary face %d: specularity outside [0,1]", bf);
+    fbf[f] = bf;
+    bf_face[bf] = f;
+    G.bf_act[bf] = fcell[f];
+    G.bf_type[bf] = cm.tag_type[tg];
+    G.bf_p[bf] = p;
+    G.bf_eps_w[bf] = cm.tag_T[tg] - opt->T_ref;
+    G.bf_area[bf] = flen[f];
+  }
+  for (int f = 0; f < nf; ++f)
+    if (fnbr[f] < 0 && fbf[f] < 0)
+      return nb_fail(h, NANOBTE_E_UNTAGGED, "cell %d has an exposed face without a boundary tag", fcell[f]);
+
+  // ---- per direction: levels (Kahn), positions, sweep records, inflow lists ----------------------------------------------------
+  const int64_t e_stride = ((int64_t)nc + 31) / 32 * 32;
+  std::vector<int32_t> a2pos((size_t)D * nc), n_lvl(D), cellat((size_t)D * e_stride, 0);
+  std::vector<std::vector<int32_t>> lvl_ptrs(D);
+  std::vector<double> gout((size_t)D * e_stride, 0.0);
+  G.bf_sn.assign((size_t)nbf * D, 0.0);
+  G.bf_mirror.assign((size_t)nbf * D, -1);
+  G.bf_inidx.assign((size_t)nbf * D, -1);
+  G.bf_opos.assign((size_t)nbf * D, -1);
+  G.dir_bin.resize(D); G.dir_nin.resize(D); G.dir_row0.resize(D);
+  int MI = 1, l_max = 0;
+  // pass 1: levels and positions
+  std::vector<int32_t> level(nc), indeg(nc), queue(nc);
+  std::vector<std::vector<double>> sn_all;  // s_d . n_f for every face, per direction, kept only transiently
+  for (int d = 0; d < D; ++d) {
+    const double sx = cm.s[3 * d], sy = cm.s[3 * d + 1];
+    for (int c = 0; c < nc; ++c) {
+      int in = 0, nin_faces = 0;
+      for (int f = m->cell_ptr[c]; f < m->cell_ptr[c + 1]; ++f) {
+        const double sn = sx * fnx[f] + sy * fny[f];
+        if (sn < 0) {
+          ++nin_faces;
+          if (fnbr[f] >= 0) ++in;
+        }
+      }
+      indeg[c] = in;
+      MI = std::max(MI, nin_faces);
+    }
+    int head = 0, tail = 0;
+    for (int c = 0; c < nc; ++c)
+      if (indeg[c] == 0) { level[c] = 0; queue[tail++] = c; }
+    int lmax_d = 0;
+    while (head < tail) {
+      const int c = queue[head++];
+      lmax_d = std::max(lmax_d, level[c]);
+      for (int f = m->cell_ptr[c]; f < m->cell_ptr[c + 1]; ++f) {
+        const int nb = fnbr[f];
+        if (nb >= 0 && sx * fnx[f] + sy * fny[f] > 0) {  // c is upwind of nb; nb's level is fixed by its LAST upwind cell
+          if (--indeg[nb] == 0) { level[nb] = level[c] + 1; queue[tail++] = nb; }
+        }
+      }
+    }
+    if (tail != nc) return nb_fail(h, NANOBTE_E_CYCLE, "upwind graph of direction %d is cyclic (%d of %d cells ordered)", d, tail, nc);
+    // Kahn's queue pops cells in non-decreasing level order, so level[c] above is the longest upwind path.
+    n_lvl[d] = lmax_d + 1;
+    l_max = std::max(l_max, n_lvl[d]);
+    std::vector<int32_t> &lp = lvl_ptrs[d];
+    lp.assign(n_lvl[d] + 1, 0);
+    for (int c = 0; c < nc; ++c) lp[level[c] + 1]++;
+    for (int l = 0; l < n_lvl[d]; ++l) lp[l + 1] += lp[l];
+    std::vector<int32_t> fill(lp.begin(), lp.end() - 1);
+    for (int c = 0; c < nc; ++c) {  // cells of a level in cell-id order
+      const int pos = fill[level[c]]++;
+      a2pos[(size_t)d * nc + c] = pos;
+      cellat[(size_t)d * e_stride + pos] = c;
+    }
+  }
+  if (MI > 7) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "a cell has %d inflow faces; at most 7 are supported", MI);
+  // pass 2: records
+  std::vector<int32_t> up((size_t)MI * D * e_stride, kNone);
+  std::vector<double> gin((size_t)MI * D * e_stride, 0.0);
+  int64_t bin_total = 0;
+  for (int d = 0; d < D; ++d) {
+    const double sx = cm.s[3 * d], sy = cm.s[3 * d + 1];
+    int nin = 0;
+    G.dir_bin[d] = bin_total;
+    G.dir_row0[d] = d * B;
+    for (int c = 0; c < nc; ++c) {
+      const int64_t at = (int64_t)d * e_stride + a2pos[(size_t)d * nc + c];
+      int k = 0;
+      double go = 0.0;
+      for (int f = m->cell_ptr[c]; f < m->cell_ptr[c + 1]; ++f) {
+        const double sn = sx * fnx[f] + sy * fny[f];
+        const double g = flen[f] * sn / vol[c];  // O1
+        if (g > 0) {
+          go += g;
+        } else if (g < 0) {
+          const int64_t r = (int64_t)k * D * e_stride + at;
+          gin[r] = -g;
+          if (fnbr[f] >= 0) {
+            up[r] = a2pos[(size_t)d * nc + fnbr[f]];
+          } else {
+            up[r] = -1 - nin;
+            G.bf_inidx[(size_t)fbf[f] * D + d] = nin++;
+          }
+          ++k;
+        }
+      }
+      gout[at] = go;
+    }
+    G.dir_nin[d] = nin;
+    bin_total += (int64_t)B * nin;
+  }
+  G.bin_total = bin_total;
+
+  // ---- closure tables -------------------------------------------------------------------------------------------------------
+  for (int bf = 0; bf < nbf; ++bf) {
+    const int f = bf_face[bf];
+    const double nrm[3] = {fnx[f], fny[f], 0.0};
+    const bool refl = G.bf_type[bf] == NANOBTE_SPECULAR || G.bf_type[bf] == NANOBTE_MIXED;
+    double den = 0.0;
+    for (int d = 0; d < D; ++d) {
+      const double sn = cm.s[3 * d] * nrm[0] + cm.s[3 * d + 1] * nrm[1] + cm.s[3 * d + 2] * nrm[2];
+      G.bf_sn[(size_t)bf * D + d] = sn;
+      if (sn < 0) {
+        den += cm.w[d] * (-sn);
+        if (refl) {
+          const int mj = nb_find_mirror(cm, d, nrm);
+          if (mj < 0) return nb_fail(h, NANOBTE_E_SPECULAR, "boundary face %d: mirror image of direction %d is not in the quadrature", bf, d);
+          G.bf_mirror[(size_t)bf * D + d] = mj;
+        }
+      } else if (sn > 0) {
+        G.bf_opos[(size_t)bf * D + d] = a2pos[(size_t)d * nc + fcell[f]];
+      }
+    }
+    G.bf_den[bf] = den;
+  }
+
+  // ---- cells: volumes, source, initial theta, diffusion stencil (two-point flux, R14e) ------------------------------------------
+  int maxf = 0;
+  for (int c = 0; c < nc; ++c) maxf = std::max(maxf, m->cell_ptr[c + 1] - m->cell_ptr[c]);
+  G.vol = vol;
+  G.Qdot_act.resize(nc); G.theta0.resize(nc);
+  G.cg_nf = maxf;
+  G.cg_nbr.assign((size_t)maxf * nc, 0);
+  G.cg_coef.assign((size_t)maxf * nc, 0.0);
+  G.cg_diag.assign(nc, 0.0);
+  G.cellbf_ptr.assign(nc + 1, 0);
+  for (int c = 0; c < nc; ++c) {
+    G.Qdot_act[c] = Qdot ? Qdot[c] : 0.0;
+    G.theta0[c] = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
+    for (int k = 0; k < maxf; ++k) G.cg_nbr[(size_t)k * nc + c] = c;
+    int k = 0;
+    for (int f = m->cell_ptr[c]; f < m->cell_ptr[c + 1]; ++f, ++k) {
+      if (fnbr[f] >= 0) {
+        const double cf = cm.kappa * flen[f] / fdist[f];
+        G.cg_nbr[(size_t)k * nc + c] = fnbr[f];
+        G.cg_coef[(size_t)k * nc + c] = cf;
+        G.cg_diag[c] += cf;
+      } else if (G.bf_type[fbf[f]] == NANOBTE_THERMALIZING) {
+        G.cg_diag[c] += cm.kappa * flen[f] / fdist[f];  // delta = 0 on the wall
+      } else {
+        G.cellbf.push_back(fbf[f]);
+      }
+    }
+    G.cellbf_ptr[c + 1] = (int32_t)G.cellbf.size();
+  }
+  G.tagface_ptr.assign(n_tags + 1, 0);
+  for (int bf = 0; bf < nbf; ++bf) G.tagface_ptr[m->bf_tag[bf] + 1]++;
+  for (int t = 0; t < n_tags; ++t) G.tagface_ptr[t + 1] += G.tagface_ptr[t];
+  G.tagface.resize(nbf);
+  {
+    std::vector<int> fill(G.tagface_ptr.begin(), G.tagface_ptr.end() - 1);
+    for (int bf = 0; bf < nbf; ++bf) G.tagface[fill[m->bf_tag[bf]]++] = bf;
+  }
+
+  // ---- launch shape: bands per CTA so that D * NBG CTAs fill the SMs a few times over ------------------------------------------
+  int BG = opt->sweep_G > 0 ? std::min(opt->sweep_G, B) : std::min(B, 8);
+  if (opt->sweep_G <= 0 && B % 8 != 0 && B <= 12) BG = B;
+  const int NBG = (B + BG - 1) / BG;
+  int threads = opt->sweep_threads > 0 ? std::min(1024, (opt->sweep_threads + 31) / 32 * 32) : 256;
+  threads = std::max(threads, (BG + 31) / 32 * 32);
+  const int cpp = threads / BG;
+
+  std::vector<int32_t> lvl_ptr((size_t)D * (l_max + 1), 0);
+  for (int d = 0; d < D; ++d) {
+    for (int l = 0; l <= l_max; ++l) lvl_ptr[(size_t)d * (l_max + 1) + l] = lvl_ptrs[d][std::min(l, n_lvl[d])];
+  }
+  std::vector<double> kA(B), kS(B), itau(B);
+  for (int b = 0; b < B; ++b) {
+    kA[b] = cm.C[b] / (cm.W * cm.tau[b]);
+    kS[b] = cm.share[b] / cm.W;
+    itau[b] = 1.0 / cm.tau[b];
+  }
+  std::vector<int32_t> dir_cls(D);
+  std::iota(dir_cls.begin(), dir_cls.end(), 0);
+
+  h->kind = 1; h->n_cells = nc; h->n_cls = D; h->n_planes = l_max; h->n_tasks = D * NBG;
+  h->sweep_G = BG; h->sweep_threads = threads; h->sweep_rmax = MI; h->pencil_axis = -1;
+  h->n_pos = nc; h->e_stride = e_stride; h->sweep_smem = 0;
+  h->T_ref = opt->T_ref;
+  h->cg_rtol = opt->cg_rtol > 0 ? opt->cg_rtol : 1e-12;
+  h->cg_max_iter = opt->cg_max_iter > 0 ? opt->cg_max_iter : 100000;
+  if (!h->uns) h->uns = new (std::nothrow) UnsArgs();
+  if (!h->uns) return nb_fail(h, NANOBTE_E_ALLOC, "host allocation failed");
+  UnsArgs &u = *h->uns;
+
+  for (int pass = 0; pass < 2; ++pass) {
+    const bool dry = pass == 0;
+    Arena A(h, dry);
+    rc = nb_upload_generic(h, A, cm, G);
+    if (rc) return nb_fail(h, rc, "device upload failed");
+    u.D = D; u.B = B; u.BG = BG; u.NBG = NBG; u.MI = MI; u.cpp = cpp; u.n_act = nc; u.l_max = l_max; u.e_stride = e_stride;
+    u.n_lvl = A.put(n_lvl);
+    u.lvl_ptr = A.put(lvl_ptr);
+    u.cell = A.put(cellat);
+    u.up = A.put(up);
+    u.gin = A.put(gin);
+    u.gout = A.put(gout);
+    u.kA = A.put(kA); u.kS = A.put(kS); u.itau = A.put(itau);
+    u.vb = h->bd.v;
+    u.theta = h->theta; u.Qdot = h->Qdot;
+    u.bin = h->bd.bin; u.dir_bin = h->bd.dir_bin; u.dir_nin = h->bd.dir_nin;
+    h->a2pos = A.put(a2pos);
+    u.a2pos = h->a2pos;
+    h->dir_cls = A.put(dir_cls);
+    u.w = h->bd.w;
+    u.s = A.put(cm.s);
+    u.theta_SI = h->theta_SI; u.theta_en = h->theta_en; u.q = h->q;
+    u.beta = cm.beta; u.Csum = cm.Csum;
+    const size_t part_n = (size_t)3 * nc + 64;  // scratch of the host-destination getters
+    h->part = A.zeros<double>(part_n);
+    double *e = A.zeros<double>((size_t)D * e_stride * B);
+    u.e = e; h->sw.e = e; h->bd.e = e; h->bd.e_stride = e_stride;
+    if (A.rc) return nb_fail(h, A.rc, "device upload failed");
+    if (dry) {
+      const size_t need = A.off + 256;
+      if (size_only) { *bytes_out = need; return 0; }
+      if (opt->workspace) {
+        if (opt->workspace_bytes < need) return nb_fail(h, NANOBTE_E_ALLOC, "workspace of %zu B given, %zu B needed", opt->workspace_bytes, need);
+        if ((uintptr_t)opt->workspace & 255) return nb_fail(h, NANOBTE_E_INVALID, "workspace must be 256-byte aligned");
+        h->arena = (char *)opt->workspace; h->arena_owned = false;
+      } else {
+        void *p = nullptr;
+        if (cudaMalloc(&p, need) != cudaSuccess) { cudaGetLastError(); return nb_fail(h, NANOBTE_E_ALLOC, "cudaMalloc of %zu B failed", need); }
+        h->arena = (char *)p; h->arena_owned = true;
+      }
+      h->arena_bytes = need;
+    }
+  }
+  NB_CUDA(h, cudaMallocHost((void **)&h->h_pinned, 64));
+  NB_CUDA(h, cudaStreamSynchronize(h->stream));  // host vectors die here
+  rc = nb_launch_boundary(h);  // initial inflow cache: thermalizing constants, zero elsewhere (R12)
+  if (rc < 0) return rc;
+  NB_CUDA(h, cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+}  // namespace
+
+extern "C" int nanobte_workspace_bytes_unstructured(const nanobte_unstructured_mesh *m, const nanobte_bands *b,
+                                                    const nanobte_quadrature *q, const nanobte_tag *tags, int32_t n_tags,
+                                                    const nanobte_options *opt, size_t *bytes_out) {
+  if (!bytes_out) return NANOBTE_E_INVALID;
+  nanobte_solver tmp;
+  int rc = build_uns(&tmp, m, b, q, tags, n_tags, nullptr, opt, true, bytes_out);
+  nb_free_unstructured(&tmp);
+  return rc;
+}
+
+extern "C" int nanobte_create_unstructured(const nanobte_unstructured_mesh *m, const nanobte_bands *b, const nanobte_quadrature *q,
+                                           const nanobte_tag *tags, int32_t n_tags, const double *Qdot,
+                                           const nanobte_options *opt, nanobte_solver **out) {
   if (!out) return NANOBTE_E_INVALID;
   nanobte_solver *h = new (std::nothrow) nanobte_solver();
+  if (!h) return NANOBTE_E_ALLOC;
   *out = h;
-  return nb_fail(h, NANOBTE_E_UNSUPPORTED, "unstructured meshes not built yet");
+  int rc = nb_check_device(h);
+  if (rc) return rc;
+  h->stream = opt ? (cudaStream_t)opt->stream : nullptr;
+  rc = build_uns(h, m, b, q, tags, n_tags, Qdot, opt, false, nullptr);
+  if (rc < 0 && h->arena && h->arena_owned) cudaFree(h->arena);
+  if (rc < 0) h->arena = nullptr;
+  return rc;
 }

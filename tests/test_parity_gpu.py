@@ -159,6 +159,54 @@ def test_finfet_cut_solve():
         assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
 
 
+# ---- unstructured polygon meshes (BASELINE.json configs[4] family): level-scheduled sweep --------------------------------------
+def test_tiny_triangles_steps():
+    pr = TINY["tri4x4"]
+    step_parity(pr, 4, T_init=random_T(pr, 5))
+
+
+def test_tiny_triangles_synthetic_and_solve():
+    pr = dict(TINY["tri4x4"])
+    pr["bands"] = small_bands(2, 21, lo=-11.3)
+    step_parity(pr, 3, T_init=random_T(pr, 6), mode="synthetic")
+    for mode in ("plain", "synthetic"):
+        r, g = RefSolver(pr), gpu_solver(pr)
+        rr, rg = r.solve(1e-11, 20000, mode), g.solve(1e-11, 20000, mode)
+        assert rr["converged"] and rg["converged"] and rg["iters"] == rr["iters"], (mode, rr, rg)
+        assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+
+
+@pytest.mark.parametrize("n,B,D,kw", [(24, 5, 16, {}), (40, 8, 16, {"sweep_threads": 128}), (33, 3, 8, {"sweep_G": 2}),
+                                      (20, 11, 8, {"sweep_G": 4, "sweep_threads": 64})])
+def test_triangles_cut_steps(n, B, D, kw):
+    """Cuts of configs[4]: jittered triangles with the circular hole, several CTAs per direction, ragged band groups."""
+    pr = wl.config_triangles(n=n, side=2e-6 * n / 320, B=B, D=D, hole_radius=300e-9 * n / 320)
+    step_parity(pr, 3, T_init=random_T(pr, 12), **kw)
+
+
+def test_triangles_cut_solve():
+    pr = wl.config_triangles(n=16, side=1e-7, B=3, D=8, hole_radius=1.5e-8)
+    r, g = RefSolver(pr), gpu_solver(pr)
+    rr, rg = r.solve(1e-9, 4000), g.solve(1e-9, 4000)
+    assert rr["converged"] and rg["converged"] and rr["iters"] == rg["iters"], (rr, rg)
+    assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+
+
+def test_polygon_quads_match_structured_on_gpu():
+    tags = [(wl.THERMALIZING, 302.0), (wl.THERMALIZING, 299.0), (wl.DIFFUSE, 0.0), (wl.SPECULAR, 0.0)]
+    bands, quad = small_bands(2, 8), wl.inplane_quadrature(8)
+    ps = wl.make_structured_problem(9, 7, 1, 7e-9, 9e-9, 1.0, bands, quad, tags, [0, 1, 2, 3, 0, 0])
+    pu = dict(ps)
+    pu["kind"] = "unstructured"
+    pu["mesh"] = wl.quads_as_unstructured(9, 7, 7e-9, 9e-9, lambda side: [0, 1, 2, 3][side], tags)
+    a, b = gpu_solver(ps), gpu_solver(pu)
+    for _ in range(4):
+        a.sweep(); b.sweep()
+        a.update_temperature(); b.update_temperature()
+    assert rel(b.get_e(), a.get_e()) <= 1e-12
+    assert np.abs(a.get_T(0) - b.get_T(0)).max() <= 1e-11
+
+
 # ---- degenerate shapes ---------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("shape", [(1, 1, 1), (7, 1, 1), (1, 9, 1), (5, 1, 3), (1, 1, 6), (2, 3, 1)])
 def test_degenerate_shapes(shape):
