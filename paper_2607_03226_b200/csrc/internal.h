@@ -19,13 +19,16 @@
 
 // ---- per-octant tables of the structured sweep -------------------------------------------------------------
 // Pencils (lines of cells along the sweep axis u) of a class are sorted by (m = v'+w', w'); the pencil index p is
-// also the pencil's slot in the shared-memory wavefront state.  Hyperplane h = u'+v'+w' holds the contiguous pencil
-// range [lo, lo+cnt) and lives at positions start + (p - lo) of every e row of the class; start is a multiple of 16
-// cells so that the per-plane table segments can be fetched with 1-D bulk TMA and every warp stores whole lines.
+// also the pencil's slot in the shared-memory wavefront state.  Each diagonal m is padded to an even number of slots
+// (padding slots are holes), so hyperplane h = u'+v'+w' holds the contiguous slot range [lo, lo+cnt) with lo and cnt
+// even and lives at positions start + (p - lo) of every e row of the class; start is a multiple of 16 cells.  Both
+// the per-plane table segments and the state-row segment that is the plane's output are therefore legal 1-D bulk
+// TMA transfers (16-byte aligned, multiple of 16 bytes).  The class's boundary-inflow row is ordered by consuming
+// hyperplane, each plane's slice [in_lo(h), in_lo(h+1)) padded to an even length for the same reason.
 struct OctTab {
   const uint2 *pen;          // [n_pen]   .x = m, .y = pencil index of the v-upwind pencil | w-upwind pencil << 16 (n_pen = none)
-  const int4 *plane;         // [H]       {lo, cnt, start, 0}
-  const uint32_t *cellinfo;  // [n_pos+16] bit0..2: u/v/w upwind value is a boundary inflow, bit3: hole, bits 4..: first inflow idx
+  const int4 *plane;         // [H+1]     {lo, cnt, start, in_lo}; entry H is the sentinel {0, 0, n_pos, n_in}
+  const uint32_t *cellinfo;  // [n_pos+16] bit0..2: u/v/w upwind value is a boundary inflow, bit3: hole, bits 4..: first inflow idx - in_lo(h)
   const double2 *tq;         // [n_pos+16] (theta, Qdot) in sweep order
   const double *rhu;         // [nu]      1/h_u in primed coordinates (non-uniform spacing only)
   const double2 *pen_rh;     // [n_pen]   (1/h_v, 1/h_w) of the pencil (non-uniform spacing only)
@@ -40,7 +43,8 @@ struct SweepArgs {
   const double *bin;         // inflow rows: class c, local row k at bin_base[c] + k * n_in[c]
   double *e;                 // [rows][e_stride]
   int64_t e_stride;
-  int32_t nu, sp, pcap;      // pencil length, state pitch (>= n_pen + 1), stage capacity in cells (multiple of 4)
+  int32_t nu, sp, pcap, gcap;  // pencil length, state pitch (>= n_pen + 1, even), table stage capacity in cells (multiple
+                             // of 4), inflow stage capacity in values (even)
 };
 
 // ---- boundary-closure kernel ----------------------------------------------------------------------------------
@@ -149,7 +153,7 @@ int nb_cg_solve(nanobte_solver *h, int *iters);
 int nb_cg_blocks(nanobte_solver *h);
 // sweep_structured.cu
 int nb_launch_sweep_structured(nanobte_solver *h);
-int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int H, int want_G, int want_threads,
+int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int gcap, int H, int want_G, int want_threads,
                                int n_sys_min_class);
 // sweep_unstructured.cu
 int nb_launch_sweep_unstructured(nanobte_solver *h);

@@ -31,7 +31,7 @@ struct OctHost {
   std::vector<int32_t> in_bf;      // inflow list: boundary face ids in consumption order
   std::vector<int32_t> bf_slot;    // [n_bf] index of the face in in_bf, or -1
   std::vector<int32_t> cell2pos;   // [n_cells]
-  int n_pen = 0, H = 0, n_pos = 0, p_max = 0;
+  int n_pen = 0, H = 0, n_pos = 0, p_max = 0, g_max = 0;
 };
 
 int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_bands *bands, const nanobte_quadrature *quad,
@@ -160,13 +160,14 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     for (double v : g.hsz[a]) uniform &= (v == g.hsz[a][0]);
 
   // ---- per class: pencils, hyperplanes, cell info, inflow lists ----------------------------------------------------------
-  int n_pen_max = 0, n_pos_max = 0, p_max = 0;
+  int n_pen_max = 0, n_pos_max = 0, p_max = 0, g_max = 0;
   for (int ci = 0; ci < ncls; ++ci) {
     OctHost &o = oct[ci];
     auto phys = [&](int axis, int x) { return o.sign[axis] > 0 ? x : g.n[axis] - 1 - x; };
     auto cell_of = [&](int u, int v, int w) { int c[3]; c[pa] = phys(pa, u); c[va] = phys(va, v); c[wa] = phys(wa, w); return g.cell(c[0], c[1], c[2]); };
     std::vector<int> pen_v, pen_w, first_of_m(nv + nw, 0), pen_of((size_t)nv * nw, -1);
     for (int mm = 0; mm <= nv + nw - 2; ++mm) {
+      if (pen_v.size() & 1) { pen_v.push_back(-1); pen_w.push_back(-1); }  // padding slot: keeps every diagonal's first slot even
       first_of_m[mm] = (int)pen_v.size();
       for (int w = std::max(0, mm - nv + 1); w <= std::min(nw - 1, mm); ++w) {
         const int v = mm - w;
@@ -175,12 +176,18 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
         if (any) { pen_of[(size_t)v + (size_t)nv * w] = (int)pen_v.size(); pen_v.push_back(v); pen_w.push_back(w); }
       }
     }
+    if (pen_v.size() & 1) { pen_v.push_back(-1); pen_w.push_back(-1); }
     first_of_m[nv + nw - 1] = (int)pen_v.size();
     o.n_pen = (int)pen_v.size();
     o.pen.resize(o.n_pen);
     o.pen_rh.resize(o.n_pen);
     for (int p = 0; p < o.n_pen; ++p) {
       const int v = pen_v[p], w = pen_w[p];
+      if (v < 0) {  // padding slot: never active (its cellinfo entries stay "hole")
+        o.pen[p] = make_uint2(0x3fffffffu, (uint32_t)o.n_pen | ((uint32_t)o.n_pen << 16));
+        o.pen_rh[p] = make_double2(0.0, 0.0);
+        continue;
+      }
       int nbv = v > 0 ? pen_of[(size_t)(v - 1) + (size_t)nv * w] : -1, nbw = w > 0 ? pen_of[(size_t)v + (size_t)nv * (w - 1)] : -1;
       if (nbv < 0) nbv = o.n_pen;  // the zero slot: such a cell always carries the boundary flag of that face
       if (nbw < 0) nbw = o.n_pen;
@@ -188,7 +195,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       o.pen_rh[p] = make_double2(1.0 / g.hsz[va][phys(va, v)], has_w ? 1.0 / g.hsz[wa][phys(wa, w)] : 0.0);
     }
     o.H = H;
-    o.plane.resize(H);
+    o.plane.resize(H + 1);
     std::vector<int> lo(H), hi(H), start(H);
     int base = 0;
     for (int hh = 0; hh < H; ++hh) {
@@ -206,8 +213,12 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     o.cell2pos.assign(nc, -1);
     o.bf_slot.assign(nbf, -1);
     const int axes[3] = {pa, va, wa};
-    for (int hh = 0; hh < H; ++hh)
+    for (int hh = 0; hh < H; ++hh) {
+      if (o.in_bf.size() & 1) o.in_bf.push_back(-1);  // every hyperplane's inflow slice starts on an even index
+      const uint32_t in_lo = (uint32_t)o.in_bf.size();
+      o.plane[hh].w = (int)in_lo;
       for (int p = lo[hh]; p < hi[hh]; ++p) {
+        if (pen_v[p] < 0) continue;
         const int u = hh - (pen_v[p] + pen_w[p]);
         const int pos = start[hh] + (p - lo[hh]);
         const int c = cell_of(u, pen_v[p], pen_w[p]);
@@ -229,16 +240,21 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
             o.in_bf.push_back(f);
           }
         }
-        if (first >= (1u << 28)) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "too many boundary inflow faces");
-        o.cellinfo[pos] = flags | (first << 4);
+        if (first - in_lo >= (1u << 28)) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "too many boundary inflow faces");
+        o.cellinfo[pos] = flags | ((first - in_lo) << 4);
         const double th0 = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
         o.tq[pos] = make_double2(th0, Qdot ? Qdot[c] : 0.0);
       }
+      o.g_max = std::max(o.g_max, (int)(o.in_bf.size() - in_lo));
+    }
+    if (o.in_bf.size() & 1) o.in_bf.push_back(-1);
+    o.plane[H] = make_int4(0, 0, o.n_pos, (int)o.in_bf.size());
     // reciprocal spacings along the sweep axis, in primed coordinates
     o.rhu.resize(nu);
     for (int u = 0; u < nu; ++u) o.rhu[u] = 1.0 / g.hsz[pa][phys(pa, u)];
     n_pen_max = std::max(n_pen_max, o.n_pen);
     p_max = std::max(p_max, o.p_max);
+    g_max = std::max(g_max, o.g_max);
     n_pos_max = std::max(n_pos_max, o.n_pos);
   }
   const int64_t e_stride = ((int64_t)n_pos_max + 31) / 32 * 32;
@@ -365,7 +381,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   // ---- sweep launch shape, tasks ---------------------------------------------------------------------------------------------------
   int nsys_min = 1 << 30;
   for (auto &o : oct) nsys_min = std::min<int>(nsys_min, (int)o.dirs.size() * B);
-  rc = nb_sweep_structured_config(h, n_pen_max, p_max, H, opt->sweep_G, opt->sweep_threads, nsys_min);
+  rc = nb_sweep_structured_config(h, n_pen_max, p_max, g_max, H, opt->sweep_G, opt->sweep_threads, nsys_min);
   if (rc) return rc;
   const int per_task = h->sweep_G;
   std::vector<int32_t> task_oct, task_row;

@@ -10,12 +10,16 @@
 // sweep: a CTA owns G systems of one octant for the entire grid and walks the hyperplanes itself.
 //   * The wavefront state -- one value per (v', w') pencil and system, i.e. the previous hyperplane -- lives in
 //     shared memory, so the v/w upwind reads never leave the SM; the u upwind value is the thread's own previous
-//     result and stays in a register.  HBM sees exactly one coalesced 8-byte streaming store per update.
+//     result and stays in a register.
 //   * Threads own pencils (lines along the sweep axis u) sorted by v'+w': the active pencils of a hyperplane are a
-//     contiguous thread range and the global store position start[h] + (p - lo[h]) is contiguous as well.
-//   * The per-cell tables of hyperplane h+1 (boundary flags / inflow index, theta, Qdot) are fetched by 1-D bulk TMA
-//     (cp.async.bulk + mbarrier complete_tx) into a two-stage shared-memory ring while hyperplane h is computed, so
-//     no global-memory round trip sits on the per-plane critical path except the (rare) boundary inflow values.
+//     contiguous slot range [lo, lo+cnt) of the state rows, and their positions in the e rows are contiguous too.
+//     So the state row segment IS the output: after every hyperplane one elected thread of a dedicated DMA warp
+//     issues one bulk TMA store (cp.async.bulk shared -> global) per system.  The compute warps never form a
+//     global address; HBM sees exactly one 8-byte streaming write per update, in >= 128-byte aligned segments.
+//   * Everything a hyperplane consumes arrives by 1-D bulk TMA one plane ahead, into a two-stage ring, on one
+//     mbarrier: the per-cell tables (flags / inflow index, theta, Qdot) and, per system, the hyperplane's slice
+//     of the lagged boundary-inflow cache (R9), which lands right behind the state row so that "upwind value" is
+//     one shared-memory load whether it is an interior neighbour or a wall.
 #include <algorithm>
 
 #include "internal.h"
@@ -49,39 +53,107 @@ __device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
+// 1-D bulk TMA shared -> global (bulk async-group completion)
+__device__ __forceinline__ void tma_store_1d(void *dst, const void *src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+// CTA-wide barrier that the compute warps and the DMA warp reach from different program points
+__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// Shared-memory carve-up (all offsets multiples of 16 bytes).
+// Shared-memory carve-up (all offsets multiples of 16 bytes).  A system's row is [ state sp | inflow stage 0 gcap |
+// inflow stage 1 gcap ] doubles, so one index addresses "upwind value" wherever it comes from.
 struct SmemLayout {
-  uint32_t tq, state, info, plane, bar, total;
+  uint32_t tq, info, rows, plane, bar, total, rp;
 };
-__host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int H) {
+__host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int gcap, int H) {
   SmemLayout L;
+  L.rp = (uint32_t)sp + 2u * (uint32_t)gcap;                 // row pitch in doubles (even)
   L.tq = 0;                                                  // [2][pcap] double2
-  L.state = L.tq + 2u * (uint32_t)pcap * 16u;                // [G][sp]   double
-  L.info = L.state + (uint32_t)G * (uint32_t)sp * 8u;        // [2][pcap] uint32
-  L.plane = L.info + 2u * (uint32_t)pcap * 4u;               // [H]       int4
-  L.bar = L.plane + (uint32_t)H * 16u;                       // [2]       mbarrier
+  L.info = L.tq + 2u * (uint32_t)pcap * 16u;                 // [2][pcap] uint32
+  L.rows = L.info + 2u * (uint32_t)pcap * 4u;                // [G][rp]   double
+  L.plane = L.rows + (uint32_t)G * L.rp * 8u;                // [H+1]     int4
+  L.bar = L.plane + ((uint32_t)H + 1u) * 16u;                // [2]       mbarrier
   L.total = L.bar + 16u;
   return L;
 }
 
+// blockDim.x = NT compute threads + 32 (the DMA warp).  R = pencils per compute thread.
 template <int G, int R, bool UNIFORM>
 __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a, const OctTab *__restrict__ octs) {
   extern __shared__ __align__(128) unsigned char smem[];
-  const int t = threadIdx.x, nt = blockDim.x;
+  const int t = threadIdx.x, nt = blockDim.x - 32;
   const int task = blockIdx.x;
   const OctTab T = octs[a.task_oct[task]];
-  const int nu = a.nu, sp = a.sp, pcap = a.pcap;
-  const SmemLayout L = smem_layout(G, sp, pcap, T.H);
+  const int nu = a.nu, sp = a.sp, pcap = a.pcap, gcap = a.gcap;
+  const SmemLayout L = smem_layout(G, sp, pcap, gcap, T.H);
   double2 *tq_s = reinterpret_cast<double2 *>(smem + L.tq);
-  double *st = reinterpret_cast<double *>(smem + L.state);
   uint32_t *info_s = reinterpret_cast<uint32_t *>(smem + L.info);
+  double *rows = reinterpret_cast<double *>(smem + L.rows);
   int4 *plane_s = reinterpret_cast<int4 *>(smem + L.plane);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smem + L.bar);
+  const uint32_t rp = L.rp;
 
   const int row_loc = a.task_row[task];
   const int n_valid = min(G, T.n_rows - row_loc);  // rows past the class's end recompute the last row and store nothing
   const int64_t row_g0 = (int64_t)T.row0 + row_loc;
+
+  for (int k = t; k <= T.H; k += blockDim.x) plane_s[k] = T.plane[k];
+  for (uint32_t k = t; k < (uint32_t)G * rp; k += blockDim.x) rows[k] = 0.0;
+  if (t == 0) {
+    mbar_init(bar, 1);
+    mbar_init(bar + 1, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  fence_proxy_async();
+  __syncthreads();
+
+  if (t >= nt) {
+    // ------------------------------------------------ DMA warp ---------------------------------------------------
+    const bool lead = t == nt;
+    double *const e0 = a.e + row_g0 * a.e_stride;
+    const double *const bin0 = a.bin + T.bin_base + (int64_t)row_loc * T.n_in;
+    auto issue_loads = [&](int h) {  // tables + inflow slices of hyperplane h into stage h & 1
+      const int4 P = plane_s[h];
+      const int s = h & 1;
+      const uint32_t c4 = ((uint32_t)P.y + 3u) & ~3u;
+      const uint32_t nin = (uint32_t)(plane_s[h + 1].w - P.w);  // even
+      mbar_expect_tx(bar + s, c4 * 20u + (uint32_t)G * nin * 8u);
+      if (c4) {
+        tma_load_1d(tq_s + (size_t)s * pcap, T.tq + P.z, c4 * 16u, bar + s);
+        tma_load_1d(info_s + (size_t)s * pcap, T.cellinfo + P.z, c4 * 4u, bar + s);
+      }
+      if (nin) {
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+          tma_load_1d(rows + (size_t)g * rp + sp + s * gcap, bin0 + (int64_t)min(g, n_valid - 1) * T.n_in + P.w, nin * 8u, bar + s);
+      }
+    };
+    if (lead) issue_loads(0);
+    for (int h = 0; h < T.H; ++h) {
+      if (lead) {
+        if (h + 1 < T.H) issue_loads(h + 1);  // stage (h+1)&1 was last read while hyperplane h-1 was computed
+        tma_store_wait_read();                // the stores of hyperplane h-1 have read the state rows
+      }
+      cta_sync();  // A: every read of hyperplane h-1 is done
+      cta_sync();  // B: hyperplane h is in the state rows (and fenced to the async proxy)
+      if (lead) {
+        const int4 P = plane_s[h];
+        if (P.y) {
+#pragma unroll
+          for (int g = 0; g < G; ++g)
+            if (g < n_valid) tma_store_1d(e0 + (int64_t)g * a.e_stride + P.z, rows + (size_t)g * rp + P.x, (uint32_t)P.y * 8u);
+        }
+        tma_store_commit();
+      }
+    }
+    if (lead) tma_store_wait_read();
+    return;
+  }
+
+  // -------------------------------------------------- compute warps ------------------------------------------------
   double cf[G][UNIFORM ? 5 : 6];
 #pragma unroll
   for (int g = 0; g < G; ++g) {
@@ -89,54 +161,26 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
 #pragma unroll
     for (int k = 0; k < (UNIFORM ? 5 : 6); ++k) cf[g][k] = a.coef[row * 8 + k];
   }
-  double *const e0 = a.e + row_g0 * a.e_stride;
-  const double *const bin0 = a.bin + T.bin_base + (int64_t)row_loc * T.n_in;
-  const int64_t e_stride = a.e_stride;
-  const int n_in = T.n_in;
-
-  // per-thread pencils
-  int pm[R];
+  // per-thread pencils: slot p = t + r*nt; upwind pencil slots (the zero slot n_pen if there is none)
   uint32_t pnb[R];
+  int pm[UNIFORM ? 1 : R];
   double rv[UNIFORM ? 1 : R], rw[UNIFORM ? 1 : R];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
     const int p = t + r * nt;
+    pnb[r] = 0;
+    if (!UNIFORM) { rv[r] = rw[r] = 0.0; pm[r] = 0; }
     if (p < T.n_pen) {
       const uint2 q = T.pen[p];
-      pm[r] = (int)q.x;
       pnb[r] = q.y;
       if (!UNIFORM) {
+        pm[r] = (int)q.x;
         const double2 rh = T.pen_rh[p];
         rv[r] = rh.x;
         rw[r] = rh.y;
       }
-    } else {
-      pm[r] = 0x3fffffff;  // never active
-      pnb[r] = 0;
-      if (!UNIFORM) rv[r] = rw[r] = 0.0;
     }
   }
-  for (int k = t; k < T.H; k += nt) plane_s[k] = T.plane[k];
-  for (int k = t; k < G; k += nt) st[(size_t)k * sp + T.n_pen] = 0.0;  // the "no upwind pencil" slot
-  if (t == 0) {
-    mbar_init(bar, 1);
-    mbar_init(bar + 1, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-
-  auto issue = [&](int h) {  // thread 0: fetch the tables of hyperplane h into stage h & 1
-    const int4 P = plane_s[h];
-    const int s = h & 1;
-    const uint32_t c4 = ((uint32_t)P.y + 3u) & ~3u;
-    mbar_expect_tx(bar + s, c4 * 20u);
-    if (c4) {
-      tma_load_1d(tq_s + (size_t)s * pcap, T.tq + P.z, c4 * 16u, bar + s);
-      tma_load_1d(info_s + (size_t)s * pcap, T.cellinfo + P.z, c4 * 4u, bar + s);
-    }
-  };
-  if (t == 0) issue(0);
-
   double res[R][G];
 #pragma unroll
   for (int r = 0; r < R; ++r)
@@ -145,46 +189,40 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
 
   for (int h = 0; h < T.H; ++h) {
     const int s = h & 1;
-    mbar_wait(bar + s, (h >> 1) & 1);
-    if (t == 0 && h + 1 < T.H) issue(h + 1);  // stage s^1 was last read before the closing barrier of step h-1
     const int4 P = plane_s[h];
+    mbar_wait(bar + s, (h >> 1) & 1);
     const double2 *tqh = tq_s + (size_t)s * pcap - P.x;
     const uint32_t *infoh = info_s + (size_t)s * pcap - P.x;
+    const uint32_t gs = (uint32_t)sp + (uint32_t)(s * gcap);  // this hyperplane's inflow stage within a row
     unsigned act = 0;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      const int u = h - pm[r];
-      if ((unsigned)u < (unsigned)nu) {
-        const int p = t + r * nt;
+      const int p = t + r * nt;
+      if ((unsigned)(p - P.x) < (unsigned)P.y) {
         const uint32_t info = infoh[p];
-        if (!(info & 8u)) {
+        if (!(info & 8u)) {  // not a hole / padding slot
           act |= 1u << r;
           const double2 tq = tqh[p];
-          const uint32_t nbv = pnb[r] & 0xffffu, nbw = pnb[r] >> 16;
+          const uint32_t gb = gs + (info >> 4);
+          const uint32_t iv = (info & 2u) ? gb + (info & 1u) : (pnb[r] & 0xffffu);
+          const uint32_t iw = (info & 4u) ? gb + (info & 1u) + ((info >> 1) & 1u) : (pnb[r] >> 16);
           double eu[G], ev[G], ew[G];
 #pragma unroll
           for (int g = 0; g < G; ++g) {
             eu[g] = res[r][g];
-            ev[g] = st[g * sp + nbv];
-            ew[g] = st[g * sp + nbw];
+            ev[g] = rows[g * rp + iv];
+            ew[g] = rows[g * rp + iw];
           }
-          if (info & 7u) {
-            const double *b = bin0 + (info >> 4);
-            const int iv = (info & 1u), iw = iv + ((info >> 1) & 1u);
+          if (info & 1u) {
 #pragma unroll
-            for (int g = 0; g < G; ++g) {
-              const double *bg = b + (int64_t)min(g, n_valid - 1) * n_in;
-              if (info & 1u) eu[g] = __ldg(bg);
-              if (info & 2u) ev[g] = __ldg(bg + iv);
-              if (info & 4u) ew[g] = __ldg(bg + iw);
-            }
+            for (int g = 0; g < G; ++g) eu[g] = rows[g * rp + gb];
           }
           if (UNIFORM) {
 #pragma unroll
             for (int g = 0; g < G; ++g)
               res[r][g] = cf[g][0] * tq.x + cf[g][1] * tq.y + cf[g][2] * eu[g] + cf[g][3] * ev[g] + cf[g][4] * ew[g];
           } else {
-            const double au = __ldg(T.rhu + u);
+            const double au = __ldg(T.rhu + min(max(h - pm[r], 0), nu - 1));
 #pragma unroll
             for (int g = 0; g < G; ++g) {
               const double gu = cf[g][3] * au, gv = cf[g][4] * rv[r], gw = cf[g][5] * rw[r];
@@ -195,21 +233,17 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
         }
       }
     }
-    __syncthreads();  // every read of hyperplane h-1 (and of stage s) is done
-    const int64_t pbase = (int64_t)P.z - P.x;
+    cta_sync();  // A: every read of hyperplane h-1 (and of stage s) is done; its stores have left the state rows
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       if (act & (1u << r)) {
         const int p = t + r * nt;
-        double *ep = e0 + pbase + p;
 #pragma unroll
-        for (int g = 0; g < G; ++g) {
-          st[g * sp + p] = res[r][g];
-          if (g < n_valid) __stcs(ep + g * e_stride, res[r][g]);
-        }
+        for (int g = 0; g < G; ++g) rows[g * rp + p] = res[r][g];
       }
     }
-    __syncthreads();  // hyperplane h is visible
+    fence_proxy_async();  // generic-proxy writes -> visible to the bulk store the DMA warp issues after B
+    cta_sync();           // B: hyperplane h is visible
   }
 }
 
@@ -236,56 +270,62 @@ sweep_fn pick(int g, int r, bool uniform) {
   switch (g) {
     case 1: return pick_r<1>(r, uniform);
     case 2: return pick_r<2>(r, uniform);
+    case 3: return pick_r<3>(r, uniform);
     case 4: return pick_r<4>(r, uniform);
   }
   return nullptr;
 }
 const int kR[7] = {1, 2, 3, 4, 5, 6, 8};
+const int kMaxCompute = 480;  // + the DMA warp = 512 threads
 
 }  // namespace
 
-// Chooses systems per CTA (G), pencils per thread (R) and threads per CTA.  want_G / want_threads: 0 = auto.
-int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int H, int want_G, int want_threads,
+// Chooses systems per CTA (G), pencils per thread (R) and compute threads per CTA.  want_G / want_threads: 0 = auto.
+// n_pen_max: pencil slots (incl. padding); p_max: largest hyperplane; gcap: largest per-hyperplane inflow slice.
+int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int gcap, int H, int want_G, int want_threads,
                                int n_sys_min_class) {
   const size_t smem_cap = 227 * 1024;
-  if (want_G != 0 && want_G != 1 && want_G != 2 && want_G != 4) return nb_fail(h, NANOBTE_E_INVALID, "sweep_G must be 0, 1, 2 or 4");
-  if (n_pen_max > 8 * 512 || n_pen_max >= 65535)
-    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section has %d pencils; the sweep kernel supports up to %d", n_pen_max, 8 * 512);
+  if (want_G < 0 || want_G > 4) return nb_fail(h, NANOBTE_E_INVALID, "sweep_G must be 0..4");
+  if (n_pen_max > 8 * kMaxCompute || n_pen_max >= 65535)
+    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section has %d pencils; the sweep kernel supports up to %d", n_pen_max,
+                   8 * kMaxCompute);
   int R = 0, T = 0;
   if (want_threads > 0) {
-    T = std::min(512, (want_threads + 31) / 32 * 32);
+    T = std::min(kMaxCompute, (want_threads + 31) / 32 * 32);
     for (int k = 0; k < 7 && !R; ++k)
       if ((long)kR[k] * T >= n_pen_max) R = kR[k];
     if (!R) return nb_fail(h, NANOBTE_E_INVALID, "sweep_threads=%d cannot cover %d pencils", want_threads, n_pen_max);
   } else {
     for (int k = 0; k < 7 && !R; ++k) {
       const int tt = ((n_pen_max + kR[k] - 1) / kR[k] + 31) / 32 * 32;
-      if (tt <= 512) { R = kR[k]; T = tt; }
+      if (tt <= kMaxCompute) { R = kR[k]; T = tt; }
     }
   }
   const int sp = (n_pen_max + 1 + 1) & ~1;
   const int pcap = (p_max + 3 + 4) & ~3;
+  gcap = (gcap + 1) & ~1;
   int G = 0;
-  const int cand[3] = {4, 2, 1};
-  for (int k = 0; k < 3 && !G; ++k) {
+  const int cand[4] = {4, 3, 2, 1};
+  for (int k = 0; k < 4 && !G; ++k) {
     const int g = cand[k];
     if (want_G > 0 && g != want_G) continue;
-    if (smem_layout(g, sp, pcap, H).total > smem_cap) continue;
+    if (smem_layout(g, sp, pcap, gcap, H).total > smem_cap) continue;
     if (want_G <= 0 && (g * R > 20 || g > std::max(1, n_sys_min_class))) continue;  // registers: 2*G*R for the results
     G = g;
   }
   if (!G) {
     if (want_G > 0) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "sweep_G=%d needs %u B of shared memory (> %zu)", want_G,
-                                   smem_layout(want_G, sp, pcap, H).total, smem_cap);
+                                   smem_layout(want_G, sp, pcap, gcap, H).total, smem_cap);
     return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section of %d pencils needs %u B of shared memory (> %zu)", n_pen_max,
-                   smem_layout(1, sp, pcap, H).total, smem_cap);
+                   smem_layout(1, sp, pcap, gcap, H).total, smem_cap);
   }
   h->sweep_G = G;
   h->sweep_rmax = R;
   h->sweep_threads = T;
-  h->sweep_smem = smem_layout(G, sp, pcap, H).total;
+  h->sweep_smem = smem_layout(G, sp, pcap, gcap, H).total;
   h->sw.sp = sp;
   h->sw.pcap = pcap;
+  h->sw.gcap = gcap;
   return 0;
 }
 
@@ -296,7 +336,7 @@ int nb_launch_sweep_structured(nanobte_solver *h) {
     NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(h->sweep_smem, 1024)));
     h->sweep_attr_set = true;
   }
-  fn<<<h->n_tasks, h->sweep_threads, h->sweep_smem, h->stream>>>(h->sw, h->d_octs);
+  fn<<<h->n_tasks, h->sweep_threads + 32, h->sweep_smem, h->stream>>>(h->sw, h->d_octs);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
   return 0;
