@@ -186,6 +186,8 @@ extern "C" void nanobte_destroy(nanobte_solver *h) {
 
 extern "C" int nanobte_sweep(nanobte_solver *h) {
   if (!h || !h->arena) return NANOBTE_E_INVALID;
+  h->swept_since_closure = true;
+  h->therm_stale = true;
   return h->kind == 0 ? nb_launch_sweep_structured(h) : nb_launch_sweep_unstructured(h);
 }
 
@@ -200,7 +202,10 @@ static int read_maxdT(nanobte_solver *h, double *out) {
 extern "C" int nanobte_update_temperature(nanobte_solver *h, double *max_dT) {
   if (!h || !h->arena) return NANOBTE_E_INVALID;
   int rc;
-  if ((rc = nb_launch_boundary(h)) < 0) return rc;  // G, face fluxes, inflow cache for the next sweep (O3)
+  if (h->swept_since_closure) {  // G, face fluxes, inflow cache for the next sweep (O3); once per sweep
+    if ((rc = nb_launch_boundary(h)) < 0) return rc;
+    h->swept_since_closure = false;
+  }
   if ((rc = nb_launch_moments(h)) < 0) return rc;   // O4
   if ((rc = nb_launch_update(h, 0)) < 0) return rc; // O5
   if (max_dT) return read_maxdT(h, max_dT);
@@ -320,13 +325,17 @@ extern "C" int nanobte_get_e(nanobte_solver *h, int32_t b0, int32_t nb, int32_t 
 
 extern "C" int nanobte_get_G(nanobte_solver *h, double *dst, int32_t dst_is_device) {
   if (!h || !h->arena || !dst) return NANOBTE_E_INVALID;
+  int rc = nb_refresh_thermalizing(h);
+  if (rc < 0) return rc;
   return copy_out(h, h->bd.G, dst, (size_t)h->n_bf * h->B, dst_is_device);
 }
 
 extern "C" int nanobte_get_boundary_heat(nanobte_solver *h, double *per_tag) {
   if (!h || !h->arena || !per_tag) return NANOBTE_E_INVALID;
   if (h->n_tags == 0) return 0;
-  int rc = nb_launch_tagheat(h);
+  int rc = nb_refresh_thermalizing(h);
+  if (rc < 0) return rc;
+  rc = nb_launch_tagheat(h);
   if (rc < 0) return rc;
   return copy_out(h, h->d_tagheat, per_tag, (size_t)h->n_tags, 0);
 }

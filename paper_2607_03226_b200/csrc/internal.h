@@ -96,6 +96,14 @@ struct nanobte_solver {
   struct UnsArgs *uns = nullptr;
 
   BoundaryArgs bd{};
+  // structured grids: closures split into a G/flux kernel over reflecting faces and an inflow-cache kernel
+  bool split_closures = false, therm_stale = true, swept_since_closure = false;
+  const int32_t *cls_inbf[NB_MAX_CLASSES] = {nullptr};  // per class: face id per inflow slot (-1 = padding)
+  int32_t cls_nin[NB_MAX_CLASSES] = {0}, cls_ndirs[NB_MAX_CLASSES] = {0};
+  const int32_t *cls_dirs = nullptr;                     // [n_cls][max_cls_dirs]
+  int max_cls_dirs = 0;
+  const int32_t *refl_faces = nullptr, *therm_faces = nullptr;
+  int n_refl = 0, n_therm = 0;
 
   // moments / update
   int32_t *cls_npos_h = nullptr;
@@ -142,7 +150,8 @@ int nb_fail(nanobte_solver *h, int code, const char *fmt, ...);
   } while (0)
 
 // kernels_common.cu
-int nb_launch_boundary(nanobte_solver *h);
+int nb_launch_boundary(nanobte_solver *h, int init = 0);
+int nb_refresh_thermalizing(nanobte_solver *h);
 int nb_launch_moments(nanobte_solver *h);
 int nb_launch_update(nanobte_solver *h, int mode /*0: theta<-theta_SI, 1: theta<-theta_SI+x*/);
 int nb_launch_get_e(nanobte_solver *h, int b0, int nb, int d0, int nd, double *dst_dev, int deviational);

@@ -3,6 +3,8 @@
 // Everything is fp64, deterministic (no floating-point atomics; fixed reduction trees).
 #include <cooperative_groups.h>
 
+#include <algorithm>
+
 #include "internal.h"
 namespace cg = cooperative_groups;
 
@@ -81,8 +83,19 @@ __global__ void __launch_bounds__(256) boundary_kernel(BoundaryRun R) {
   }
 }
 
-int nb_launch_boundary(nanobte_solver *h) {
+static int launch_closure_G(nanobte_solver *h, const int32_t *faces, int n_faces);
+static int launch_closure_inflow(nanobte_solver *h, int init);
+
+int nb_launch_boundary(nanobte_solver *h, int init) {
   if (h->n_bf == 0) return 0;
+  if (h->split_closures) {
+    h->therm_stale = true;
+    if (init) return launch_closure_inflow(h, 1);
+    if (h->n_refl == 0) return 0;
+    int rc = launch_closure_G(h, h->refl_faces, h->n_refl);
+    if (rc < 0) return rc;
+    return launch_closure_inflow(h, 0);
+  }
   BoundaryRun R;
   R.a = h->bd;
   R.W = h->W;
@@ -92,6 +105,175 @@ int nb_launch_boundary(nanobte_solver *h) {
   boundary_kernel<<<(h->n_bf + wpb - 1) / wpb, wpb * 32, smem, h->stream>>>(R);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+// =================================================================================================================
+// (a3) structured grids: the closures as two kernels whose global accesses follow the memory layout.
+//   closure_G_kernel      one warp per (boundary face, chunk of bands), lanes over the OUTGOING directions: gathers
+//                         eps at the wall cell (one 8-byte value per (direction, band) row -- inherently one sector
+//                         each), G_bf (R7) and the face flux (O8).  The incoming half of the flux needs no second
+//                         gather: the inflow the last sweep consumed was C_b dT_w/W (thermalizing) or built from
+//                         eps^{n-1} with G^{n-1}, and sum_in w (s.n) inflow = -den * G^{n-1} for diffuse, specular and
+//                         mixed walls alike because the quadrature is mirror symmetric about the wall (weights
+//                         checked at create), so  F_bf = v_b (gnum^n - den * X),  X = C_b dT_w/W  or  G^{n-1}_bf.
+//   closure_inflow_kernel one thread per (octant class, slot of its inflow row, direction of the class): writes the
+//                         inflow cache in exactly the order the sweep's bulk loads read it -> coalesced stores;
+//                         the specular part gathers eps of the mirrored direction (R8).
+// Thermalizing faces never change their inflow (written once at create) and their G / flux are diagnostics only:
+// they are skipped per iteration and evaluated on demand (get_G, get_boundary_heat).
+// =================================================================================================================
+struct ClosureArgs {
+  BoundaryArgs a;
+  double W;
+  const int32_t *faces;     // face list this launch covers
+  int32_t n_faces, bands_per_chunk;
+};
+
+template <int K>  // K = ceil(D / 32) directions per lane
+__global__ void __launch_bounds__(256) closure_G_kernel(ClosureArgs R) {
+  const BoundaryArgs &a = R.a;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int fi = blockIdx.x * (blockDim.x >> 5) + wib;
+  if (fi >= R.n_faces) return;
+  const int bf = R.faces[fi];
+  const size_t row = (size_t)bf * a.D;
+  const double *src[K];
+  double wsn[K];
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    const int d = lane + 32 * k;
+    wsn[k] = 0.0;
+    src[k] = a.e;
+    if (d < a.D) {
+      const double sn = a.bf_sn[row + d];
+      if (sn > 0.0) {
+        wsn[k] = a.w[d] * sn;
+        src[k] = a.e + (int64_t)a.dir_row0[d] * a.e_stride + a.bf_opos[row + d];
+      }
+    }
+  }
+  const double den = a.bf_den[bf], dTw = a.bf_eps_w[bf];
+  const bool therm = a.bf_type[bf] == NANOBTE_THERMALIZING;
+  const int b_lo = blockIdx.y * R.bands_per_chunk, b_hi = min(a.B, b_lo + R.bands_per_chunk);
+  constexpr int UB = 6;
+  for (int b0 = b_lo; b0 < b_hi; b0 += UB) {
+    double acc[UB];
+#pragma unroll
+    for (int j = 0; j < UB; ++j) {
+      acc[j] = 0.0;
+      const int b = min(b0 + j, b_hi - 1);
+#pragma unroll
+      for (int k = 0; k < K; ++k)
+        if (wsn[k] != 0.0) acc[j] += wsn[k] * __ldcs(src[k] + (int64_t)b * a.e_stride);
+    }
+#pragma unroll
+    for (int j = 0; j < UB; ++j) acc[j] = warp_sum(acc[j]);
+#pragma unroll
+    for (int j = 0; j < UB; ++j) {
+      const int b = b0 + j;
+      if (lane == j && b < b_hi) {
+        const size_t o = (size_t)bf * a.B + b;
+        const double Gold = a.G[o];
+        a.G[o] = den > 0.0 ? acc[j] / den : 0.0;
+        const double X = therm ? a.C[b] * dTw / R.W : Gold;
+        a.faceflux[o] = a.v[b] * (acc[j] - den * X);
+      }
+    }
+  }
+}
+
+struct InflowArgs {
+  BoundaryArgs a;
+  double W;
+  const int32_t *cls_inbf[NB_MAX_CLASSES];  // per class: face id of every slot of the inflow row (-1 = padding)
+  int32_t cls_nin[NB_MAX_CLASSES], cls_ndirs[NB_MAX_CLASSES];
+  const int32_t *cls_dirs;                   // [n_cls][max_dirs]
+  int32_t max_dirs, init;
+};
+
+__global__ void __launch_bounds__(128) closure_inflow_kernel(InflowArgs R) {
+  const BoundaryArgs &a = R.a;
+  const int c = blockIdx.y, kd = blockIdx.z;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (kd >= R.cls_ndirs[c] || idx >= R.cls_nin[c]) return;
+  const int bf = R.cls_inbf[c][idx];
+  if (bf < 0) return;
+  const int type = a.bf_type[bf];
+  const int d = R.cls_dirs[c * R.max_dirs + kd];
+  const int64_t n_in = a.dir_nin[d];
+  double *dst = a.bin + a.dir_bin[d] + idx;
+  if (type == NANOBTE_THERMALIZING) {
+    if (R.init) {
+      const double dTw = a.bf_eps_w[bf];
+      for (int b = 0; b < a.B; ++b) dst[b * n_in] = a.C[b] * dTw / R.W;  // R6
+    }
+    return;
+  }
+  if (R.init) return;  // eps^0 = 0 (R12): reflecting walls start from a zero cache
+  const double *Gf = a.G + (size_t)bf * a.B;
+  if (type == NANOBTE_DIFFUSE) {
+    for (int b = 0; b < a.B; ++b) dst[b * n_in] = Gf[b];  // R7
+    return;
+  }
+  const double p = type == NANOBTE_SPECULAR ? 1.0 : a.bf_p[bf];
+  const int md = a.bf_mirror[(size_t)bf * a.D + d];
+  const double *src = a.e + (int64_t)a.dir_row0[md] * a.e_stride + a.bf_opos[(size_t)bf * a.D + md];
+  constexpr int UB = 6;
+  for (int b0 = 0; b0 < a.B; b0 += UB) {
+    double spec[UB];
+#pragma unroll
+    for (int j = 0; j < UB; ++j) spec[j] = __ldcs(src + (int64_t)min(b0 + j, a.B - 1) * a.e_stride);
+#pragma unroll
+    for (int j = 0; j < UB; ++j)
+      if (b0 + j < a.B) dst[(b0 + j) * n_in] = type == NANOBTE_SPECULAR ? spec[j] : p * spec[j] + (1.0 - p) * Gf[b0 + j];  // R8
+  }
+}
+
+static int launch_closure_G(nanobte_solver *h, const int32_t *faces, int n_faces) {
+  if (n_faces == 0) return 0;
+  ClosureArgs R;
+  R.a = h->bd; R.W = h->W; R.faces = faces; R.n_faces = n_faces;
+  const int chunks = std::max(1, std::min((h->B + 5) / 6, (4 * h->n_sm * 8 + n_faces - 1) / n_faces));
+  R.bands_per_chunk = ((h->B + chunks - 1) / chunks + 5) / 6 * 6;
+  dim3 grid((n_faces + 7) / 8, (h->B + R.bands_per_chunk - 1) / R.bands_per_chunk);
+  const int K = (h->D + 31) / 32;
+  switch (K) {
+    case 1: closure_G_kernel<1><<<grid, 256, 0, h->stream>>>(R); break;
+    case 2: closure_G_kernel<2><<<grid, 256, 0, h->stream>>>(R); break;
+    case 3: closure_G_kernel<3><<<grid, 256, 0, h->stream>>>(R); break;
+    case 4: closure_G_kernel<4><<<grid, 256, 0, h->stream>>>(R); break;
+    default: return nb_fail(h, NANOBTE_E_UNSUPPORTED, "internal: closure_G_kernel supports up to 128 directions");
+  }
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+static int launch_closure_inflow(nanobte_solver *h, int init) {
+  InflowArgs R;
+  R.a = h->bd; R.W = h->W; R.cls_dirs = h->cls_dirs; R.max_dirs = h->max_cls_dirs; R.init = init;
+  int nin_max = 0;
+  for (int c = 0; c < NB_MAX_CLASSES; ++c) {
+    R.cls_inbf[c] = h->cls_inbf[c];
+    R.cls_nin[c] = h->cls_nin[c];
+    R.cls_ndirs[c] = h->cls_ndirs[c];
+    nin_max = std::max(nin_max, h->cls_nin[c]);
+  }
+  if (nin_max == 0) return 0;
+  dim3 grid((nin_max + 127) / 128, h->n_cls, h->max_cls_dirs);
+  closure_inflow_kernel<<<grid, 128, 0, h->stream>>>(R);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+// Diagnostics of the thermalizing faces (G, face flux) from the current eps; called by the getters that expose them.
+int nb_refresh_thermalizing(nanobte_solver *h) {
+  if (!h->split_closures || !h->therm_stale) return 0;
+  int rc = launch_closure_G(h, h->therm_faces, h->n_therm);
+  if (rc < 0) return rc;
+  h->therm_stale = false;
   return 0;
 }
 

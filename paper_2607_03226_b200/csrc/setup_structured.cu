@@ -285,6 +285,8 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
           int &mj = mirror_tab[(size_t)side * D + d];
           if (mj == -2) mj = nb_find_mirror(cm, d, nrm);
           if (mj < 0) return nb_fail(h, NANOBTE_E_SPECULAR, "boundary face %d: mirror image of direction %d is not in the quadrature", f, d);
+          if (std::fabs(cm.w[mj] - cm.w[d]) > 1e-13 * cm.w[d])
+            return nb_fail(h, NANOBTE_E_SPECULAR, "boundary face %d: direction %d and its mirror image %d carry different weights", f, d, mj);
           G.bf_mirror[(size_t)f * D + d] = mj;
         }
       } else if (sn > 0) {
@@ -312,6 +314,14 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     }
   }
   G.bin_total = tot;
+  // closure launch lists: reflecting faces (every iteration), thermalizing faces (diagnostics on demand), class directions
+  std::vector<int32_t> refl_faces, therm_faces;
+  for (int f = 0; f < nbf; ++f) (G.bf_type[f] == NANOBTE_THERMALIZING ? therm_faces : refl_faces).push_back(f);
+  int max_cls_dirs = 0;
+  for (auto &o : oct) max_cls_dirs = std::max<int>(max_cls_dirs, (int)o.dirs.size());
+  std::vector<int32_t> cls_dirs((size_t)ncls * max_cls_dirs, 0);
+  for (int ci = 0; ci < ncls; ++ci)
+    for (size_t k = 0; k < oct[ci].dirs.size(); ++k) cls_dirs[(size_t)ci * max_cls_dirs + k] = oct[ci].dirs[k];
 
   // ---- per-row coefficient tables ----------------------------------------------------------------------------------------------
   std::vector<double> coef((size_t)D * B * 8, 0.0);
@@ -381,6 +391,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   // ---- sweep launch shape, tasks ---------------------------------------------------------------------------------------------------
   int nsys_min = 1 << 30;
   for (auto &o : oct) nsys_min = std::min<int>(nsys_min, (int)o.dirs.size() * B);
+  h->uniform = uniform;
   rc = nb_sweep_structured_config(h, n_pen_max, p_max, g_max, H, opt->sweep_G, opt->sweep_threads, nsys_min);
   if (rc) return rc;
   const int per_task = h->sweep_G;
@@ -417,6 +428,9 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     for (int ci = 0; ci < ncls; ++ci) {
       OctHost &o = oct[ci];
       OctTab &t = tabs[ci];
+      h->cls_inbf[ci] = A.put(o.in_bf);
+      h->cls_nin[ci] = (int32_t)o.in_bf.size();
+      h->cls_ndirs[ci] = (int32_t)o.dirs.size();
       t.pen = A.put(o.pen);
       t.plane = A.put(o.plane);
       t.cellinfo = A.put(o.cellinfo);
@@ -429,6 +443,13 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       t.n_pen = o.n_pen; t.H = o.H; t.n_pos = o.n_pos; t.n_in = (int)o.in_bf.size();
       t.row0 = cls_row0[ci]; t.n_rows = h->cls_nsys[ci]; t.p_max = o.p_max;
     }
+    h->cls_dirs = A.put(cls_dirs);
+    h->max_cls_dirs = max_cls_dirs;
+    h->refl_faces = A.put(refl_faces);
+    h->therm_faces = A.put(therm_faces);
+    h->n_refl = (int)refl_faces.size();
+    h->n_therm = (int)therm_faces.size();
+    h->split_closures = D <= 128;  // closure_G_kernel keeps ceil(D/32) <= 4 directions per lane
     h->d_octs = A.put(tabs);
     h->sw.task_oct = A.put(task_oct);
     h->sw.task_row = A.put(task_row);
@@ -460,7 +481,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   NB_CUDA(h, cudaMallocHost((void **)&h->h_pinned, 64));
   NB_CUDA(h, cudaStreamSynchronize(h->stream));  // host vectors die here
   // initial inflow cache: thermalizing constants, zero elsewhere (eps^0 = 0, R12)
-  rc = nb_launch_boundary(h);
+  rc = nb_launch_boundary(h, 1);
   if (rc < 0) return rc;
   NB_CUDA(h, cudaStreamSynchronize(h->stream));
   return 0;

@@ -16,7 +16,7 @@
 //     So the state row segment IS the output: after every hyperplane one elected thread of a dedicated DMA warp
 //     issues one bulk TMA store (cp.async.bulk shared -> global) per system.  The compute warps never form a
 //     global address; HBM sees exactly one 8-byte streaming write per update, in >= 128-byte aligned segments.
-//   * Everything a hyperplane consumes arrives by 1-D bulk TMA one plane ahead, into a two-stage ring, on one
+//   * Everything a hyperplane consumes arrives by 1-D bulk TMA two planes ahead, into a two-stage ring, on one
 //     mbarrier: the per-cell tables (flags / inflow index, theta, Qdot) and, per system, the hyperplane's slice
 //     of the lagged boundary-inflow cache (R9), which lands right behind the state row so that "upwind value" is
 //     one shared-memory load whether it is an interior neighbour or a wall.
@@ -131,13 +131,15 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
           tma_load_1d(rows + (size_t)g * rp + sp + s * gcap, bin0 + (int64_t)min(g, n_valid - 1) * T.n_in + P.w, nin * 8u, bar + s);
       }
     };
-    if (lead) issue_loads(0);
+    if (lead) {
+      issue_loads(0);
+      if (T.H > 1) issue_loads(1);
+    }
     for (int h = 0; h < T.H; ++h) {
-      if (lead) {
-        if (h + 1 < T.H) issue_loads(h + 1);  // stage (h+1)&1 was last read while hyperplane h-1 was computed
-        tma_store_wait_read();                // the stores of hyperplane h-1 have read the state rows
-      }
-      cta_sync();  // A: every read of hyperplane h-1 is done
+      if (lead) tma_store_wait_read();  // the stores of hyperplane h-1 have read the state rows
+      cta_sync();  // A: every read of hyperplane h-1 and of stage h&1 is done
+      // two planes ahead, and ahead of this plane's stores in the TMA queue
+      if (lead && h + 2 < T.H) issue_loads(h + 2);
       cta_sync();  // B: hyperplane h is in the state rows (and fenced to the async proxy)
       if (lead) {
         const int4 P = plane_s[h];
@@ -187,9 +189,11 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
 #pragma unroll
     for (int g = 0; g < G; ++g) res[r][g] = 0.0;
 
+  int4 Pn = plane_s[0];
   for (int h = 0; h < T.H; ++h) {
     const int s = h & 1;
-    const int4 P = plane_s[h];
+    const int4 P = Pn;
+    Pn = plane_s[h + 1];
     mbar_wait(bar + s, (h >> 1) & 1);
     const double2 *tqh = tq_s + (size_t)s * pcap - P.x;
     const uint32_t *infoh = info_s + (size_t)s * pcap - P.x;
@@ -249,11 +253,15 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
 
 // ---- host side: variant table ---------------------------------------------------------------------------------------
 typedef void (*sweep_fn)(const SweepArgs, const OctTab *);
+constexpr int kMaxGR = 24;  // registers: 2*G*R hold the results of a hyperplane; larger products spill
 
 template <int G>
 sweep_fn pick_r(int r, bool uniform) {
-#define NB_CASE(RR) \
-  case RR: return uniform ? sweep_structured_kernel<G, RR, true> : sweep_structured_kernel<G, RR, false>;
+#define NB_CASE(RR)                                                                                         \
+  case RR:                                                                                                  \
+    if constexpr (G * RR <= kMaxGR / 2) { if (!uniform) return sweep_structured_kernel<G, RR, false>; }          \
+    if constexpr (G * RR <= kMaxGR) { if (uniform) return sweep_structured_kernel<G, RR, true>; }                 \
+    break;
   switch (r) {
     NB_CASE(1)
     NB_CASE(2)
@@ -262,6 +270,8 @@ sweep_fn pick_r(int r, bool uniform) {
     NB_CASE(5)
     NB_CASE(6)
     NB_CASE(8)
+    NB_CASE(10)
+    NB_CASE(12)
   }
 #undef NB_CASE
   return nullptr;
@@ -275,7 +285,8 @@ sweep_fn pick(int g, int r, bool uniform) {
   }
   return nullptr;
 }
-const int kR[7] = {1, 2, 3, 4, 5, 6, 8};
+const int kR[9] = {1, 2, 3, 4, 5, 6, 8, 10, 12};
+const int kNR = 9;
 const int kMaxCompute = 480;  // + the DMA warp = 512 threads
 
 }  // namespace
@@ -286,17 +297,17 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
                                int n_sys_min_class) {
   const size_t smem_cap = 227 * 1024;
   if (want_G < 0 || want_G > 4) return nb_fail(h, NANOBTE_E_INVALID, "sweep_G must be 0..4");
-  if (n_pen_max > 8 * kMaxCompute || n_pen_max >= 65535)
+  if (n_pen_max > 12 * kMaxCompute || n_pen_max >= 65535)
     return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section has %d pencils; the sweep kernel supports up to %d", n_pen_max,
-                   8 * kMaxCompute);
+                   12 * kMaxCompute);
   int R = 0, T = 0;
   if (want_threads > 0) {
     T = std::min(kMaxCompute, (want_threads + 31) / 32 * 32);
-    for (int k = 0; k < 7 && !R; ++k)
+    for (int k = 0; k < kNR && !R; ++k)
       if ((long)kR[k] * T >= n_pen_max) R = kR[k];
     if (!R) return nb_fail(h, NANOBTE_E_INVALID, "sweep_threads=%d cannot cover %d pencils", want_threads, n_pen_max);
   } else {
-    for (int k = 0; k < 7 && !R; ++k) {
+    for (int k = 0; k < kNR && !R; ++k) {
       const int tt = ((n_pen_max + kR[k] - 1) / kR[k] + 31) / 32 * 32;
       if (tt <= kMaxCompute) { R = kR[k]; T = tt; }
     }
@@ -310,12 +321,13 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
     const int g = cand[k];
     if (want_G > 0 && g != want_G) continue;
     if (smem_layout(g, sp, pcap, gcap, H).total > smem_cap) continue;
-    if (want_G <= 0 && (g * R > 20 || g > std::max(1, n_sys_min_class))) continue;  // registers: 2*G*R for the results
+    if (g * R > (h->uniform ? kMaxGR : kMaxGR / 2)) continue;  // the non-uniform variant carries 5 more registers per pencil
+    if (want_G <= 0 && g > std::max(1, n_sys_min_class)) continue;
     G = g;
   }
   if (!G) {
-    if (want_G > 0) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "sweep_G=%d needs %u B of shared memory (> %zu)", want_G,
-                                   smem_layout(want_G, sp, pcap, gcap, H).total, smem_cap);
+    if (want_G > 0) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "sweep_G=%d with %d pencils per thread needs %u B of shared memory (cap %zu) and G*R <= %d",
+                                   want_G, R, smem_layout(want_G, sp, pcap, gcap, H).total, smem_cap, kMaxGR);
     return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section of %d pencils needs %u B of shared memory (> %zu)", n_pen_max,
                    smem_layout(1, sp, pcap, gcap, H).total, smem_cap);
   }

@@ -588,7 +588,7 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
   }
   NB_CUDA(h, cudaMallocHost((void **)&h->h_pinned, 64));
   NB_CUDA(h, cudaStreamSynchronize(h->stream));  // host vectors die here
-  rc = nb_launch_boundary(h);  // initial inflow cache: thermalizing constants, zero elsewhere (R12)
+  rc = nb_launch_boundary(h, 1);  // initial inflow cache: thermalizing constants, zero elsewhere (R12)
   if (rc < 0) return rc;
   NB_CUDA(h, cudaStreamSynchronize(h->stream));
   return 0;
