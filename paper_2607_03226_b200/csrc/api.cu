@@ -1,6 +1,7 @@
 // api.cu -- the C-ABI entry points of libnanobte that do not depend on the mesh kind, plus the host-side
 // validation and the upload of the tables both kinds share.  See include/nanobte.h for the contract.
 #include <algorithm>
+#include <cstdlib>
 
 #include "host_util.h"
 
@@ -168,6 +169,49 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
   h->cg_rhs = A.zeros<double>(na);
   h->cg_scal = A.zeros<double>(16);
   h->cg_partial = A.zeros<double>(4 * 2048);
+  // fused CG plan: contiguous chunks of cells, one per CTA; halo = neighbours owned by other CTAs
+  {
+    const int n = (int)na, nf = g.cg_nf;
+    const int threads = 512;
+    int nblk = std::max(1, std::min(h->n_sm, (n + 255) / 256));
+    int chunk = (n + nblk - 1) / nblk;
+    nblk = (n + chunk - 1) / chunk;
+    const int cpt = chunk <= threads ? 1 : chunk <= 2 * threads ? 2 : chunk <= 4 * threads ? 4 : 0;
+    std::vector<int32_t> nloc((size_t)nf * n), hptr(nblk + 1, 0), hidx;
+    int nh_cap = 0;
+    for (int k = 0; k < nblk; ++k) {
+      const int a0 = k * chunk, a1 = std::min(n, a0 + chunk);
+      std::vector<int32_t> halo;
+      for (int i = a0; i < a1; ++i)
+        for (int f = 0; f < nf; ++f) {
+          const int j = g.cg_nbr[(size_t)f * n + i];
+          if (g.cg_coef[(size_t)f * n + i] != 0.0 && (j < a0 || j >= a1)) halo.push_back(j);
+        }
+      std::sort(halo.begin(), halo.end());
+      halo.erase(std::unique(halo.begin(), halo.end()), halo.end());
+      for (int i = a0; i < a1; ++i)
+        for (int f = 0; f < nf; ++f) {
+          const int j = g.cg_nbr[(size_t)f * n + i];
+          int32_t loc = i - a0;  // faces without a neighbour carry coefficient 0 and point at the cell itself
+          if (g.cg_coef[(size_t)f * n + i] != 0.0)
+            loc = (j >= a0 && j < a1) ? j - a0 : chunk + (int32_t)(std::lower_bound(halo.begin(), halo.end(), j) - halo.begin());
+          nloc[(size_t)f * n + i] = loc;
+        }
+      hidx.insert(hidx.end(), halo.begin(), halo.end());
+      hptr[k + 1] = (int32_t)hidx.size();
+      nh_cap = std::max(nh_cap, (int)halo.size());
+    }
+    h->cgf_nblk = nblk; h->cgf_chunk = chunk; h->cgf_cpt = cpt; h->cgf_nh_cap = nh_cap;
+    h->cgf_smem = (3 * (size_t)chunk + 2 * (size_t)nh_cap) * sizeof(double) + (size_t)nh_cap * sizeof(int32_t) + 1024;
+    h->cgf_ok = cpt > 0 && chunk + nh_cap < 65536 && (nf == 3 || nf == 4 || nf == 6) && h->cgf_smem <= 200 * 1024;
+    h->cg_force_generic = std::getenv("NANOBTE_CG_GENERIC") != nullptr;  // test hook: the multi-pass fallback kernel
+    h->cgf_nloc = A.put(nloc);
+    h->cgf_hptr = A.put(hptr);
+    h->cgf_hidx = A.put(hidx);
+    h->cgf_w = A.zeros<double>(2 * na);
+    h->cgf_part = A.zeros<double>((size_t)4 * nblk + 8);
+    h->cgf_bar = A.zeros<unsigned int>(4);
+  }
   h->tagface_ptr = A.put(g.tagface_ptr);
   h->tagface = A.put(g.tagface);
   h->d_tagheat = A.zeros<double>((size_t)std::max(1, c.n_tags));

@@ -120,6 +120,275 @@ __global__ void __launch_bounds__(256) cg_kernel(CgArgs a) {
   if (tid == 0) *a.iters_out = (unsigned long long)it;
 }
 
+// =================================================================================================================
+// Fused variant (the one used whenever the plan built at create fits): one CTA per contiguous chunk of cells, the
+// CTA's slice of every CG vector in registers, the residual of the chunk plus its halo in shared memory, and ONE
+// grid barrier per iteration.
+//   * Single-reduction CG (Chronopoulos & Gear): with s = A p and w = A r kept by recurrence,
+//       beta = g_k / g_{k-1},  alpha = g_k / (d_k - beta g_k / alpha_{k-1}),  g = (r, r),  d = (w, r),
+//       p <- r + beta p,  s <- w + beta s,  x <- x + alpha p,  r <- r - alpha s,  w <- A r
+//     so both dot products of an iteration are reduced together.  Same iterates as textbook CG in exact arithmetic.
+//   * No halo exchange of r: a CTA applies the same two recurrences (s, r) to its halo cells, redundantly and with
+//     bit-identical arithmetic, reading only the owner's published w.  Hence the barrier that completes the
+//     reduction is the only grid-wide synchronisation of an iteration.
+//   * Reductions are fixed trees (per-CTA partials summed in CTA order by every warp): bitwise reproducible and
+//     identical in every CTA, which is what keeps the redundant halo copies consistent.
+// =================================================================================================================
+struct CgfArgs {
+  int32_t n, nf, nblk, chunk, nh_cap, max_iter, B;
+  const int32_t *nloc;
+  const double *coef, *diag, *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
+  const int32_t *cellbf_ptr, *cellbf, *hptr, *hidx;
+  double *x, *w, *part;
+  unsigned int *bar;
+  unsigned long long *iters_out;
+  double beta, rtol;
+};
+
+__device__ __forceinline__ void grid_barrier(unsigned int *bar, unsigned int target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned int v;
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
+    do {
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+    } while (v < target);
+  }
+  __syncthreads();
+}
+
+constexpr int kCgfThreads = 512;
+#ifdef NB_CG_PROFILE
+__device__ unsigned long long nb_cg_prof[8];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define NB_STAMP(k) do { if (blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_ = gtime(); nb_cg_prof[k] += t_ - t_last; t_last = t_; } } while (0)
+#else
+#define NB_STAMP(k) do {} while (0)
+#endif
+
+template <int NF, int CPT>
+__global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
+  extern __shared__ __align__(16) unsigned char cgf_smem[];
+  double *r_loc = reinterpret_cast<double *>(cgf_smem);           // [chunk + nh_cap]
+  double *s_h = r_loc + a.chunk + a.nh_cap;                       // [nh_cap]
+  double *x_s = s_h + a.nh_cap;                                   // [chunk]  solution (kept out of the registers)
+  double *p_s = x_s + a.chunk;                                    // [chunk]  search direction
+  int32_t *hidx_s = reinterpret_cast<int32_t *>(p_s + a.chunk);   // [nh_cap]
+  __shared__ double red[2 * (kCgfThreads / 32)];
+  __shared__ double gd[2];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int k = blockIdx.x, a0 = k * a.chunk, nown = min(a.n, a0 + a.chunk) - a0;
+  const int h0 = a.hptr[k], nh = a.hptr[k + 1] - h0;
+  const int n = a.n;
+  for (int j = tid; j < nh; j += kCgfThreads) {
+    hidx_s[j] = a.hidx[h0 + j];
+    s_h[j] = 0.0;
+  }
+  double cf[CPT][NF], dg[CPT], r[CPT], s[CPT], wv[CPT];
+  uint16_t nl[CPT][NF];  // local indices < 65536 (checked when the plan is built)
+#pragma unroll
+  for (int c = 0; c < CPT; ++c) {
+    const int li = tid + c * kCgfThreads, i = a0 + li;
+    s[c] = wv[c] = r[c] = dg[c] = 0.0;
+    if (li < a.chunk) x_s[li] = p_s[li] = 0.0;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { cf[c][f] = 0.0; nl[c][f] = 0; }
+    if (li < nown) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        cf[c][f] = a.coef[(size_t)f * n + i];
+        nl[c][f] = (uint16_t)a.nloc[(size_t)f * n + i];
+      }
+      dg[c] = a.diag[i];
+      double rhs = a.vol[i] * a.beta * (a.theta_SI[i] - a.theta_prev[i]);   // R14c
+      for (int q = a.cellbf_ptr[i]; q < a.cellbf_ptr[i + 1]; ++q) {         // R14c'
+        const int bf = a.cellbf[q];
+        double F = 0.0;
+        for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
+        rhs += a.bf_area[bf] * F;
+      }
+      r[c] = rhs;
+      r_loc[li] = rhs;
+      a.w[(size_t)n + i] = rhs;  // publish r_0 through the second w buffer
+    }
+  }
+  unsigned int epoch = 1;
+  grid_barrier(a.bar, epoch++ * a.nblk);
+  for (int j = tid; j < nh; j += kCgfThreads) r_loc[a.chunk + j] = __ldcg(a.w + (size_t)n + hidx_s[j]);
+  __syncthreads();
+
+  // w = A r on the chunk, the two partial dot products, publication of w; reads r_loc
+  auto apply_and_reduce = [&](int par_out) {
+    double g = 0.0, d = 0.0;
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+      const int li = tid + c * kCgfThreads;
+      if (li < nown) {
+        double acc = dg[c] * r[c];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) acc -= cf[c][f] * r_loc[nl[c][f]];
+        wv[c] = acc;
+        a.w[(size_t)par_out * n + a0 + li] = acc;
+        g += r[c] * r[c];
+        d += acc * r[c];
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      g += __shfl_xor_sync(0xffffffffu, g, o);
+      d += __shfl_xor_sync(0xffffffffu, d, o);
+    }
+    if (lane == 0) { red[2 * wid] = g; red[2 * wid + 1] = d; }
+    __syncthreads();
+    if (wid == 0) {
+      double G = lane < kCgfThreads / 32 ? red[2 * lane] : 0.0, D = lane < kCgfThreads / 32 ? red[2 * lane + 1] : 0.0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        G += __shfl_xor_sync(0xffffffffu, G, o);
+        D += __shfl_xor_sync(0xffffffffu, D, o);
+      }
+      if (lane == 0) *reinterpret_cast<double2 *>(a.part + ((size_t)par_out * a.nblk + k) * 2) = make_double2(G, D);
+    }
+  };
+  apply_and_reduce(0);
+  grid_barrier(a.bar, epoch++ * a.nblk);
+
+  double g_prev = 1.0, alpha_prev = 1.0, stop2 = 0.0;
+  int it = 0;
+#ifdef NB_CG_PROFILE
+  unsigned long long t_last = gtime();
+#endif
+  for (;; ++it) {
+    const int par = it & 1;
+    // Issue every global load of the iteration first (per-CTA partials and the owners' w of the first halo batch):
+    // one L2 round trip after the barrier instead of two.
+    const double *pp = a.part + (size_t)par * a.nblk * 2;
+    const double *wp = a.w + (size_t)par * n;
+    constexpr int NP = 5, HB = 10;
+    double2 pv[NP];
+    if (wid == 0) {  // one warp per CTA reads the partials: 2368 warps hammering the same 19 lines is an L2 hot spot
+#pragma unroll
+      for (int u = 0; u < NP; ++u) {
+        const int q = lane + 32 * u;
+        pv[u] = q < a.nblk ? __ldcg(reinterpret_cast<const double2 *>(pp) + q) : make_double2(0.0, 0.0);
+      }
+    }
+    double wh[HB];
+#pragma unroll
+    for (int q = 0; q < HB; ++q) {
+      const int j = tid + q * kCgfThreads;
+      wh[q] = j < nh ? __ldcg(wp + hidx_s[j]) : 0.0;
+    }
+    // fixed summation order -> the same bits in every CTA
+    if (wid == 0) {
+      double g = 0.0, d = 0.0;
+#pragma unroll
+      for (int u = 0; u < NP; ++u) {
+        g += pv[u].x;
+        d += pv[u].y;
+      }
+      for (int q = lane + 32 * NP; q < a.nblk; q += 32) {  // more than 160 CTAs: not on B200
+        const double2 v = __ldcg(reinterpret_cast<const double2 *>(pp) + q);
+        g += v.x;
+        d += v.y;
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        g += __shfl_xor_sync(0xffffffffu, g, o);
+        d += __shfl_xor_sync(0xffffffffu, d, o);
+      }
+      if (lane == 0) { gd[0] = g; gd[1] = d; }
+    }
+    __syncthreads();
+    const double g = gd[0], d = gd[1];
+    if (it == 0) stop2 = a.rtol * a.rtol * g;
+    if (!(g > stop2) || it >= a.max_iter) break;
+    NB_STAMP(0);
+    const double bet = it ? g / g_prev : 0.0;
+    const double alpha = it ? g / (d - bet * g / alpha_prev) : g / d;
+    // halo copies: same recurrences as the owner, owner's w
+#pragma unroll
+    for (int q = 0; q < HB; ++q) {
+      const int j = tid + q * kCgfThreads;
+      if (j < nh) {
+        const double sh = fma(bet, s_h[j], wh[q]);
+        s_h[j] = sh;
+        r_loc[a.chunk + j] = fma(-alpha, sh, r_loc[a.chunk + j]);
+      }
+    }
+    for (int j = tid + HB * kCgfThreads; j < nh; j += kCgfThreads) {  // very large halos: one more round trip each
+      const double sh = fma(bet, s_h[j], __ldcg(wp + hidx_s[j]));
+      s_h[j] = sh;
+      r_loc[a.chunk + j] = fma(-alpha, sh, r_loc[a.chunk + j]);
+    }
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+      const int li = tid + c * kCgfThreads;
+      if (li < nown) {
+        const double pc = fma(bet, p_s[li], r[c]);
+        p_s[li] = pc;
+        s[c] = fma(bet, s[c], wv[c]);
+        x_s[li] = fma(alpha, pc, x_s[li]);
+        r[c] = fma(-alpha, s[c], r[c]);
+        r_loc[li] = r[c];
+      }
+    }
+    __syncthreads();
+    NB_STAMP(1);
+    apply_and_reduce(par ^ 1);
+    NB_STAMP(2);
+    grid_barrier(a.bar, epoch++ * a.nblk);
+    NB_STAMP(3);
+    g_prev = g;
+    alpha_prev = alpha;
+  }
+#pragma unroll
+  for (int c = 0; c < CPT; ++c) {
+    const int li = tid + c * kCgfThreads;
+    if (li < nown) a.x[a0 + li] = x_s[li];
+  }
+  if (k == 0 && tid == 0) *a.iters_out = (unsigned long long)it;
+}
+
+typedef void (*cgf_fn)(CgfArgs);
+template <int NF>
+static cgf_fn cgf_pick_cpt(int cpt) {
+  switch (cpt) {
+    case 1: return cg_fused_kernel<NF, 1>;
+    case 2: return cg_fused_kernel<NF, 2>;
+    case 4: return cg_fused_kernel<NF, 4>;
+  }
+  return nullptr;
+}
+static cgf_fn cgf_pick(int nf, int cpt) {
+  switch (nf) {
+    case 3: return cgf_pick_cpt<3>(cpt);
+    case 4: return cgf_pick_cpt<4>(cpt);
+    case 6: return cgf_pick_cpt<6>(cpt);
+  }
+  return nullptr;
+}
+
+static int cg_solve_fused(nanobte_solver *h) {
+  cgf_fn fn = cgf_pick(h->cg_nf, h->cgf_cpt);
+  if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "internal: no fused CG variant for nf=%d cpt=%d", h->cg_nf, h->cgf_cpt);
+  CgfArgs a;
+  a.n = h->n_act; a.nf = h->cg_nf; a.nblk = h->cgf_nblk; a.chunk = h->cgf_chunk; a.nh_cap = h->cgf_nh_cap;
+  a.max_iter = h->cg_max_iter; a.B = h->B;
+  a.nloc = h->cgf_nloc; a.coef = h->cg_coef; a.diag = h->cg_diag; a.vol = h->vol;
+  a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev; a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area;
+  a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf; a.hptr = h->cgf_hptr; a.hidx = h->cgf_hidx;
+  a.x = h->cg_x; a.w = h->cgf_w; a.part = h->cgf_part; a.bar = h->cgf_bar;
+  a.iters_out = h->d_maxdT + 1;
+  a.beta = h->beta; a.rtol = h->cg_rtol;
+  NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->cgf_smem));
+  NB_CUDA(h, cudaMemsetAsync(h->cgf_bar, 0, sizeof(unsigned int), h->stream));
+  void *args[] = {&a};
+  NB_CUDA(h, cudaLaunchCooperativeKernel((void *)fn, dim3(h->cgf_nblk), dim3(kCgfThreads), args, h->cgf_smem, h->stream));
+  h->launches++;
+  return 0;
+}
+
 int nb_cg_blocks(nanobte_solver *h) {
   int per_sm = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cg_kernel, 256, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
@@ -129,6 +398,8 @@ int nb_cg_blocks(nanobte_solver *h) {
 }
 
 int nb_cg_solve(nanobte_solver *h, int *iters) {
+  if (iters) *iters = -1;  // read back by the caller together with max|dT|
+  if (h->cgf_ok && !h->cg_force_generic) return cg_solve_fused(h);
   CgArgs a;
   a.n = h->n_act; a.nf = h->cg_nf; a.max_iter = h->cg_max_iter; a.B = h->B;
   a.nbr = h->cg_nbr; a.coef = h->cg_coef; a.diag = h->cg_diag;
@@ -144,3 +415,15 @@ int nb_cg_solve(nanobte_solver *h, int *iters) {
   if (iters) *iters = -1;  // read back by the caller together with max|dT|
   return 0;
 }
+
+#ifdef NB_CG_PROFILE
+extern "C" int nanobte_debug_cg_prof(unsigned long long *out, int reset) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, nb_cg_prof, sizeof(nb_cg_prof));
+  if (reset) {
+    unsigned long long z[8] = {0};
+    cudaMemcpyToSymbol(nb_cg_prof, z, sizeof(z));
+  }
+  return 0;
+}
+#endif

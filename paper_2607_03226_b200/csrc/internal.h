@@ -130,6 +130,16 @@ struct nanobte_solver {
   double *cg_x = nullptr, *cg_r = nullptr, *cg_p0 = nullptr, *cg_p1 = nullptr, *cg_rhs = nullptr, *cg_scal = nullptr;
   double *cg_partial = nullptr;
   int cg_blocks = 0;
+  // fused CG (cg.cu, cg_fused_kernel): cells cut into one contiguous chunk per CTA, vectors on chip
+  bool cgf_ok = false, cg_force_generic = false;
+  int cgf_nblk = 0, cgf_chunk = 0, cgf_cpt = 0, cgf_nh_cap = 0;
+  size_t cgf_smem = 0;
+  const int32_t *cgf_nloc = nullptr;   // [nf][n] index of the neighbour inside its owner CTA's local vector
+  const int32_t *cgf_hptr = nullptr;   // [nblk+1] halo lists
+  const int32_t *cgf_hidx = nullptr;   // global cell index of every halo entry
+  double *cgf_w = nullptr;             // [2][n]   A r, published every iteration (double buffered)
+  double *cgf_part = nullptr;          // [2][nblk][2] per-CTA partial dot products (double buffered)
+  unsigned int *cgf_bar = nullptr;     // grid barrier counter
 
   // boundary heat
   const int32_t *tagface_ptr = nullptr, *tagface = nullptr;  // CSR faces per tag
