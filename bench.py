@@ -181,9 +181,8 @@ def run_oracle(pr, mode, steps, warmup, n_bands):
 # ---------------------------------------------------------------------------------------------------------------------
 def main():
     args = parse_args()
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2607_03226_b200 import replicas
+    rank, world, local = replicas.env_rank()
     pr = make_problem(args.workload)
     mode = args.mode or pr["mode"]
 
@@ -207,10 +206,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: libnanobte has no CPU fallback")
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dist = replicas.init("nccl", torch.device("cuda", local))
     from paper_2607_03226_b200 import build as nb_build
     from paper_2607_03226_b200 import workloads as wl
     if rank == 0:
@@ -245,10 +241,7 @@ def main():
             ev[3].record()
 
     def barrier():
-        torch.cuda.synchronize()
-        if dist:
-            dist.barrier()
-            torch.cuda.synchronize()
+        replicas.barrier(dist, torch.cuda.synchronize)
 
     # ---- device-resident arm -------------------------------------------------------------------------------------
     for _ in range(args.warmup):
@@ -267,12 +260,9 @@ def main():
     sweep_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     update_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
     cg_ms = float(np.mean([e[2].elapsed_time(e[3]) for e in evs])) if synthetic else 0.0
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if dist:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = replicas.max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * upd / (ms_per_step * 1e-3)
+    value = replicas.whole_job_rate(upd, world, ms_per_step * 1e-3)
 
     # ---- end-to-end arm: host buffers through the C ABI, copies inside the timed region ------------------------------
     T_host = torch.empty(g.n_cells, dtype=torch.float64).pin_memory()
@@ -298,11 +288,8 @@ def main():
         e2e_step()
     barrier()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if dist:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_s = float(t.item())
-    e2e = {"value": world * upd / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(g.n_cells * 8),
+    e2e_s = replicas.max_over_ranks(e2e_s, dist, "cuda")
+    e2e = {"value": replicas.whole_job_rate(upd, world, e2e_s), "unit": UNIT, "h2d_bytes_per_step": int(g.n_cells * 8),
            "d2h_bytes_per_step": int(g.n_cells * 8 + 16), "ms_per_step": e2e_s * 1e3}
 
     # ---- roofline of the dominant kernel (the sweep): 8 algorithmic bytes per update ----------

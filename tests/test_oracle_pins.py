@@ -395,3 +395,20 @@ def test_error_paths():
     with pytest.raises(OracleError) as e:
         r.solve(1e-9, 5, "synthetic")
     assert e.value.code == -9
+
+
+def test_golden_config0_file_matches_oracle_and_fixed_point():
+    """tests/golden/config0_oracle.txt is what the committed script wrote from oracle/ only, and is itself within the
+    stopping error of the dense fixed point (P2): a stored value that both the oracle and the GPU tests answer to."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config0_oracle.txt")
+    lines = open(path).read().splitlines()
+    iters = int([ln for ln in lines if ln.startswith("# iterations")][0].split()[-1])
+    T = np.array([[float(x) for x in ln.split()] for ln in lines if not ln.startswith("#")]).reshape(-1)
+    pr = wl.config_gray_square()
+    r = RefSolver(pr)
+    res = r.solve(pr["tol"], pr["max_iter"])
+    assert res["iters"] == iters == 35
+    assert np.abs(r.get_T(0) - T).max() < 1e-12
+    _, th_fp = fvgeom.Geom(pr).fixed_point()
+    assert np.abs((T - 300.0) - th_fp).max() < 5e-10
