@@ -27,7 +27,8 @@
 // hyperplane, each plane's slice [in_lo(h), in_lo(h+1)) padded to an even length for the same reason.
 struct OctTab {
   const uint2 *pen;          // [n_pen]   .x = m, .y = pencil index of the v-upwind pencil | w-upwind pencil << 16 (n_pen = none)
-  const int4 *plane;         // [H+1]     {lo, cnt, start, in_lo}; entry H is the sentinel {0, 0, n_pos, n_in}
+  const int4 *plane;         // [H+1][2]  {wall lo, wall cnt, interior lo, interior cnt}, {start, in_lo, 0, 0}; entry H is the
+                             //           sentinel {0,0,0,0}, {n_pos, n_in, 0, 0}
   const uint32_t *cellinfo;  // [n_pos+16] bit0..2: u/v/w upwind value is a boundary inflow, bit3: hole, bits 4..: first inflow idx - in_lo(h)
   const double2 *tq;         // [n_pos+16] (theta, Qdot) in sweep order
   const double *rhu;         // [nu]      1/h_u in primed coordinates (non-uniform spacing only)
@@ -102,6 +103,10 @@ struct nanobte_solver {
   int32_t cls_nin[NB_MAX_CLASSES] = {0}, cls_ndirs[NB_MAX_CLASSES] = {0};
   const int32_t *cls_dirs = nullptr;                     // [n_cls][max_cls_dirs]
   int max_cls_dirs = 0;
+  const int32_t *cls_outbf[NB_MAX_CLASSES] = {nullptr}, *cls_outpos[NB_MAX_CLASSES] = {nullptr};  // outgoing wall cells per class
+  const uint8_t *cls_outord[NB_MAX_CLASSES] = {nullptr}, *bf_nord = nullptr;
+  int32_t cls_nout[NB_MAX_CLASSES] = {0};
+  double *g_partial = nullptr;                            // [4][n_bf][B] per-class shares of gnum
   const int32_t *refl_faces = nullptr, *therm_faces = nullptr;
   int n_refl = 0, n_therm = 0;
 

@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(256) boundary_kernel(BoundaryRun R) {
   }
 }
 
-static int launch_closure_G(nanobte_solver *h, const int32_t *faces, int n_faces);
+static int launch_closure_G(nanobte_solver *h, const int32_t *faces, int n_faces, int therm);
 static int launch_closure_inflow(nanobte_solver *h, int init);
 
 int nb_launch_boundary(nanobte_solver *h, int init) {
@@ -92,7 +92,7 @@ int nb_launch_boundary(nanobte_solver *h, int init) {
     h->therm_stale = true;
     if (init) return launch_closure_inflow(h, 1);
     if (h->n_refl == 0) return 0;
-    int rc = launch_closure_G(h, h->refl_faces, h->n_refl);
+    int rc = launch_closure_G(h, h->refl_faces, h->n_refl, 0);
     if (rc < 0) return rc;
     return launch_closure_inflow(h, 0);
   }
@@ -110,10 +110,12 @@ int nb_launch_boundary(nanobte_solver *h, int init) {
 
 // =================================================================================================================
 // (a3) structured grids: the closures as two kernels whose global accesses follow the memory layout.
-//   closure_G_kernel      one warp per (boundary face, chunk of bands), lanes over the OUTGOING directions: gathers
-//                         eps at the wall cell (one 8-byte value per (direction, band) row -- inherently one sector
-//                         each), G_bf (R7) and the face flux (O8).  The incoming half of the flux needs no second
-//                         gather: the inflow the last sweep consumed was C_b dT_w/W (thermalizing) or built from
+//   closure_gsum_kernel   one thread per (octant class, wall cell that is outgoing for the class, chunk of bands): the
+//                         class's share of gnum = sum_out w (s.n) eps.  Lanes run over wall cells in position
+//                         order, which are contiguous in every e row (a hyperplane stores its wall cells first).
+//   closure_gcomb_kernel  G_bf (R7) from the class partials in fixed order, and the face flux (O8).  The incoming
+//                         half of the flux needs no gather: the inflow the last sweep consumed was C_b dT_w/W
+//                         (thermalizing) or built from
 //                         eps^{n-1} with G^{n-1}, and sum_in w (s.n) inflow = -den * G^{n-1} for diffuse, specular and
 //                         mixed walls alike because the quadrature is mirror symmetric about the wall (weights
 //                         checked at create), so  F_bf = v_b (gnum^n - den * X),  X = C_b dT_w/W  or  G^{n-1}_bf.
@@ -123,64 +125,75 @@ int nb_launch_boundary(nanobte_solver *h, int init) {
 // Thermalizing faces never change their inflow (written once at create) and their G / flux are diagnostics only:
 // they are skipped per iteration and evaluated on demand (get_G, get_boundary_heat).
 // =================================================================================================================
-struct ClosureArgs {
+struct GsumArgs {
   BoundaryArgs a;
-  double W;
-  const int32_t *faces;     // face list this launch covers
-  int32_t n_faces, bands_per_chunk;
+  const int32_t *out_bf[NB_MAX_CLASSES];   // per class: boundary faces that are OUTGOING for the class, in position order
+  const int32_t *out_pos[NB_MAX_CLASSES];  //            position of the wall cell in the class's e rows
+  const uint8_t *out_ord[NB_MAX_CLASSES];  //            which of the face's outgoing classes this is (0..3)
+  int32_t cls_nout[NB_MAX_CLASSES], cls_ndirs[NB_MAX_CLASSES];
+  const int32_t *cls_dirs;                 // [n_cls][max_dirs]
+  int32_t max_dirs, bands_per_chunk, therm;  // therm: 1 = thermalizing faces only, 0 = all the others
+  double *partial;                         // [4][n_bf][B]
 };
 
-template <int K>  // K = ceil(D / 32) directions per lane
-__global__ void __launch_bounds__(256) closure_G_kernel(ClosureArgs R) {
+// gnum partials: sum over the directions of ONE class of w (s.n) eps at the wall cell.  Lanes run over the wall cells
+// of a class in position order -- contiguous in every e row because a hyperplane stores its wall cells first.
+constexpr int kGsumUB = 6;
+__global__ void __launch_bounds__(128) closure_gsum_kernel(GsumArgs R) {
   const BoundaryArgs &a = R.a;
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  const int fi = blockIdx.x * (blockDim.x >> 5) + wib;
-  if (fi >= R.n_faces) return;
-  const int bf = R.faces[fi];
-  const size_t row = (size_t)bf * a.D;
-  const double *src[K];
-  double wsn[K];
+  const int c = blockIdx.y;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= R.cls_nout[c]) return;
+  const int bf = R.out_bf[c][j];
+  if ((a.bf_type[bf] == NANOBTE_THERMALIZING) != (R.therm != 0)) return;
+  const int b_lo = blockIdx.z * R.bands_per_chunk;
+  const int nb = min(a.B - b_lo, R.bands_per_chunk);
+  const double *src0 = a.e + R.out_pos[c][j] + (int64_t)b_lo * a.e_stride;
+  const double *sn = a.bf_sn + (size_t)bf * a.D;
+  for (int b0 = 0; b0 < nb; b0 += kGsumUB) {
+    double acc[kGsumUB];
 #pragma unroll
-  for (int k = 0; k < K; ++k) {
-    const int d = lane + 32 * k;
-    wsn[k] = 0.0;
-    src[k] = a.e;
-    if (d < a.D) {
-      const double sn = a.bf_sn[row + d];
-      if (sn > 0.0) {
-        wsn[k] = a.w[d] * sn;
-        src[k] = a.e + (int64_t)a.dir_row0[d] * a.e_stride + a.bf_opos[row + d];
-      }
+    for (int u = 0; u < kGsumUB; ++u) acc[u] = 0.0;
+    for (int kd = 0; kd < R.cls_ndirs[c]; ++kd) {
+      const int d = R.cls_dirs[c * R.max_dirs + kd];
+      const double wsn = a.w[d] * sn[d];
+      const double *src = src0 + ((int64_t)a.dir_row0[d] + b0) * a.e_stride;
+      double v[kGsumUB];
+#pragma unroll
+      for (int u = 0; u < kGsumUB; ++u) v[u] = __ldcs(src + (int64_t)min(u, nb - 1 - b0) * a.e_stride);
+#pragma unroll
+      for (int u = 0; u < kGsumUB; ++u) acc[u] += wsn * v[u];
     }
+    double *dst = R.partial + ((size_t)R.out_ord[c][j] * a.n_bf + bf) * a.B + b_lo + b0;
+#pragma unroll
+    for (int u = 0; u < kGsumUB; ++u)
+      if (b0 + u < nb) dst[u] = acc[u];
   }
-  const double den = a.bf_den[bf], dTw = a.bf_eps_w[bf];
-  const bool therm = a.bf_type[bf] == NANOBTE_THERMALIZING;
-  const int b_lo = blockIdx.y * R.bands_per_chunk, b_hi = min(a.B, b_lo + R.bands_per_chunk);
-  constexpr int UB = 6;
-  for (int b0 = b_lo; b0 < b_hi; b0 += UB) {
-    double acc[UB];
-#pragma unroll
-    for (int j = 0; j < UB; ++j) {
-      acc[j] = 0.0;
-      const int b = min(b0 + j, b_hi - 1);
-#pragma unroll
-      for (int k = 0; k < K; ++k)
-        if (wsn[k] != 0.0) acc[j] += wsn[k] * __ldcs(src[k] + (int64_t)b * a.e_stride);
-    }
-#pragma unroll
-    for (int j = 0; j < UB; ++j) acc[j] = warp_sum(acc[j]);
-#pragma unroll
-    for (int j = 0; j < UB; ++j) {
-      const int b = b0 + j;
-      if (lane == j && b < b_hi) {
-        const size_t o = (size_t)bf * a.B + b;
-        const double Gold = a.G[o];
-        a.G[o] = den > 0.0 ? acc[j] / den : 0.0;
-        const double X = therm ? a.C[b] * dTw / R.W : Gold;
-        a.faceflux[o] = a.v[b] * (acc[j] - den * X);
-      }
-    }
-  }
+}
+
+struct GcombArgs {
+  BoundaryArgs a;
+  double W;
+  const int32_t *faces;      // face list this launch covers
+  const uint8_t *nord;       // [n_bf] number of outgoing classes of the face
+  const double *partial;
+  int32_t n_faces;
+};
+
+// G_bf = (sum of the class partials, fixed order) / den (R7); face flux (O8) with the lagged inflow in closed form.
+__global__ void __launch_bounds__(256) closure_gcomb_kernel(GcombArgs R) {
+  const BoundaryArgs &a = R.a;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (int64_t)R.n_faces * a.B) return;
+  const int bf = R.faces[i / a.B], b = (int)(i % a.B);
+  double gnum = 0.0;
+  for (int o = 0; o < R.nord[bf]; ++o) gnum += R.partial[((size_t)o * a.n_bf + bf) * a.B + b];
+  const double den = a.bf_den[bf];
+  const size_t k = (size_t)bf * a.B + b;
+  const double Gold = a.G[k];
+  a.G[k] = den > 0.0 ? gnum / den : 0.0;
+  const double X = a.bf_type[bf] == NANOBTE_THERMALIZING ? a.C[b] * a.bf_eps_w[bf] / R.W : Gold;
+  a.faceflux[k] = a.v[b] * (gnum - den * X);
 }
 
 struct InflowArgs {
@@ -230,21 +243,25 @@ __global__ void __launch_bounds__(128) closure_inflow_kernel(InflowArgs R) {
   }
 }
 
-static int launch_closure_G(nanobte_solver *h, const int32_t *faces, int n_faces) {
+static int launch_closure_G(nanobte_solver *h, const int32_t *faces, int n_faces, int therm) {
   if (n_faces == 0) return 0;
-  ClosureArgs R;
-  R.a = h->bd; R.W = h->W; R.faces = faces; R.n_faces = n_faces;
-  const int chunks = std::max(1, std::min((h->B + 5) / 6, (4 * h->n_sm * 8 + n_faces - 1) / n_faces));
-  R.bands_per_chunk = ((h->B + chunks - 1) / chunks + 5) / 6 * 6;
-  dim3 grid((n_faces + 7) / 8, (h->B + R.bands_per_chunk - 1) / R.bands_per_chunk);
-  const int K = (h->D + 31) / 32;
-  switch (K) {
-    case 1: closure_G_kernel<1><<<grid, 256, 0, h->stream>>>(R); break;
-    case 2: closure_G_kernel<2><<<grid, 256, 0, h->stream>>>(R); break;
-    case 3: closure_G_kernel<3><<<grid, 256, 0, h->stream>>>(R); break;
-    case 4: closure_G_kernel<4><<<grid, 256, 0, h->stream>>>(R); break;
-    default: return nb_fail(h, NANOBTE_E_UNSUPPORTED, "internal: closure_G_kernel supports up to 128 directions");
+  GsumArgs S;
+  S.a = h->bd; S.cls_dirs = h->cls_dirs; S.max_dirs = h->max_cls_dirs; S.therm = therm; S.partial = h->g_partial;
+  int nout_max = 0;
+  for (int c = 0; c < NB_MAX_CLASSES; ++c) {
+    S.out_bf[c] = h->cls_outbf[c]; S.out_pos[c] = h->cls_outpos[c]; S.out_ord[c] = h->cls_outord[c];
+    S.cls_nout[c] = h->cls_nout[c]; S.cls_ndirs[c] = h->cls_ndirs[c];
+    nout_max = std::max(nout_max, h->cls_nout[c]);
   }
+  S.bands_per_chunk = kGsumUB;
+  dim3 grid((nout_max + 127) / 128, h->n_cls, (h->B + kGsumUB - 1) / kGsumUB);
+  closure_gsum_kernel<<<grid, 128, 0, h->stream>>>(S);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  GcombArgs R;
+  R.a = h->bd; R.W = h->W; R.faces = faces; R.nord = h->bf_nord; R.partial = h->g_partial; R.n_faces = n_faces;
+  const int64_t n = (int64_t)n_faces * h->B;
+  closure_gcomb_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(R);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
   return 0;
@@ -271,7 +288,7 @@ static int launch_closure_inflow(nanobte_solver *h, int init) {
 // Diagnostics of the thermalizing faces (G, face flux) from the current eps; called by the getters that expose them.
 int nb_refresh_thermalizing(nanobte_solver *h) {
   if (!h->split_closures || !h->therm_stale) return 0;
-  int rc = launch_closure_G(h, h->therm_faces, h->n_therm);
+  int rc = launch_closure_G(h, h->therm_faces, h->n_therm, 1);
   if (rc < 0) return rc;
   h->therm_stale = false;
   return 0;

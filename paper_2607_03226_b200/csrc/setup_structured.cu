@@ -31,6 +31,8 @@ struct OctHost {
   std::vector<int32_t> in_bf;      // inflow list: boundary face ids in consumption order
   std::vector<int32_t> bf_slot;    // [n_bf] index of the face in in_bf, or -1
   std::vector<int32_t> cell2pos;   // [n_cells]
+  std::vector<int32_t> out_bf, out_pos;  // faces that are outgoing for the class and their wall cell's position, position order
+  std::vector<uint8_t> out_ord;    // rank of the class among the face's outgoing classes
   int n_pen = 0, H = 0, n_pos = 0, p_max = 0, g_max = 0;
 };
 
@@ -159,25 +161,56 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   for (int a = 0; a < dim; ++a)
     for (double v : g.hsz[a]) uniform &= (v == g.hsz[a][0]);
 
+  // ---- pencils (physical coordinates): which exist, which touch a +-v / +-w boundary face ---------------------------------------
+  std::vector<uint8_t> pen_any((size_t)nv * nw, 0), pen_wall((size_t)nv * nw, 0);
+  for (int w = 0; w < nw; ++w)
+    for (int v = 0; v < nv; ++v)
+      for (int u = 0; u < nu; ++u) {
+        int c[3]; c[pa] = u; c[va] = v; c[wa] = w;
+        if (!g.act[g.cell(c[0], c[1], c[2])]) continue;
+        pen_any[(size_t)v + (size_t)nv * w] = 1;
+        for (int axis : {va, wa}) {
+          if (axis == wa && !has_w) continue;
+          for (int sgn = -1; sgn <= 1; sgn += 2) {
+            int nb[3] = {c[0], c[1], c[2]};
+            nb[axis] += sgn;
+            if (!(g.inside(nb) && g.act[g.cell(nb[0], nb[1], nb[2])])) pen_wall[(size_t)v + (size_t)nv * w] = 1;
+          }
+        }
+      }
+
   // ---- per class: pencils, hyperplanes, cell info, inflow lists ----------------------------------------------------------
   int n_pen_max = 0, n_pos_max = 0, p_max = 0, g_max = 0;
+  std::vector<uint8_t> bf_nord(nbf, 0);  // outgoing classes per face (4 in 3-D, 2 in 2-D)
   for (int ci = 0; ci < ncls; ++ci) {
     OctHost &o = oct[ci];
     auto phys = [&](int axis, int x) { return o.sign[axis] > 0 ? x : g.n[axis] - 1 - x; };
     auto cell_of = [&](int u, int v, int w) { int c[3]; c[pa] = phys(pa, u); c[va] = phys(va, v); c[wa] = phys(wa, w); return g.cell(c[0], c[1], c[2]); };
-    std::vector<int> pen_v, pen_w, first_of_m(nv + nw, 0), pen_of((size_t)nv * nw, -1);
-    for (int mm = 0; mm <= nv + nw - 2; ++mm) {
-      if (pen_v.size() & 1) { pen_v.push_back(-1); pen_w.push_back(-1); }  // padding slot: keeps every diagonal's first slot even
-      first_of_m[mm] = (int)pen_v.size();
-      for (int w = std::max(0, mm - nv + 1); w <= std::min(nw - 1, mm); ++w) {
-        const int v = mm - w;
-        bool any = false;
-        for (int u = 0; u < nu && !any; ++u) any = g.act[cell_of(u, v, w)];
-        if (any) { pen_of[(size_t)v + (size_t)nv * w] = (int)pen_v.size(); pen_v.push_back(v); pen_w.push_back(w); }
+    // Slot order: wall pencils first (those with a boundary face on a +-v or +-w side somewhere along the pencil),
+    // then interior pencils; each group sorted by (m = v'+w', w') with every diagonal padded to an even slot count.
+    // A hyperplane's active slots are then two contiguous ranges, one per group, and its wall cells are contiguous
+    // in every e row -- which is what lets the closure kernels read the walls with coalesced loads.
+    std::vector<int> pen_v, pen_w, pen_of((size_t)nv * nw, -1);
+    std::vector<int> first_of_m[2] = {std::vector<int>(nv + nw, 0), std::vector<int>(nv + nw, 0)};
+    int n_wall_slots = 0;
+    for (int grp = 0; grp < 2; ++grp) {
+      for (int mm = 0; mm <= nv + nw - 2; ++mm) {
+        if (pen_v.size() & 1) { pen_v.push_back(-1); pen_w.push_back(-1); }  // padding slot: keeps every diagonal's first slot even
+        first_of_m[grp][mm] = (int)pen_v.size();
+        for (int w = std::max(0, mm - nv + 1); w <= std::min(nw - 1, mm); ++w) {
+          const int v = mm - w;
+          const size_t pv = (size_t)phys(va, v) + (size_t)nv * phys(wa, w);
+          if (!pen_any[pv] || (pen_wall[pv] ? 0 : 1) != grp) continue;
+          pen_of[(size_t)v + (size_t)nv * w] = (int)pen_v.size();
+          pen_v.push_back(v);
+          pen_w.push_back(w);
+        }
       }
+      if (pen_v.size() & 1) { pen_v.push_back(-1); pen_w.push_back(-1); }
+      first_of_m[grp][nv + nw - 1] = (int)pen_v.size();
+      if (grp == 0) n_wall_slots = (int)pen_v.size();
     }
-    if (pen_v.size() & 1) { pen_v.push_back(-1); pen_w.push_back(-1); }
-    first_of_m[nv + nw - 1] = (int)pen_v.size();
+    (void)n_wall_slots;
     o.n_pen = (int)pen_v.size();
     o.pen.resize(o.n_pen);
     o.pen_rh.resize(o.n_pen);
@@ -195,17 +228,20 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       o.pen_rh[p] = make_double2(1.0 / g.hsz[va][phys(va, v)], has_w ? 1.0 / g.hsz[wa][phys(wa, w)] : 0.0);
     }
     o.H = H;
-    o.plane.resize(H + 1);
-    std::vector<int> lo(H), hi(H), start(H);
+    o.plane.resize(2 * (size_t)(H + 1));
+    std::vector<int> wlo(H), wcnt(H), ilo(H), icnt(H), start(H);
     int base = 0;
     for (int hh = 0; hh < H; ++hh) {
       const int mlo = std::max(0, hh - nu + 1), mhi = std::min(hh, nv + nw - 2);
-      lo[hh] = first_of_m[mlo];
-      hi[hh] = mhi >= mlo ? first_of_m[mhi + 1] : lo[hh];
+      wlo[hh] = first_of_m[0][mlo];
+      wcnt[hh] = mhi >= mlo ? first_of_m[0][mhi + 1] - wlo[hh] : 0;
+      ilo[hh] = first_of_m[1][mlo];
+      icnt[hh] = mhi >= mlo ? first_of_m[1][mhi + 1] - ilo[hh] : 0;
       start[hh] = (base + 15) / 16 * 16;  // 128-byte aligned e segments, 16-byte aligned table segments (bulk TMA)
-      base = start[hh] + (hi[hh] - lo[hh]);
-      o.plane[hh] = make_int4(lo[hh], hi[hh] - lo[hh], start[hh], 0);
-      o.p_max = std::max(o.p_max, hi[hh] - lo[hh]);
+      base = start[hh] + wcnt[hh] + icnt[hh];
+      o.plane[2 * hh] = make_int4(wlo[hh], wcnt[hh], ilo[hh], icnt[hh]);
+      o.plane[2 * hh + 1] = make_int4(start[hh], 0, 0, 0);
+      o.p_max = std::max(o.p_max, wcnt[hh] + icnt[hh]);
     }
     o.n_pos = base;
     o.cellinfo.assign((size_t)o.n_pos + 16, 8u);
@@ -216,11 +252,12 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     for (int hh = 0; hh < H; ++hh) {
       if (o.in_bf.size() & 1) o.in_bf.push_back(-1);  // every hyperplane's inflow slice starts on an even index
       const uint32_t in_lo = (uint32_t)o.in_bf.size();
-      o.plane[hh].w = (int)in_lo;
-      for (int p = lo[hh]; p < hi[hh]; ++p) {
+      o.plane[2 * hh + 1].y = (int)in_lo;
+      for (int k = 0; k < wcnt[hh] + icnt[hh]; ++k) {  // position order: wall slots, then interior slots
+        const int p = k < wcnt[hh] ? wlo[hh] + k : ilo[hh] + (k - wcnt[hh]);
         if (pen_v[p] < 0) continue;
         const int u = hh - (pen_v[p] + pen_w[p]);
-        const int pos = start[hh] + (p - lo[hh]);
+        const int pos = start[hh] + k;
         const int c = cell_of(u, pen_v[p], pen_w[p]);
         if (!g.act[c]) continue;  // hole
         o.cell2pos[c] = pos;
@@ -240,6 +277,17 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
             o.in_bf.push_back(f);
           }
         }
+        for (int k2 = 0; k2 < (has_w ? 3 : 2); ++k2) {  // faces this class leaves the domain through, in position order
+          const int axis = axes[k2];
+          int nb[3] = {ijk[0], ijk[1], ijk[2]};
+          nb[axis] += o.sign[axis];
+          if (!(g.inside(nb) && g.act[g.cell(nb[0], nb[1], nb[2])])) {
+            const int f = facebf[(size_t)c * 6 + 2 * axis + (o.sign[axis] > 0 ? 1 : 0)];
+            o.out_bf.push_back(f);
+            o.out_pos.push_back(pos);
+            o.out_ord.push_back(bf_nord[f]++);
+          }
+        }
         if (first - in_lo >= (1u << 28)) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "too many boundary inflow faces");
         o.cellinfo[pos] = flags | ((first - in_lo) << 4);
         const double th0 = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
@@ -248,7 +296,8 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       o.g_max = std::max(o.g_max, (int)(o.in_bf.size() - in_lo));
     }
     if (o.in_bf.size() & 1) o.in_bf.push_back(-1);
-    o.plane[H] = make_int4(0, 0, o.n_pos, (int)o.in_bf.size());
+    o.plane[2 * (size_t)H] = make_int4(0, 0, 0, 0);
+    o.plane[2 * (size_t)H + 1] = make_int4(o.n_pos, (int)o.in_bf.size(), 0, 0);
     // reciprocal spacings along the sweep axis, in primed coordinates
     o.rhu.resize(nu);
     for (int u = 0; u < nu; ++u) o.rhu[u] = 1.0 / g.hsz[pa][phys(pa, u)];
@@ -428,6 +477,10 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     for (int ci = 0; ci < ncls; ++ci) {
       OctHost &o = oct[ci];
       OctTab &t = tabs[ci];
+      h->cls_outbf[ci] = A.put(o.out_bf);
+      h->cls_outpos[ci] = A.put(o.out_pos);
+      h->cls_outord[ci] = A.put(o.out_ord);
+      h->cls_nout[ci] = (int32_t)o.out_bf.size();
       h->cls_inbf[ci] = A.put(o.in_bf);
       h->cls_nin[ci] = (int32_t)o.in_bf.size();
       h->cls_ndirs[ci] = (int32_t)o.dirs.size();
@@ -449,7 +502,9 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     h->therm_faces = A.put(therm_faces);
     h->n_refl = (int)refl_faces.size();
     h->n_therm = (int)therm_faces.size();
-    h->split_closures = D <= 128;  // closure_G_kernel keeps ceil(D/32) <= 4 directions per lane
+    h->bf_nord = A.put(bf_nord);
+    h->g_partial = A.zeros<double>((size_t)4 * nbf * B);
+    h->split_closures = true;
     h->d_octs = A.put(tabs);
     h->sw.task_oct = A.put(task_oct);
     h->sw.task_row = A.put(task_row);

@@ -74,8 +74,8 @@ __host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int g
   L.tq = 0;                                                  // [2][pcap] double2
   L.info = L.tq + 2u * (uint32_t)pcap * 16u;                 // [2][pcap] uint32
   L.rows = L.info + 2u * (uint32_t)pcap * 4u;                // [G][rp]   double
-  L.plane = L.rows + (uint32_t)G * L.rp * 8u;                // [H+1]     int4
-  L.bar = L.plane + ((uint32_t)H + 1u) * 16u;                // [2]       mbarrier
+  L.plane = L.rows + (uint32_t)G * L.rp * 8u;                // [H+1][2]  int4
+  L.bar = L.plane + ((uint32_t)H + 1u) * 32u;                // [2]       mbarrier
   L.total = L.bar + 16u;
   return L;
 }
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
   const int n_valid = min(G, T.n_rows - row_loc);  // rows past the class's end recompute the last row and store nothing
   const int64_t row_g0 = (int64_t)T.row0 + row_loc;
 
-  for (int k = t; k <= T.H; k += blockDim.x) plane_s[k] = T.plane[k];
+  for (int k = t; k < 2 * (T.H + 1); k += blockDim.x) plane_s[k] = T.plane[k];
   for (uint32_t k = t; k < (uint32_t)G * rp; k += blockDim.x) rows[k] = 0.0;
   if (t == 0) {
     mbar_init(bar, 1);
@@ -116,19 +116,19 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
     double *const e0 = a.e + row_g0 * a.e_stride;
     const double *const bin0 = a.bin + T.bin_base + (int64_t)row_loc * T.n_in;
     auto issue_loads = [&](int h) {  // tables + inflow slices of hyperplane h into stage h & 1
-      const int4 P = plane_s[h];
+      const int4 P = plane_s[2 * h], Q = plane_s[2 * h + 1];
       const int s = h & 1;
-      const uint32_t c4 = ((uint32_t)P.y + 3u) & ~3u;
-      const uint32_t nin = (uint32_t)(plane_s[h + 1].w - P.w);  // even
+      const uint32_t c4 = ((uint32_t)(P.y + P.w) + 3u) & ~3u;
+      const uint32_t nin = (uint32_t)(plane_s[2 * h + 3].y - Q.y);  // even
       mbar_expect_tx(bar + s, c4 * 20u + (uint32_t)G * nin * 8u);
       if (c4) {
-        tma_load_1d(tq_s + (size_t)s * pcap, T.tq + P.z, c4 * 16u, bar + s);
-        tma_load_1d(info_s + (size_t)s * pcap, T.cellinfo + P.z, c4 * 4u, bar + s);
+        tma_load_1d(tq_s + (size_t)s * pcap, T.tq + Q.x, c4 * 16u, bar + s);
+        tma_load_1d(info_s + (size_t)s * pcap, T.cellinfo + Q.x, c4 * 4u, bar + s);
       }
       if (nin) {
 #pragma unroll
         for (int g = 0; g < G; ++g)
-          tma_load_1d(rows + (size_t)g * rp + sp + s * gcap, bin0 + (int64_t)min(g, n_valid - 1) * T.n_in + P.w, nin * 8u, bar + s);
+          tma_load_1d(rows + (size_t)g * rp + sp + s * gcap, bin0 + (int64_t)min(g, n_valid - 1) * T.n_in + Q.y, nin * 8u, bar + s);
       }
     };
     if (lead) {
@@ -142,12 +142,14 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
       if (lead && h + 2 < T.H) issue_loads(h + 2);
       cta_sync();  // B: hyperplane h is in the state rows (and fenced to the async proxy)
       if (lead) {
-        const int4 P = plane_s[h];
-        if (P.y) {
+        const int4 P = plane_s[2 * h];
+        const int start = plane_s[2 * h + 1].x;
 #pragma unroll
-          for (int g = 0; g < G; ++g)
-            if (g < n_valid) tma_store_1d(e0 + (int64_t)g * a.e_stride + P.z, rows + (size_t)g * rp + P.x, (uint32_t)P.y * 8u);
-        }
+        for (int g = 0; g < G; ++g)
+          if (g < n_valid) {  // the plane's wall cells, then its interior cells: two contiguous slot ranges
+            if (P.y) tma_store_1d(e0 + (int64_t)g * a.e_stride + start, rows + (size_t)g * rp + P.x, (uint32_t)P.y * 8u);
+            if (P.w) tma_store_1d(e0 + (int64_t)g * a.e_stride + start + P.y, rows + (size_t)g * rp + P.z, (uint32_t)P.w * 8u);
+          }
         tma_store_commit();
       }
     }
@@ -192,21 +194,23 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
   int4 Pn = plane_s[0];
   for (int h = 0; h < T.H; ++h) {
     const int s = h & 1;
-    const int4 P = Pn;
-    Pn = plane_s[h + 1];
+    const int4 P = Pn;  // {first wall slot, wall slots, first interior slot, interior slots} of this hyperplane
+    Pn = plane_s[2 * h + 2];
     mbar_wait(bar + s, (h >> 1) & 1);
-    const double2 *tqh = tq_s + (size_t)s * pcap - P.x;
-    const uint32_t *infoh = info_s + (size_t)s * pcap - P.x;
+    const double2 *tqh = tq_s + (size_t)s * pcap;
+    const uint32_t *infoh = info_s + (size_t)s * pcap;
     const uint32_t gs = (uint32_t)sp + (uint32_t)(s * gcap);  // this hyperplane's inflow stage within a row
     unsigned act = 0;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       const int p = t + r * nt;
-      if ((unsigned)(p - P.x) < (unsigned)P.y) {
-        const uint32_t info = infoh[p];
+      const unsigned kw = (unsigned)(p - P.x), ki = (unsigned)(p - P.z);
+      if (kw < (unsigned)P.y || ki < (unsigned)P.w) {
+        const unsigned k = kw < (unsigned)P.y ? kw : ki + (unsigned)P.y;  // index within the plane's segment
+        const uint32_t info = infoh[k];
         if (!(info & 8u)) {  // not a hole / padding slot
           act |= 1u << r;
-          const double2 tq = tqh[p];
+          const double2 tq = tqh[k];
           const uint32_t gb = gs + (info >> 4);
           const uint32_t iv = (info & 2u) ? gb + (info & 1u) : (pnb[r] & 0xffffu);
           const uint32_t iw = (info & 4u) ? gb + (info & 1u) + ((info >> 1) & 1u) : (pnb[r] >> 16);
