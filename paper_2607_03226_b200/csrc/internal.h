@@ -27,10 +27,13 @@
 // hyperplane, each plane's slice [in_lo(h), in_lo(h+1)) padded to an even length for the same reason.
 struct OctTab {
   const uint2 *pen;          // [n_pen]   .x = m, .y = pencil index of the v-upwind pencil | w-upwind pencil << 16 (n_pen = none)
-  const int4 *plane;         // [H+1][2]  {wall lo, wall cnt, interior lo, interior cnt}, {start, in_lo, 0, 0}; entry H is the
-                             //           sentinel {0,0,0,0}, {n_pos, n_in, 0, 0}
-  const uint32_t *cellinfo;  // [n_pos+16] bit0..2: u/v/w upwind value is a boundary inflow, bit3: hole, bits 4..: first inflow idx - in_lo(h)
-  const double2 *tq;         // [n_pos+16] (theta, Qdot) in sweep order
+  const int4 *plane;         // [H+1][2]  {wall lo, wall cnt, interior lo, interior cnt}, {start, in_lo, q_lo, 0}; entry H is the
+                             //           sentinel {0,0,0,0}, {n_pos, n_in, n_q, 0}
+  const double2 *tq;         // [n_pos+16] per position in sweep order: .x = theta, .y = bit pattern of a 64-bit record:
+                             //   bit 0..2 u/v/w upwind value is a boundary inflow, bit 3 hole / padding, bit 4 source cell,
+                             //   bits 5..17 first inflow index - in_lo(h), bits 18..31 index into the plane's qlist slice,
+                             //   bits 32..47 slot of the v-upwind pencil, bits 48..63 slot of the w-upwind pencil
+  const double *qlist;       // Qdot of the source cells in sweep order; hyperplane h owns [q_lo(h), q_lo(h+1)), even length
   const double *rhu;         // [nu]      1/h_u in primed coordinates (non-uniform spacing only)
   const double2 *pen_rh;     // [n_pen]   (1/h_v, 1/h_w) of the pencil (non-uniform spacing only)
   int64_t bin_base;          // offset of the class's first inflow row in bin
@@ -44,8 +47,8 @@ struct SweepArgs {
   const double *bin;         // inflow rows: class c, local row k at bin_base[c] + k * n_in[c]
   double *e;                 // [rows][e_stride]
   int64_t e_stride;
-  int32_t nu, sp, pcap, gcap;  // pencil length, state pitch (>= n_pen + 1, even), table stage capacity in cells (multiple
-                             // of 4), inflow stage capacity in values (even)
+  int32_t nu, sp, pcap, gcap, qcap;  // pencil length, state pitch (>= n_pen + 1, even), table stage capacity in cells
+                             // (multiple of 4), inflow / source stage capacities in values (even)
 };
 
 // ---- boundary-closure kernel ----------------------------------------------------------------------------------
@@ -177,7 +180,7 @@ int nb_cg_solve(nanobte_solver *h, int *iters);
 int nb_cg_blocks(nanobte_solver *h);
 // sweep_structured.cu
 int nb_launch_sweep_structured(nanobte_solver *h);
-int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int gcap, int H, int want_G, int want_threads,
+int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int gcap, int qcap, int H, int want_G, int want_threads,
                                int n_sys_min_class);
 // sweep_unstructured.cu
 int nb_launch_sweep_unstructured(nanobte_solver *h);

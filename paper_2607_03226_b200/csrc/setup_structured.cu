@@ -8,6 +8,8 @@
 
 namespace {
 
+inline double __longlong_as_double_host(uint64_t v) { double d; std::memcpy(&d, &v, sizeof(d)); return d; }
+
 struct Grid {
   int n[3];
   std::vector<double> hsz[3];
@@ -24,8 +26,8 @@ struct OctHost {
   std::vector<int> dirs;
   std::vector<uint2> pen;
   std::vector<int4> plane;
-  std::vector<uint32_t> cellinfo;
-  std::vector<double2> tq;
+  std::vector<double2> tq;         // per position: .x = theta, .y = bit pattern of (info | upwind slots << 32)
+  std::vector<double> qlist;       // Qdot of the source cells, position order, each hyperplane's slice padded to even
   std::vector<double> rhu;
   std::vector<double2> pen_rh;
   std::vector<int32_t> in_bf;      // inflow list: boundary face ids in consumption order
@@ -33,7 +35,7 @@ struct OctHost {
   std::vector<int32_t> cell2pos;   // [n_cells]
   std::vector<int32_t> out_bf, out_pos;  // faces that are outgoing for the class and their wall cell's position, position order
   std::vector<uint8_t> out_ord;    // rank of the class among the face's outgoing classes
-  int n_pen = 0, H = 0, n_pos = 0, p_max = 0, g_max = 0;
+  int n_pen = 0, H = 0, n_pos = 0, p_max = 0, g_max = 0, q_max = 0;
 };
 
 int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_bands *bands, const nanobte_quadrature *quad,
@@ -180,7 +182,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       }
 
   // ---- per class: pencils, hyperplanes, cell info, inflow lists ----------------------------------------------------------
-  int n_pen_max = 0, n_pos_max = 0, p_max = 0, g_max = 0;
+  int n_pen_max = 0, n_pos_max = 0, p_max = 0, g_max = 0, q_max = 0;
   std::vector<uint8_t> bf_nord(nbf, 0);  // outgoing classes per face (4 in 3-D, 2 in 2-D)
   for (int ci = 0; ci < ncls; ++ci) {
     OctHost &o = oct[ci];
@@ -244,8 +246,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       o.p_max = std::max(o.p_max, wcnt[hh] + icnt[hh]);
     }
     o.n_pos = base;
-    o.cellinfo.assign((size_t)o.n_pos + 16, 8u);
-    o.tq.assign((size_t)o.n_pos + 16, make_double2(0.0, 0.0));
+    o.tq.assign((size_t)o.n_pos + 16, make_double2(0.0, __longlong_as_double_host(8ull)));  // holes / padding
     o.cell2pos.assign(nc, -1);
     o.bf_slot.assign(nbf, -1);
     const int axes[3] = {pa, va, wa};
@@ -253,6 +254,9 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       if (o.in_bf.size() & 1) o.in_bf.push_back(-1);  // every hyperplane's inflow slice starts on an even index
       const uint32_t in_lo = (uint32_t)o.in_bf.size();
       o.plane[2 * hh + 1].y = (int)in_lo;
+      if (o.qlist.size() & 1) o.qlist.push_back(0.0);
+      const uint32_t q_lo = (uint32_t)o.qlist.size();
+      o.plane[2 * hh + 1].z = (int)q_lo;
       for (int k = 0; k < wcnt[hh] + icnt[hh]; ++k) {  // position order: wall slots, then interior slots
         const int p = k < wcnt[hh] ? wlo[hh] + k : ilo[hh] + (k - wcnt[hh]);
         if (pen_v[p] < 0) continue;
@@ -288,22 +292,32 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
             o.out_ord.push_back(bf_nord[f]++);
           }
         }
-        if (first - in_lo >= (1u << 28)) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "too many boundary inflow faces");
-        o.cellinfo[pos] = flags | ((first - in_lo) << 4);
+        if (first - in_lo >= (1u << 13)) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "a hyperplane has more than 8191 boundary inflow faces");
+        uint32_t info = flags | ((first - in_lo) << 5);
+        const double qc = Qdot ? Qdot[c] : 0.0;
+        if (qc != 0.0) {
+          const uint32_t qi = (uint32_t)o.qlist.size() - q_lo;
+          if (qi >= (1u << 14)) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "a hyperplane has more than 16383 source cells");
+          info |= 16u | (qi << 18);
+          o.qlist.push_back(qc);
+        }
         const double th0 = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
-        o.tq[pos] = make_double2(th0, Qdot ? Qdot[c] : 0.0);
+        o.tq[pos] = make_double2(th0, __longlong_as_double_host((uint64_t)info | ((uint64_t)o.pen[p].y << 32)));
       }
       o.g_max = std::max(o.g_max, (int)(o.in_bf.size() - in_lo));
+      o.q_max = std::max(o.q_max, (int)(o.qlist.size() - q_lo));
     }
     if (o.in_bf.size() & 1) o.in_bf.push_back(-1);
+    if (o.qlist.size() & 1) o.qlist.push_back(0.0);
     o.plane[2 * (size_t)H] = make_int4(0, 0, 0, 0);
-    o.plane[2 * (size_t)H + 1] = make_int4(o.n_pos, (int)o.in_bf.size(), 0, 0);
+    o.plane[2 * (size_t)H + 1] = make_int4(o.n_pos, (int)o.in_bf.size(), (int)o.qlist.size(), 0);
     // reciprocal spacings along the sweep axis, in primed coordinates
     o.rhu.resize(nu);
     for (int u = 0; u < nu; ++u) o.rhu[u] = 1.0 / g.hsz[pa][phys(pa, u)];
     n_pen_max = std::max(n_pen_max, o.n_pen);
     p_max = std::max(p_max, o.p_max);
     g_max = std::max(g_max, o.g_max);
+    q_max = std::max(q_max, o.q_max);
     n_pos_max = std::max(n_pos_max, o.n_pos);
   }
   const int64_t e_stride = ((int64_t)n_pos_max + 31) / 32 * 32;
@@ -441,7 +455,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   int nsys_min = 1 << 30;
   for (auto &o : oct) nsys_min = std::min<int>(nsys_min, (int)o.dirs.size() * B);
   h->uniform = uniform;
-  rc = nb_sweep_structured_config(h, n_pen_max, p_max, g_max, H, opt->sweep_G, opt->sweep_threads, nsys_min);
+  rc = nb_sweep_structured_config(h, n_pen_max, p_max, g_max, q_max, H, opt->sweep_G, opt->sweep_threads, nsys_min);
   if (rc) return rc;
   const int per_task = h->sweep_G;
   std::vector<int32_t> task_oct, task_row;
@@ -486,7 +500,8 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       h->cls_ndirs[ci] = (int32_t)o.dirs.size();
       t.pen = A.put(o.pen);
       t.plane = A.put(o.plane);
-      t.cellinfo = A.put(o.cellinfo);
+      o.qlist.resize((size_t)o.n_pos + 2 * (size_t)H + 16, 0.0);  // fixed capacity: the arena size must not depend on Qdot
+      t.qlist = A.put(o.qlist);
       double2 *tq = A.put(o.tq);
       t.tq = tq;
       h->tq[ci] = tq;

@@ -66,14 +66,14 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // Shared-memory carve-up (all offsets multiples of 16 bytes).  A system's row is [ state sp | inflow stage 0 gcap |
 // inflow stage 1 gcap ] doubles, so one index addresses "upwind value" wherever it comes from.
 struct SmemLayout {
-  uint32_t tq, info, rows, plane, bar, total, rp;
+  uint32_t tq, q, rows, plane, bar, total, rp;
 };
-__host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int gcap, int H) {
+__host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int gcap, int qcap, int H) {
   SmemLayout L;
   L.rp = (uint32_t)sp + 2u * (uint32_t)gcap;                 // row pitch in doubles (even)
   L.tq = 0;                                                  // [2][pcap] double2
-  L.info = L.tq + 2u * (uint32_t)pcap * 16u;                 // [2][pcap] uint32
-  L.rows = L.info + 2u * (uint32_t)pcap * 4u;                // [G][rp]   double
+  L.q = L.tq + 2u * (uint32_t)pcap * 16u;                    // [2][qcap] double
+  L.rows = L.q + 2u * (uint32_t)qcap * 8u;                   // [G][rp]   double
   L.plane = L.rows + (uint32_t)G * L.rp * 8u;                // [H+1][2]  int4
   L.bar = L.plane + ((uint32_t)H + 1u) * 32u;                // [2]       mbarrier
   L.total = L.bar + 16u;
@@ -87,10 +87,10 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
   const int t = threadIdx.x, nt = blockDim.x - 32;
   const int task = blockIdx.x;
   const OctTab T = octs[a.task_oct[task]];
-  const int nu = a.nu, sp = a.sp, pcap = a.pcap, gcap = a.gcap;
-  const SmemLayout L = smem_layout(G, sp, pcap, gcap, T.H);
+  const int nu = a.nu, sp = a.sp, pcap = a.pcap, gcap = a.gcap, qcap = a.qcap;
+  const SmemLayout L = smem_layout(G, sp, pcap, gcap, qcap, T.H);
   double2 *tq_s = reinterpret_cast<double2 *>(smem + L.tq);
-  uint32_t *info_s = reinterpret_cast<uint32_t *>(smem + L.info);
+  double *q_s = reinterpret_cast<double *>(smem + L.q);
   double *rows = reinterpret_cast<double *>(smem + L.rows);
   int4 *plane_s = reinterpret_cast<int4 *>(smem + L.plane);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smem + L.bar);
@@ -120,11 +120,10 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
       const int s = h & 1;
       const uint32_t c4 = ((uint32_t)(P.y + P.w) + 3u) & ~3u;
       const uint32_t nin = (uint32_t)(plane_s[2 * h + 3].y - Q.y);  // even
-      mbar_expect_tx(bar + s, c4 * 20u + (uint32_t)G * nin * 8u);
-      if (c4) {
-        tma_load_1d(tq_s + (size_t)s * pcap, T.tq + Q.x, c4 * 16u, bar + s);
-        tma_load_1d(info_s + (size_t)s * pcap, T.cellinfo + Q.x, c4 * 4u, bar + s);
-      }
+      const uint32_t nq = (uint32_t)(plane_s[2 * h + 3].z - Q.z);   // even
+      mbar_expect_tx(bar + s, c4 * 16u + nq * 8u + (uint32_t)G * nin * 8u);
+      if (c4) tma_load_1d(tq_s + (size_t)s * pcap, T.tq + Q.x, c4 * 16u, bar + s);
+      if (nq) tma_load_1d(q_s + (size_t)s * qcap, T.qlist + Q.z, nq * 8u, bar + s);
       if (nin) {
 #pragma unroll
         for (int g = 0; g < G; ++g)
@@ -166,18 +165,15 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
     for (int k = 0; k < (UNIFORM ? 5 : 6); ++k) cf[g][k] = a.coef[row * 8 + k];
   }
   // per-thread pencils: slot p = t + r*nt; upwind pencil slots (the zero slot n_pen if there is none)
-  uint32_t pnb[R];
   int pm[UNIFORM ? 1 : R];
   double rv[UNIFORM ? 1 : R], rw[UNIFORM ? 1 : R];
 #pragma unroll
   for (int r = 0; r < R; ++r) {
     const int p = t + r * nt;
-    pnb[r] = 0;
     if (!UNIFORM) { rv[r] = rw[r] = 0.0; pm[r] = 0; }
-    if (p < T.n_pen) {
+    if (!UNIFORM && p < T.n_pen) {
       const uint2 q = T.pen[p];
-      pnb[r] = q.y;
-      if (!UNIFORM) {
+      {
         pm[r] = (int)q.x;
         const double2 rh = T.pen_rh[p];
         rv[r] = rh.x;
@@ -198,7 +194,7 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
     Pn = plane_s[2 * h + 2];
     mbar_wait(bar + s, (h >> 1) & 1);
     const double2 *tqh = tq_s + (size_t)s * pcap;
-    const uint32_t *infoh = info_s + (size_t)s * pcap;
+    const double *qh = q_s + (size_t)s * qcap;
     const uint32_t gs = (uint32_t)sp + (uint32_t)(s * gcap);  // this hyperplane's inflow stage within a row
     unsigned act = 0;
 #pragma unroll
@@ -207,13 +203,15 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
       const unsigned kw = (unsigned)(p - P.x), ki = (unsigned)(p - P.z);
       if (kw < (unsigned)P.y || ki < (unsigned)P.w) {
         const unsigned k = kw < (unsigned)P.y ? kw : ki + (unsigned)P.y;  // index within the plane's segment
-        const uint32_t info = infoh[k];
+        double2 tq = tqh[k];
+        const uint64_t rec = (uint64_t)__double_as_longlong(tq.y);
+        const uint32_t info = (uint32_t)rec, pnb = (uint32_t)(rec >> 32);
         if (!(info & 8u)) {  // not a hole / padding slot
           act |= 1u << r;
-          const double2 tq = tqh[k];
-          const uint32_t gb = gs + (info >> 4);
-          const uint32_t iv = (info & 2u) ? gb + (info & 1u) : (pnb[r] & 0xffffu);
-          const uint32_t iw = (info & 4u) ? gb + (info & 1u) + ((info >> 1) & 1u) : (pnb[r] >> 16);
+          tq.y = (info & 16u) ? qh[info >> 18] : 0.0;  // Qdot of a source cell
+          const uint32_t gb = gs + ((info >> 5) & 0x1fffu);
+          const uint32_t iv = (info & 2u) ? gb + (info & 1u) : (pnb & 0xffffu);
+          const uint32_t iw = (info & 4u) ? gb + (info & 1u) + ((info >> 1) & 1u) : (pnb >> 16);
           double eu[G], ev[G], ew[G];
 #pragma unroll
           for (int g = 0; g < G; ++g) {
@@ -297,7 +295,7 @@ const int kMaxCompute = 480;  // + the DMA warp = 512 threads
 
 // Chooses systems per CTA (G), pencils per thread (R) and compute threads per CTA.  want_G / want_threads: 0 = auto.
 // n_pen_max: pencil slots (incl. padding); p_max: largest hyperplane; gcap: largest per-hyperplane inflow slice.
-int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int gcap, int H, int want_G, int want_threads,
+int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int gcap, int qcap, int H, int want_G, int want_threads,
                                int n_sys_min_class) {
   const size_t smem_cap = 227 * 1024;
   if (want_G < 0 || want_G > 4) return nb_fail(h, NANOBTE_E_INVALID, "sweep_G must be 0..4");
@@ -319,29 +317,31 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
   const int sp = (n_pen_max + 1 + 1) & ~1;
   const int pcap = (p_max + 3 + 4) & ~3;
   gcap = (gcap + 1) & ~1;
+  qcap = (qcap + 1) & ~1;
   int G = 0;
   const int cand[4] = {4, 3, 2, 1};
   for (int k = 0; k < 4 && !G; ++k) {
     const int g = cand[k];
     if (want_G > 0 && g != want_G) continue;
-    if (smem_layout(g, sp, pcap, gcap, H).total > smem_cap) continue;
+    if (smem_layout(g, sp, pcap, gcap, qcap, H).total > smem_cap) continue;
     if (g * R > (h->uniform ? kMaxGR : kMaxGR / 2)) continue;  // the non-uniform variant carries 5 more registers per pencil
     if (want_G <= 0 && g > std::max(1, n_sys_min_class)) continue;
     G = g;
   }
   if (!G) {
     if (want_G > 0) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "sweep_G=%d with %d pencils per thread needs %u B of shared memory (cap %zu) and G*R <= %d",
-                                   want_G, R, smem_layout(want_G, sp, pcap, gcap, H).total, smem_cap, kMaxGR);
+                                   want_G, R, smem_layout(want_G, sp, pcap, gcap, qcap, H).total, smem_cap, kMaxGR);
     return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section of %d pencils needs %u B of shared memory (> %zu)", n_pen_max,
-                   smem_layout(1, sp, pcap, gcap, H).total, smem_cap);
+                   smem_layout(1, sp, pcap, gcap, qcap, H).total, smem_cap);
   }
   h->sweep_G = G;
   h->sweep_rmax = R;
   h->sweep_threads = T;
-  h->sweep_smem = smem_layout(G, sp, pcap, gcap, H).total;
+  h->sweep_smem = smem_layout(G, sp, pcap, gcap, qcap, H).total;
   h->sw.sp = sp;
   h->sw.pcap = pcap;
   h->sw.gcap = gcap;
+  h->sw.qcap = qcap;
   return 0;
 }
 
