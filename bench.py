@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--cpu-sample-bands", type=int, default=0, help="bands in the oracle's sample (0 = auto)")
     ap.add_argument("--sweep-G", type=int, default=0)
     ap.add_argument("--sweep-threads", type=int, default=0)
+    ap.add_argument("--sweep-variant", type=int, default=0)
     return ap.parse_args()
 
 
@@ -216,7 +217,7 @@ def main():
     from paper_2607_03226_b200.binding import Solver
 
     t_c0 = time.perf_counter()
-    g = Solver(pr, sweep_G=args.sweep_G, sweep_threads=args.sweep_threads)
+    g = Solver(pr, sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_variant=args.sweep_variant)
     torch.cuda.synchronize()
     create_s = time.perf_counter() - t_c0
     upd = wl.n_updates(pr)

@@ -116,8 +116,9 @@ typedef struct {
   size_t workspace_bytes;
   double cg_rtol;               /* <= 0 -> 1e-12 (R14e)                                            */
   int32_t cg_max_iter;          /* <= 0 -> 100000                                                  */
-  int32_t sweep_G;              /* tuning: systems per CTA in the structured sweep (1,2,4); 0 = auto */
-  int32_t sweep_threads;        /* tuning: threads per CTA of the structured sweep (<= 512); 0 = auto */
+  int32_t sweep_G;              /* tuning: systems per CTA in the structured sweep (1..4); 0 = auto   */
+  int32_t sweep_threads;        /* tuning: compute threads per CTA of the structured sweep (<= 480); 0 = auto */
+  int32_t sweep_variant;        /* tuning: 0 = auto, 3 = single-buffered state (any spacing), 4 = double-buffered (uniform) */
 } nanobte_options;
 
 /* Layout / schedule facts of a created solver (for reporting and roofline arithmetic). */
@@ -126,7 +127,7 @@ typedef struct {
   int32_t n_octants;            /* direction classes in use (structured) / D (unstructured)       */
   int32_t n_planes;             /* hyperplanes per octant (structured) / max levels per direction */
   int32_t n_tasks;              /* CTAs per sweep launch                                           */
-  int32_t sweep_G, sweep_threads, sweep_rmax, pencil_axis;
+  int32_t sweep_G, sweep_threads, sweep_rmax, pencil_axis;  /* sweep_rmax: pencils per thread, 0 for the double-buffered variant */
   int64_t n_pos;                /* e slots per (band,direction) incl. holes and padding            */
   int64_t n_inflow;             /* sum over directions of boundary-inflow values per band          */
   size_t device_bytes;          /* total device memory in use by the solver                        */

@@ -57,7 +57,7 @@ class UnstructuredMesh(C.Structure):
 class Options(C.Structure):
     _fields_ = [("T_ref", C.c_double), ("T_init", _dp), ("stream", C.c_void_p), ("workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("cg_rtol", C.c_double), ("cg_max_iter", C.c_int32),
-                ("sweep_G", C.c_int32), ("sweep_threads", C.c_int32)]
+                ("sweep_G", C.c_int32), ("sweep_threads", C.c_int32), ("sweep_variant", C.c_int32)]
 
 
 class Info(C.Structure):
@@ -172,11 +172,11 @@ class _Marshalled:
         self.n_bf = len(k["bt"])
 
 
-def workspace_bytes(problem, sweep_G=0, sweep_threads=0):
+def workspace_bytes(problem, sweep_G=0, sweep_threads=0, sweep_variant=0):
     """Device bytes a Solver for this problem needs (host-only call; also validates the problem)."""
     lib = load()
     ms = _Marshalled(problem)
-    opt = Options(float(problem["T_ref"]), None, None, None, 0, 0.0, 0, sweep_G, sweep_threads)
+    opt = Options(float(problem["T_ref"]), None, None, None, 0, 0.0, 0, sweep_G, sweep_threads, sweep_variant)
     out = C.c_size_t()
     fn = lib.nanobte_workspace_bytes_structured if ms.kind == "structured" else lib.nanobte_workspace_bytes_unstructured
     rc = fn(C.byref(ms.mesh), C.byref(ms.bands), C.byref(ms.quad), ms.tags, ms.n_tags, C.byref(opt), C.byref(out))
@@ -189,7 +189,7 @@ class Solver:
     """One problem instance on the current CUDA device (same call shapes as the C ABI)."""
 
     def __init__(self, problem, T_init=None, cg_rtol=1e-12, cg_max_iter=100000, share=None, sweep_G=0,
-                 sweep_threads=0, own_workspace=True):
+                 sweep_threads=0, sweep_variant=0, own_workspace=True):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("nanobte needs a CUDA device (sm_100); there is no CPU fallback")
@@ -200,7 +200,7 @@ class Solver:
         self.B, self.D = ms.bands.B, ms.quad.D
         self.stream = torch.cuda.current_stream()
         opt = Options(float(problem["T_ref"]), _p(ms.keep["Ti"], _dp), C.c_void_p(self.stream.cuda_stream), None, 0,
-                      float(cg_rtol), int(cg_max_iter), int(sweep_G), int(sweep_threads))
+                      float(cg_rtol), int(cg_max_iter), int(sweep_G), int(sweep_threads), int(sweep_variant))
         structured = ms.kind == "structured"
         self._ws = None
         if own_workspace:  # device memory is a torch tensor (PyTorch: buffers and streams only)

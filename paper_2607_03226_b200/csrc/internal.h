@@ -90,7 +90,7 @@ struct nanobte_solver {
 
   // structured sweep
   SweepArgs sw{};
-  int sweep_G = 1, sweep_threads = 0, sweep_rmax = 1, n_tasks = 0, pencil_axis = 0, n_planes = 0;
+  int sweep_G = 1, sweep_threads = 0, sweep_rmax = 1, n_tasks = 0, pencil_axis = 0, n_planes = 0, sweep_variant = 3;
   bool uniform = true, sweep_attr_set = false;
   const OctTab *d_octs = nullptr;
   size_t sweep_smem = 0;
@@ -181,7 +181,7 @@ int nb_cg_blocks(nanobte_solver *h);
 // sweep_structured.cu
 int nb_launch_sweep_structured(nanobte_solver *h);
 int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int gcap, int qcap, int H, int want_G, int want_threads,
-                               int n_sys_min_class);
+                               int n_sys_min_class, int want_variant, int n_sys_total);
 // sweep_unstructured.cu
 int nb_launch_sweep_unstructured(nanobte_solver *h);
 void nb_free_unstructured(nanobte_solver *h);

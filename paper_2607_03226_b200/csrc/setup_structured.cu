@@ -455,7 +455,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   int nsys_min = 1 << 30;
   for (auto &o : oct) nsys_min = std::min<int>(nsys_min, (int)o.dirs.size() * B);
   h->uniform = uniform;
-  rc = nb_sweep_structured_config(h, n_pen_max, p_max, g_max, q_max, H, opt->sweep_G, opt->sweep_threads, nsys_min);
+  rc = nb_sweep_structured_config(h, n_pen_max, p_max, g_max, q_max, H, opt->sweep_G, opt->sweep_threads, nsys_min, opt->sweep_variant, B * D);
   if (rc) return rc;
   const int per_task = h->sweep_G;
   std::vector<int32_t> task_oct, task_row;

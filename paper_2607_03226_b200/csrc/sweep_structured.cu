@@ -253,6 +253,168 @@ __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a
   }
 }
 
+// =================================================================================================================
+// Double-buffered variant (uniform spacing; sweep_variant = 4, not the default: measured on B200 it halves the fixed
+// per-hyperplane cost but its fourth shared-memory access per update -- the u-upwind value -- costs more than that on
+// the large grids, where the shared-memory pipe is the busiest unit).  The state rows exist
+// twice: hyperplane h is written to buffer h&1 while buffer (h-1)&1 is read, so
+//   * there is ONE CTA barrier per hyperplane and no write phase (results go straight to shared memory),
+//   * cells are assigned to threads per hyperplane (thread t takes the plane's cells t, t+nt, ...), so no
+//     iteration is spent on pencils that are not active in this plane, and nothing per pencil lives in registers:
+//     the u-upwind value is the pencil's own slot in the other buffer, the upwind slots come with the cell record.
+// Row of a system: [ state buffer 0 | state buffer 1 | inflow stage 0 | inflow stage 1 ].
+// =================================================================================================================
+struct SmemLayoutDB {
+  uint32_t tq, q, rows, plane, bar, total, rp;
+};
+__host__ __device__ inline SmemLayoutDB smem_layout_db(int G, int sp, int pcap, int gcap, int qcap, int H) {
+  SmemLayoutDB L;
+  L.rp = 2u * (uint32_t)sp + 2u * (uint32_t)gcap;
+  L.tq = 0;                                                  // [2][pcap] double2 records
+  L.q = L.tq + 2u * (uint32_t)pcap * 16u;                    // [2][qcap] double
+  L.rows = L.q + 2u * (uint32_t)qcap * 8u;                   // [G][rp]   double
+  L.plane = L.rows + (uint32_t)G * L.rp * 8u;                // [H+1][2]  int4
+  L.bar = L.plane + ((uint32_t)H + 1u) * 32u;                // [2]       mbarrier
+  L.total = L.bar + 16u;
+  return L;
+}
+
+template <int G>
+__global__ void __launch_bounds__(512) sweep_structured_db_kernel(const SweepArgs a, const OctTab *__restrict__ octs) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int t = threadIdx.x, nt = blockDim.x - 32;
+  const int task = blockIdx.x;
+  const OctTab T = octs[a.task_oct[task]];
+  const int sp = a.sp, pcap = a.pcap, gcap = a.gcap, qcap = a.qcap;
+  const SmemLayoutDB L = smem_layout_db(G, sp, pcap, gcap, qcap, T.H);
+  double2 *tq_s = reinterpret_cast<double2 *>(smem + L.tq);
+  double *q_s = reinterpret_cast<double *>(smem + L.q);
+  double *rows = reinterpret_cast<double *>(smem + L.rows);
+  int4 *plane_s = reinterpret_cast<int4 *>(smem + L.plane);
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + L.bar);
+  const uint32_t rp = L.rp;
+
+  const int row_loc = a.task_row[task];
+  const int n_valid = min(G, T.n_rows - row_loc);
+  const int64_t row_g0 = (int64_t)T.row0 + row_loc;
+
+  for (int k = t; k < 2 * (T.H + 1); k += blockDim.x) plane_s[k] = T.plane[k];
+  for (uint32_t k = t; k < (uint32_t)G * rp; k += blockDim.x) rows[k] = 0.0;
+  if (t == 0) {
+    mbar_init(bar, 1);
+    mbar_init(bar + 1, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  fence_proxy_async();
+  __syncthreads();
+
+  if (t >= nt) {
+    // ------------------------------------------------ DMA warp ---------------------------------------------------
+    const bool lead = t == nt;
+    double *const e0 = a.e + row_g0 * a.e_stride;
+    const double *const bin0 = a.bin + T.bin_base + (int64_t)row_loc * T.n_in;
+    auto issue_loads = [&](int h) {
+      const int4 P = plane_s[2 * h], Q = plane_s[2 * h + 1];
+      const int s = h & 1;
+      const uint32_t c4 = ((uint32_t)(P.y + P.w) + 3u) & ~3u;
+      const uint32_t nin = (uint32_t)(plane_s[2 * h + 3].y - Q.y);
+      const uint32_t nq = (uint32_t)(plane_s[2 * h + 3].z - Q.z);
+      mbar_expect_tx(bar + s, c4 * 16u + nq * 8u + (uint32_t)G * nin * 8u);
+      if (c4) tma_load_1d(tq_s + (size_t)s * pcap, T.tq + Q.x, c4 * 16u, bar + s);
+      if (nq) tma_load_1d(q_s + (size_t)s * qcap, T.qlist + Q.z, nq * 8u, bar + s);
+      if (nin) {
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+          tma_load_1d(rows + (size_t)g * rp + 2 * sp + s * gcap, bin0 + (int64_t)min(g, n_valid - 1) * T.n_in + Q.y, nin * 8u, bar + s);
+      }
+    };
+    if (lead) {
+      issue_loads(0);
+      if (T.H > 1) issue_loads(1);
+    }
+    for (int h = 0; h < T.H; ++h) {
+      // the stores of hyperplane h-1 have read buffer (h-1)&1, which hyperplane h+1 overwrites after this barrier
+      if (lead) tma_store_wait_read();
+      cta_sync();  // hyperplane h is complete in buffer h&1; stage h&1 is free
+      if (lead) {
+        const int4 P = plane_s[2 * h];
+        const int start = plane_s[2 * h + 1].x;
+        const double *buf = rows + (size_t)(h & 1) * sp;
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+          if (g < n_valid) {
+            if (P.y) tma_store_1d(e0 + (int64_t)g * a.e_stride + start, buf + (size_t)g * rp + P.x, (uint32_t)P.y * 8u);
+            if (P.w) tma_store_1d(e0 + (int64_t)g * a.e_stride + start + P.y, buf + (size_t)g * rp + P.z, (uint32_t)P.w * 8u);
+          }
+        tma_store_commit();
+        if (h + 2 < T.H) issue_loads(h + 2);
+      }
+    }
+    if (lead) tma_store_wait_read();
+    return;
+  }
+
+  // -------------------------------------------------- compute warps ------------------------------------------------
+  double cf[G][5];
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    const int64_t row = row_g0 + min(g, n_valid - 1);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) cf[g][k] = a.coef[row * 8 + k];
+  }
+  int4 Pn = plane_s[0];
+  for (int h = 0; h < T.H; ++h) {
+    const int s = h & 1;
+    const int4 P = Pn;
+    Pn = plane_s[2 * h + 2];
+    const int ntot = P.y + P.w;
+    const uint32_t prev = (uint32_t)((s ^ 1) * sp), cur = (uint32_t)(s * sp);
+    const uint32_t gs = 2u * (uint32_t)sp + (uint32_t)(s * gcap);
+    const double2 *tqh = tq_s + (size_t)s * pcap;
+    const double *qh = q_s + (size_t)s * qcap;
+    mbar_wait(bar + s, (h >> 1) & 1);
+    for (int k0 = t; k0 < ntot; k0 += 2 * nt) {  // two cells per trip: all shared-memory loads before the first store
+      double res[2][G];
+      uint32_t slot[2];
+      bool on[2];
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int k = k0 + j * nt;
+        on[j] = false;
+        slot[j] = 0;
+        if (k < ntot) {
+          double2 tq = tqh[k];
+          const uint64_t rec = (uint64_t)__double_as_longlong(tq.y);
+          const uint32_t info = (uint32_t)rec, pnb = (uint32_t)(rec >> 32);
+          if (!(info & 8u)) {
+            on[j] = true;
+            const uint32_t p = k < P.y ? (uint32_t)(P.x + k) : (uint32_t)(P.z + k - P.y);
+            slot[j] = p;
+            const double qd = (info & 16u) ? qh[info >> 18] : 0.0;
+            const uint32_t gb = gs + ((info >> 5) & 0x1fffu);
+            const uint32_t iu = (info & 1u) ? gb : prev + p;
+            const uint32_t iv = (info & 2u) ? gb + (info & 1u) : prev + (pnb & 0xffffu);
+            const uint32_t iw = (info & 4u) ? gb + (info & 1u) + ((info >> 1) & 1u) : prev + (pnb >> 16);
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+              const double *rg = rows + g * rp;
+              res[j][g] = cf[g][0] * tq.x + cf[g][1] * qd + cf[g][2] * rg[iu] + cf[g][3] * rg[iv] + cf[g][4] * rg[iw];
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < 2; ++j)
+        if (on[j]) {
+#pragma unroll
+          for (int g = 0; g < G; ++g) rows[g * rp + cur + slot[j]] = res[j][g];
+        }
+    }
+    fence_proxy_async();
+    cta_sync();
+  }
+}
+
 // ---- host side: variant table ---------------------------------------------------------------------------------------
 typedef void (*sweep_fn)(const SweepArgs, const OctTab *);
 constexpr int kMaxGR = 24;  // registers: 2*G*R hold the results of a hyperplane; larger products spill
@@ -296,7 +458,7 @@ const int kMaxCompute = 480;  // + the DMA warp = 512 threads
 // Chooses systems per CTA (G), pencils per thread (R) and compute threads per CTA.  want_G / want_threads: 0 = auto.
 // n_pen_max: pencil slots (incl. padding); p_max: largest hyperplane; gcap: largest per-hyperplane inflow slice.
 int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int gcap, int qcap, int H, int want_G, int want_threads,
-                               int n_sys_min_class) {
+                               int n_sys_min_class, int want_variant, int n_sys_total) {
   const size_t smem_cap = 227 * 1024;
   if (want_G < 0 || want_G > 4) return nb_fail(h, NANOBTE_E_INVALID, "sweep_G must be 0..4");
   if (n_pen_max > 12 * kMaxCompute || n_pen_max >= 65535)
@@ -326,6 +488,8 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
     if (smem_layout(g, sp, pcap, gcap, qcap, H).total > smem_cap) continue;
     if (g * R > (h->uniform ? kMaxGR : kMaxGR / 2)) continue;  // the non-uniform variant carries 5 more registers per pencil
     if (want_G <= 0 && g > std::max(1, n_sys_min_class)) continue;
+    // small problems: rather more CTAs than more systems per CTA, until the machine has two CTAs per SM to run
+    if (want_G <= 0 && g > 1 && (long)((n_sys_total + g - 1) / g) < 2L * h->n_sm) continue;
     G = g;
   }
   if (!G) {
@@ -333,6 +497,33 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
                                    want_G, R, smem_layout(want_G, sp, pcap, gcap, qcap, H).total, smem_cap, kMaxGR);
     return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section of %d pencils needs %u B of shared memory (> %zu)", n_pen_max,
                    smem_layout(1, sp, pcap, gcap, qcap, H).total, smem_cap);
+  }
+  // double-buffered variant: uniform spacing only, on request
+  h->sweep_variant = 3;
+  if (h->uniform && want_variant == 4) {
+    int Gd = 0;
+    for (int k = 0; k < 4 && !Gd; ++k) {
+      const int g = cand[k];
+      if (want_G > 0 && g != want_G) continue;
+      if (smem_layout_db(g, sp, pcap, gcap, qcap, H).total > smem_cap) continue;
+      if (want_G <= 0 && g > std::max(1, n_sys_min_class)) continue;
+      Gd = g;
+    }
+    if (Gd) {
+      h->sweep_variant = 4;
+      h->sweep_G = Gd;
+      h->sweep_rmax = 0;
+      h->sweep_threads = want_threads > 0 ? T : std::min(kMaxCompute, std::max(32, (p_max / 2 + 31) / 32 * 32));
+      h->sweep_smem = smem_layout_db(Gd, sp, pcap, gcap, qcap, H).total;
+      h->sw.sp = sp;
+      h->sw.pcap = pcap;
+      h->sw.gcap = gcap;
+      h->sw.qcap = qcap;
+      return 0;
+    }
+    if (want_variant == 4) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "the double-buffered sweep does not fit in shared memory");
+  } else if (want_variant == 4) {
+    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "the double-buffered sweep needs uniform spacing");
   }
   h->sweep_G = G;
   h->sweep_rmax = R;
@@ -346,7 +537,17 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
 }
 
 int nb_launch_sweep_structured(nanobte_solver *h) {
-  sweep_fn fn = pick(h->sweep_G, h->sweep_rmax, h->uniform);
+  sweep_fn fn = nullptr;
+  if (h->sweep_variant == 4) {
+    switch (h->sweep_G) {
+      case 1: fn = sweep_structured_db_kernel<1>; break;
+      case 2: fn = sweep_structured_db_kernel<2>; break;
+      case 3: fn = sweep_structured_db_kernel<3>; break;
+      case 4: fn = sweep_structured_db_kernel<4>; break;
+    }
+  } else {
+    fn = pick(h->sweep_G, h->sweep_rmax, h->uniform);
+  }
   if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "no sweep kernel variant for G=%d R=%d", h->sweep_G, h->sweep_rmax);
   if (!h->sweep_attr_set) {
     NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(h->sweep_smem, 1024)));

@@ -66,10 +66,11 @@ def step_parity(pr, n_steps=3, T_init=None, mode="plain", **kw):
 
 
 # ---- tiny meshes: every closure type, non-uniform spacing, a masked L-shape ------------------------------------------
+@pytest.mark.parametrize("variant", [0, 4])  # 0: auto (single-buffered sweep), 4: double-buffered sweep
 @pytest.mark.parametrize("name", [k for k in TINY if TINY[k]["kind"] == "structured"])
-def test_tiny_steps(name):
+def test_tiny_steps(name, variant):
     pr = TINY[name]
-    step_parity(pr, 4, T_init=random_T(pr, 5))
+    step_parity(pr, 4, T_init=random_T(pr, 5), sweep_variant=variant)
 
 
 @pytest.mark.parametrize("name", [k for k in TINY if TINY[k]["kind"] == "structured"])
@@ -107,7 +108,8 @@ def test_config0_gray_square_full():
 
 
 @pytest.mark.parametrize("kw", [{}, {"sweep_G": 1}, {"sweep_G": 2, "sweep_threads": 64}, {"sweep_G": 4},
-                                {"sweep_G": 1, "sweep_threads": 32}])
+                                {"sweep_G": 1, "sweep_threads": 32}, {"sweep_variant": 4}, {"sweep_variant": 4, "sweep_G": 2},
+                                {"sweep_variant": 4, "sweep_G": 3, "sweep_threads": 96}])
 def test_config1_nongray_square_full(kw):
     pr = wl.config_nongray_square()
     step_parity(pr, 2, **kw)
@@ -123,7 +125,9 @@ def test_config1_solve():
 
 # ---- cuts of configs[2] (cube) and configs[3] (finfet): several tiles and ragged tails ---------------------------------------
 @pytest.mark.parametrize("n,kw", [(12, {}), (20, {"sweep_G": 1}), (20, {"sweep_G": 2}), (20, {"sweep_G": 4, "sweep_threads": 128}),
-                                  (33, {"sweep_G": 2, "sweep_threads": 160}), (24, {"sweep_G": 1, "sweep_threads": 96})])
+                                  (33, {"sweep_G": 2, "sweep_threads": 160}), (24, {"sweep_G": 1, "sweep_threads": 96}),
+                                  (20, {"sweep_variant": 4}), (33, {"sweep_variant": 4, "sweep_G": 2, "sweep_threads": 160}),
+                                  (24, {"sweep_variant": 4, "sweep_G": 3}), (17, {"sweep_variant": 3, "sweep_G": 3})])
 def test_cube_cut_steps(n, kw):
     pr = wl.config_cube(n=n, B=3, n_polar=4, n_azim=8)
     step_parity(pr, 3, T_init=random_T(pr, 9), **kw)
@@ -142,7 +146,8 @@ def test_cube_cut_solve_both_modes():
     assert np.abs(Ts["plain"] - Ts["synthetic"]).max() < 1e-6  # P6 on the GPU side
 
 
-@pytest.mark.parametrize("shape,kw", [((16, 8, 8), {}), ((32, 16, 16), {"sweep_G": 2}), ((24, 12, 12), {"sweep_G": 1})])
+@pytest.mark.parametrize("shape,kw", [((16, 8, 8), {}), ((32, 16, 16), {"sweep_G": 2}), ((24, 12, 12), {"sweep_G": 1}),
+                                      ((32, 16, 16), {"sweep_variant": 4}), ((24, 12, 12), {"sweep_variant": 4, "sweep_G": 3})])
 def test_finfet_cut_steps(shape, kw):
     nx, ny, nz = shape
     pr = wl.config_finfet(nx=nx, ny=ny, nz=nz, B=3, n_polar=2, n_azim=8)
