@@ -14,6 +14,7 @@
 // level -- no dependent-launch chain (~1,500 levels), upwind chunks are re-read from L2 where the same CTA wrote
 // them one level earlier.  The per-(direction, position) geometry records are prefetched one pass ahead.
 #include <algorithm>
+#include <cstdlib>
 #include <map>
 #include <numeric>
 
@@ -21,6 +22,7 @@
 
 struct UnsArgs {
   int32_t D, B, BG, NBG, MI, cpp;   // bands per CTA, band groups, max inflow faces per cell, cells per pass
+  int32_t rcap;                     // positions held by the shared-memory ring (power of two)
   int32_t n_act, l_max;
   int64_t e_stride;                 // positions per direction (n_act rounded up)
   const int32_t *n_lvl;             // [D]
@@ -47,8 +49,20 @@ namespace {
 constexpr int32_t kNone = INT32_MIN;
 
 // ---- (a5) the sweep -----------------------------------------------------------------------------------------------------
+// Upwind references carry their class in the top bits (decided once at create):
+//   kUpRing  the upwind cell lies within the last `rcap` positions before the end of this cell's level: its value is
+//            still in the CTA's shared-memory ring (positions are written in increasing order, slot = pos mod rcap);
+//   kUpOld   the upwind cell's level is at least 3 levels back: final and visible long before this cell's turn, so
+//            the value is fetched from global memory a whole item ahead, off the per-level critical path;
+//   neither  (a level wider than the ring) read from global memory after the level barrier.
+// Per thread the work items (its cells, in level order) run through a three-stage pipeline: geometry record two
+// items ahead, operand values (theta, Qdot, inflow, old upwind values) one item ahead, compute now.  Between two
+// level barriers a thread therefore touches only registers and shared memory.
+constexpr int32_t kUpRing = 1 << 29, kUpOld = 1 << 28, kUpMask = (1 << 28) - 1;
+
 template <int MI>
-__global__ void __launch_bounds__(1024) sweep_unstructured_kernel(const UnsArgs a) {
+__global__ void __launch_bounds__(256, 3) sweep_unstructured_kernel(const UnsArgs a) {
+  extern __shared__ double ring[];  // [rcap][BG]
   const int d = blockIdx.x / a.NBG, bg = blockIdx.x % a.NBG;
   const int slot0 = threadIdx.x / a.BG, bl = threadIdx.x - slot0 * a.BG;
   const int b = bg * a.BG + bl;
@@ -63,70 +77,105 @@ __global__ void __launch_bounds__(1024) sweep_unstructured_kernel(const UnsArgs 
   const int32_t *const lp = a.lvl_ptr + (int64_t)d * (a.l_max + 1);
   const int64_t kstride = (int64_t)a.D * a.e_stride;
   const int n_lvl = a.n_lvl[d], cpp = a.cpp;
+  const int rmask = a.rcap - 1, BG = a.BG;
 
-  // record of the first position this thread will touch; afterwards always one pass ahead
-  int c_n = 0, up_n[MI];
-  double go_n = 0.0, gi_n[MI];
-  auto fetch = [&](int pos) {
-    c_n = __ldg(cell + pos);
-    go_n = __ldg(gout + pos);
+  struct Rec {
+    int c, pos, lvl;
+    double go;
+    int up[MI];
+    double gi[MI];
+  };
+  auto fetch_rec = [&](Rec &r, int pos, int lvl) {
+    r.pos = pos;
+    r.lvl = lvl;
+    r.c = __ldg(cell + pos);
+    r.go = __ldg(gout + pos);
 #pragma unroll
     for (int k = 0; k < MI; ++k) {
-      up_n[k] = __ldg(a.up + k * kstride + dbase + pos);
-      gi_n[k] = __ldg(a.gin + k * kstride + dbase + pos);
+      r.up[k] = __ldg(a.up + k * kstride + dbase + pos);
+      r.gi[k] = __ldg(a.gin + k * kstride + dbase + pos);
     }
   };
-  int lo = lp[0], hi = n_lvl > 0 ? lp[1] : 0;
-  int pos = lo + slot0;
-  // the next position this thread handles, possibly in a later level
-  auto next_pos = [&](int p, int &l, int &l_lo, int &l_hi) {
-    p += cpp;
-    while (p >= l_hi && l + 1 < n_lvl) {
-      ++l;
-      l_lo = l_hi;
-      l_hi = lp[l + 1];
-      p = l_lo + slot0;
+  // item cursor: the thread's next position at or after p in level order (n_lvl = exhausted)
+  int cl = 0, clo = lp[0], chi = n_lvl > 0 ? lp[1] : 0, cp = clo + slot0;
+  auto settle = [&]() {
+    while (cp >= chi && cl < n_lvl) {
+      ++cl;
+      if (cl < n_lvl) {
+        clo = chi;
+        chi = lp[cl + 1];
+        cp = clo + slot0;
+      }
     }
-    return p;
   };
-  int l_f = 0, lo_f = lo, hi_f = hi;  // fetch cursor
-  int p_f = pos;
-  while (p_f >= hi_f && l_f + 1 < n_lvl) {
-    ++l_f;
-    lo_f = hi_f;
-    hi_f = lp[l_f + 1];
-    p_f = lo_f + slot0;
+  auto advance = [&]() {
+    cp += cpp;
+    settle();
+  };
+  constexpr int QD = 1;   // records in flight behind stage V (deeper queues spill under the 3-CTA register cap)
+  Rec rV, rQ[QD];         // stage V: record arrived, values (being) fetched; rQ: records in flight, oldest first
+  bool hasV = false, vIssued = false;
+  int nQ = 0;
+  double thV = 0.0, qV = 0.0, valV[MI];
+  auto issue_vals = [&]() {  // operands of stage V that do not depend on the sweep's recent output
+    thV = a.theta[rV.c];
+    qV = a.Qdot[rV.c];
+#pragma unroll
+    for (int k = 0; k < MI; ++k) {
+      const int u = rV.up[k];
+      valV[k] = 0.0;
+      if (u != kNone) {
+        if (u < 0) valV[k] = bind[-1 - u];
+        else if (u & kUpOld) valV[k] = ed[(int64_t)(u & kUpMask) * a.B];
+      }
+    }
+    vIssued = true;
+  };
+  if (live) {
+    settle();
+    if (cl < n_lvl) { fetch_rec(rV, cp, cl); hasV = true; advance(); }
+#pragma unroll
+    for (int j = 0; j < QD; ++j)
+      if (cl < n_lvl) { fetch_rec(rQ[j], cp, cl); nQ = j + 1; advance(); }
   }
-  bool have = live && p_f < hi_f;
-  if (have) fetch(p_f);
 
   for (int l = 0; l < n_lvl; ++l) {
-    lo = lp[l];
-    hi = lp[l + 1];
-    if (live) {
-      for (pos = lo + slot0; pos < hi; pos += cpp) {
-        // pos == p_f by construction: consume the prefetched record, start the next fetch
-        const int c = c_n;
-        const double go = go_n;
-        int up[MI];
-        double gi[MI];
+    // levels <= l-1 are complete and visible here
+    if (hasV && !vIssued && rV.lvl <= l + 2) issue_vals();
+    while (hasV && rV.lvl == l) {
+      if (!vIssued) issue_vals();
+      const int pos = rV.pos;
+      double num = kA * thV + kS * qV;
+      const double den = itau + vb * rV.go;
 #pragma unroll
-        for (int k = 0; k < MI; ++k) {
-          up[k] = up_n[k];
-          gi[k] = gi_n[k];
-        }
-        p_f = next_pos(p_f, l_f, lo_f, hi_f);
-        if (p_f < hi_f) fetch(p_f);
-        double num = kA * a.theta[c] + kS * a.Qdot[c];
-        const double den = itau + vb * go;
-#pragma unroll
-        for (int k = 0; k < MI; ++k) {
-          if (up[k] != kNone) {
-            const double val = up[k] >= 0 ? ed[(int64_t)up[k] * a.B] : bind[-1 - up[k]];
-            num += vb * gi[k] * val;
+      for (int k = 0; k < MI; ++k) {
+        const int u = rV.up[k];
+        if (u != kNone) {
+          double val = valV[k];
+          if (u >= 0 && !(u & kUpOld)) {
+            const int up = u & kUpMask;
+            val = (u & kUpRing) ? ring[(up & rmask) * BG + bl] : ed[(int64_t)up * a.B];
           }
+          num += vb * rV.gi[k] * val;
         }
-        ed[(int64_t)pos * a.B] = num / den;
+      }
+      const double res = num / den;
+      ed[(int64_t)pos * a.B] = res;
+      ring[(pos & rmask) * BG + bl] = res;
+      // shift the pipeline
+      hasV = nQ > 0;
+      vIssued = false;
+      if (hasV) {
+        rV = rQ[0];
+#pragma unroll
+        for (int j = 0; j + 1 < QD; ++j) rQ[j] = rQ[j + 1];
+        --nQ;
+        if (cl < n_lvl) {  // the queue is full whenever items remain, so the new record goes to the last slot
+          fetch_rec(rQ[QD - 1], cp, cl);
+          ++nQ;
+          advance();
+        }
+        if (rV.lvl <= l + 2) issue_vals();
       }
     }
     __syncthreads();  // level l is visible to the whole CTA (it alone reads these rows)
@@ -225,7 +274,11 @@ int nb_launch_sweep_unstructured(nanobte_solver *h) {
   const UnsArgs &a = *h->uns;
   uns_fn fn = pick_uns(a.MI);
   if (!fn) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "cells with more than 7 inflow faces are not supported");
-  fn<<<a.D * a.NBG, h->sweep_threads, 0, h->stream>>>(a);
+  if (!h->sweep_attr_set) {
+    NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(h->sweep_smem, 1024)));
+    h->sweep_attr_set = true;
+  }
+  fn<<<a.D * a.NBG, h->sweep_threads, h->sweep_smem, h->stream>>>(a);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
   return 0;
@@ -516,9 +569,30 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
   int BG = opt->sweep_G > 0 ? std::min(opt->sweep_G, B) : std::min(B, 8);
   if (opt->sweep_G <= 0 && B % 8 != 0 && B <= 12) BG = B;
   const int NBG = (B + BG - 1) / BG;
-  int threads = opt->sweep_threads > 0 ? std::min(1024, (opt->sweep_threads + 31) / 32 * 32) : 256;
+  int threads = opt->sweep_threads > 0 ? std::min(256, (opt->sweep_threads + 31) / 32 * 32) : 256;
   threads = std::max(threads, (BG + 31) / 32 * 32);
   const int cpp = threads / BG;
+  // shared-memory ring of the CTA's most recent outputs: the largest power of two of positions within 64 KB
+  int rcap = 64;
+  while ((size_t)rcap * 2 * BG * sizeof(double) <= 64 * 1024 && rcap * 2 <= (1 << 20)) rcap *= 2;
+  if (nc >= (1 << 28)) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "more than 2^28 cells");
+  // class of every upwind reference (see the kernel): ring / old / neither
+  {
+    std::vector<int32_t> lvl_of(nc);
+    for (int d = 0; d < D; ++d) {
+      const std::vector<int32_t> &lp = lvl_ptrs[d];
+      for (int l = 0; l < n_lvl[d]; ++l)
+        for (int pos = lp[l]; pos < lp[l + 1]; ++pos) lvl_of[pos] = l;
+      for (int k = 0; k < MI; ++k)
+        for (int pos = 0; pos < nc; ++pos) {
+          int32_t &u = up[(size_t)k * D * e_stride + (size_t)d * e_stride + pos];
+          if (u < 0) continue;  // none or boundary inflow
+          const int l = lvl_of[pos];
+          if (u >= lp[l + 1] - rcap) u |= kUpRing;
+          else if (lvl_of[u] <= l - 3) u |= kUpOld;
+        }
+    }
+  }
 
   std::vector<int32_t> lvl_ptr((size_t)D * (l_max + 1), 0);
   for (int d = 0; d < D; ++d) {
@@ -535,7 +609,7 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
 
   h->kind = 1; h->n_cells = nc; h->n_cls = D; h->n_planes = l_max; h->n_tasks = D * NBG;
   h->sweep_G = BG; h->sweep_threads = threads; h->sweep_rmax = MI; h->pencil_axis = -1;
-  h->n_pos = nc; h->e_stride = e_stride; h->sweep_smem = 0;
+  h->n_pos = nc; h->e_stride = e_stride; h->sweep_smem = (size_t)rcap * BG * sizeof(double);
   h->T_ref = opt->T_ref;
   h->cg_rtol = opt->cg_rtol > 0 ? opt->cg_rtol : 1e-12;
   h->cg_max_iter = opt->cg_max_iter > 0 ? opt->cg_max_iter : 100000;
@@ -548,7 +622,7 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
     Arena A(h, dry);
     rc = nb_upload_generic(h, A, cm, G);
     if (rc) return nb_fail(h, rc, "device upload failed");
-    u.D = D; u.B = B; u.BG = BG; u.NBG = NBG; u.MI = MI; u.cpp = cpp; u.n_act = nc; u.l_max = l_max; u.e_stride = e_stride;
+    u.D = D; u.B = B; u.BG = BG; u.NBG = NBG; u.MI = MI; u.cpp = cpp; u.rcap = rcap; u.n_act = nc; u.l_max = l_max; u.e_stride = e_stride;
     u.n_lvl = A.put(n_lvl);
     u.lvl_ptr = A.put(lvl_ptr);
     u.cell = A.put(cellat);
