@@ -275,3 +275,10 @@ def test_errors_on_gpu():
     with pytest.raises(NanoBTEError) as e:
         g.solve(1e-9, 5, "synthetic")
     assert e.value.code == -9
+
+
+def test_generic_cg_kernel_matches_oracle(monkeypatch):
+    """The multi-pass CG kernel (fallback for meshes whose chunk or halo does not fit the fused kernel)."""
+    monkeypatch.setenv("NANOBTE_CG_GENERIC", "1")
+    pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
+    step_parity(pr, 2, T_init=random_T(pr, 4), mode="synthetic")
