@@ -185,27 +185,27 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
     s_h[j] = 0.0;
   }
   // Stencil of the thread's cells: in registers up to 2 cells per thread; with 4 the 48 coefficient registers would
-  // spill, so they are re-read every iteration through the read-only path (100 KB per CTA: L1-resident).
+  // spill, so the coefficients are re-read every iteration through the read-only path (95 KB per CTA: L1-resident).
   constexpr bool kStencilInRegs = CPT <= 2;
   constexpr int CR = kStencilInRegs ? CPT : 1;
   double cf[CR][NF], dg[CPT], r[CPT], s[CPT], wv[CPT];
-  uint16_t nl[CR][NF];  // local indices < 65536 (checked when the plan is built)
+  uint16_t nl[CPT][NF];  // local indices < 65536 (checked when the plan is built); always in registers
 #pragma unroll
   for (int c = 0; c < CPT; ++c) {
     const int li = tid + c * kCgfThreads, i = a0 + li;
     s[c] = wv[c] = r[c] = dg[c] = 0.0;
     if (li < a.chunk) x_s[li] = p_s[li] = 0.0;
 #pragma unroll
-    if (kStencilInRegs)
 #pragma unroll
-      for (int f = 0; f < NF; ++f) { cf[c % CR][f] = 0.0; nl[c % CR][f] = 0; }
+    for (int f = 0; f < NF; ++f) {
+      nl[c][f] = 0;
+      if (kStencilInRegs) cf[c % CR][f] = 0.0;
+    }
     if (li < nown) {
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        if (kStencilInRegs) {
-          cf[c % CR][f] = a.coef[(size_t)f * n + i];
-          nl[c % CR][f] = (uint16_t)a.nloc[(size_t)f * n + i];
-        }
+        nl[c][f] = (uint16_t)a.nloc[(size_t)f * n + i];
+        if (kStencilInRegs) cf[c % CR][f] = a.coef[(size_t)f * n + i];
       }
       dg[c] = a.diag[i];
       double rhs = a.vol[i] * a.beta * (a.theta_SI[i] - a.theta_prev[i]);   // R14c
@@ -235,8 +235,8 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
         double acc = dg[c] * r[c];
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-          if (kStencilInRegs) acc -= cf[c % CR][f] * r_loc[nl[c % CR][f]];
-          else acc -= __ldg(a.coef + (size_t)f * n + a0 + li) * r_loc[__ldg(a.nloc + (size_t)f * n + a0 + li)];
+          if (kStencilInRegs) acc -= cf[c % CR][f] * r_loc[nl[c][f]];
+          else acc -= __ldg(a.coef + (size_t)f * n + a0 + li) * r_loc[nl[c][f]];
         }
         wv[c] = acc;
         a.w[(size_t)par_out * n + a0 + li] = acc;
