@@ -21,6 +21,7 @@
 //     of the lagged boundary-inflow cache (R9), which lands right behind the state row so that "upwind value" is
 //     one shared-memory load whether it is an interior neighbour or a wall.
 #include <algorithm>
+#include <cstdlib>
 
 #include "internal.h"
 
@@ -68,9 +69,9 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 struct SmemLayout {
   uint32_t tq, q, rows, plane, bar, total, rp;
 };
-__host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int gcap, int qcap, int H) {
+__host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int gcap, int qcap, int H, int rp_fixed) {
   SmemLayout L;
-  L.rp = (uint32_t)sp + 2u * (uint32_t)gcap;                 // row pitch in doubles (even)
+  L.rp = rp_fixed ? (uint32_t)rp_fixed : (uint32_t)sp + 2u * (uint32_t)gcap;  // row pitch in doubles (even)
   L.tq = 0;                                                  // [2][pcap] double2
   L.q = L.tq + 2u * (uint32_t)pcap * 16u;                    // [2][qcap] double
   L.rows = L.q + 2u * (uint32_t)qcap * 8u;                   // [G][rp]   double
@@ -80,21 +81,23 @@ __host__ __device__ inline SmemLayout smem_layout(int G, int sp, int pcap, int g
   return L;
 }
 
-// blockDim.x = NT compute threads + 32 (the DMA warp).  R = pencils per compute thread.
-template <int G, int R, bool UNIFORM>
+// blockDim.x = NT compute threads + 32 (the DMA warp).  R = pencils per compute thread.  RP > 0: the row pitch is this
+// compile-time constant (>= sp + 2 gcap), so the per-system shared-memory offsets g*RP*8 fold into the LDS/STS
+// instructions as immediates (27 % of the executed instructions were the IMADs that formed them); RP = 0: run-time pitch.
+template <int G, int R, bool UNIFORM, int RP>
 __global__ void __launch_bounds__(512) sweep_structured_kernel(const SweepArgs a, const OctTab *__restrict__ octs) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int t = threadIdx.x, nt = blockDim.x - 32;
   const int task = blockIdx.x;
   const OctTab T = octs[a.task_oct[task]];
   const int nu = a.nu, sp = a.sp, pcap = a.pcap, gcap = a.gcap, qcap = a.qcap;
-  const SmemLayout L = smem_layout(G, sp, pcap, gcap, qcap, T.H);
+  const SmemLayout L = smem_layout(G, sp, pcap, gcap, qcap, T.H, RP);
   double2 *tq_s = reinterpret_cast<double2 *>(smem + L.tq);
   double *q_s = reinterpret_cast<double *>(smem + L.q);
   double *rows = reinterpret_cast<double *>(smem + L.rows);
   int4 *plane_s = reinterpret_cast<int4 *>(smem + L.plane);
   uint64_t *bar = reinterpret_cast<uint64_t *>(smem + L.bar);
-  const uint32_t rp = L.rp;
+  const uint32_t rp = RP ? (uint32_t)RP : L.rp;
 
   const int row_loc = a.task_row[task];
   const int n_valid = min(G, T.n_rows - row_loc);  // rows past the class's end recompute the last row and store nothing
@@ -419,12 +422,12 @@ __global__ void __launch_bounds__(512) sweep_structured_db_kernel(const SweepArg
 typedef void (*sweep_fn)(const SweepArgs, const OctTab *);
 constexpr int kMaxGR = 24;  // registers: 2*G*R hold the results of a hyperplane; larger products spill
 
-template <int G>
+template <int G, int RP>
 sweep_fn pick_r(int r, bool uniform) {
-#define NB_CASE(RR)                                                                                         \
-  case RR:                                                                                                  \
-    if constexpr (G * RR <= kMaxGR / 2) { if (!uniform) return sweep_structured_kernel<G, RR, false>; }          \
-    if constexpr (G * RR <= kMaxGR) { if (uniform) return sweep_structured_kernel<G, RR, true>; }                 \
+#define NB_CASE(RR)                                                                                              \
+  case RR:                                                                                                       \
+    if constexpr (RP == 0 && G * RR <= kMaxGR / 2) { if (!uniform) return sweep_structured_kernel<G, RR, false, 0>; } \
+    if constexpr (G * RR <= kMaxGR && (RP == 0 || (G >= 2 && RR >= 4 && RR <= 6))) { if (uniform) return sweep_structured_kernel<G, RR, true, RP>; } \
     break;
   switch (r) {
     NB_CASE(1)
@@ -440,12 +443,25 @@ sweep_fn pick_r(int r, bool uniform) {
 #undef NB_CASE
   return nullptr;
 }
-sweep_fn pick(int g, int r, bool uniform) {
+template <int RP>
+sweep_fn pick_g(int g, int r, bool uniform) {
   switch (g) {
-    case 1: return pick_r<1>(r, uniform);
-    case 2: return pick_r<2>(r, uniform);
-    case 3: return pick_r<3>(r, uniform);
-    case 4: return pick_r<4>(r, uniform);
+    case 1: return pick_r<1, RP>(r, uniform);
+    case 2: return pick_r<2, RP>(r, uniform);
+    case 3: return pick_r<3, RP>(r, uniform);
+    case 4: return pick_r<4, RP>(r, uniform);
+  }
+  return nullptr;
+}
+// compile-time row pitches on offer (doubles); a grid whose rows need more, or a small launch shape, runs with RP = 0
+const int kRowPitch[4] = {2048, 3072, 4096, 5120};
+sweep_fn pick(int g, int r, bool uniform, int rp) {
+  switch (rp) {
+    case 0: return pick_g<0>(g, r, uniform);
+    case 2048: return pick_g<2048>(g, r, uniform);
+    case 3072: return pick_g<3072>(g, r, uniform);
+    case 4096: return pick_g<4096>(g, r, uniform);
+    case 5120: return pick_g<5120>(g, r, uniform);
   }
   return nullptr;
 }
@@ -485,7 +501,7 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
   for (int k = 0; k < 4 && !G; ++k) {
     const int g = cand[k];
     if (want_G > 0 && g != want_G) continue;
-    if (smem_layout(g, sp, pcap, gcap, qcap, H).total > smem_cap) continue;
+    if (smem_layout(g, sp, pcap, gcap, qcap, H, 0).total > smem_cap) continue;
     if (g * R > (h->uniform ? kMaxGR : kMaxGR / 2)) continue;  // the non-uniform variant carries 5 more registers per pencil
     if (want_G <= 0 && g > std::max(1, n_sys_min_class)) continue;
     // small problems: rather more CTAs than more systems per CTA, until the machine has two CTAs per SM to run
@@ -494,9 +510,9 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
   }
   if (!G) {
     if (want_G > 0) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "sweep_G=%d with %d pencils per thread needs %u B of shared memory (cap %zu) and G*R <= %d",
-                                   want_G, R, smem_layout(want_G, sp, pcap, gcap, qcap, H).total, smem_cap, kMaxGR);
+                                   want_G, R, smem_layout(want_G, sp, pcap, gcap, qcap, H, 0).total, smem_cap, kMaxGR);
     return nb_fail(h, NANOBTE_E_UNSUPPORTED, "grid cross-section of %d pencils needs %u B of shared memory (> %zu)", n_pen_max,
-                   smem_layout(1, sp, pcap, gcap, qcap, H).total, smem_cap);
+                   smem_layout(1, sp, pcap, gcap, qcap, H, 0).total, smem_cap);
   }
   // double-buffered variant: uniform spacing only, on request
   h->sweep_variant = 3;
@@ -528,7 +544,14 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
   h->sweep_G = G;
   h->sweep_rmax = R;
   h->sweep_threads = T;
-  h->sweep_smem = smem_layout(G, sp, pcap, gcap, qcap, H).total;
+  h->sweep_rp = 0;
+  const char *rp_env = std::getenv("NANOBTE_SWEEP_RP");  // tuning hook: 0 forces the run-time pitch
+  // measured on B200: -6 % on config 4 (G = 4, R = 5), but +30 % with 10 pencils per thread (config 3), hence R <= 6
+  if (h->uniform && G >= 2 && R >= 4 && R <= 6 && !(rp_env && std::atoi(rp_env) == 0)) {
+    for (int k = 0; k < 4 && !h->sweep_rp; ++k)
+      if (kRowPitch[k] >= sp + 2 * gcap && smem_layout(G, sp, pcap, gcap, qcap, H, kRowPitch[k]).total <= smem_cap) h->sweep_rp = kRowPitch[k];
+  }
+  h->sweep_smem = smem_layout(G, sp, pcap, gcap, qcap, H, h->sweep_rp).total;
   h->sw.sp = sp;
   h->sw.pcap = pcap;
   h->sw.gcap = gcap;
@@ -546,7 +569,7 @@ int nb_launch_sweep_structured(nanobte_solver *h) {
       case 4: fn = sweep_structured_db_kernel<4>; break;
     }
   } else {
-    fn = pick(h->sweep_G, h->sweep_rmax, h->uniform);
+    fn = pick(h->sweep_G, h->sweep_rmax, h->uniform, h->sweep_rp);
   }
   if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "no sweep kernel variant for G=%d R=%d", h->sweep_G, h->sweep_rmax);
   if (!h->sweep_attr_set) {
