@@ -1,6 +1,7 @@
 // api.cu -- the C-ABI entry points of libnanobte that do not depend on the mesh kind, plus the host-side
 // validation and the upload of the tables both kinds share.  See include/nanobte.h for the contract.
 #include <algorithm>
+#include <numeric>
 #include <cstdlib>
 
 #include "host_util.h"
@@ -169,7 +170,8 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
   h->cg_rhs = A.zeros<double>(na);
   h->cg_scal = A.zeros<double>(16);
   h->cg_partial = A.zeros<double>(4 * 2048);
-  // fused CG plan: contiguous chunks of cells, one per CTA; halo = neighbours owned by other CTAs
+  // fused CG plan: the cells are renumbered so that every CTA owns a contiguous range that is also compact in space
+  // (recursive coordinate bisection with prescribed part sizes: small halos); halo = neighbours owned by other CTAs
   {
     const int n = (int)na, nf = g.cg_nf;
     const int threads = 512;
@@ -177,6 +179,46 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
     int chunk = (n + nblk - 1) / nblk;
     nblk = (n + chunk - 1) / chunk;
     const int cpt = chunk <= threads ? 1 : chunk <= 2 * threads ? 2 : chunk <= 4 * threads ? 4 : 0;
+    std::vector<int32_t> perm(n), inv(n);  // perm: CG index -> active index
+    std::iota(perm.begin(), perm.end(), 0);
+    if ((int)g.cg_xyz.size() == 3 * n && nblk > 1) {
+      struct Job { int lo, hi, p0, p1; };
+      std::vector<Job> stack{{0, n, 0, nblk}};
+      while (!stack.empty()) {
+        const Job J = stack.back();
+        stack.pop_back();
+        if (J.p1 - J.p0 <= 1) continue;
+        double mn[3] = {1e300, 1e300, 1e300}, mx[3] = {-1e300, -1e300, -1e300};
+        for (int i = J.lo; i < J.hi; ++i)
+          for (int k = 0; k < 3; ++k) {
+            const double v = g.cg_xyz[3 * (size_t)perm[i] + k];
+            mn[k] = std::min(mn[k], v);
+            mx[k] = std::max(mx[k], v);
+          }
+        int ax = 0;
+        for (int k = 1; k < 3; ++k) if (mx[k] - mn[k] > mx[ax] - mn[ax]) ax = k;
+        const int pm = (J.p0 + J.p1) / 2;
+        const int mid = std::min(J.hi, J.lo + (pm - J.p0) * chunk);  // parts p0..pm-1 are full chunks
+        std::nth_element(perm.begin() + J.lo, perm.begin() + mid, perm.begin() + J.hi, [&](int32_t x, int32_t y) {
+          const double vx = g.cg_xyz[3 * (size_t)x + ax], vy = g.cg_xyz[3 * (size_t)y + ax];
+          return vx < vy || (vx == vy && x < y);
+        });
+        stack.push_back({J.lo, mid, J.p0, pm});
+        stack.push_back({mid, J.hi, pm, J.p1});
+      }
+      for (int k = 0; k < nblk; ++k)  // deterministic, memory-friendly order inside a chunk
+        std::sort(perm.begin() + k * chunk, perm.begin() + std::min(n, (k + 1) * chunk));
+    }
+    for (int i = 0; i < n; ++i) inv[perm[i]] = i;
+    std::vector<double> coef_p((size_t)nf * n), diag_p(n);
+    std::vector<int32_t> nbr_p((size_t)nf * n);
+    for (int i = 0; i < n; ++i) {
+      diag_p[i] = g.cg_diag[perm[i]];
+      for (int f = 0; f < nf; ++f) {
+        coef_p[(size_t)f * n + i] = g.cg_coef[(size_t)f * n + perm[i]];
+        nbr_p[(size_t)f * n + i] = inv[g.cg_nbr[(size_t)f * n + perm[i]]];
+      }
+    }
     std::vector<int32_t> nloc((size_t)nf * n), hptr(nblk + 1, 0), hidx;
     int nh_cap = 0;
     for (int k = 0; k < nblk; ++k) {
@@ -184,16 +226,16 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
       std::vector<int32_t> halo;
       for (int i = a0; i < a1; ++i)
         for (int f = 0; f < nf; ++f) {
-          const int j = g.cg_nbr[(size_t)f * n + i];
-          if (g.cg_coef[(size_t)f * n + i] != 0.0 && (j < a0 || j >= a1)) halo.push_back(j);
+          const int j = nbr_p[(size_t)f * n + i];
+          if (coef_p[(size_t)f * n + i] != 0.0 && (j < a0 || j >= a1)) halo.push_back(j);
         }
       std::sort(halo.begin(), halo.end());
       halo.erase(std::unique(halo.begin(), halo.end()), halo.end());
       for (int i = a0; i < a1; ++i)
         for (int f = 0; f < nf; ++f) {
-          const int j = g.cg_nbr[(size_t)f * n + i];
+          const int j = nbr_p[(size_t)f * n + i];
           int32_t loc = i - a0;  // faces without a neighbour carry coefficient 0 and point at the cell itself
-          if (g.cg_coef[(size_t)f * n + i] != 0.0)
+          if (coef_p[(size_t)f * n + i] != 0.0)
             loc = (j >= a0 && j < a1) ? j - a0 : chunk + (int32_t)(std::lower_bound(halo.begin(), halo.end(), j) - halo.begin());
           nloc[(size_t)f * n + i] = loc;
         }
@@ -201,6 +243,9 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
       hptr[k + 1] = (int32_t)hidx.size();
       nh_cap = std::max(nh_cap, (int)halo.size());
     }
+    h->cgf_perm = A.put(perm);
+    h->cgf_coef = A.put(coef_p);
+    h->cgf_diag = A.put(diag_p);
     h->cgf_nblk = nblk; h->cgf_chunk = chunk; h->cgf_cpt = cpt; h->cgf_nh_cap = nh_cap;
     h->cgf_smem = (3 * (size_t)chunk + 2 * (size_t)nh_cap) * sizeof(double) + (size_t)nh_cap * sizeof(int32_t) + 1024;
     h->cgf_ok = cpt > 0 && chunk + nh_cap < 65536 && (nf == 3 || nf == 4 || nf == 6) && h->cgf_smem <= 200 * 1024;

@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(256) cg_kernel(CgArgs a) {
 // =================================================================================================================
 struct CgfArgs {
   int32_t n, nf, nblk, chunk, nh_cap, max_iter, B;
-  const int32_t *nloc;
+  const int32_t *nloc, *perm;
   const double *coef, *diag, *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
   const int32_t *cellbf_ptr, *cellbf, *hptr, *hidx;
   double *x, *w, *part;
@@ -208,8 +208,9 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
         if (kStencilInRegs) cf[c % CR][f] = a.coef[(size_t)f * n + i];
       }
       dg[c] = a.diag[i];
-      double rhs = a.vol[i] * a.beta * (a.theta_SI[i] - a.theta_prev[i]);   // R14c
-      for (int q = a.cellbf_ptr[i]; q < a.cellbf_ptr[i + 1]; ++q) {         // R14c'
+      const int io = a.perm[i];  // the cell in the solver's own (active) numbering
+      double rhs = a.vol[io] * a.beta * (a.theta_SI[io] - a.theta_prev[io]);  // R14c
+      for (int q = a.cellbf_ptr[io]; q < a.cellbf_ptr[io + 1]; ++q) {        // R14c'
         const int bf = a.cellbf[q];
         double F = 0.0;
         for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
@@ -356,7 +357,7 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
 #pragma unroll
   for (int c = 0; c < CPT; ++c) {
     const int li = tid + c * kCgfThreads;
-    if (li < nown) a.x[a0 + li] = x_s[li];
+    if (li < nown) a.x[a.perm[a0 + li]] = x_s[li];
   }
   if (k == 0 && tid == 0) *a.iters_out = (unsigned long long)it;
 }
@@ -386,7 +387,7 @@ static int cg_solve_fused(nanobte_solver *h) {
   CgfArgs a;
   a.n = h->n_act; a.nf = h->cg_nf; a.nblk = h->cgf_nblk; a.chunk = h->cgf_chunk; a.nh_cap = h->cgf_nh_cap;
   a.max_iter = h->cg_max_iter; a.B = h->B;
-  a.nloc = h->cgf_nloc; a.coef = h->cg_coef; a.diag = h->cg_diag; a.vol = h->vol;
+  a.nloc = h->cgf_nloc; a.perm = h->cgf_perm; a.coef = h->cgf_coef; a.diag = h->cgf_diag; a.vol = h->vol;
   a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev; a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area;
   a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf; a.hptr = h->cgf_hptr; a.hidx = h->cgf_hidx;
   a.x = h->cg_x; a.w = h->cgf_w; a.part = h->cgf_part; a.bar = h->cgf_bar;

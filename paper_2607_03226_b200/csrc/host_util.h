@@ -79,6 +79,7 @@ struct GenericTables {
   std::vector<int32_t> cg_nbr;
   std::vector<double> cg_coef, cg_diag;
   std::vector<int32_t> cellbf_ptr, cellbf;
+  std::vector<double> cg_xyz;      // [n][3] cell centres in any consistent unit (partitioning of the CG only)
   std::vector<int32_t> tagface_ptr, tagface;
   int64_t bin_total = 0;
 };

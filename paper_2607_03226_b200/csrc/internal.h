@@ -142,6 +142,8 @@ struct nanobte_solver {
   bool cgf_ok = false, cg_force_generic = false;
   int cgf_nblk = 0, cgf_chunk = 0, cgf_cpt = 0, cgf_nh_cap = 0;
   size_t cgf_smem = 0;
+  const int32_t *cgf_perm = nullptr;   // [n] CG index -> active cell index (spatially compact chunks)
+  const double *cgf_coef = nullptr, *cgf_diag = nullptr;  // stencil in CG order
   const int32_t *cgf_nloc = nullptr;   // [nf][n] index of the neighbour inside its owner CTA's local vector
   const int32_t *cgf_hptr = nullptr;   // [nblk+1] halo lists
   const int32_t *cgf_hidx = nullptr;   // global cell index of every halo entry

@@ -411,6 +411,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   // ---- cells: volumes, source, initial theta, diffusion stencil ------------------------------------------------------------------
   G.vol.resize(na); G.Qdot_act.resize(na); G.theta0.resize(na);
   G.cg_nf = nside;
+  G.cg_xyz.assign((size_t)3 * na, 0.0);
   G.cg_nbr.assign((size_t)nside * na, 0);
   G.cg_coef.assign((size_t)nside * na, 0.0);
   G.cg_diag.assign(na, 0.0);
@@ -420,6 +421,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     int ijk[3] = {c % g.n[0], (c / g.n[0]) % g.n[1], c / (g.n[0] * g.n[1])};
     const double hh[3] = {g.hsz[0][ijk[0]], g.hsz[1][ijk[1]], dim == 3 ? g.hsz[2][ijk[2]] : 1.0};
     G.vol[a] = hh[0] * hh[1] * hh[2];
+    for (int k = 0; k < 3; ++k) G.cg_xyz[3 * (size_t)a + k] = ijk[k];
     G.Qdot_act[a] = Qdot ? Qdot[c] : 0.0;
     G.theta0[a] = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
     for (int side = 0; side < nside; ++side) {

@@ -537,7 +537,10 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
   G.cg_coef.assign((size_t)maxf * nc, 0.0);
   G.cg_diag.assign(nc, 0.0);
   G.cellbf_ptr.assign(nc + 1, 0);
+  G.cg_xyz.assign((size_t)3 * nc, 0.0);
   for (int c = 0; c < nc; ++c) {
+    G.cg_xyz[3 * (size_t)c] = cen[2 * c];
+    G.cg_xyz[3 * (size_t)c + 1] = cen[2 * c + 1];
     G.Qdot_act[c] = Qdot ? Qdot[c] : 0.0;
     G.theta0[c] = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
     for (int k = 0; k < maxf; ++k) G.cg_nbr[(size_t)k * nc + c] = c;
