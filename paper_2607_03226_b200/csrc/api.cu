@@ -219,6 +219,17 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
         nbr_p[(size_t)f * n + i] = inv[g.cg_nbr[(size_t)f * n + perm[i]]];
       }
     }
+    // face-uniform stencil (uniform structured grids): every face slot has one coefficient value, or none
+    bool uni = nf <= 6;
+    double cfu[6] = {0, 0, 0, 0, 0, 0};
+    for (int f = 0; f < nf && uni; ++f)
+      for (int i = 0; i < n && uni; ++i) {
+        const double c = coef_p[(size_t)f * n + i];
+        if (c == 0.0) continue;
+        if (cfu[f] == 0.0) cfu[f] = c;
+        uni = cfu[f] == c;
+      }
+    if (std::getenv("NANOBTE_CG_NO_UNI")) uni = false;  // test hook: the general stencil path
     std::vector<int32_t> nloc((size_t)nf * n), hptr(nblk + 1, 0), hidx;
     int nh_cap = 0;
     for (int k = 0; k < nblk; ++k) {
@@ -246,6 +257,13 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
     h->cgf_perm = A.put(perm);
     h->cgf_coef = A.put(coef_p);
     h->cgf_diag = A.put(diag_p);
+    nh_cap += 1;  // one more slot that is in nobody's halo: stays zero
+    if (uni)      // a missing neighbour reads the zero slot (its coefficient is the face's, not 0)
+      for (int i = 0; i < n; ++i)
+        for (int f = 0; f < nf; ++f)
+          if (coef_p[(size_t)f * n + i] == 0.0) nloc[(size_t)f * n + i] = chunk + nh_cap - 1;
+    h->cgf_uni = uni;
+    for (int f = 0; f < 6; ++f) h->cgf_cfu[f] = cfu[f];
     h->cgf_nblk = nblk; h->cgf_chunk = chunk; h->cgf_cpt = cpt; h->cgf_nh_cap = nh_cap;
     h->cgf_smem = (3 * (size_t)chunk + 2 * (size_t)nh_cap) * sizeof(double) + (size_t)nh_cap * sizeof(int32_t) + 1024;
     h->cgf_ok = cpt > 0 && chunk + nh_cap < 65536 && (nf == 3 || nf == 4 || nf == 6) && h->cgf_smem <= 200 * 1024;

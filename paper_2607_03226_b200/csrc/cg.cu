@@ -143,6 +143,7 @@ struct CgfArgs {
   unsigned int *bar;
   unsigned long long *iters_out;
   double beta, rtol;
+  double cfu[6];  // face-uniform stencil: the one non-zero coefficient of every face slot
 };
 
 __device__ __forceinline__ void grid_barrier(unsigned int *bar, unsigned int target) {
@@ -166,7 +167,9 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 #define NB_STAMP(k) do {} while (0)
 #endif
 
-template <int NF, int CPT>
+// UNI: every face slot carries one coefficient value or none (uniform structured grids).  The coefficients are then
+// kernel parameters, and a missing neighbour points at a slot of r_loc that stays zero.
+template <int NF, int CPT, bool UNI>
 __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
   extern __shared__ __align__(16) unsigned char cgf_smem[];
   double *r_loc = reinterpret_cast<double *>(cgf_smem);           // [chunk + nh_cap]
@@ -184,9 +187,10 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
     hidx_s[j] = a.hidx[h0 + j];
     s_h[j] = 0.0;
   }
+  if (tid == 0) r_loc[a.chunk + a.nh_cap - 1] = 0.0;  // the last halo slot belongs to no CTA's halo: the zero slot
   // Stencil of the thread's cells: in registers up to 2 cells per thread; with 4 the 48 coefficient registers would
   // spill, so the coefficients are re-read every iteration through the read-only path (95 KB per CTA: L1-resident).
-  constexpr bool kStencilInRegs = CPT <= 2;
+  constexpr bool kStencilInRegs = CPT <= 2 && !UNI;
   constexpr int CR = kStencilInRegs ? CPT : 1;
   double cf[CR][NF], dg[CPT], r[CPT], s[CPT], wv[CPT];
   uint16_t nl[CPT][NF];  // local indices < 65536 (checked when the plan is built); always in registers
@@ -236,7 +240,8 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
         double acc = dg[c] * r[c];
 #pragma unroll
         for (int f = 0; f < NF; ++f) {
-          if (kStencilInRegs) acc -= cf[c % CR][f] * r_loc[nl[c][f]];
+          if (UNI) acc -= a.cfu[f] * r_loc[nl[c][f]];
+          else if (kStencilInRegs) acc -= cf[c % CR][f] * r_loc[nl[c][f]];
           else acc -= __ldg(a.coef + (size_t)f * n + a0 + li) * r_loc[nl[c][f]];
         }
         wv[c] = acc;
@@ -363,26 +368,26 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
 }
 
 typedef void (*cgf_fn)(CgfArgs);
-template <int NF>
+template <int NF, bool UNI>
 static cgf_fn cgf_pick_cpt(int cpt) {
   switch (cpt) {
-    case 1: return cg_fused_kernel<NF, 1>;
-    case 2: return cg_fused_kernel<NF, 2>;
-    case 4: return cg_fused_kernel<NF, 4>;
+    case 1: return cg_fused_kernel<NF, 1, UNI>;
+    case 2: return cg_fused_kernel<NF, 2, UNI>;
+    case 4: return cg_fused_kernel<NF, 4, UNI>;
   }
   return nullptr;
 }
-static cgf_fn cgf_pick(int nf, int cpt) {
+static cgf_fn cgf_pick(int nf, int cpt, bool uni) {
   switch (nf) {
-    case 3: return cgf_pick_cpt<3>(cpt);
-    case 4: return cgf_pick_cpt<4>(cpt);
-    case 6: return cgf_pick_cpt<6>(cpt);
+    case 3: return uni ? cgf_pick_cpt<3, true>(cpt) : cgf_pick_cpt<3, false>(cpt);
+    case 4: return uni ? cgf_pick_cpt<4, true>(cpt) : cgf_pick_cpt<4, false>(cpt);
+    case 6: return uni ? cgf_pick_cpt<6, true>(cpt) : cgf_pick_cpt<6, false>(cpt);
   }
   return nullptr;
 }
 
 static int cg_solve_fused(nanobte_solver *h) {
-  cgf_fn fn = cgf_pick(h->cg_nf, h->cgf_cpt);
+  cgf_fn fn = cgf_pick(h->cg_nf, h->cgf_cpt, h->cgf_uni);
   if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "internal: no fused CG variant for nf=%d cpt=%d", h->cg_nf, h->cgf_cpt);
   CgfArgs a;
   a.n = h->n_act; a.nf = h->cg_nf; a.nblk = h->cgf_nblk; a.chunk = h->cgf_chunk; a.nh_cap = h->cgf_nh_cap;
@@ -393,6 +398,7 @@ static int cg_solve_fused(nanobte_solver *h) {
   a.x = h->cg_x; a.w = h->cgf_w; a.part = h->cgf_part; a.bar = h->cgf_bar;
   a.iters_out = h->d_maxdT + 1;
   a.beta = h->beta; a.rtol = h->cg_rtol;
+  for (int f = 0; f < 6; ++f) a.cfu[f] = h->cgf_cfu[f];
   NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->cgf_smem));
   NB_CUDA(h, cudaMemsetAsync(h->cgf_bar, 0, sizeof(unsigned int), h->stream));
   void *args[] = {&a};

@@ -139,7 +139,8 @@ struct nanobte_solver {
   double *cg_partial = nullptr;
   int cg_blocks = 0;
   // fused CG (cg.cu, cg_fused_kernel): cells cut into one contiguous chunk per CTA, vectors on chip
-  bool cgf_ok = false, cg_force_generic = false;
+  bool cgf_ok = false, cg_force_generic = false, cgf_uni = false;
+  double cgf_cfu[6] = {0, 0, 0, 0, 0, 0};  // face-uniform stencil coefficients (cgf_uni)
   int cgf_nblk = 0, cgf_chunk = 0, cgf_cpt = 0, cgf_nh_cap = 0;
   size_t cgf_smem = 0;
   const int32_t *cgf_perm = nullptr;   // [n] CG index -> active cell index (spatially compact chunks)
