@@ -98,6 +98,7 @@ struct nanobte_solver {
 
   // unstructured sweep (see sweep_unstructured.cu)
   struct UnsArgs *uns = nullptr;
+  bool uns_staged = false;
 
   BoundaryArgs bd{};
   // structured grids: closures split into a G/flux kernel over reflecting faces and an inflow-cache kernel

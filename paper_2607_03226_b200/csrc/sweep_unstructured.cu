@@ -23,6 +23,14 @@
 struct UnsArgs {
   int32_t D, B, BG, NBG, MI, cpp;   // bands per CTA, band groups, max inflow faces per cell, cells per pass
   int32_t rcap;                     // positions held by the shared-memory ring (power of two)
+  // staged variant (sweep_unstructured_staged_kernel)
+  int32_t st_BG, st_NBG, st_threads, st_vr, st_rr, st_sr;  // bands per CTA, groups, threads, ring capacities (powers of two)
+  const int32_t *st_up;             // [MI][D][e_stride] upwind codes: ring / side / late
+  const int32_t *side_ptr;          // [D][l_max+2] first side entry of each level (per direction)
+  const int32_t *side_src;          // per direction from side_base[d]: >= 0 position in e, < 0: -1 - inflow index
+  const int64_t *side_base;         // [D]
+  double *thetaP;                   // [D][e_stride] theta in sweep order (refreshed before every sweep)
+  const double *QP;                 // [D][e_stride] Qdot in sweep order
   int32_t n_act, l_max;
   int64_t e_stride;                 // positions per direction (n_act rounded up)
   const int32_t *n_lvl;             // [D]
@@ -182,6 +190,146 @@ __global__ void __launch_bounds__(256, 3) sweep_unstructured_kernel(const UnsArg
   }
 }
 
+// ---- (a5) staged variant --------------------------------------------------------------------------------------------
+// Same arithmetic, but between two level barriers a thread touches only shared memory:
+//   * the per-position records (theta and Qdot pre-permuted per direction, outflow sum, inflow coefficients, upwind
+//     codes) stream into a ring of `rr` positions by cp.async, up to rr positions ahead of the level in progress;
+//   * an upwind value is read from the value ring (the last `vr` outputs), or -- wall inflow and upwind cells at
+//     least 3 levels back -- from a side ring that cp.async fills 2 levels ahead (the sources are final by then);
+//     the rare reference in between (a level wider than the ring) is a global load after the barrier.
+//   * one CTA per SM: (direction, group of bands) with 32 cells per pass; every thread issues its share of the
+//     copies at the top of a level, commits one group per level and waits for the previous level's group before
+//     the barrier, so a copy has a level time to land.  create() checks the spans that make this safe
+//     (3 consecutive levels fit the record ring, their side entries the side ring) and falls back otherwise.
+constexpr int32_t kStRing = 1 << 29, kStSide = 1 << 28, kStIn = 1 << 27, kStMask = (1 << 27) - 1;
+
+__device__ __forceinline__ void cp_async8(void *dst, const void *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void *dst, const void *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+
+__global__ void theta_permute_kernel(const UnsArgs a) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (int64_t)a.D * a.e_stride) return;
+  const int pos = (int)(i % a.e_stride);
+  if (pos < a.n_act) a.thetaP[i] = a.theta[a.cell[i]];
+}
+
+template <int MI>
+__global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const UnsArgs a) {
+  extern __shared__ __align__(16) unsigned char st_smem[];
+  const int BG = a.st_BG, VR = a.st_vr, RR = a.st_rr, SR = a.st_sr;
+  double *vring = reinterpret_cast<double *>(st_smem);  // [VR][BG]
+  double *side = vring + (size_t)VR * BG;                // [SR][BG]
+  double *th_s = side + (size_t)SR * BG;                 // [RR]
+  double *q_s = th_s + RR;
+  double *go_s = q_s + RR;
+  double *gi_s = go_s + RR;                              // [MI][RR]
+  int32_t *up_s = reinterpret_cast<int32_t *>(gi_s + (size_t)MI * RR);  // [MI][RR]
+  const int d = blockIdx.x / a.st_NBG, bg = blockIdx.x % a.st_NBG;
+  const int tid = threadIdx.x, nth = blockDim.x;
+  const int slot0 = tid / BG, bl = tid - slot0 * BG;
+  const int b = bg * BG + bl;
+  const bool live = b < a.B && slot0 < 32;
+  const int bb = min(b, a.B - 1);
+  const double kA = a.kA[bb], kS = a.kS[bb], itau = a.itau[bb], vb = a.vb[bb];
+  const int64_t dbase = (int64_t)d * a.e_stride;
+  double *const ed = a.e + dbase * a.B + bb;
+  const double *const eband0 = a.e + dbase * a.B + (int64_t)bg * BG;          // + src * B + band within group
+  const double *const bin0 = a.bin + a.dir_bin[d] + (int64_t)bg * BG * a.dir_nin[d];
+  const int64_t nin = a.dir_nin[d];
+  const double *const bin_b = a.bin + a.dir_bin[d] + (int64_t)bb * nin;
+  const int32_t *const lp = a.lvl_ptr + (int64_t)d * (a.l_max + 1);
+  const int32_t *const sp = a.side_ptr + (int64_t)d * (a.l_max + 2);
+  const int32_t *const ssrc = a.side_src + a.side_base[d];
+  const int64_t kstride = (int64_t)a.D * a.e_stride;
+  const int n_lvl = a.n_lvl[d], n_act = a.n_act;
+  const int nbg = min(BG, a.B - bg * BG);  // bands of this group that exist
+
+  int pf = 0, sf = 0;  // next record position / side entry to request (identical in every thread)
+  // Side copies: the thread (cell slot slot0, band bl) copies band bl of the entries sf + slot0, sf + slot0 + 32, ...
+  // (no index arithmetic beyond an add); the sources of the next level's first two are prefetched into registers.
+  constexpr int PRE = 2;
+  int pre_src[PRE], pre_sf = -1;
+  auto prefetch_src = [&](int s0, int s1) {
+    pre_sf = s0;
+#pragma unroll
+    for (int i = 0; i < PRE; ++i) {
+      const int e = s0 + slot0 + 32 * i;
+      pre_src[i] = (live && e < s1) ? __ldg(ssrc + e) : 0;
+    }
+  };
+  auto issue = [&](int pf_end, int sf_end) {
+    for (int p = pf + tid; p < pf_end; p += nth) {
+      const int s = p & (RR - 1);
+      const int64_t g = dbase + p;
+      cp_async8(th_s + s, a.thetaP + g);
+      cp_async8(q_s + s, a.QP + g);
+      cp_async8(go_s + s, a.gout + g);
+#pragma unroll
+      for (int k = 0; k < MI; ++k) {
+        cp_async8(gi_s + k * RR + s, a.gin + k * kstride + g);
+        cp_async4(up_s + k * RR + s, a.st_up + k * kstride + g);
+      }
+    }
+    pf = max(pf, pf_end);
+    if (live) {
+      const bool hit = pre_sf == sf;
+      int i = 0;
+      for (int e = sf + slot0; e < sf_end; e += 32, ++i) {
+        const int src = (hit && i < PRE) ? (i == 0 ? pre_src[0] : pre_src[1]) : __ldg(ssrc + e);
+        const double *from = src >= 0 ? ed + (int64_t)src * a.B : bin_b + (-1 - src);
+        cp_async8(side + (size_t)(e & (SR - 1)) * BG + bl, from);
+      }
+    }
+    sf = max(sf, sf_end);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  // prologue: everything the first levels need, fully landed
+  issue(min(n_act, RR), min(sp[min(2, n_lvl)], SR));
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  // level table entries one level ahead in registers: no global load sits between a barrier and the level's work
+  int lo = lp[0], hi = n_lvl > 0 ? lp[1] : 0, hi_n = lp[min(2, n_lvl)];
+  int sp_l = sp[0], sp_l4 = sp[min(3, n_lvl)], sp_n = sp[min(1, n_lvl)], sp_n4 = sp[min(4, n_lvl)];
+  prefetch_src(sf, max(sf, min(sp_l4, sp_l + SR)));
+  __syncthreads();
+
+  for (int l = 0; l < n_lvl; ++l) {
+    issue(min(n_act, lo + RR), min(sp_l4, sp_l + SR));
+    // next level's table entries and side sources, in flight while this level is computed
+    const int hi_nn = lp[min(l + 3, n_lvl)];
+    const int sp_nn = sp[min(l + 2, n_lvl)], sp_nn4 = sp[min(l + 5, n_lvl)];
+    prefetch_src(sf, max(sf, min(sp_n4, sp_n + SR)));
+    if (live) {
+      for (int pos = lo + slot0; pos < hi; pos += 32) {
+        const int s = pos & (RR - 1);
+        double num = kA * th_s[s] + kS * q_s[s];
+        const double den = itau + vb * go_s[s];
+#pragma unroll
+        for (int k = 0; k < MI; ++k) {
+          const int u = up_s[k * RR + s];
+          if (u != kNone) {
+            const int x = u & kStMask;
+            const double val = (u & kStRing) ? vring[(size_t)(x & (VR - 1)) * BG + bl]
+                               : (u & kStSide) ? side[(size_t)(x & (SR - 1)) * BG + bl]
+                               : (u & kStIn) ? bin_b[x] : ed[(int64_t)x * a.B];  // the last two: late, from global memory
+            num += vb * gi_s[k * RR + s] * val;
+          }
+        }
+        const double res = num / den;
+        ed[(int64_t)pos * a.B] = res;
+        vring[(size_t)(pos & (VR - 1)) * BG + bl] = res;
+      }
+    }
+    asm volatile("cp.async.wait_group 1;" ::: "memory");
+    __syncthreads();
+    lo = hi; hi = hi_n; hi_n = hi_nn;
+    sp_l = sp_n; sp_l4 = sp_n4; sp_n = sp_nn; sp_n4 = sp_nn4;
+  }
+}
+
 // ---- (a6) moments in the per-direction layout: one warp per cell, lanes over bands, directions in order ---------------------
 __global__ void __launch_bounds__(256) moments_unstructured_kernel(const UnsArgs a) {
   extern __shared__ double sm[];  // w[D], s[D][3]
@@ -270,8 +418,33 @@ uns_fn pick_uns(int mi) {
 
 }  // namespace
 
+typedef void (*uns_st_fn)(const UnsArgs);
+static uns_st_fn pick_uns_staged(int mi) {
+  switch (mi) {
+    case 1: return sweep_unstructured_staged_kernel<1>;
+    case 2: return sweep_unstructured_staged_kernel<2>;
+    case 3: return sweep_unstructured_staged_kernel<3>;
+    case 4: return sweep_unstructured_staged_kernel<4>;
+  }
+  return nullptr;
+}
+
 int nb_launch_sweep_unstructured(nanobte_solver *h) {
   const UnsArgs &a = *h->uns;
+  if (h->uns_staged) {
+    uns_st_fn fs = pick_uns_staged(a.MI);
+    const int64_t n = (int64_t)a.D * a.e_stride;
+    theta_permute_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(a);
+    h->launches++;
+    if (!h->sweep_attr_set) {
+      NB_CUDA(h, cudaFuncSetAttribute(fs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->sweep_smem));
+      h->sweep_attr_set = true;
+    }
+    fs<<<a.D * a.st_NBG, a.st_threads, h->sweep_smem, h->stream>>>(a);
+    h->launches++;
+    NB_CUDA(h, cudaGetLastError());
+    return 0;
+  }
   uns_fn fn = pick_uns(a.MI);
   if (!fn) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "cells with more than 7 inflow faces are not supported");
   if (!h->sweep_attr_set) {
@@ -597,6 +770,67 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
     }
   }
 
+  // ---- staged variant: launch shape, upwind codes, side lists, spans ---------------------------------------------------------
+  int st_NBG = std::max(1, std::min(B, h->n_sm / std::max(1, D)));
+  int st_BG = opt->sweep_G > 0 ? std::min(opt->sweep_G, B) : (B + st_NBG - 1) / st_NBG;
+  st_BG = std::min(st_BG, 20);
+  st_NBG = (B + st_BG - 1) / st_BG;
+  const int st_threads = (32 * st_BG + 31) / 32 * 32;
+  // shared-memory budget of the one CTA per SM: record ring (fixed), a side ring of 64 entries, the rest for the value ring
+  const size_t st_budget = 225 * 1024;
+  const size_t st_rec = (size_t)1024 * ((3 + MI) * sizeof(double) + MI * sizeof(int32_t));
+  int st_sr = 64, st_vr = 64;
+  while (st_rec + (size_t)st_sr * st_BG * sizeof(double) + (size_t)st_vr * 2 * st_BG * sizeof(double) + 64 <= st_budget && st_vr < 4096) st_vr *= 2;
+  while (st_rec + (size_t)st_sr * 2 * st_BG * sizeof(double) + (size_t)st_vr * st_BG * sizeof(double) + 64 <= st_budget && st_sr < 1024) st_sr *= 2;
+  const int st_rr = 1024;
+  bool staged = MI <= 4 && std::getenv("NANOBTE_UNS_PLAIN") == nullptr;
+  std::vector<int32_t> st_up(up.size(), kNone), side_ptr((size_t)D * (l_max + 2), 0), side_src;
+  std::vector<int64_t> side_base(D, 0);
+  long n_late = 0;
+  {
+    std::vector<int32_t> lvl_of(nc);
+    for (int d = 0; d < D && staged; ++d) {
+      const std::vector<int32_t> &lp = lvl_ptrs[d];
+      for (int l = 0; l < n_lvl[d]; ++l)
+        for (int pos = lp[l]; pos < lp[l + 1]; ++pos) lvl_of[pos] = l;
+      side_base[d] = (int64_t)side_src.size();
+      int32_t ns = 0;
+      for (int l = 0; l < n_lvl[d]; ++l) {
+        side_ptr[(size_t)d * (l_max + 2) + l] = ns;
+        for (int pos = lp[l]; pos < lp[l + 1]; ++pos)
+          for (int k = 0; k < MI; ++k) {
+            const size_t r = (size_t)k * D * e_stride + (size_t)d * e_stride + pos;
+            const int32_t u = up[r] == kNone ? kNone : (up[r] < 0 ? up[r] : (up[r] & kUpMask));
+            if (u == kNone) continue;
+            if (u >= 0 && u >= lp[l + 1] - st_vr) { st_up[r] = kStRing | u; continue; }
+            // wall inflow, or final long before its turn: side ring -- if the entry can be requested in time (entries of
+            // level l are requested at level l-2, at most st_sr beyond the first entry of that level)
+            const int32_t first = side_ptr[(size_t)d * (l_max + 2) + std::max(0, l - 2)];
+            if ((u < 0 || lvl_of[u] <= l - 3) && ns - first < st_sr) {
+              st_up[r] = kStSide | ns++;
+              side_src.push_back(u);
+              continue;
+            }
+            st_up[r] = u < 0 ? (kStIn | (-1 - u)) : u;  // late: global load after the level barrier
+            ++n_late;
+          }
+      }
+      for (int l = n_lvl[d]; l < l_max + 2; ++l) side_ptr[(size_t)d * (l_max + 2) + l] = ns;
+      if (ns >= (1 << 27) || nc >= (1 << 27)) staged = false;
+      for (int l = 0; l < n_lvl[d] && staged; ++l) {  // three consecutive levels must fit the rings
+        const int l4 = std::min(l + 3, n_lvl[d]);
+        if (lp[l4] - lp[l] > st_rr) { staged = false; if (std::getenv("NANOBTE_DEBUG")) fprintf(stderr, "staged off: dir %d level %d span %d > %d\n", d, l, lp[l4] - lp[l], st_rr); }
+      }
+    }
+  }
+  const size_t st_smem = ((size_t)st_vr * st_BG + (size_t)st_sr * st_BG + (size_t)st_rr * (3 + MI)) * sizeof(double) +
+                         (size_t)st_rr * MI * sizeof(int32_t) + 64;
+  if (st_smem > 227 * 1024 - 512) staged = false;
+  if (std::getenv("NANOBTE_DEBUG")) fprintf(stderr, "unstructured sweep: staged %d BG %d NBG %d vr %d sr %d smem %zu MI %d late refs %ld side entries %zu\n", (int)staged, st_BG, st_NBG, st_vr, st_sr, st_smem, MI, n_late, side_src.size());
+  std::vector<double> QP((size_t)D * e_stride, 0.0);
+  for (int d = 0; d < D; ++d)
+    for (int pos = 0; pos < nc; ++pos) QP[(size_t)d * e_stride + pos] = Qdot ? Qdot[cellat[(size_t)d * e_stride + pos]] : 0.0;
+
   std::vector<int32_t> lvl_ptr((size_t)D * (l_max + 1), 0);
   for (int d = 0; d < D; ++d) {
     for (int l = 0; l <= l_max; ++l) lvl_ptr[(size_t)d * (l_max + 1) + l] = lvl_ptrs[d][std::min(l, n_lvl[d])];
@@ -613,6 +847,11 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
   h->kind = 1; h->n_cells = nc; h->n_cls = D; h->n_planes = l_max; h->n_tasks = D * NBG;
   h->sweep_G = BG; h->sweep_threads = threads; h->sweep_rmax = MI; h->pencil_axis = -1;
   h->n_pos = nc; h->e_stride = e_stride; h->sweep_smem = (size_t)rcap * BG * sizeof(double);
+  h->uns_staged = staged;
+  if (staged) {
+    h->sweep_smem = st_smem;
+    h->n_tasks = D * st_NBG; h->sweep_G = st_BG; h->sweep_threads = st_threads;
+  }
   h->T_ref = opt->T_ref;
   h->cg_rtol = opt->cg_rtol > 0 ? opt->cg_rtol : 1e-12;
   h->cg_max_iter = opt->cg_max_iter > 0 ? opt->cg_max_iter : 100000;
@@ -626,6 +865,13 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
     rc = nb_upload_generic(h, A, cm, G);
     if (rc) return nb_fail(h, rc, "device upload failed");
     u.D = D; u.B = B; u.BG = BG; u.NBG = NBG; u.MI = MI; u.cpp = cpp; u.rcap = rcap; u.n_act = nc; u.l_max = l_max; u.e_stride = e_stride;
+    u.st_BG = st_BG; u.st_NBG = st_NBG; u.st_threads = st_threads; u.st_vr = st_vr; u.st_rr = st_rr; u.st_sr = st_sr;
+    u.st_up = A.put(st_up);
+    u.side_ptr = A.put(side_ptr);
+    u.side_src = A.put(side_src);
+    u.side_base = A.put(side_base);
+    u.thetaP = A.zeros<double>((size_t)D * e_stride);
+    u.QP = A.put(QP);
     u.n_lvl = A.put(n_lvl);
     u.lvl_ptr = A.put(lvl_ptr);
     u.cell = A.put(cellat);
