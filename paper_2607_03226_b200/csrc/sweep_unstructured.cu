@@ -201,7 +201,9 @@ __global__ void __launch_bounds__(256, 3) sweep_unstructured_kernel(const UnsArg
 //     copies at the top of a level, commits one group per level and waits for the previous level's group before
 //     the barrier, so a copy has a level time to land.  create() checks the spans that make this safe
 //     (3 consecutive levels fit the record ring, their side entries the side ring) and falls back otherwise.
-constexpr int32_t kStRing = 1 << 29, kStSide = 1 << 28, kStIn = 1 << 27, kStMask = (1 << 27) - 1;
+// upwind codes: >= 0 shared-memory offset (slot * BG) in the value ring or the side ring behind it; kStLate (sign bit
+// set, != kNone): position in e, or with kStIn an index into the band's inflow row
+constexpr int32_t kStLate = INT32_MIN | (1 << 30), kStIn = 1 << 27, kStMask = (1 << 27) - 1;
 
 __device__ __forceinline__ void cp_async8(void *dst, const void *src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
@@ -311,14 +313,12 @@ __global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const
         for (int k = 0; k < MI; ++k) {
           const int u = up_s[k * RR + s];
           if (u != kNone) {
-            const int x = u & kStMask;
-            const double val = (u & kStRing) ? vring[(size_t)(x & (VR - 1)) * BG + bl]
-                               : (u & kStSide) ? side[(size_t)(x & (SR - 1)) * BG + bl]
-                               : (u & kStIn) ? bin_b[x] : ed[(int64_t)x * a.B];  // the last two: late, from global memory
+            // ring and side references carry their shared-memory offset (slot * BG) ready-made; the rest is late
+            const double val = u >= 0 ? vring[u + bl] : (u & kStIn) ? bin_b[u & kStMask] : ed[(int64_t)(u & kStMask) * a.B];
             num += vb * gi_s[k * RR + s] * val;
           }
         }
-        const double res = num / den;
+        const double res = num * __drcp_rn(den);  // within 1 ulp of num / den
         ed[(int64_t)pos * a.B] = res;
         vring[(size_t)(pos & (VR - 1)) * BG + bl] = res;
       }
@@ -802,16 +802,17 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
             const size_t r = (size_t)k * D * e_stride + (size_t)d * e_stride + pos;
             const int32_t u = up[r] == kNone ? kNone : (up[r] < 0 ? up[r] : (up[r] & kUpMask));
             if (u == kNone) continue;
-            if (u >= 0 && u >= lp[l + 1] - st_vr) { st_up[r] = kStRing | u; continue; }
+            if (u >= 0 && u >= lp[l + 1] - st_vr) { st_up[r] = (u & (st_vr - 1)) * st_BG; continue; }  // offset in the value ring
             // wall inflow, or final long before its turn: side ring -- if the entry can be requested in time (entries of
             // level l are requested at level l-2, at most st_sr beyond the first entry of that level)
             const int32_t first = side_ptr[(size_t)d * (l_max + 2) + std::max(0, l - 2)];
             if ((u < 0 || lvl_of[u] <= l - 3) && ns - first < st_sr) {
-              st_up[r] = kStSide | ns++;
+              st_up[r] = (st_vr + (ns & (st_sr - 1))) * st_BG;  // offset in the side ring, which follows the value ring
+              ++ns;
               side_src.push_back(u);
               continue;
             }
-            st_up[r] = u < 0 ? (kStIn | (-1 - u)) : u;  // late: global load after the level barrier
+            st_up[r] = kStLate | (u < 0 ? (kStIn | (-1 - u)) : u);  // late: global load after the level barrier
             ++n_late;
           }
       }
