@@ -305,7 +305,8 @@ __global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const
     const int sp_nn = sp[min(l + 2, n_lvl)], sp_nn4 = sp[min(l + 5, n_lvl)];
     prefetch_src(sf, max(sf, min(sp_n4, sp_n + SR)));
     if (live) {
-      for (int pos = lo + slot0; pos < hi; pos += 32) {
+      double *ep = ed + (int64_t)(lo + slot0) * a.B;  // this thread's output, advanced by pointer (no 64-bit multiply per cell)
+      for (int pos = lo + slot0; pos < hi; pos += 32, ep += 32 * (int64_t)a.B) {
         const int s = pos & (RR - 1);
         double num = kA * th_s[s] + kS * q_s[s];
         const double den = itau + vb * go_s[s];
@@ -319,7 +320,7 @@ __global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const
           }
         }
         const double res = num * __drcp_rn(den);  // within 1 ulp of num / den
-        ed[(int64_t)pos * a.B] = res;
+        *ep = res;
         vring[(size_t)(pos & (VR - 1)) * BG + bl] = res;
       }
     }
@@ -330,34 +331,47 @@ __global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const
   }
 }
 
-// ---- (a6) moments in the per-direction layout: one warp per cell, lanes over bands, directions in order ---------------------
+// ---- (a6) moments in the per-direction layout: one warp per cell; a lane is (direction within a group of 4, band
+// modulo 8), so every 8-lane group reads 64 contiguous bytes of one (direction, cell) chunk and all lanes stay busy for
+// any band count; the direction loop is unrolled for memory-level parallelism.  Fixed shuffle tree: deterministic.
 __global__ void __launch_bounds__(256) moments_unstructured_kernel(const UnsArgs a) {
-  extern __shared__ double sm[];  // w[D], s[D][3]
-  for (int k = threadIdx.x; k < a.D; k += blockDim.x) sm[k] = a.w[k];
-  for (int k = threadIdx.x; k < 3 * a.D; k += blockDim.x) sm[a.D + k] = a.w[k / 3] * a.s[k];
+  extern __shared__ double sm[];  // w[D], w s[D][3], 1/tau[B], v[B]
+  double *wsm = sm, *wss = sm + a.D, *its = sm + 4 * a.D, *vbs = its + a.B;
+  for (int k = threadIdx.x; k < a.D; k += blockDim.x) wsm[k] = a.w[k];
+  for (int k = threadIdx.x; k < 3 * a.D; k += blockDim.x) wss[k] = a.w[k / 3] * a.s[k];
+  for (int k = threadIdx.x; k < a.B; k += blockDim.x) { its[k] = a.itau[k]; vbs[k] = a.vb[k]; }
   __syncthreads();
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, dl = lane >> 3, b8 = lane & 7;
   const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (c >= a.n_act) return;
   double A1 = 0.0, A2 = 0.0, qx = 0.0, qy = 0.0, qz = 0.0;
-  for (int b0 = 0; b0 < a.B; b0 += 32) {
-    const int b = b0 + lane;
-    double E = 0.0, Fx = 0.0, Fy = 0.0, Fz = 0.0;
-    if (b < a.B) {
-      for (int d = 0; d < a.D; ++d) {
-        const int64_t pos = a.a2pos[(int64_t)d * a.n_act + c];
-        const double v = __ldcs(a.e + ((int64_t)d * a.e_stride + pos) * a.B + b);
-        E += sm[d] * v;
-        Fx += sm[a.D + 3 * d] * v;
-        Fy += sm[a.D + 3 * d + 1] * v;
-        Fz += sm[a.D + 3 * d + 2] * v;
+  for (int d0 = 0; d0 < a.D; d0 += 16) {  // 4 direction groups of 4 in flight
+    int64_t base[4];
+    int dd[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      dd[u] = d0 + 4 * u + dl;
+      base[u] = dd[u] < a.D ? ((int64_t)dd[u] * a.e_stride + __ldg(a.a2pos + (int64_t)dd[u] * a.n_act + c)) * a.B : -1;
+    }
+    for (int b0 = 0; b0 < a.B; b0 += 8) {
+      const int b = b0 + b8;
+      if (b < a.B) {
+        double v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = base[u] >= 0 ? __ldcs(a.e + base[u] + b) : 0.0;
+        const double it = its[b], vb = vbs[b];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (base[u] >= 0) {
+            const double wv = wsm[dd[u]] * v[u];
+            A1 += it * wv;                         // Eq. 5 numerator
+            A2 += wv;                              // R13
+            qx += vb * (wss[3 * dd[u]] * v[u]);    // Eq. 7
+            qy += vb * (wss[3 * dd[u] + 1] * v[u]);
+            qz += vb * (wss[3 * dd[u] + 2] * v[u]);
+          }
+        }
       }
-      const double it = a.itau[b], vb = a.vb[b];
-      A1 += E * it;  // Eq. 5 numerator
-      A2 += E;       // R13
-      qx += vb * Fx; // Eq. 7
-      qy += vb * Fy;
-      qz += vb * Fz;
     }
   }
 #pragma unroll
@@ -460,7 +474,7 @@ int nb_launch_sweep_unstructured(nanobte_solver *h) {
 int nb_launch_moments_unstructured(nanobte_solver *h) {
   const UnsArgs &a = *h->uns;
   const int wpb = 8;
-  moments_unstructured_kernel<<<(a.n_act + wpb - 1) / wpb, wpb * 32, (size_t)4 * a.D * sizeof(double), h->stream>>>(a);
+  moments_unstructured_kernel<<<(a.n_act + wpb - 1) / wpb, wpb * 32, ((size_t)4 * a.D + 2 * a.B) * sizeof(double), h->stream>>>(a);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
   return 0;
