@@ -282,3 +282,19 @@ def test_generic_cg_kernel_matches_oracle(monkeypatch):
     monkeypatch.setenv("NANOBTE_CG_GENERIC", "1")
     pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
     step_parity(pr, 2, T_init=random_T(pr, 4), mode="synthetic")
+
+
+def test_unstructured_fallback_kernel_matches_oracle(monkeypatch):
+    """The ring + register-pipeline sweep that `create` falls back to when a mesh's level spans do not fit the staged
+    kernel's rings."""
+    monkeypatch.setenv("NANOBTE_UNS_PLAIN", "1")
+    pr = wl.config_triangles(n=24, side=2e-6 * 24 / 320, B=5, D=16, hole_radius=300e-9 * 24 / 320)
+    step_parity(pr, 3, T_init=random_T(pr, 12))
+
+
+def test_general_cg_stencil_on_a_uniform_grid(monkeypatch):
+    """The per-cell stencil path of the fused CG (what non-uniform and unstructured meshes use), forced on a grid that
+    would take the face-uniform path."""
+    monkeypatch.setenv("NANOBTE_CG_NO_UNI", "1")
+    pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
+    step_parity(pr, 2, T_init=random_T(pr, 4), mode="synthetic")
