@@ -39,12 +39,13 @@ SMI_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.acti
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="finfet")
     ap.add_argument("--mode", default=None, help="plain | synthetic (default: the config's own)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-convergence", action="store_true", help="skip the time-to-convergence run")
     ap.add_argument("--cpu-sample-bands", type=int, default=0, help="bands in the oracle's sample (0 = auto)")
     ap.add_argument("--sweep-G", type=int, default=0)
     ap.add_argument("--sweep-threads", type=int, default=0)
@@ -321,6 +322,17 @@ def main():
            "breakdown_ms": {"sweep": sweep_ms, "closures_moments_update": update_ms, "cg": cg_ms},
            "create_s": create_s, "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
     g.close()
+    # ---- time to convergence (north_star: reported beside the per-iteration numbers): a fresh solver, solve() to the
+    # workload's own tolerance, wall clock around the call (one 16-byte D2H per iteration is part of it)
+    if not args.no_convergence:
+        g2 = Solver(pr, sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_variant=args.sweep_variant)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        res = g2.solve(pr["tol"], pr["max_iter"], mode)
+        torch.cuda.synchronize()
+        out["time_to_convergence"] = {"seconds": time.perf_counter() - t0, "iterations": res["iters"],
+                                      "converged": res["converged"], "tol_K": pr["tol"], "last_dT_K": res["last_dT"]}
+        g2.close()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         nb = args.cpu_sample_bands or auto_sample_bands(pr)
         val, dt, cores, sample = run_oracle(pr, mode, 2, 1, nb)
