@@ -25,12 +25,12 @@ struct UnsArgs {
   int32_t rcap;                     // positions held by the shared-memory ring (power of two)
   // staged variant (sweep_unstructured_staged_kernel)
   int32_t st_BG, st_NBG, st_threads, st_vr, st_rr, st_sr;  // bands per CTA, groups, threads, ring capacities (powers of two)
-  const int32_t *st_up;             // [MI][D][e_stride] upwind codes: ring / side / late
+  char *st_rec;                     // [D][e_stride] records of st_rsb bytes: theta, Qdot, outflow sum, inflow
+                                    // coefficients [MI], upwind codes [MI] (theta refreshed before every sweep)
+  int32_t st_rsb;
   const int32_t *side_ptr;          // [D][l_max+2] first side entry of each level (per direction)
   const int32_t *side_src;          // per direction from side_base[d]: >= 0 position in e, < 0: -1 - inflow index
   const int64_t *side_base;         // [D]
-  double *thetaP;                   // [D][e_stride] theta in sweep order (refreshed before every sweep)
-  const double *QP;                 // [D][e_stride] Qdot in sweep order
   int32_t n_act, l_max;
   int64_t e_stride;                 // positions per direction (n_act rounded up)
   const int32_t *n_lvl;             // [D]
@@ -208,15 +208,15 @@ constexpr int32_t kStLate = INT32_MIN | (1 << 30), kStIn = 1 << 27, kStMask = (1
 __device__ __forceinline__ void cp_async8(void *dst, const void *src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
 }
-__device__ __forceinline__ void cp_async4(void *dst, const void *src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+__device__ __forceinline__ void cp_async16(void *dst, const void *src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
 }
 
 __global__ void theta_permute_kernel(const UnsArgs a) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= (int64_t)a.D * a.e_stride) return;
   const int pos = (int)(i % a.e_stride);
-  if (pos < a.n_act) a.thetaP[i] = a.theta[a.cell[i]];
+  if (pos < a.n_act) *reinterpret_cast<double *>(a.st_rec + i * a.st_rsb) = a.theta[a.cell[i]];
 }
 
 template <int MI>
@@ -225,11 +225,8 @@ __global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const
   const int BG = a.st_BG, VR = a.st_vr, RR = a.st_rr, SR = a.st_sr;
   double *vring = reinterpret_cast<double *>(st_smem);  // [VR][BG]
   double *side = vring + (size_t)VR * BG;                // [SR][BG]
-  double *th_s = side + (size_t)SR * BG;                 // [RR]
-  double *q_s = th_s + RR;
-  double *go_s = q_s + RR;
-  double *gi_s = go_s + RR;                              // [MI][RR]
-  int32_t *up_s = reinterpret_cast<int32_t *>(gi_s + (size_t)MI * RR);  // [MI][RR]
+  constexpr int RSB = (24 + 12 * MI + 15) / 16 * 16, NQ = RSB / 16;  // record: th, q, go, gi[MI] doubles, up[MI] ints
+  char *rec_s = reinterpret_cast<char *>(side + (size_t)SR * BG);  // [RR] records
   const int d = blockIdx.x / a.st_NBG, bg = blockIdx.x % a.st_NBG;
   const int tid = threadIdx.x, nth = blockDim.x;
   const int slot0 = tid / BG, bl = tid - slot0 * BG;
@@ -266,15 +263,9 @@ __global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const
   auto issue = [&](int pf_end, int sf_end) {
     for (int p = pf + tid; p < pf_end; p += nth) {
       const int s = p & (RR - 1);
-      const int64_t g = dbase + p;
-      cp_async8(th_s + s, a.thetaP + g);
-      cp_async8(q_s + s, a.QP + g);
-      cp_async8(go_s + s, a.gout + g);
+      const char *src = a.st_rec + (dbase + p) * RSB;
 #pragma unroll
-      for (int k = 0; k < MI; ++k) {
-        cp_async8(gi_s + k * RR + s, a.gin + k * kstride + g);
-        cp_async4(up_s + k * RR + s, a.st_up + k * kstride + g);
-      }
+      for (int i = 0; i < NQ; ++i) cp_async16(rec_s + (size_t)s * RSB + 16 * i, src + 16 * i);
     }
     pf = max(pf, pf_end);
     if (live) {
@@ -308,15 +299,23 @@ __global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const
       double *ep = ed + (int64_t)(lo + slot0) * a.B;  // this thread's output, advanced by pointer (no 64-bit multiply per cell)
       for (int pos = lo + slot0; pos < hi; pos += 32, ep += 32 * (int64_t)a.B) {
         const int s = pos & (RR - 1);
-        double num = kA * th_s[s] + kS * q_s[s];
-        const double den = itau + vb * go_s[s];
+        // the whole record in NQ 16-byte shared-memory loads
+        uint4 raw[NQ];
+#pragma unroll
+        for (int i = 0; i < NQ; ++i) raw[i] = reinterpret_cast<const uint4 *>(rec_s + (size_t)s * RSB)[i];
+        double rd[3 + MI];
+        int32_t ru[MI];
+        memcpy(rd, raw, sizeof(rd));
+        memcpy(ru, reinterpret_cast<const char *>(raw) + sizeof(rd), sizeof(ru));
+        double num = kA * rd[0] + kS * rd[1];
+        const double den = itau + vb * rd[2];
 #pragma unroll
         for (int k = 0; k < MI; ++k) {
-          const int u = up_s[k * RR + s];
+          const int u = ru[k];
           if (u != kNone) {
             // ring and side references carry their shared-memory offset (slot * BG) ready-made; the rest is late
             const double val = u >= 0 ? vring[u + bl] : (u & kStIn) ? bin_b[u & kStMask] : ed[(int64_t)(u & kStMask) * a.B];
-            num += vb * gi_s[k * RR + s] * val;
+            num += vb * rd[3 + k] * val;
           }
         }
         const double res = num * __drcp_rn(den);  // within 1 ulp of num / den
@@ -792,10 +791,10 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
   const int st_threads = (32 * st_BG + 31) / 32 * 32;
   // shared-memory budget of the one CTA per SM: record ring (fixed), a side ring of 64 entries, the rest for the value ring
   const size_t st_budget = 225 * 1024;
-  const size_t st_rec = (size_t)1024 * ((3 + MI) * sizeof(double) + MI * sizeof(int32_t));
+  const size_t st_rec_smem = (size_t)1024 * ((24 + 12 * MI + 15) / 16 * 16);
   int st_sr = 64, st_vr = 64;
-  while (st_rec + (size_t)st_sr * st_BG * sizeof(double) + (size_t)st_vr * 2 * st_BG * sizeof(double) + 64 <= st_budget && st_vr < 4096) st_vr *= 2;
-  while (st_rec + (size_t)st_sr * 2 * st_BG * sizeof(double) + (size_t)st_vr * st_BG * sizeof(double) + 64 <= st_budget && st_sr < 1024) st_sr *= 2;
+  while (st_rec_smem + (size_t)st_sr * st_BG * sizeof(double) + (size_t)st_vr * 2 * st_BG * sizeof(double) + 64 <= st_budget && st_vr < 4096) st_vr *= 2;
+  while (st_rec_smem + (size_t)st_sr * 2 * st_BG * sizeof(double) + (size_t)st_vr * st_BG * sizeof(double) + 64 <= st_budget && st_sr < 1024) st_sr *= 2;
   const int st_rr = 1024;
   bool staged = MI <= 4 && std::getenv("NANOBTE_UNS_PLAIN") == nullptr;
   std::vector<int32_t> st_up(up.size(), kNone), side_ptr((size_t)D * (l_max + 2), 0), side_src;
@@ -838,13 +837,25 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
       }
     }
   }
-  const size_t st_smem = ((size_t)st_vr * st_BG + (size_t)st_sr * st_BG + (size_t)st_rr * (3 + MI)) * sizeof(double) +
-                         (size_t)st_rr * MI * sizeof(int32_t) + 64;
+  const size_t st_smem = ((size_t)st_vr * st_BG + (size_t)st_sr * st_BG) * sizeof(double) + st_rec_smem + 64;
   if (st_smem > 227 * 1024 - 512) staged = false;
   if (std::getenv("NANOBTE_DEBUG")) fprintf(stderr, "unstructured sweep: staged %d BG %d NBG %d vr %d sr %d smem %zu MI %d late refs %ld side entries %zu\n", (int)staged, st_BG, st_NBG, st_vr, st_sr, st_smem, MI, n_late, side_src.size());
-  std::vector<double> QP((size_t)D * e_stride, 0.0);
-  for (int d = 0; d < D; ++d)
-    for (int pos = 0; pos < nc; ++pos) QP[(size_t)d * e_stride + pos] = Qdot ? Qdot[cellat[(size_t)d * e_stride + pos]] : 0.0;
+  const int st_rsb = (24 + 12 * MI + 15) / 16 * 16;
+  std::vector<char> st_rec(staged ? (size_t)D * e_stride * st_rsb : 16, 0);
+  if (staged)
+    for (int d = 0; d < D; ++d)
+      for (int pos = 0; pos < nc; ++pos) {
+        const size_t at = (size_t)d * e_stride + pos;
+        char *rec = &st_rec[at * st_rsb];
+        double dv[3 + 7] = {0.0, Qdot ? Qdot[cellat[at]] : 0.0, gout[at]};
+        int32_t uv[7];
+        for (int k = 0; k < MI; ++k) {
+          dv[3 + k] = gin[(size_t)k * D * e_stride + at];
+          uv[k] = st_up[(size_t)k * D * e_stride + at];
+        }
+        std::memcpy(rec, dv, sizeof(double) * (3 + MI));
+        std::memcpy(rec + sizeof(double) * (3 + MI), uv, sizeof(int32_t) * MI);
+      }
 
   std::vector<int32_t> lvl_ptr((size_t)D * (l_max + 1), 0);
   for (int d = 0; d < D; ++d) {
@@ -881,12 +892,11 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
     if (rc) return nb_fail(h, rc, "device upload failed");
     u.D = D; u.B = B; u.BG = BG; u.NBG = NBG; u.MI = MI; u.cpp = cpp; u.rcap = rcap; u.n_act = nc; u.l_max = l_max; u.e_stride = e_stride;
     u.st_BG = st_BG; u.st_NBG = st_NBG; u.st_threads = st_threads; u.st_vr = st_vr; u.st_rr = st_rr; u.st_sr = st_sr;
-    u.st_up = A.put(st_up);
+    u.st_rec = A.put(st_rec);
+    u.st_rsb = st_rsb;
     u.side_ptr = A.put(side_ptr);
     u.side_src = A.put(side_src);
     u.side_base = A.put(side_base);
-    u.thetaP = A.zeros<double>((size_t)D * e_stride);
-    u.QP = A.put(QP);
     u.n_lvl = A.put(n_lvl);
     u.lvl_ptr = A.put(lvl_ptr);
     u.cell = A.put(cellat);
