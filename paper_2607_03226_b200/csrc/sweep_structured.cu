@@ -491,6 +491,8 @@ int nb_sweep_structured_config(nanobte_solver *h, int n_pen_max, int p_max, int 
       const int tt = ((n_pen_max + kR[k] - 1) / kR[k] + 31) / 32 * 32;
       if (tt <= kMaxCompute) { R = kR[k]; T = tt; }
     }
+    // with several pencils per thread the CTA is alone on its SM anyway: more warps hide more latency (config 3: -2 %)
+    if (R >= 4) T = kMaxCompute;
   }
   const int sp = (n_pen_max + 1 + 1) & ~1;
   const int pcap = (p_max + 3 + 4) & ~3;
