@@ -34,6 +34,14 @@
  * exceptions cross the ABI, no global state; nanobte_last_error(h) gives the message.  There is NO CPU
  * fallback: without a CUDA device of compute capability 10.x every create_* fails with NANOBTE_E_ARCH.
  * A solver handle is not thread-safe.
+ *
+ * NANOBTE_E_SPECULAR is also returned when a direction and its mirror image carry different weights: the face
+ * flux of reflecting walls is evaluated in closed form and relies on that symmetry.
+ *
+ * Environment hooks, read at create, for tests and tuning only (each selects another of the library's own CUDA
+ * paths; none of them leaves the GPU): NANOBTE_CG_GENERIC=1 (multi-pass CG kernel), NANOBTE_CG_NO_UNI=1 (per-cell CG
+ * stencil on uniform grids), NANOBTE_UNS_PLAIN=1 (non-staged unstructured sweep), NANOBTE_SWEEP_RP=0 (run-time row
+ * pitch in the structured sweep), NANOBTE_DEBUG=1 (launch-shape decisions on stderr).
  */
 #ifndef NANOBTE_H
 #define NANOBTE_H
