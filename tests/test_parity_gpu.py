@@ -298,3 +298,23 @@ def test_general_cg_stencil_on_a_uniform_grid(monkeypatch):
     monkeypatch.setenv("NANOBTE_CG_NO_UNI", "1")
     pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
     step_parity(pr, 2, T_init=random_T(pr, 4), mode="synthetic")
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6])
+def test_random_masks(seed):
+    """Random masks (holes inside pencils, isolated cells, walls of every type on interior faces) in both sweep
+    variants: stresses the wall-first slot order, the padding slots and the inflow / source index packing."""
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = int(rng.integers(3, 12)), int(rng.integers(2, 9)), int(rng.integers(1, 7))
+    active = (rng.random(nx * ny * nz) > 0.3).astype(np.uint8)
+    active[int(rng.integers(0, nx * ny * nz))] = 1
+    tags = [(wl.THERMALIZING, 303.0), (wl.THERMALIZING, 298.0), (wl.DIFFUSE, 0.0), (wl.SPECULAR, 0.0), (wl.MIXED, 0.0)]
+    side_tags = [int(t) for t in rng.permutation(5)] + [int(rng.integers(0, 5))]
+    if 0 not in side_tags and 1 not in side_tags:
+        side_tags[0] = 0
+    quad = wl.product_quadrature(2, 8) if nz > 1 else wl.inplane_quadrature(8)
+    Q = np.where(rng.random(nx * ny * nz) > 0.6, 1e17 * rng.random(nx * ny * nz), 0.0)
+    pr = wl.make_structured_problem(nx, ny, nz, 7e-9, 9e-9, 11e-9, small_bands(3, seed), quad, tags, side_tags,
+                                    active=active, Qdot=Q, p_seed=seed)
+    for variant in (0, 4):
+        step_parity(pr, 3, T_init=random_T(pr, seed), sweep_variant=variant)
