@@ -318,3 +318,15 @@ def test_random_masks(seed):
                                     active=active, Qdot=Q, p_seed=seed)
     for variant in (0, 4):
         step_parity(pr, 3, T_init=random_T(pr, seed), sweep_variant=variant)
+
+
+def test_library_owned_memory_matches_caller_owned_workspace():
+    """options.workspace == NULL: the library allocates its arena itself (cudaMalloc) -- same results, bit for bit."""
+    pr = wl.config_cube(n=10, B=2, n_polar=2, n_azim=8)
+    outs = []
+    for own in (True, False):
+        g = gpu_solver(pr, own_workspace=own)
+        g.solve(1e-9, 5, "synthetic")
+        outs.append((g.get_T(0).copy(), g.get_e(0, 1, 0, 3).copy()))
+        g.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
