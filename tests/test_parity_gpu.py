@@ -330,3 +330,17 @@ def test_library_owned_memory_matches_caller_owned_workspace():
         outs.append((g.get_T(0).copy(), g.get_e(0, 1, 0, 3).copy()))
         g.close()
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+def test_finfet_mid_cut_solve_synthetic():
+    """A cut large enough for the CG to run on many CTA chunks (halo recurrences, grid barrier): converged field and
+    outer iteration count against the oracle."""
+    pr = wl.config_finfet(nx=32, ny=16, nz=16, B=4, n_polar=2, n_azim=8)
+    r, g = RefSolver(pr), gpu_solver(pr)
+    rr, rg = r.solve(1e-9, 5000, "synthetic"), g.solve(1e-9, 5000, "synthetic")
+    assert rr["converged"] and rg["converged"], (rr, rg)
+    assert rr["iters"] == rg["iters"], (rr, rg)
+    assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+    hg, hr = g.get_history(), r.get_history()
+    np.testing.assert_allclose(hg[0], hr[0], rtol=1e-6, atol=1e-14)
+    assert np.abs(hg[1] - hr[1]).max() <= max(2, int(hr[1].max()) // 20)  # CG iterations per outer iteration
