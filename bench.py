@@ -280,7 +280,7 @@ def main():
             g.diffusion_correct()           # D2H: max|dT|, CG iterations
         else:
             g.update_temperature(sync=True)
-        T_np[:] = g.get_T(0)                # D2H: n_cells doubles
+        g.get_T(0, out=T_np)                # D2H: n_cells doubles, straight into the pinned buffer
 
     for _ in range(min(2, args.warmup)):
         e2e_step()

@@ -292,7 +292,13 @@ class Solver:
         a = np.empty(shape)
         return a, a.ctypes.data_as(C.c_void_p)
 
-    def get_T(self, which=0, device=False):
+    def get_T(self, which=0, device=False, out=None):
+        """`out`: optional host destination (a contiguous float64 numpy array of n_cells, e.g. the numpy view of a pinned
+        torch tensor, which makes the device-to-host copy a true DMA)."""
+        if out is not None and not device:
+            assert out.dtype == np.float64 and out.size == self.n_cells and out.flags["C_CONTIGUOUS"]
+            self._chk(self._lib.nanobte_get_T(self._h, int(which), out.ctypes.data_as(C.c_void_p), 0))
+            return out
         out, p = self._out((self.n_cells,), device)
         self._chk(self._lib.nanobte_get_T(self._h, int(which), p, int(device)))
         return out
