@@ -194,7 +194,6 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     // in every e row -- which is what lets the closure kernels read the walls with coalesced loads.
     std::vector<int> pen_v, pen_w, pen_of((size_t)nv * nw, -1);
     std::vector<int> first_of_m[2] = {std::vector<int>(nv + nw, 0), std::vector<int>(nv + nw, 0)};
-    int n_wall_slots = 0;
     for (int grp = 0; grp < 2; ++grp) {
       for (int mm = 0; mm <= nv + nw - 2; ++mm) {
         if (pen_v.size() & 1) { pen_v.push_back(-1); pen_w.push_back(-1); }  // padding slot: keeps every diagonal's first slot even
@@ -210,9 +209,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       }
       if (pen_v.size() & 1) { pen_v.push_back(-1); pen_w.push_back(-1); }
       first_of_m[grp][nv + nw - 1] = (int)pen_v.size();
-      if (grp == 0) n_wall_slots = (int)pen_v.size();
     }
-    (void)n_wall_slots;
     o.n_pen = (int)pen_v.size();
     o.pen.resize(o.n_pen);
     o.pen_rh.resize(o.n_pen);

@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(256, 3) sweep_unstructured_kernel(const UnsArg
     settle();
   };
   constexpr int QD = 1;   // records in flight behind stage V (deeper queues spill under the 3-CTA register cap)
-  Rec rV, rQ[QD];         // stage V: record arrived, values (being) fetched; rQ: records in flight, oldest first
+  Rec rV{}, rQ[QD];       // stage V: record arrived, values (being) fetched; rQ: records in flight, oldest first
   bool hasV = false, vIssued = false;
   int nQ = 0;
   double thV = 0.0, qV = 0.0, valV[MI];
@@ -236,16 +236,12 @@ __global__ void __launch_bounds__(640, 1) sweep_unstructured_staged_kernel(const
   const double kA = a.kA[bb], kS = a.kS[bb], itau = a.itau[bb], vb = a.vb[bb];
   const int64_t dbase = (int64_t)d * a.e_stride;
   double *const ed = a.e + dbase * a.B + bb;
-  const double *const eband0 = a.e + dbase * a.B + (int64_t)bg * BG;          // + src * B + band within group
-  const double *const bin0 = a.bin + a.dir_bin[d] + (int64_t)bg * BG * a.dir_nin[d];
   const int64_t nin = a.dir_nin[d];
   const double *const bin_b = a.bin + a.dir_bin[d] + (int64_t)bb * nin;
   const int32_t *const lp = a.lvl_ptr + (int64_t)d * (a.l_max + 1);
   const int32_t *const sp = a.side_ptr + (int64_t)d * (a.l_max + 2);
   const int32_t *const ssrc = a.side_src + a.side_base[d];
-  const int64_t kstride = (int64_t)a.D * a.e_stride;
   const int n_lvl = a.n_lvl[d], n_act = a.n_act;
-  const int nbg = min(BG, a.B - bg * BG);  // bands of this group that exist
 
   int pf = 0, sf = 0;  // next record position / side entry to request (identical in every thread)
   // Side copies: the thread (cell slot slot0, band bl) copies band bl of the entries sf + slot0, sf + slot0 + 32, ...
