@@ -274,6 +274,9 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
     h->cgf_w = A.zeros<double>(2 * na);
     h->cgf_part = A.zeros<double>((size_t)4 * nblk + 8);
     h->cgf_bar = A.zeros<unsigned int>(4);
+    h->cgf_xprev = A.zeros<double>(2 * na);
+    h->cgf_gpart = A.zeros<double>((size_t)8 * nblk + 8);
+    h->cgf_recycle = std::getenv("NANOBTE_CG_NO_RECYCLE") == nullptr;
   }
   h->tagface_ptr = A.put(g.tagface_ptr);
   h->tagface = A.put(g.tagface);

@@ -141,7 +141,10 @@ struct nanobte_solver {
   int cg_blocks = 0;
   // fused CG (cg.cu, cg_fused_kernel): cells cut into one contiguous chunk per CTA, vectors on chip
   bool cgf_ok = false, cg_force_generic = false, cgf_uni = false;
-  double cgf_cfu[6] = {0, 0, 0, 0, 0, 0};  // face-uniform stencil coefficients (cgf_uni)
+  double cgf_cfu[6] = {0, 0, 0, 0, 0, 0};
+  bool cgf_recycle = true;              // Galerkin initial guess from the last two CG solutions
+  int cgf_nprev = 0;
+  double *cgf_xprev = nullptr, *cgf_gpart = nullptr;  // face-uniform stencil coefficients (cgf_uni)
   int cgf_nblk = 0, cgf_chunk = 0, cgf_cpt = 0, cgf_nh_cap = 0;
   size_t cgf_smem = 0;
   const int32_t *cgf_perm = nullptr;   // [n] CG index -> active cell index (spatially compact chunks)

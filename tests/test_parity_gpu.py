@@ -60,7 +60,9 @@ def step_parity(pr, n_steps=3, T_init=None, mode="plain", **kw):
             (ir, d2r), (ig, d2g) = r.diffusion_correct(), g.diffusion_correct()
             a, b = g.get_T(0) - pr["T_ref"], r.get_T(0) - pr["T_ref"]
             assert rel(a, b) <= 1e-9, f"synthetic step {n}: {rel(a, b):.3e}"
-            assert abs(ig - ir) <= max(2, ir // 20)
+            # the GPU CG starts from a recycled initial guess: same system, same stopping rule,
+            # so it never needs noticeably more iterations than the oracle's CG from zero
+            assert ig <= ir + max(2, ir // 20)
     g.close()
     r.close()
 
@@ -343,4 +345,4 @@ def test_finfet_mid_cut_solve_synthetic():
     assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
     hg, hr = g.get_history(), r.get_history()
     np.testing.assert_allclose(hg[0], hr[0], rtol=1e-6, atol=1e-14)
-    assert np.abs(hg[1] - hr[1]).max() <= max(2, int(hr[1].max()) // 20)  # CG iterations per outer iteration
+    assert (hg[1] - hr[1]).max() <= max(2, int(hr[1].max()) // 20)  # CG iterations per outer iteration: never noticeably more
