@@ -40,7 +40,7 @@
  *
  * Environment hooks, read at create, for tests and tuning only (each selects another of the library's own CUDA
  * paths; none of them leaves the GPU): NANOBTE_CG_GENERIC=1 (multi-pass CG kernel), NANOBTE_CG_NO_UNI=1 (per-cell CG
- * stencil on uniform grids), NANOBTE_UNS_PLAIN=1 (non-staged unstructured sweep), NANOBTE_SWEEP_RP=0 (run-time row
+ * stencil on uniform grids), NANOBTE_CG_NO_RECYCLE=1 (CG from zero instead of the recycled initial guess), NANOBTE_UNS_PLAIN=1 (non-staged unstructured sweep), NANOBTE_SWEEP_RP=0 (run-time row
  * pitch in the structured sweep), NANOBTE_DEBUG=1 (launch-shape decisions on stderr).
  */
 #ifndef NANOBTE_H
