@@ -346,3 +346,17 @@ def test_finfet_mid_cut_solve_synthetic():
     hg, hr = g.get_history(), r.get_history()
     np.testing.assert_allclose(hg[0], hr[0], rtol=1e-6, atol=1e-14)
     assert (hg[1] - hr[1]).max() <= max(2, int(hr[1].max()) // 20)  # CG iterations per outer iteration: never noticeably more
+
+
+def test_cg_from_zero_matches_oracle_counts(monkeypatch):
+    """Without the recycled initial guess the GPU CG is the oracle's CG (from zero, unpreconditioned): the iteration
+    counts agree within rounding effects, in both directions."""
+    monkeypatch.setenv("NANOBTE_CG_NO_RECYCLE", "1")
+    pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
+    r, g = RefSolver(pr), gpu_solver(pr)
+    for _ in range(4):
+        r.sweep(); g.sweep()
+        r.update_temperature(); g.update_temperature()
+        (ir, _), (ig, _) = r.diffusion_correct(), g.diffusion_correct()
+        assert abs(ig - ir) <= max(2, ir // 20)
+    assert rel(g.get_T(0) - pr["T_ref"], r.get_T(0) - pr["T_ref"]) <= 1e-9
