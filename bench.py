@@ -137,13 +137,14 @@ def measured_peaks():
 # CPU oracle leg (cpu_baseline / --impl reference)
 # ---------------------------------------------------------------------------------------------------------------------
 def oracle_sample_problem(pr, n_bands):
-    """Same mesh, quadrature, tags and source; the first n_bands bands of the table.  (band, direction) systems are
-    independent, so the cost per update is the workload's own."""
+    """Same mesh, quadrature, tags and source; the first n_bands bands of the table, each with the source share it has
+    in the full table.  (band, direction) systems are independent, so the cost per update is the workload's own."""
     B = len(pr["bands"]["C"])
     n_bands = max(1, min(B, n_bands))
     sub = dict(pr)
     sub["bands"] = {k: np.ascontiguousarray(v[:n_bands]) for k, v in pr["bands"].items()}
-    return sub, n_bands
+    C = np.asarray(pr["bands"]["C"], dtype=np.float64)
+    return sub, n_bands, C[:n_bands] / C.sum()
 
 
 def auto_sample_bands(pr, target_updates=1.0e8):
@@ -152,32 +153,52 @@ def auto_sample_bands(pr, target_updates=1.0e8):
     return int(max(1, min(len(pr["bands"]["C"]), round(target_updates / per_band))))
 
 
-def run_oracle(pr, mode, steps, warmup, n_bands):
-    """Times `steps` oracle source iterations on the sample; returns (updates/s, seconds per step, cores, sample text)."""
+def run_oracle(pr, mode, steps, warmup, n_bands, threads):
+    """Times the oracle PER PHASE on a band sample of the workload and extrapolates to the full band table:
+
+        t_step(full) = (t_sweep + t_moments) * B / n_bands + t_cg
+
+    The sweep (O2/O3) and the moment pass (O4) cost the same per (cell, band, direction) update whatever the band, so
+    they scale with the band count; the diffusion correction (O6, CG on the full mesh) does not depend on the band
+    count at all, so it is taken as measured (a sample that divides the fixed CG cost by the sample's updates
+    understates the CPU rate).  Returns a dict."""
     from oracle.ref import RefSolver
     from paper_2607_03226_b200 import workloads as wl
-    sub, nb = oracle_sample_problem(pr, n_bands)
-    cores = len(os.sched_getaffinity(0))
-    r = RefSolver(sub, threads=cores)
-    cores = r.threads
-
-    def step():
+    sub, nb, share = oracle_sample_problem(pr, n_bands)
+    B = len(pr["bands"]["C"])
+    r = RefSolver(sub, threads=threads, share=share)
+    threads = r.threads
+    synthetic = mode == "synthetic"
+    t = {"sweep": 0.0, "moments": 0.0, "cg": 0.0}
+    cg_iters = []
+    for k in range(warmup + steps):
+        t0 = time.perf_counter()
         r.sweep()
+        t1 = time.perf_counter()
         r.update_temperature()
-        if mode == "synthetic":
-            r.diffusion_correct()
-
-    for _ in range(warmup):
-        step()
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        step()
-    dt = (time.perf_counter() - t0) / max(1, steps)
-    upd = wl.n_updates(sub)
+        t2 = time.perf_counter()
+        if synthetic:
+            it, _ = r.diffusion_correct()
+        t3 = time.perf_counter()
+        if k >= warmup:
+            t["sweep"] += t1 - t0
+            t["moments"] += t2 - t1
+            t["cg"] += t3 - t2
+            if synthetic:
+                cg_iters.append(it)
     r.close()
-    sample = (f"{pr['name']}: same mesh/quadrature/walls/source, first {nb} of {len(pr['bands']['C'])} bands "
-              f"({upd} updates per step), {steps} timed steps after {warmup} warm-up, mode {mode}")
-    return upd / dt, dt, cores, sample
+    for k in t:
+        t[k] /= max(1, steps)
+    scale = B / nb
+    t_full = (t["sweep"] + t["moments"]) * scale + t["cg"]
+    upd_full = wl.n_updates(pr)
+    return {"value": upd_full / t_full, "s_per_step_full": t_full, "cores": threads,
+            "sweep_updates_per_s": wl.n_updates(sub) / t["sweep"],
+            "phases_s_sample": dict(t), "phases_s_full": {"sweep": t["sweep"] * scale, "moments": t["moments"] * scale, "cg": t["cg"]},
+            "cg_iters_per_step": float(np.mean(cg_iters)) if cg_iters else 0.0,
+            "sample": (f"{pr['name']}: same mesh/quadrature/walls/source, first {nb} of {B} bands ({wl.n_updates(sub)} updates per "
+                       f"sample step), {steps} timed steps after {warmup} warm-up, mode {mode}; sweep and moments timed separately "
+                       f"and scaled by {B}/{nb}, CG (full mesh, band independent) as measured")}
 
 
 # ---------------------------------------------------------------------------------------------------------------------
@@ -191,14 +212,18 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return 0
-        nb = args.cpu_sample_bands or auto_sample_bands(pr, 4.0e7)
-        steps, warmup = max(1, min(args.steps, 5)), max(1, min(args.warmup, 1))
-        val, dt, cores, sample = run_oracle(pr, mode, steps, warmup, nb)
+        nb = args.cpu_sample_bands or auto_sample_bands(pr, 6.0e7)
+        steps, warmup = max(1, min(args.steps, 3)), max(1, min(args.warmup, 1))
+        cores = len(os.sched_getaffinity(0))
+        o = run_oracle(pr, mode, steps, warmup, nb, cores)
+        val = o["value"]
         out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-               "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+               "warmup": warmup, "ms_per_step": o["s_per_step_full"] * 1e3, "higher_is_better": True, "scaling": "weak",
                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-               "config": workload_config(pr, mode, {"note": "CPU oracle on a bounded sample; ms_per_step is per sample step"}),
-               "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+               "config": workload_config(pr, mode, {"note": "CPU oracle; per-phase timing on a band sample, extrapolated to the full "
+                                                            "band table (ms_per_step is that extrapolation)"}),
+               "cpu_baseline": {"value": val, "unit": UNIT, "cores": o["cores"], "kind": "oracle", "sample": o["sample"],
+                                "phases_s_full": o["phases_s_full"], "cg_iters_per_step": o["cg_iters_per_step"]},
                "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                "gpu_launches": 0}
         print(json.dumps(out))
@@ -217,26 +242,30 @@ def main():
         dist.barrier()
     from paper_2607_03226_b200.binding import Solver
 
+    skw = dict(sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_variant=args.sweep_variant)
     t_c0 = time.perf_counter()
-    g = Solver(pr, sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_variant=args.sweep_variant)
+    g = Solver(pr, **skw)
     torch.cuda.synchronize()
     create_s = time.perf_counter() - t_c0
     upd = wl.n_updates(pr)
     synthetic = mode == "synthetic"
 
-    def step(ev=None):
+    def step(s, ev=None, cg=None):
+        """One source iteration through the C ABI: sweep (a2-a5), closures + moments + update (a3, a6, a8), CG (a7)."""
         if ev is not None:
             ev[0].record()
-        g.sweep()
+        s.sweep()
         if ev is not None:
             ev[1].record()
         if synthetic:
-            g.update_temperature(sync=False)
+            s.update_temperature(sync=False)
             if ev is not None:
                 ev[2].record()
-            g.diffusion_correct()
+            it, _ = s.diffusion_correct()
+            if cg is not None:
+                cg.append(it)
         else:
-            g.update_temperature(sync=True)
+            s.update_temperature(sync=True)
             if ev is not None:
                 ev[2].record()
         if ev is not None:
@@ -245,16 +274,17 @@ def main():
     def barrier():
         replicas.barrier(dist, torch.cuda.synchronize)
 
-    # ---- device-resident arm -------------------------------------------------------------------------------------
+    # ---- device-resident arm: outer iterations W+1 .. W+K of the solve from T_ref ------------------------------------
     for _ in range(args.warmup):
-        step()
+        step(g)
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
     sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local)
     l0 = g.launches
+    cg_dev = []
     barrier()
     sampler.start()
     for k in range(args.steps):
-        step(evs[k])
+        step(g, evs[k], cg_dev)
     barrier()
     clocks = sampler.stop()
     launches = g.launches - l0
@@ -265,49 +295,56 @@ def main():
     total_ms = replicas.max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / args.steps
     value = replicas.whole_job_rate(upd, world, ms_per_step * 1e-3)
+    info = dict(g.info)
+    g.close()
 
-    # ---- end-to-end arm: host buffers through the C ABI, copies inside the timed region ------------------------------
+    # ---- end-to-end arm: the SAME outer iterations (fresh solver, same warm-up), host buffers through the C ABI, the
+    # host<->device copies of every step inside the timed region ----------------------------------------------------------
+    g = Solver(pr, **skw)
     T_host = torch.empty(g.n_cells, dtype=torch.float64).pin_memory()
     T_host.copy_(torch.as_tensor(g.get_T(0)))
     T_np = T_host.numpy()
-    e2e_steps = args.steps
+    cg_e2e = []
 
-    def e2e_step():
+    def e2e_step(cg=None):
         g.set_T(T_np)                       # H2D: n_cells doubles from pinned host memory
-        g.sweep()
-        if synthetic:
-            g.update_temperature(sync=False)
-            g.diffusion_correct()           # D2H: max|dT|, CG iterations
-        else:
-            g.update_temperature(sync=True)
+        step(g, None, cg)                   # D2H inside: max|dT| (+ CG iterations)
         g.get_T(0, out=T_np)                # D2H: n_cells doubles, straight into the pinned buffer
 
-    for _ in range(min(2, args.warmup)):
+    for _ in range(args.warmup):
         e2e_step()
     barrier()
     t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        e2e_step()
+    for _ in range(args.steps):
+        e2e_step(cg_e2e)
     barrier()
-    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    e2e_s = (time.perf_counter() - t0) / args.steps
     e2e_s = replicas.max_over_ranks(e2e_s, dist, "cuda")
     e2e = {"value": replicas.whole_job_rate(upd, world, e2e_s), "unit": UNIT, "h2d_bytes_per_step": int(g.n_cells * 8),
-           "d2h_bytes_per_step": int(g.n_cells * 8 + 16), "ms_per_step": e2e_s * 1e3}
+           "d2h_bytes_per_step": int(g.n_cells * 8 + 16), "ms_per_step": e2e_s * 1e3,
+           "cg_iters_per_step": float(np.mean(cg_e2e)) if cg_e2e else 0.0,
+           "note": "same outer iterations as the device arm (fresh solver, same warm-up); timed with the host clock around "
+                   "barrier + synchronize"}
+    g.close()
 
     # ---- roofline of the dominant kernel (the sweep): 8 algorithmic bytes per update ----------
     peak, peak_src = measured_peaks()
     alg_bytes = 8.0 * upd
     achieved = alg_bytes / (sweep_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "sweep_structured_kernel" if pr["kind"] == "structured" else "sweep_unstructured_kernel",
+    kernel = ("sweep_structured_kernel" if pr["kind"] == "structured" else
+              ("sweep_unstructured_staged_kernel" if info.get("sweep_rmax", 0) == 0 else "sweep_unstructured_kernel"))
+    roofline = {"bound": "hbm", "kernel": kernel,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                 "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": sweep_ms,
                 "moments_pass": {"achieved": alg_bytes / (update_ms * 1e-3) / 1e9, "launch_ms": update_ms,
                                  "note": "closures + moments + update; 8 B/update read"}}
-    tr = os.path.join(ROOT, "profiles", "traffic.json")  # written by hand from the ncu --set full capture
+    tr = os.path.join(ROOT, "profiles", "traffic.json")  # copied from ncu --set full captures; each entry names its capture
     if os.path.exists(tr):
         try:
-            roofline["traffic"] = json.load(open(tr)).get(pr["name"], {}).get("sweep_dram_bytes_per_launch")
+            ent = json.load(open(tr)).get(pr["name"], {})
+            roofline["traffic"] = ent.get("sweep_dram_bytes_per_launch")
+            roofline["traffic_source"] = {k: ent.get(k) for k in ("capture", "commit", "kernel") if k in ent}
         except Exception:
             pass
 
@@ -315,29 +352,40 @@ def main():
            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
            "config": workload_config(pr, mode, {"parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-                                                "sweep": {k: g.info[k] for k in ("sweep_G", "sweep_threads", "sweep_rmax", "n_tasks", "n_planes",
+                                                "sweep": {k: info[k] for k in ("sweep_G", "sweep_threads", "sweep_rmax", "n_tasks", "n_planes",
                                                                                "sweep_smem_bytes", "pencil_axis")},
-                                                "device_bytes": g.info["device_bytes"]}),
+                                                "cg": {k: info[k] for k in ("cg_fused", "cg_cells_per_thread", "cg_ctas", "cg_face_uniform",
+                                                                            "cg_recycle")},
+                                                "device_bytes": info["device_bytes"]}),
            "sweep_updates_per_s": world * upd / (sweep_ms * 1e-3), "s_per_iteration": ms_per_step * 1e-3,
            "breakdown_ms": {"sweep": sweep_ms, "closures_moments_update": update_ms, "cg": cg_ms},
+           "cg_iters_per_step": float(np.mean(cg_dev)) if cg_dev else 0.0,
            "create_s": create_s, "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
-    g.close()
     # ---- time to convergence (north_star: reported beside the per-iteration numbers): a fresh solver, solve() to the
     # workload's own tolerance, wall clock around the call (one 16-byte D2H per iteration is part of it)
     if not args.no_convergence:
-        g2 = Solver(pr, sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_variant=args.sweep_variant)
+        g2 = Solver(pr, **skw)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         res = g2.solve(pr["tol"], pr["max_iter"], mode)
         torch.cuda.synchronize()
         out["time_to_convergence"] = {"seconds": time.perf_counter() - t0, "iterations": res["iters"],
-                                      "converged": res["converged"], "tol_K": pr["tol"], "last_dT_K": res["last_dT"]}
+                                      "converged": res["converged"], "tol_K": pr["tol"], "last_dT_K": res["last_dT"],
+                                      "cg_iters_total": int(g2.get_history()[1].sum())}
         g2.close()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        # the oracle as it stands on this box's host cores: all cores and one core, per phase
+        cores = len(os.sched_getaffinity(0))
         nb = args.cpu_sample_bands or auto_sample_bands(pr)
-        val, dt, cores, sample = run_oracle(pr, mode, 2, 1, nb)
-        out["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
-                               "s_per_sample_step": dt}
+        oN = run_oracle(pr, mode, 2, 1, nb, cores)
+        o1 = run_oracle(pr, mode, 1, 0, 1 if wl.n_updates(pr) > 1e7 else nb, 1)
+        out["cpu_baseline"] = {"value": oN["value"], "unit": UNIT, "cores": oN["cores"], "kind": "oracle", "sample": oN["sample"],
+                               "s_per_step_full": oN["s_per_step_full"], "phases_s_full": oN["phases_s_full"],
+                               "sweep_updates_per_s": oN["sweep_updates_per_s"], "cg_iters_per_step": oN["cg_iters_per_step"],
+                               "one_thread": {k: o1[k] for k in ("value", "cores", "s_per_step_full", "phases_s_full",
+                                                                  "sweep_updates_per_s", "sample")}}
+        if "time_to_convergence" in out:
+            out["cpu_baseline"]["time_to_convergence_extrapolated_s"] = oN["s_per_step_full"] * out["time_to_convergence"]["iterations"]
     if rank == 0:
         print(json.dumps(out))
     if dist:

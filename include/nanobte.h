@@ -41,7 +41,8 @@
  * Environment hooks, read at create, for tests and tuning only (each selects another of the library's own CUDA
  * paths; none of them leaves the GPU): NANOBTE_CG_GENERIC=1 (multi-pass CG kernel), NANOBTE_CG_NO_UNI=1 (per-cell CG
  * stencil on uniform grids), NANOBTE_CG_NO_RECYCLE=1 (CG from zero instead of the recycled initial guess), NANOBTE_UNS_PLAIN=1 (non-staged unstructured sweep), NANOBTE_SWEEP_RP=0 (run-time row
- * pitch in the structured sweep), NANOBTE_DEBUG=1 (launch-shape decisions on stderr).
+ * pitch in the structured sweep), NANOBTE_CG_NBLK=k (at most k CTAs in the fused CG: more cells per thread on small
+ * meshes).
  */
 #ifndef NANOBTE_H
 #define NANOBTE_H
@@ -140,6 +141,12 @@ typedef struct {
   int64_t n_inflow;             /* sum over directions of boundary-inflow values per band          */
   size_t device_bytes;          /* total device memory in use by the solver                        */
   size_t sweep_smem_bytes;
+  /* which CG kernel nanobte_diffusion_correct launches */
+  int32_t cg_fused;             /* 1: one-barrier fused kernel, 0: multi-pass fallback                */
+  int32_t cg_cells_per_thread;  /* fused kernel: 1, 2, 4 or 8                                      */
+  int32_t cg_ctas;              /* CTAs of the cooperative launch (0 before the first fallback launch) */
+  int32_t cg_face_uniform;      /* fused kernel: face-uniform stencil (uniform structured grids)   */
+  int32_t cg_recycle;           /* fused kernel: recycled initial guess on                         */
 } nanobte_info;
 
 /* Bytes of device workspace create_* would need for this problem (same validation as create). */
@@ -172,11 +179,14 @@ int nanobte_sweep(nanobte_solver *);
 int nanobte_update_temperature(nanobte_solver *, double *max_dT);
 
 /* (a7) synthetic correction after update_temperature: CG on the two-point-flux diffusion operator,
- * T <- T_SI + delta (R14).  cg_iters/max_dT host pointers or NULL; synchronises. */
+ * T <- T_SI + delta (R14).  cg_iters/max_dT host pointers or NULL; synchronises.
+ * Returns NANOBTE_NOT_CONVERGED (state valid, T updated with the last CG iterate) when the CG stopped on
+ * options.cg_max_iter with ||r|| > cg_rtol ||rhs||. */
 int nanobte_diffusion_correct(nanobte_solver *, int32_t *cg_iters, double *max_dT);
 
 /* (a8) outer loop until max|dT| < tol or max_iter sweeps (R11).  Synchronises once per iteration
- * (one double device->host). */
+ * (one double device->host).  Starts the recycled CG guess afresh, so the result does not depend on earlier
+ * calls on the handle.  NANOBTE_NOT_CONVERGED also when the last synthetic correction's CG did not converge. */
 int nanobte_solve(nanobte_solver *, double tol, int32_t max_iter, int32_t mode, int32_t *iters_out,
                   double *last_dT_out);
 

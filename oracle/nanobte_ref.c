@@ -91,7 +91,7 @@ static int finish_setup(nanobte_ref *h, int B, const double *C, const double *v,
   }
   for (int b = 0; b < B; ++b) h->share[b] = share ? share[b] : C[b] / h->Csum; /* PAPER.md:178 */
   h->W = 0.0; /* W_Omega = sum_i w_i, Eq. 11 PAPER.md:91 */
-  double ws[3] = {0, 0, 0}, sxx = 0.0;
+  double ws[3] = {0, 0, 0}, tr = 0.0;
   for (int i = 0; i < D; ++i) {
     if (!(w[i] > 0)) FAIL(h, NBR_E_QUADRATURE, "weight %d not positive", i);
     double nn = sqrt(dot3(s + 3 * i, s + 3 * i));
@@ -102,14 +102,16 @@ static int finish_setup(nanobte_ref *h, int B, const double *C, const double *v,
       ws[k] += w[i] * s[3 * i + k];
     }
     h->W += w[i];
-    sxx += w[i] * s[3 * i] * s[3 * i];
+    for (int k = 0; k < h->dim; ++k) tr += w[i] * s[3 * i + k] * s[3 * i + k];
   }
   for (int k = 0; k < h->dim; ++k)
     if (fabs(ws[k]) > 1e-12 * h->W) FAIL(h, NBR_E_QUADRATURE, "sum_i w_i s_i != 0 (component %d: %g)", k, ws[k]);
-  /* kappa_bulk = sum_b C_b v_b^2 tau_b * (sum_i w_i s_ix^2 / W)  (R14d) */
+  /* kappa_bulk (R14d): kinetic value with the isotropic part of the discrete second angular moment,
+   *   kappa = sum_b C_b v_b^2 tau_b * trace_dim(sum_i w_i s_i s_i^T) / (dim W)
+   * = (1/3) sum C v^2 tau for unit vectors in 3-D, (1/2) sum C v^2 tau for in-plane unit vectors in 2-D. */
   h->kappa = 0.0;
   for (int b = 0; b < B; ++b) h->kappa += C[b] * v[b] * v[b] * tau[b];
-  h->kappa *= sxx / h->W;
+  h->kappa *= tr / (h->dim * h->W);
   for (int t = 0; t < n_tags; ++t) {
     if (tag_type[t] < 0 || tag_type[t] > 3) FAIL(h, NBR_E_INVALID, "tag %d: unknown type %d", t, tag_type[t]);
     h->tag_type[t] = tag_type[t];

@@ -54,51 +54,94 @@ int nb_check_device(nanobte_solver *h) {
   return 0;
 }
 
+// Host-side validation of the band table, the quadrature and the tag table, and the scalars derived from them:
+//   W = sum_i w_i (Eq. 11), beta = sum_b C_b / tau_b (denominator of Eq. 5), sum_b C_b (R13),
+//   source shares C_b / sum C (R5) and kappa_bulk (R14d).
+// kappa_bulk is the kinetic conductivity with the isotropic part of the quadrature's second moment tensor
+// M = sum_i w_i s_i s_i^T / W:  kappa = (trace of M over the mesh's own dimensions / dim) * sum_b C_b v_b^2 tau_b.
+namespace {
+struct AngularMoments {
+  double zeroth = 0.0, first[3] = {0.0, 0.0, 0.0}, second_diag[3] = {0.0, 0.0, 0.0};
+};
+const char *check_bands(const nanobte_bands &t, int &bad) {
+  for (bad = 0; bad < t.B; ++bad)
+    if (!(t.C[bad] > 0.0 && t.v[bad] > 0.0 && t.tau[bad] > 0.0)) return "band %d: heat capacity, group velocity and relaxation time must all be positive";
+  return nullptr;
+}
+}  // namespace
+
+// Number of SMs of the current device if there is one (the plan built by workspace_bytes_* must match create's);
+// leaves the default (148, B200) on a machine without a GPU, where only the host-side sizing runs.
+void nb_query_sm_count(nanobte_solver *h) {
+  int n = 0, dev = 0, sms = 0;
+  if (cudaGetDeviceCount(&n) == cudaSuccess && n > 0 && cudaGetDevice(&dev) == cudaSuccess &&
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+    h->n_sm = sms;
+  cudaGetLastError();
+}
+
 int nb_validate_common(nanobte_solver *h, int dim, const nanobte_bands *bands, const nanobte_quadrature *quad,
                        const nanobte_tag *tags, int n_tags, Common &c) {
-  if (!bands || !quad || (n_tags > 0 && !tags)) return nb_fail(h, NANOBTE_E_INVALID, "null argument");
-  const int B = bands->B, D = quad->D;
-  if (B < 1 || D < 1 || n_tags < 0) return nb_fail(h, NANOBTE_E_INVALID, "B, D must be >= 1");
-  if (!bands->C || !bands->v || !bands->tau || !quad->s || !quad->w) return nb_fail(h, NANOBTE_E_INVALID, "null table");
-  c.B = B; c.D = D; c.dim = dim; c.n_tags = n_tags;
-  c.C.assign(bands->C, bands->C + B);
-  c.v.assign(bands->v, bands->v + B);
-  c.tau.assign(bands->tau, bands->tau + B);
-  c.share.resize(B);
-  c.Csum = 0; c.beta = 0;
-  for (int b = 0; b < B; ++b) {
-    if (!(c.C[b] > 0) || !(c.v[b] > 0) || !(c.tau[b] > 0))
-      return nb_fail(h, NANOBTE_E_INVALID, "band %d: C, v, tau must be > 0", b);
-    c.Csum += c.C[b];
-    c.beta += c.C[b] / c.tau[b];  // denominator of Eq. 5
-  }
-  for (int b = 0; b < B; ++b) c.share[b] = bands->src_share ? bands->src_share[b] : c.C[b] / c.Csum;
-  c.s.assign(quad->s, quad->s + 3 * (size_t)D);
-  c.w.assign(quad->w, quad->w + D);
-  c.W = 0;  // W_Omega, Eq. 11
-  double ws[3] = {0, 0, 0}, sxx = 0;
-  for (int i = 0; i < D; ++i) {
-    if (!(c.w[i] > 0)) return nb_fail(h, NANOBTE_E_QUADRATURE, "weight %d not positive", i);
-    const double *s = &c.s[3 * i];
-    double nn = std::sqrt(s[0] * s[0] + s[1] * s[1] + s[2] * s[2]);
-    if (std::fabs(nn - 1.0) > 1e-12) return nb_fail(h, NANOBTE_E_QUADRATURE, "direction %d is not a unit vector", i);
-    for (int k = 0; k < 3; ++k) ws[k] += c.w[i] * s[k];
-    c.W += c.w[i];
-    sxx += c.w[i] * s[0] * s[0];
-  }
-  for (int k = 0; k < dim; ++k)
-    if (std::fabs(ws[k]) > 1e-12 * c.W)
-      return nb_fail(h, NANOBTE_E_QUADRATURE, "sum_i w_i s_i != 0 (component %d: %g)", k, ws[k]);
-  c.kappa = 0;  // R14d
-  for (int b = 0; b < B; ++b) c.kappa += c.C[b] * c.v[b] * c.v[b] * c.tau[b];
-  c.kappa *= sxx / c.W;
-  c.tag_type.resize(n_tags);
-  c.tag_T.resize(n_tags);
+  if (bands == nullptr || quad == nullptr) return nb_fail(h, NANOBTE_E_INVALID, "band table and quadrature are required");
+  if (n_tags < 0 || (n_tags > 0 && tags == nullptr)) return nb_fail(h, NANOBTE_E_INVALID, "tag table missing");
+  if (bands->B < 1 || bands->C == nullptr || bands->v == nullptr || bands->tau == nullptr)
+    return nb_fail(h, NANOBTE_E_INVALID, "band table needs B >= 1 and the arrays C, v, tau");
+  if (quad->D < 1 || quad->s == nullptr || quad->w == nullptr)
+    return nb_fail(h, NANOBTE_E_INVALID, "quadrature needs D >= 1 and the arrays s, w");
+  c.dim = dim;
+  c.n_tags = n_tags;
+
+  // tags first: cheapest, and independent of everything else
+  c.tag_type.clear();
+  c.tag_T.clear();
   for (int t = 0; t < n_tags; ++t) {
-    if (tags[t].type < 0 || tags[t].type > 3) return nb_fail(h, NANOBTE_E_INVALID, "tag %d: unknown type %d", t, tags[t].type);
-    c.tag_type[t] = tags[t].type;
-    c.tag_T[t] = tags[t].T_wall;
+    const int ty = tags[t].type;
+    if (ty != NANOBTE_THERMALIZING && ty != NANOBTE_DIFFUSE && ty != NANOBTE_SPECULAR && ty != NANOBTE_MIXED)
+      return nb_fail(h, NANOBTE_E_INVALID, "tag %d has type %d; known types are 0..3", t, ty);
+    c.tag_type.push_back(ty);
+    c.tag_T.push_back(tags[t].T_wall);
   }
+
+  // quadrature: unit vectors, positive weights, vanishing first moment (the T_ref part of q then drops out of Eq. 7)
+  c.D = quad->D;
+  c.s.assign(quad->s, quad->s + 3 * (size_t)c.D);
+  c.w.assign(quad->w, quad->w + c.D);
+  AngularMoments am;
+  for (int i = 0; i < c.D; ++i) {
+    const double wi = c.w[i], *si = &c.s[3 * (size_t)i];
+    if (!(wi > 0.0)) return nb_fail(h, NANOBTE_E_QUADRATURE, "quadrature weight %d is %g; weights must be positive", i, wi);
+    const double len2 = si[0] * si[0] + si[1] * si[1] + si[2] * si[2];
+    if (std::fabs(std::sqrt(len2) - 1.0) > 1e-12) return nb_fail(h, NANOBTE_E_QUADRATURE, "direction %d has length %.15g, not 1", i, std::sqrt(len2));
+    am.zeroth += wi;
+    for (int a = 0; a < 3; ++a) {
+      am.first[a] += wi * si[a];
+      am.second_diag[a] += wi * si[a] * si[a];
+    }
+  }
+  c.W = am.zeroth;
+  for (int a = 0; a < dim; ++a)
+    if (std::fabs(am.first[a]) > 1e-12 * c.W)
+      return nb_fail(h, NANOBTE_E_QUADRATURE, "first angular moment does not vanish: sum_i w_i s_i[%d] = %g", a, am.first[a]);
+
+  // bands
+  c.B = bands->B;
+  int bad = 0;
+  if (const char *msg = check_bands(*bands, bad)) return nb_fail(h, NANOBTE_E_INVALID, msg, bad);
+  c.C.assign(bands->C, bands->C + c.B);
+  c.v.assign(bands->v, bands->v + c.B);
+  c.tau.assign(bands->tau, bands->tau + c.B);
+  c.Csum = std::accumulate(c.C.begin(), c.C.end(), 0.0);
+  c.beta = 0.0;
+  double cv2tau = 0.0;
+  for (int b = 0; b < c.B; ++b) {
+    c.beta += c.C[b] / c.tau[b];
+    cv2tau += c.C[b] * c.v[b] * c.v[b] * c.tau[b];
+  }
+  c.share.resize(c.B);
+  for (int b = 0; b < c.B; ++b) c.share[b] = bands->src_share != nullptr ? bands->src_share[b] : c.C[b] / c.Csum;
+  double trace = 0.0;
+  for (int a = 0; a < dim; ++a) trace += am.second_diag[a];
+  c.kappa = cv2tau * trace / (dim * c.W);
   return 0;
 }
 
@@ -176,9 +219,11 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
     const int n = (int)na, nf = g.cg_nf;
     const int threads = 512;
     int nblk = std::max(1, std::min(h->n_sm, (n + 255) / 256));
+    if (const char *env = std::getenv("NANOBTE_CG_NBLK"))  // test hook: fewer, larger chunks (more cells per thread) on small meshes
+      nblk = std::max(1, std::min(nblk, std::atoi(env)));
     int chunk = (n + nblk - 1) / nblk;
     nblk = (n + chunk - 1) / chunk;
-    const int cpt = chunk <= threads ? 1 : chunk <= 2 * threads ? 2 : chunk <= 4 * threads ? 4 : 0;
+    const int cpt = chunk <= threads ? 1 : chunk <= 2 * threads ? 2 : chunk <= 4 * threads ? 4 : chunk <= 8 * threads ? 8 : 0;
     std::vector<int32_t> perm(n), inv(n);  // perm: CG index -> active index
     std::iota(perm.begin(), perm.end(), 0);
     if ((int)g.cg_xyz.size() == 3 * n && nblk > 1) {
@@ -330,12 +375,16 @@ extern "C" int nanobte_diffusion_correct(nanobte_solver *h, int32_t *cg_iters, d
   if ((rc = nb_launch_update(h, 1)) < 0) return rc;
   double d = 0;
   if ((rc = read_maxdT(h, &d)) < 0) return rc;
-  if (cg_iters) {
-    unsigned long long it;
-    memcpy(&it, h->h_pinned + 1, sizeof(it));
-    *cg_iters = (int32_t)it;
-  }
+  unsigned long long it;
+  memcpy(&it, h->h_pinned + 1, sizeof(it));
+  const bool cg_failed = (it >> 40) & 1ull;  // the CG kernels flag "stopped on cg_max_iter above the tolerance"
+  if (cg_iters) *cg_iters = (int32_t)(it & 0xffffffffull);
   if (max_dT) *max_dT = d;
+  if (cg_failed) {
+    h->cgf_nprev = 0;  // do not recycle a solution that is not one
+    nb_fail(h, NANOBTE_NOT_CONVERGED, "CG stopped at cg_max_iter = %d above rtol = %g", h->cg_max_iter, h->cg_rtol);
+    return NANOBTE_NOT_CONVERGED;
+  }
   return 0;
 }
 
@@ -346,8 +395,10 @@ extern "C" int nanobte_solve(nanobte_solver *h, double tol, int32_t max_iter, in
   if (mode == 1 && !h->any_therm) return nb_fail(h, NANOBTE_E_SINGULAR, "synthetic mode needs at least one thermalizing face");
   h->hist_dT.clear();
   h->hist_cg.clear();
+  h->cgf_nprev = 0;  // a solve never depends on what the handle did before (recycled CG guesses start afresh)
   double dT = INFINITY;
   int n = 0, rc = NANOBTE_NOT_CONVERGED, r;
+  bool cg_failed = false;
   while (n < max_iter) {
     int cg = 0;
     if ((r = nanobte_sweep(h)) < 0) return r;
@@ -356,12 +407,13 @@ extern "C" int nanobte_solve(nanobte_solver *h, double tol, int32_t max_iter, in
     } else {
       if ((r = nanobte_update_temperature(h, nullptr)) < 0) return r;
       if ((r = nanobte_diffusion_correct(h, &cg, &dT)) < 0) return r;
+      cg_failed = r == NANOBTE_NOT_CONVERGED;
     }
     ++n;
     h->hist_dT.push_back(dT);
     h->hist_cg.push_back(cg);
     if (dT < tol) {
-      rc = NANOBTE_OK;
+      rc = cg_failed ? NANOBTE_NOT_CONVERGED : NANOBTE_OK;  // an outer iterate built on an unconverged CG is not a converged state
       break;
     }
   }
@@ -466,6 +518,9 @@ extern "C" int nanobte_get_info(const nanobte_solver *h, nanobte_info *o) {
   o->n_octants = h->n_cls; o->n_planes = h->n_planes; o->n_tasks = h->n_tasks; o->sweep_G = h->sweep_G;
   o->sweep_threads = h->sweep_threads; o->sweep_rmax = h->sweep_rmax; o->pencil_axis = h->pencil_axis; o->n_pos = h->n_pos;
   o->n_inflow = h->n_inflow; o->device_bytes = h->arena_bytes; o->sweep_smem_bytes = h->sweep_smem;
+  const bool fused = h->cgf_ok && !h->cg_force_generic;
+  o->cg_fused = fused; o->cg_cells_per_thread = fused ? h->cgf_cpt : 0; o->cg_ctas = fused ? h->cgf_nblk : h->cg_blocks;
+  o->cg_face_uniform = fused && h->cgf_uni; o->cg_recycle = fused && h->cgf_recycle;
   return 0;
 }
 

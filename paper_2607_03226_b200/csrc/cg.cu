@@ -12,6 +12,9 @@
 #include "internal.h"
 namespace cg = cooperative_groups;
 
+// bit set in the iteration count the kernels report when the loop ended on max_iter with ||r|| > rtol ||rhs||
+constexpr unsigned long long kCgNotConverged = 1ull << 40;
+
 struct CgArgs {
   int32_t n, nf, max_iter, B;
   const int32_t *nbr;    // [nf][n]  neighbour (active index); entries without a neighbour point at the cell itself
@@ -117,7 +120,7 @@ __global__ void __launch_bounds__(256) cg_kernel(CgArgs a) {
     double *t = pold; pold = pnew; pnew = t;
     ++it;
   }
-  if (tid == 0) *a.iters_out = (unsigned long long)it;
+  if (tid == 0) *a.iters_out = (unsigned long long)it | (rr > stop2 ? kCgNotConverged : 0ull);
 }
 
 // =================================================================================================================
@@ -163,13 +166,6 @@ __device__ __forceinline__ void grid_barrier(unsigned int *bar, unsigned int tar
 }
 
 constexpr int kCgfThreads = 512;
-#ifdef NB_CG_PROFILE
-__device__ unsigned long long nb_cg_prof[8];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define NB_STAMP(k) do { if (blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_ = gtime(); nb_cg_prof[k] += t_ - t_last; t_last = t_; } } while (0)
-#else
-#define NB_STAMP(k) do {} while (0)
-#endif
 
 // UNI: every face slot carries one coefficient value or none (uniform structured grids).  The coefficients are then
 // kernel parameters, and a missing neighbour points at a slot of r_loc that stays zero.
@@ -203,7 +199,6 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
     const int li = tid + c * kCgfThreads, i = a0 + li;
     s[c] = wv[c] = r[c] = dg[c] = 0.0;
     if (li < a.chunk) x_s[li] = p_s[li] = 0.0;
-#pragma unroll
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       nl[c][f] = 0;
@@ -367,9 +362,7 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
 
   double g_prev = 1.0, alpha_prev = 1.0, stop2 = 0.0;
   int it = 0;
-#ifdef NB_CG_PROFILE
-  unsigned long long t_last = gtime();
-#endif
+  bool not_converged = false;
   for (;; ++it) {
     const int par = it & 1;
     // Issue every global load of the iteration first (per-CTA partials and the owners' w of the first halo batch):
@@ -414,8 +407,8 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
     __syncthreads();
     const double g = gd[0], d = gd[1];
     if (it == 0) stop2 = a.rtol * a.rtol * (bb_total >= 0.0 ? bb_total : g);
-    if (!(g > stop2) || it >= a.max_iter) break;
-    NB_STAMP(0);
+    if (!(g > stop2)) break;
+    if (it >= a.max_iter) { not_converged = true; break; }
     const double bet = it ? g / g_prev : 0.0;
     const double alpha = it ? g / (d - bet * g / alpha_prev) : g / d;
     // halo copies: same recurrences as the owner, owner's w
@@ -446,11 +439,8 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
       }
     }
     __syncthreads();
-    NB_STAMP(1);
     apply_and_reduce(par ^ 1);
-    NB_STAMP(2);
     grid_barrier(a.bar, epoch++ * a.nblk);
-    NB_STAMP(3);
     g_prev = g;
     alpha_prev = alpha;
   }
@@ -463,7 +453,7 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
       a.xprev[a0 + li] = x_s[li];
     }
   }
-  if (k == 0 && tid == 0) *a.iters_out = (unsigned long long)it;
+  if (k == 0 && tid == 0) *a.iters_out = (unsigned long long)it | (not_converged ? kCgNotConverged : 0ull);
 }
 
 typedef void (*cgf_fn)(CgfArgs);
@@ -473,6 +463,7 @@ static cgf_fn cgf_pick_cpt(int cpt) {
     case 1: return cg_fused_kernel<NF, 1, UNI>;
     case 2: return cg_fused_kernel<NF, 2, UNI>;
     case 4: return cg_fused_kernel<NF, 4, UNI>;
+    case 8: return cg_fused_kernel<NF, 8, UNI>;
   }
   return nullptr;
 }
@@ -534,15 +525,3 @@ int nb_cg_solve(nanobte_solver *h, int *iters) {
   if (iters) *iters = -1;  // read back by the caller together with max|dT|
   return 0;
 }
-
-#ifdef NB_CG_PROFILE
-extern "C" int nanobte_debug_cg_prof(unsigned long long *out, int reset) {
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(out, nb_cg_prof, sizeof(nb_cg_prof));
-  if (reset) {
-    unsigned long long z[8] = {0};
-    cudaMemcpyToSymbol(nb_cg_prof, z, sizeof(z));
-  }
-  return 0;
-}
-#endif

@@ -57,6 +57,7 @@ struct Common {
 int nb_validate_common(nanobte_solver *h, int dim, const nanobte_bands *bands, const nanobte_quadrature *quad,
                        const nanobte_tag *tags, int n_tags, Common &c);
 int nb_check_device(nanobte_solver *h);
+void nb_query_sm_count(nanobte_solver *h);
 // Finds j with s_j == s_d - 2 (s_d.n) n  (squared distance < 1e-18), or -1.
 int nb_find_mirror(const Common &c, int d, const double n[3]);
 

@@ -91,7 +91,7 @@ struct nanobte_solver {
   // structured sweep
   SweepArgs sw{};
   int sweep_G = 1, sweep_threads = 0, sweep_rmax = 1, n_tasks = 0, pencil_axis = 0, n_planes = 0, sweep_variant = 3, sweep_rp = 0;
-  bool uniform = true, sweep_attr_set = false;
+  bool uniform = true;
   const OctTab *d_octs = nullptr;
   size_t sweep_smem = 0;
   int64_t n_pos = 0, n_inflow = 0, e_stride = 0;

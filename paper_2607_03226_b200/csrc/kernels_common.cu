@@ -231,6 +231,10 @@ __global__ void __launch_bounds__(128) closure_inflow_kernel(InflowArgs R) {
   }
   const double p = type == NANOBTE_SPECULAR ? 1.0 : a.bf_p[bf];
   const int md = a.bf_mirror[(size_t)bf * a.D + d];
+  if (md < 0) {  // s_d . n == 0 exactly (R15): the face carries nothing for d; the sweep multiplies this slot by |s.n|/h = 0
+    for (int b = 0; b < a.B; ++b) dst[b * n_in] = 0.0;
+    return;
+  }
   const double *src = a.e + (int64_t)a.dir_row0[md] * a.e_stride + a.bf_opos[(size_t)bf * a.D + md];
   constexpr int UB = 6;
   for (int b0 = 0; b0 < a.B; b0 += UB) {

@@ -563,6 +563,7 @@ extern "C" int nanobte_workspace_bytes_structured(const nanobte_structured_mesh 
                                                   const nanobte_options *opt, size_t *bytes_out) {
   if (!bytes_out) return NANOBTE_E_INVALID;
   nanobte_solver tmp;
+  nb_query_sm_count(&tmp);
   return build(&tmp, m, b, q, tags, n_tags, nullptr, opt, true, bytes_out);
 }
 

@@ -574,10 +574,9 @@ int nb_launch_sweep_structured(nanobte_solver *h) {
     fn = pick(h->sweep_G, h->sweep_rmax, h->uniform, h->sweep_rp);
   }
   if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "no sweep kernel variant for G=%d R=%d", h->sweep_G, h->sweep_rmax);
-  if (!h->sweep_attr_set) {
-    NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(h->sweep_smem, 1024)));
-    h->sweep_attr_set = true;
-  }
+  // the attribute belongs to the function, not to this solver: another solver that picked the same instantiation may have
+  // set a smaller cap since our last launch, so it is (re)set before every launch
+  NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(h->sweep_smem, 1024)));
   fn<<<h->n_tasks, h->sweep_threads + 32, h->sweep_smem, h->stream>>>(h->sw, h->d_octs);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());

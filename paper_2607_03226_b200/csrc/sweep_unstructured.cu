@@ -445,10 +445,8 @@ int nb_launch_sweep_unstructured(nanobte_solver *h) {
     const int64_t n = (int64_t)a.D * a.e_stride;
     theta_permute_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(a);
     h->launches++;
-    if (!h->sweep_attr_set) {
-      NB_CUDA(h, cudaFuncSetAttribute(fs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->sweep_smem));
-      h->sweep_attr_set = true;
-    }
+    // per-function attribute, shared by every solver in the process: set before every launch
+    NB_CUDA(h, cudaFuncSetAttribute(fs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->sweep_smem));
     fs<<<a.D * a.st_NBG, a.st_threads, h->sweep_smem, h->stream>>>(a);
     h->launches++;
     NB_CUDA(h, cudaGetLastError());
@@ -456,10 +454,7 @@ int nb_launch_sweep_unstructured(nanobte_solver *h) {
   }
   uns_fn fn = pick_uns(a.MI);
   if (!fn) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "cells with more than 7 inflow faces are not supported");
-  if (!h->sweep_attr_set) {
-    NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(h->sweep_smem, 1024)));
-    h->sweep_attr_set = true;
-  }
+  NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(h->sweep_smem, 1024)));
   fn<<<a.D * a.NBG, h->sweep_threads, h->sweep_smem, h->stream>>>(a);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
@@ -829,13 +824,12 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
       if (ns >= (1 << 27) || nc >= (1 << 27)) staged = false;
       for (int l = 0; l < n_lvl[d] && staged; ++l) {  // three consecutive levels must fit the rings
         const int l4 = std::min(l + 3, n_lvl[d]);
-        if (lp[l4] - lp[l] > st_rr) { staged = false; if (std::getenv("NANOBTE_DEBUG")) fprintf(stderr, "staged off: dir %d level %d span %d > %d\n", d, l, lp[l4] - lp[l], st_rr); }
+        if (lp[l4] - lp[l] > st_rr) staged = false;
       }
     }
   }
   const size_t st_smem = ((size_t)st_vr * st_BG + (size_t)st_sr * st_BG) * sizeof(double) + st_rec_smem + 64;
   if (st_smem > 227 * 1024 - 512) staged = false;
-  if (std::getenv("NANOBTE_DEBUG")) fprintf(stderr, "unstructured sweep: staged %d BG %d NBG %d vr %d sr %d smem %zu MI %d late refs %ld side entries %zu\n", (int)staged, st_BG, st_NBG, st_vr, st_sr, st_smem, MI, n_late, side_src.size());
   const int st_rsb = (24 + 12 * MI + 15) / 16 * 16;
   std::vector<char> st_rec(staged ? (size_t)D * e_stride * st_rsb : 16, 0);
   if (staged)
@@ -945,6 +939,7 @@ extern "C" int nanobte_workspace_bytes_unstructured(const nanobte_unstructured_m
                                                     const nanobte_options *opt, size_t *bytes_out) {
   if (!bytes_out) return NANOBTE_E_INVALID;
   nanobte_solver tmp;
+  nb_query_sm_count(&tmp);
   int rc = build_uns(&tmp, m, b, q, tags, n_tags, nullptr, opt, true, bytes_out);
   nb_free_unstructured(&tmp);
   return rc;

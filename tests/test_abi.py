@@ -30,12 +30,28 @@ def test_exports_every_declared_symbol(lib):
         assert hasattr(lib, name), name
 
 
-def test_struct_layouts_match_header(lib):
-    # sizes the C compiler gives the ABI structs (LP64): a drifted ctypes mirror would corrupt every call
-    assert C.sizeof(binding.Bands) == 40 and C.sizeof(binding.Quadrature) == 24 and C.sizeof(binding.Tag) == 16
-    assert C.sizeof(binding.StructuredMesh) == 88 and C.sizeof(binding.UnstructuredMesh) == 64
-    assert C.sizeof(binding.Options) == 64
-    assert C.sizeof(binding.Info) == 88
+def test_struct_layouts_match_header(lib, tmp_path):
+    """Sizes and field offsets the C compiler gives the ABI structs of include/nanobte.h (gcc, LP64) against the ctypes
+    mirrors in binding.py: a drifted mirror would corrupt every call."""
+    import subprocess
+    structs = {"nanobte_bands": binding.Bands, "nanobte_quadrature": binding.Quadrature, "nanobte_tag": binding.Tag,
+               "nanobte_structured_mesh": binding.StructuredMesh, "nanobte_unstructured_mesh": binding.UnstructuredMesh,
+               "nanobte_options": binding.Options, "nanobte_info": binding.Info}
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "nanobte.h"', 'int main(void) {']
+    for cname, cls in structs.items():
+        lines.append(f'printf("{cname} %zu\\n", sizeof({cname}));')
+        for fname, _ in cls._fields_:
+            lines.append(f'printf("{cname}.{fname} %zu\\n", offsetof({cname}, {fname}));')
+    lines += ['return 0;', '}']
+    src = tmp_path / "abi.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "abi"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    got = dict(ln.split() for ln in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.splitlines())
+    for cname, cls in structs.items():
+        assert int(got[cname]) == C.sizeof(cls), cname
+        for fname, _ in cls._fields_:
+            assert int(got[f"{cname}.{fname}"]) == getattr(cls, fname).offset, f"{cname}.{fname}"
 
 
 def test_strerror(lib):

@@ -129,6 +129,99 @@ def test_fullsize_moments_and_energy_identity(name):
     g.close()
 
 
+# ---- full MESH, few bands: every kernel of the step at the mesh size (and launch shape class) bench.py times ---------------------------
+FULLMESH = {
+    # name: (problem factory, mode, expected cells per thread of the fused CG)
+    "cube": (lambda: wl.config_cube(B=3, n_polar=2, n_azim=8, mode="synthetic"), "synthetic", 4),
+    "finfet": (lambda: wl.config_finfet(B=3, n_polar=2, n_azim=8), "synthetic", 4),
+    "finfet_96x48x48": (lambda: wl.config_finfet(nx=96, ny=48, nz=48, B=2, n_polar=2, n_azim=8), "synthetic", 2),
+    "cube_72": (lambda: wl.config_cube(n=72, B=2, n_polar=2, n_azim=8, mode="synthetic"), "synthetic", 8),
+    "triangles": (lambda: wl.config_triangles(B=3, D=16), "plain", None),
+}
+
+
+@pytest.mark.parametrize("name", list(FULLMESH))
+def test_fullmesh_few_bands_steps(name):
+    """The FULL mesh of configs 2-4 (and two meshes that put 2 and 8 cells on a CG thread) with a 2-3-band table on both
+    sides: eps, theta_SI, theta_en, q, G, boundary heat and theta after diffusion_correct, element by element against
+    the oracle for 3 steps.  Runs cg_fused_kernel<6,4,uni> with 148 CTAs, its halo batches and tail, update_kernel's class
+    combine and the closures at the mesh size of the bench."""
+    from paper_2607_03226_b200.binding import Solver
+    make, mode, cpt = FULLMESH[name]
+    pr = make()
+    g, r = Solver(pr), RefSolver(pr)
+    if cpt is not None:
+        assert g.info["cg_fused"] == 1 and g.info["cg_cells_per_thread"] == cpt, g.info
+        if cpt >= 4:
+            assert g.info["cg_ctas"] == 148
+    rng = np.random.default_rng(11)
+    T0 = pr["T_ref"] + rng.uniform(-2.0, 2.0, n_cells_of(pr))
+    g.set_T(T0)
+    r.set_T(T0)
+    Tr = pr["T_ref"]
+    for n in range(3):
+        g.sweep()
+        r.sweep()
+        for b in range(len(pr["bands"]["C"])):
+            eg, er = g.get_e(b, 1)[0], r.get_e(b, 1)[0]
+            assert rel(eg, er) <= TOL_SWEEP, f"{name} sweep {n} band {b}: {rel(eg, er):.3e}"
+            del eg, er
+        dg, dr = g.update_temperature(), r.update_temperature()
+        assert abs(dg - dr) <= 1e-9 * abs(dr) + 1e-13
+        for which in (0, 1, 2):
+            a, b = g.get_T(which) - Tr, r.get_T(which) - Tr
+            assert rel(a, b) <= TOL_SWEEP, f"{name} update {n}: T[{which}] {rel(a, b):.3e}"
+        assert rel(g.get_q(), r.get_q()) <= TOL_SWEEP, f"{name} update {n}: q"
+        assert rel(g.get_G(), r.get_G()) <= TOL_SWEEP, f"{name} update {n}: G"
+        Hg, Hr = g.get_boundary_heat(), r.get_boundary_heat()
+        assert np.abs(Hg - Hr).max() <= 1e-9 * np.abs(Hr).max()
+        if mode == "synthetic":
+            (ir, _), (ig, _) = r.diffusion_correct(), g.diffusion_correct()
+            a, b = g.get_T(0) - Tr, r.get_T(0) - Tr
+            # CG to rtol 1e-12 on both sides; the compared field carries rtol x condition number (DESIGN.md R14e)
+            assert rel(a, b) <= 1e-9, f"{name} synthetic step {n}: {rel(a, b):.3e}"
+            assert ig <= ir + max(2, ir // 20), (ig, ir)
+    g.close()
+    r.close()
+
+
+# ---- converged runs at full size against the oracle's stored fields ---------------------------------------------------------------------
+def test_config1_nongray_square_full_solve():
+    """configs[1] at its full 128 x 128 size: the oracle converges it in seconds (11 iterations)."""
+    from paper_2607_03226_b200.binding import Solver
+    pr = wl.config_nongray_square()
+    r, g = RefSolver(pr), Solver(pr)
+    rr, rg = r.solve(pr["tol"], pr["max_iter"]), g.solve(pr["tol"], pr["max_iter"])
+    assert rr["converged"] and rg["converged"] and rr["iters"] == rg["iters"], (rr, rg)
+    assert np.abs(g.get_T(0) - r.get_T(0)).max() <= 1e-8
+    np.testing.assert_allclose(g.get_history()[0], r.get_history()[0], rtol=1e-6, atol=1e-14)
+    g.close()
+    r.close()
+
+
+@pytest.mark.parametrize("name,mode", [("cube", "plain"), ("cube", "synthetic"), ("finfet", "synthetic"), ("triangles", "plain")])
+def test_fullsize_converged_against_golden(name, mode):
+    """north_star: converged T within 1e-8 K of the oracle's with an identical iteration count, on the full configs.
+    tests/golden/<name>_<mode>_oracle.npz is the oracle's own converged run (written by make_fullsize_golden.py from
+    oracle/ only)."""
+    from paper_2607_03226_b200.binding import Solver
+    path = os.path.join(GOLDEN, f"{name}_{mode}_oracle.npz")
+    if not os.path.exists(path):
+        pytest.fail(f"{path} missing: run python tests/golden/make_fullsize_golden.py {name} {mode}")
+    gold = np.load(path)
+    pr = wl.CONFIGS[name]()
+    assert str(gold["problem"]) == pr["name"] and float(gold["tol"]) == pr["tol"]
+    g = Solver(pr)
+    res = g.solve(pr["tol"], pr["max_iter"], mode)
+    assert res["converged"] and res["iters"] == int(gold["iters"]), (res, int(gold["iters"]))
+    m = pr["mesh"]
+    act = np.ones(g.n_cells, dtype=bool) if (pr["kind"] == "unstructured" or m["active"] is None) else np.asarray(m["active"]).reshape(-1) != 0
+    T = g.get_T(0)[act]
+    assert np.abs(T - gold["T_active"]).max() <= 1e-8, np.abs(T - gold["T_active"]).max()
+    np.testing.assert_allclose(g.get_history()[0], gold["hist_dT"], rtol=1e-6, atol=1e-14)
+    g.close()
+
+
 def test_config0_against_golden_file():
     """tests/golden/config0_oracle.txt (written by make_config0_golden.py from oracle/ only)."""
     from paper_2607_03226_b200.binding import Solver

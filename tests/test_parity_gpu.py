@@ -360,3 +360,80 @@ def test_cg_from_zero_matches_oracle_counts(monkeypatch):
         (ir, _), (ig, _) = r.diffusion_correct(), g.diffusion_correct()
         assert abs(ig - ir) <= max(2, ir // 20)
     assert rel(g.get_T(0) - pr["T_ref"], r.get_T(0) - pr["T_ref"]) <= 1e-9
+
+
+# ---- fused-CG instantiations: 2, 4 and 8 cells per thread, halo batches beyond the unrolled ones ------------------------------------
+@pytest.mark.parametrize("nblk,cpt", [(6, 2), (3, 4), (2, 8)])
+@pytest.mark.parametrize("hook", ["", "NANOBTE_CG_NO_UNI", "NANOBTE_CG_NO_RECYCLE"])
+def test_fused_cg_cells_per_thread_on_cuts(monkeypatch, nblk, cpt, hook):
+    """NANOBTE_CG_NBLK caps the CTA count of the fused CG so that a cut runs the kernel instantiations the full-size
+    configs use (4 cells per thread on configs 2-4; 2 and 8 on meshes around them), with the face-uniform and the
+    general stencil, with and without the recycled guess: element-wise against the oracle for 3 synthetic steps."""
+    monkeypatch.setenv("NANOBTE_CG_NBLK", str(nblk))
+    if hook:
+        monkeypatch.setenv(hook, "1")
+    pr = wl.config_finfet(nx=32, ny=16, nz=16, B=3, n_polar=2, n_azim=8)
+    g = gpu_solver(pr)
+    assert g.info["cg_fused"] == 1 and g.info["cg_cells_per_thread"] == cpt and g.info["cg_ctas"] <= nblk, g.info
+    assert g.info["cg_face_uniform"] == (0 if hook == "NANOBTE_CG_NO_UNI" else 1)
+    g.close()
+    step_parity(pr, 3, T_init=random_T(pr, 10), mode="synthetic")
+
+
+def test_cg_not_converged_is_reported():
+    """cg_max_iter too small: diffusion_correct and solve say NOT_CONVERGED (1) instead of OK."""
+    pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
+    g = gpu_solver(pr, cg_max_iter=5)
+    g.sweep()
+    g.update_temperature()
+    rc = g._lib.nanobte_diffusion_correct(g._h, None, None)
+    assert rc == 1
+    res = g.solve(1e-9, 3, "synthetic")
+    assert not res["converged"]
+    g.close()
+
+
+# ---- ADVICE r1: two live structured solvers that share a kernel instantiation with different shared-memory sizes ----------------------
+def test_interleaved_big_and_small_solvers():
+    big = wl.config_cube(n=28, B=3, n_polar=2, n_azim=8)
+    small = wl.config_cube(n=8, B=3, n_polar=2, n_azim=8)
+    kw = {"sweep_G": 2, "sweep_threads": 128}
+    gb, gs = gpu_solver(big, **kw), gpu_solver(small, **kw)
+    rb, rs = RefSolver(big), RefSolver(small)
+    assert gb.info["sweep_smem_bytes"] > 2 * gs.info["sweep_smem_bytes"]
+    for _ in range(3):  # big, small, big, ...: the per-function shared-memory cap must follow the launching solver
+        gb.sweep(); rb.sweep()
+        gs.sweep(); rs.sweep()
+        compare_state(gb, rb, big, "big")
+        compare_state(gs, rs, small, "small")
+        gb.update_temperature(); rb.update_temperature()
+        gs.update_temperature(); rs.update_temperature()
+    for s in (gb, gs, rb, rs):
+        s.close()
+
+
+# ---- ADVICE r1 / R15: directions exactly parallel to grid faces ---------------------------------------------------------------------------
+def axis_parallel_quadrature(dim):
+    if dim == 2:
+        a = np.sqrt(0.5)
+        s = np.array([[1, 0, 0], [a, a, 0], [0, 1, 0], [-a, a, 0], [-1, 0, 0], [-a, -a, 0], [0, -1, 0], [a, -a, 0]], dtype=np.float64)
+        return {"s": s, "w": np.full(8, 2 * np.pi / 8), "dim": 2}
+    a = 1.0 / np.sqrt(3.0)
+    axes = [[1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1]]
+    diag = [[sx * a, sy * a, sz * a] for sx in (1, -1) for sy in (1, -1) for sz in (1, -1)]
+    s = np.array(axes + diag, dtype=np.float64)
+    w = np.concatenate([np.full(6, 4 * np.pi * 0.4 / 6), np.full(8, 4 * np.pi * 0.6 / 8)])
+    return {"s": s, "w": w, "dim": 3}
+
+
+@pytest.mark.parametrize("shape", [(6, 5, 1), (5, 4, 3)])
+@pytest.mark.parametrize("mode", ["plain", "synthetic"])
+def test_axis_parallel_directions(shape, mode):
+    """A component of s exactly 0 (s.n = 0 on some faces, R15): such a face carries nothing for that direction, on every
+    wall type; the oracle drops the face from both sums, the CUDA path multiplies a finite cache slot by 0."""
+    nx, ny, nz = shape
+    tags = [(wl.THERMALIZING, 303.0), (wl.MIXED, 0.0), (wl.SPECULAR, 0.0), (wl.DIFFUSE, 0.0), (wl.SPECULAR, 0.0)]
+    bands = small_bands(2, 31, lo=-11.3)
+    pr = wl.make_structured_problem(nx, ny, nz, 7e-9, 7e-9, 7e-9, bands, axis_parallel_quadrature(3 if nz > 1 else 2), tags,
+                                    [0, 1, 2, 3, 4, 2], Qdot=np.full(nx * ny * nz, 2e16), p_seed=5)
+    step_parity(pr, 4, T_init=random_T(pr, 8), mode=mode)
