@@ -245,6 +245,7 @@ def main():
     skw = dict(sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_variant=args.sweep_variant)
     t_c0 = time.perf_counter()
     g = Solver(pr, **skw)
+    g.set_keep_e(False)  # the sweeps of an iteration leave eps where solve() leaves it (on chip where the kernel can)
     torch.cuda.synchronize()
     create_s = time.perf_counter() - t_c0
     upd = wl.n_updates(pr)
@@ -301,6 +302,7 @@ def main():
     # ---- end-to-end arm: the SAME outer iterations (fresh solver, same warm-up), host buffers through the C ABI, the
     # host<->device copies of every step inside the timed region ----------------------------------------------------------
     g = Solver(pr, **skw)
+    g.set_keep_e(False)
     T_host = torch.empty(g.n_cells, dtype=torch.float64).pin_memory()
     T_host.copy_(torch.as_tensor(g.get_T(0)))
     T_np = T_host.numpy()

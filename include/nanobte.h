@@ -127,7 +127,9 @@ typedef struct {
   int32_t cg_max_iter;          /* <= 0 -> 100000                                                  */
   int32_t sweep_G;              /* tuning: systems per CTA in the structured sweep (1..4); 0 = auto   */
   int32_t sweep_threads;        /* tuning: compute threads per CTA of the structured sweep (<= 480); 0 = auto */
-  int32_t sweep_variant;        /* tuning: 0 = auto, 3 = single-buffered state (any spacing), 4 = double-buffered (uniform) */
+  int32_t sweep_variant;        /* 0 = auto; 3 = hyperplane sweep, single-buffered state (any spacing); 4 = hyperplane sweep,
+                                   double-buffered (uniform); 5 = tile-dataflow sweep with fused moments (3-D, uniform;
+                                   what auto picks there unless sweep_G / sweep_threads are given)              */
 } nanobte_options;
 
 /* Layout / schedule facts of a created solver (for reporting and roofline arithmetic). */
@@ -147,6 +149,7 @@ typedef struct {
   int32_t cg_ctas;              /* CTAs of the cooperative launch (0 before the first fallback launch) */
   int32_t cg_face_uniform;      /* fused kernel: face-uniform stencil (uniform structured grids)   */
   int32_t cg_recycle;           /* fused kernel: recycled initial guess on                         */
+  int32_t sweep_variant;        /* 3 / 4: hyperplane kernels, 5: tile-dataflow sweep with fused moments, 1: unstructured level sweep */
 } nanobte_info;
 
 /* Bytes of device workspace create_* would need for this problem (same validation as create). */
@@ -172,6 +175,10 @@ void nanobte_destroy(nanobte_solver *);
  * 110.  Boundary inflow values are the ones cached by the previous nanobte_update_temperature (R9: lagged);
  * before the first update they are the thermalizing constants and zero elsewhere (R12).  Asynchronous. */
 int nanobte_sweep(nanobte_solver *);
+/* keep != 0 (the default): nanobte_sweep leaves the distribution in device memory for nanobte_get_e.  keep == 0: on
+ * grids swept by the tile-dataflow kernel nanobte_sweep keeps it on chip, exactly as the sweeps inside nanobte_step /
+ * nanobte_solve do (see nanobte_step); the other sweep kernels always store it and ignore the setting. */
+int nanobte_set_keep_e(nanobte_solver *, int32_t keep);
 
 /* (a6) moments + closure refresh + plain update: T_SI (Eq. 5), T_energy (R13), q (Eq. 7), diffuse averages G
  * and the boundary inflow cache for the next sweep (R6-R8), T <- T_SI (Eq. 6).  max_dT (host pointer or
@@ -183,6 +190,15 @@ int nanobte_update_temperature(nanobte_solver *, double *max_dT);
  * Returns NANOBTE_NOT_CONVERGED (state valid, T updated with the last CG iterate) when the CG stopped on
  * options.cg_max_iter with ||r|| > cg_rtol ||rhs||. */
 int nanobte_diffusion_correct(nanobte_solver *, int32_t *cg_iters, double *max_dT);
+
+/* One source iteration as nanobte_solve runs it: sweep, closures + moments + update and, in synthetic mode, the CG
+ * correction.  On grids swept by the tile-dataflow kernel the sweep of a step keeps the
+ * distribution on chip (the moments are reduced inside the sweep; only wall-cell values and tile faces
+ * go to memory); nanobte_get_e afterwards first runs one storing sweep from the current T and wall cache, i.e. it
+ * returns the distribution the NEXT iteration would compute (equal to the last one to the solve tolerance at
+ * convergence).  nanobte_sweep always stores the distribution.  max_dT / cg_iters: host pointers or NULL; synchronises.
+ * Return values as nanobte_diffusion_correct. */
+int nanobte_step(nanobte_solver *, int32_t mode, double *max_dT, int32_t *cg_iters);
 
 /* (a8) outer loop until max|dT| < tol or max_iter sweeps (R11).  Synchronises once per iteration
  * (one double device->host).  Starts the recycled CG guess afresh, so the result does not depend on earlier

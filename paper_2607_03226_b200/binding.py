@@ -21,7 +21,7 @@ ERRORS = {0: "OK", 1: "NOT_CONVERGED", -1: "INVALID", -2: "ALLOC", -3: "CUDA", -
 EXPORTS = [
     "nanobte_workspace_bytes_structured", "nanobte_workspace_bytes_unstructured", "nanobte_create_structured",
     "nanobte_create_unstructured", "nanobte_destroy", "nanobte_sweep", "nanobte_update_temperature",
-    "nanobte_diffusion_correct", "nanobte_solve", "nanobte_set_T", "nanobte_get_T", "nanobte_get_q", "nanobte_get_e",
+    "nanobte_diffusion_correct", "nanobte_step", "nanobte_set_keep_e", "nanobte_solve", "nanobte_set_T", "nanobte_get_T", "nanobte_get_q", "nanobte_get_e",
     "nanobte_get_G", "nanobte_get_boundary_heat", "nanobte_get_history", "nanobte_get_info", "nanobte_launch_count",
     "nanobte_kappa", "nanobte_strerror", "nanobte_last_error",
 ]
@@ -67,7 +67,7 @@ class Info(C.Structure):
                 ("sweep_rmax", C.c_int32), ("pencil_axis", C.c_int32), ("n_pos", C.c_int64), ("n_inflow", C.c_int64),
                 ("device_bytes", C.c_size_t), ("sweep_smem_bytes", C.c_size_t), ("cg_fused", C.c_int32),
                 ("cg_cells_per_thread", C.c_int32), ("cg_ctas", C.c_int32), ("cg_face_uniform", C.c_int32),
-                ("cg_recycle", C.c_int32)]
+                ("cg_recycle", C.c_int32), ("sweep_variant", C.c_int32)]
 
 
 class NanoBTEError(RuntimeError):
@@ -100,6 +100,8 @@ def load():
     lib.nanobte_sweep.argtypes = [vp]
     lib.nanobte_update_temperature.argtypes = [vp, _dp]
     lib.nanobte_diffusion_correct.argtypes = [vp, _ip, _dp]
+    lib.nanobte_step.argtypes = [vp, C.c_int32, _dp, _ip]
+    lib.nanobte_set_keep_e.argtypes = [vp, C.c_int32]
     lib.nanobte_solve.argtypes = [vp, C.c_double, C.c_int32, C.c_int32, _ip, _dp]
     lib.nanobte_set_T.argtypes = [vp, vp, C.c_int32]
     lib.nanobte_get_T.argtypes = [vp, C.c_int32, vp, C.c_int32]
@@ -257,6 +259,9 @@ class Solver:
     def sweep(self):
         self._chk(self._lib.nanobte_sweep(self._h))
 
+    def set_keep_e(self, keep):
+        self._chk(self._lib.nanobte_set_keep_e(self._h, 1 if keep else 0))
+
     def update_temperature(self, sync=True):
         if not sync:
             self._chk(self._lib.nanobte_update_temperature(self._h, None))
@@ -269,6 +274,12 @@ class Solver:
         it, d = C.c_int32(), C.c_double()
         self._chk(self._lib.nanobte_diffusion_correct(self._h, C.byref(it), C.byref(d)))
         return it.value, d.value
+
+    def step(self, mode="plain"):
+        """One source iteration as solve() runs it; returns (max|dT|, CG iterations)."""
+        it, d = C.c_int32(), C.c_double()
+        self._chk(self._lib.nanobte_step(self._h, 1 if mode in (1, "synthetic") else 0, C.byref(d), C.byref(it)))
+        return d.value, it.value
 
     def solve(self, tol, max_iter, mode="plain"):
         it, d = C.c_int32(), C.c_double()

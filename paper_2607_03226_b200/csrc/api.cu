@@ -4,6 +4,7 @@
 #include <numeric>
 #include <cstdlib>
 
+#include "brick.h"
 #include "host_util.h"
 
 int nb_fail(nanobte_solver *h, int code, const char *fmt, ...) {
@@ -334,16 +335,30 @@ extern "C" void nanobte_destroy(nanobte_solver *h) {
   if (!h) return;
   if (h->stream || h->arena) cudaStreamSynchronize(h->stream);
   nb_free_unstructured(h);
+  nb_free_brick(h);
   if (h->arena && h->arena_owned) cudaFree(h->arena);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;
 }
 
-extern "C" int nanobte_sweep(nanobte_solver *h) {
-  if (!h || !h->arena) return NANOBTE_E_INVALID;
+// One transport sweep.  keep_e = 0 lets the tile-dataflow sweep leave the distribution on chip (moments and wall values
+// are all the iteration needs); the other sweeps always store it.
+static int sweep_internal(nanobte_solver *h, int keep_e) {
   h->swept_since_closure = true;
   h->therm_stale = true;
+  if (h->brick) return nb_launch_sweep_brick(h, keep_e);
   return h->kind == 0 ? nb_launch_sweep_structured(h) : nb_launch_sweep_unstructured(h);
+}
+
+extern "C" int nanobte_sweep(nanobte_solver *h) {
+  if (!h || !h->arena) return NANOBTE_E_INVALID;
+  return sweep_internal(h, h->keep_e ? 1 : 0);
+}
+
+extern "C" int nanobte_set_keep_e(nanobte_solver *h, int32_t keep) {
+  if (!h) return NANOBTE_E_INVALID;
+  h->keep_e = keep != 0;
+  return 0;
 }
 
 static int read_maxdT(nanobte_solver *h, double *out) {
@@ -401,7 +416,7 @@ extern "C" int nanobte_solve(nanobte_solver *h, double tol, int32_t max_iter, in
   bool cg_failed = false;
   while (n < max_iter) {
     int cg = 0;
-    if ((r = nanobte_sweep(h)) < 0) return r;
+    if ((r = sweep_internal(h, 0)) < 0) return r;
     if (mode == 0) {
       if ((r = nanobte_update_temperature(h, &dT)) < 0) return r;
     } else {
@@ -420,6 +435,24 @@ extern "C" int nanobte_solve(nanobte_solver *h, double tol, int32_t max_iter, in
   if (iters_out) *iters_out = n;
   if (last_dT_out) *last_dT_out = dT;
   return rc;
+}
+
+extern "C" int nanobte_step(nanobte_solver *h, int32_t mode, double *max_dT, int32_t *cg_iters) {
+  if (!h || !h->arena) return NANOBTE_E_INVALID;
+  if (mode != 0 && mode != 1) return nb_fail(h, NANOBTE_E_INVALID, "mode must be 0 (plain) or 1 (synthetic)");
+  if (mode == 1 && !h->any_therm) return nb_fail(h, NANOBTE_E_SINGULAR, "synthetic mode needs at least one thermalizing face");
+  int r;
+  double dT = 0.0;
+  if ((r = sweep_internal(h, 0)) < 0) return r;
+  if (cg_iters) *cg_iters = 0;
+  if (mode == 0) {
+    r = nanobte_update_temperature(h, &dT);
+  } else {
+    if ((r = nanobte_update_temperature(h, nullptr)) < 0) return r;
+    r = nanobte_diffusion_correct(h, cg_iters, &dT);
+  }
+  if (max_dT) *max_dT = dT;
+  return r;
 }
 
 // ---- getters / setters ---------------------------------------------------------------------------------------
@@ -473,6 +506,10 @@ extern "C" int nanobte_get_e(nanobte_solver *h, int32_t b0, int32_t nb, int32_t 
   if (!h || !h->arena || !dst) return NANOBTE_E_INVALID;
   if (b0 < 0 || nb < 0 || b0 + nb > h->B || d0 < 0 || nd < 0 || d0 + nd > h->D)
     return nb_fail(h, NANOBTE_E_INVALID, "band/direction range");
+  if (h->brick && !h->brick->e_valid) {  // the last sweep kept the distribution on chip: sweep once more, storing it
+    int rc = sweep_internal(h, 1);
+    if (rc < 0) return rc;
+  }
   if (dst_is_device) return nb_launch_get_e(h, b0, nb, d0, nd, dst, deviational);
   // host destination: one (band, direction) row at a time through the part[] scratch
   for (int b = 0; b < nb; ++b)
@@ -521,6 +558,7 @@ extern "C" int nanobte_get_info(const nanobte_solver *h, nanobte_info *o) {
   const bool fused = h->cgf_ok && !h->cg_force_generic;
   o->cg_fused = fused; o->cg_cells_per_thread = fused ? h->cgf_cpt : 0; o->cg_ctas = fused ? h->cgf_nblk : h->cg_blocks;
   o->cg_face_uniform = fused && h->cgf_uni; o->cg_recycle = fused && h->cgf_recycle;
+  o->sweep_variant = h->kind == 1 ? 1 : h->sweep_variant;
   return 0;
 }
 

@@ -96,6 +96,10 @@ struct nanobte_solver {
   size_t sweep_smem = 0;
   int64_t n_pos = 0, n_inflow = 0, e_stride = 0;
 
+  // tile-dataflow sweep with fused moments (brick.h); non-null = this path is the solver's sweep
+  struct BrickState *brick = nullptr;
+  bool keep_e = true;  // nanobte_sweep stores the distribution (nanobte_set_keep_e)
+
   // unstructured sweep (see sweep_unstructured.cu)
   struct UnsArgs *uns = nullptr;
   bool uns_staged = false;
@@ -176,6 +180,7 @@ int nb_fail(nanobte_solver *h, int code, const char *fmt, ...);
 
 // kernels_common.cu
 int nb_launch_boundary(nanobte_solver *h, int init = 0);
+int nb_launch_gcomb(nanobte_solver *h, const int32_t *faces, int n_faces, const uint8_t *nord);
 int nb_refresh_thermalizing(nanobte_solver *h);
 int nb_launch_moments(nanobte_solver *h);
 int nb_launch_update(nanobte_solver *h, int mode /*0: theta<-theta_SI, 1: theta<-theta_SI+x*/);

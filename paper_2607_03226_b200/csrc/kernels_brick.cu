@@ -1,0 +1,285 @@
+// kernels_brick.cu -- closures (a3), moment combine + temperature update (a6, a8) and exports for the row spaces of the
+// tile-dataflow sweep (brick.h).  Same arithmetic as the kernels in kernels_common.cu, other addresses:
+//   wall rows    eps of the cells with an outgoing boundary face, [row][system] per (class, group)
+//   inflow rows  what the sweep reads at a wall (R6-R9), [row][system] per (class, group)
+#include <algorithm>
+
+#include "brick.h"
+
+namespace {
+
+__device__ __forceinline__ double nanmax_d(double a, double b) { return !(b <= a) ? b : a; }
+
+struct BrickClosureArgs {
+  BoundaryArgs a;
+  double W;
+  const BrickCG *cgs;
+  const int32_t *cg_of;      // [n_cls][B]
+  const int32_t *dir_local;  // [D]
+  const int32_t *dir_cls;    // [D]
+  const int32_t *cls_dirs;   // [n_cls][max_dirs]
+  int32_t max_dirs;
+  const double *wall;
+  double *inf;
+  // gsum
+  const int32_t *out_bf[NB_MAX_CLASSES], *out_row[NB_MAX_CLASSES];
+  const uint8_t *out_ord[NB_MAX_CLASSES];
+  int32_t n_out[NB_MAX_CLASSES];
+  int32_t therm;             // 1: thermalizing faces only, 0: all the others
+  double *partial;           // [4][n_bf][B]
+  // inflow
+  const int32_t *in_row[NB_MAX_CLASSES], *in_bf[NB_MAX_CLASSES];
+  int32_t n_in[NB_MAX_CLASSES];
+  const int32_t *bf_wrow;    // [n_cls][n_bf]
+  int32_t init;
+};
+
+// gnum share of one class: sum over the class's directions of w (s.n) eps at the wall cell (R7).  One thread per
+// (outgoing face entry, band); the directions of a (cell, band) are contiguous in the wall row.
+__global__ void __launch_bounds__(128) brick_gsum_kernel(const BrickClosureArgs R) {
+  const BoundaryArgs &a = R.a;
+  const int c = blockIdx.y;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)R.n_out[c] * a.B) return;
+  const int j = (int)(idx / a.B), b = (int)(idx % a.B);
+  const int bf = R.out_bf[c][j];
+  if ((a.bf_type[bf] == NANOBTE_THERMALIZING) != (R.therm != 0)) return;
+  const BrickCG G = R.cgs[R.cg_of[c * a.B + b]];
+  const double *src = R.wall + G.wall_base + (int64_t)R.out_row[c][j] * G.S + (b - G.b0) * G.nd;
+  const double *sn = a.bf_sn + (size_t)bf * a.D;
+  double acc = 0.0;
+  for (int dl = 0; dl < G.nd; ++dl) {
+    const int d = R.cls_dirs[c * R.max_dirs + dl];
+    acc += a.w[d] * sn[d] * src[dl];
+  }
+  R.partial[((size_t)R.out_ord[c][j] * a.n_bf + bf) * a.B + b] = acc;
+}
+
+// Inflow rows of the boundary faces (R6-R8, lagged R9): one CTA per (row, (class, group)), lanes = systems.
+__global__ void __launch_bounds__(kBrickMaxS) brick_inflow_kernel(const BrickClosureArgs R) {
+  const BoundaryArgs &a = R.a;
+  const BrickCG G = R.cgs[blockIdx.y];
+  const int c = G.cls, k = blockIdx.x, s = threadIdx.x;
+  if (k >= R.n_in[c] || s >= G.S) return;
+  const int bf = R.in_bf[c][k];
+  const int type = a.bf_type[bf];
+  double *dst = R.inf + G.inf_base + (int64_t)R.in_row[c][k] * G.S + s;
+  const int b = G.b0 + s / G.nd;
+  if (type == NANOBTE_THERMALIZING) {
+    if (R.init) *dst = a.C[b] * a.bf_eps_w[bf] / R.W;  // R6; never changes afterwards
+    return;
+  }
+  if (R.init) return;  // eps^0 = 0 (R12)
+  const double Gf = a.G[(size_t)bf * a.B + b];
+  if (type == NANOBTE_DIFFUSE) {
+    *dst = Gf;  // R7
+    return;
+  }
+  const int d = R.cls_dirs[c * R.max_dirs + s % G.nd];
+  const int md = a.bf_mirror[(size_t)bf * a.D + d];
+  if (md < 0) {  // s_d . n == 0 exactly (R15): the sweep multiplies this row by 0
+    *dst = 0.0;
+    return;
+  }
+  const int cm = R.dir_cls[md];
+  const BrickCG Gm = R.cgs[R.cg_of[cm * a.B + b]];
+  const double spec = R.wall[Gm.wall_base + (int64_t)R.bf_wrow[(size_t)cm * a.n_bf + bf] * Gm.S + (b - Gm.b0) * Gm.nd + R.dir_local[md]];
+  *dst = type == NANOBTE_SPECULAR ? spec : a.bf_p[bf] * spec + (1.0 - a.bf_p[bf]) * Gf;  // R8
+}
+
+// Combine the partials of every (class, group) per cell in fixed order, update T, track max |dT|, refresh the
+// sweep-order copies of theta.
+struct BrickUpdateArgs {
+  int32_t n_act, n_cls, n_cg, mode;
+  const BrickCG *cgs;
+  const double *part;
+  int32_t npos[NB_MAX_CLASSES];
+  const int32_t *a2pos;  // [n_cls][n_act]
+  double *th[NB_MAX_CLASSES];
+  double *theta, *theta_prev, *theta_SI, *theta_en, *q;
+  const double *x;
+  double beta, Csum;
+  unsigned long long *maxdT;
+};
+
+__global__ void __launch_bounds__(256) brick_update_kernel(const BrickUpdateArgs u) {
+  __shared__ double red[8];
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  double d = 0.0;
+  if (a < u.n_act) {
+    double th;
+    if (u.mode == 0) {
+      double m[5] = {0, 0, 0, 0, 0};
+      for (int g = 0; g < u.n_cg; ++g) {
+        const int c = u.cgs[g].cls;
+        const double *p = u.part + u.cgs[g].part_base + u.a2pos[(size_t)c * u.n_act + a];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) m[k] += p[(size_t)k * u.npos[c]];
+      }
+      th = m[0] / u.beta;               // Eq. 5
+      u.theta_SI[a] = th;
+      u.theta_en[a] = m[1] / u.Csum;    // R13
+      u.q[3 * (size_t)a] = m[2];        // Eq. 7
+      u.q[3 * (size_t)a + 1] = m[3];
+      u.q[3 * (size_t)a + 2] = m[4];
+      u.theta_prev[a] = u.theta[a];
+    } else {
+      th = u.theta_SI[a] + u.x[a];      // R14a
+    }
+    u.theta[a] = th;                    // Eq. 6
+    d = fabs(th - u.theta_prev[a]);
+    for (int c = 0; c < u.n_cls; ++c) u.th[c][u.a2pos[(size_t)c * u.n_act + a]] = th;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) d = nanmax_d(d, __shfl_xor_sync(0xffffffffu, d, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = d;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    d = threadIdx.x < (blockDim.x >> 5) ? red[threadIdx.x] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) d = nanmax_d(d, __shfl_xor_sync(0xffffffffu, d, o));
+    if (threadIdx.x == 0) atomicMax(u.maxdT, (unsigned long long)__double_as_longlong(d));
+  }
+}
+
+__global__ void brick_set_theta_kernel(int n_act, int n_cls, const int32_t *act2cell, const double *T, double T_ref,
+                                       double *theta, const int32_t *a2pos, BrickUpdateArgs u) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= n_act) return;
+  const double th = T[act2cell[a]] - T_ref;
+  theta[a] = th;
+  for (int c = 0; c < n_cls; ++c) u.th[c][a2pos[(size_t)c * n_act + a]] = th;
+}
+
+struct BrickGetEArgs {
+  int32_t n_cells, n_act, B, b0, nb, d0, nd;
+  const int32_t *cell2act, *a2pos, *dir_cls, *dir_local, *cg_of;
+  const BrickCG *cgs;
+  const double *e, *C;
+  double off_scale;
+  double *dst;
+};
+
+__global__ void brick_get_e_kernel(const BrickGetEArgs g) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= g.n_cells) return;
+  const int bi = blockIdx.y / g.nd, di = blockIdx.y % g.nd;
+  const int b = g.b0 + bi, d = g.d0 + di;
+  const int a = g.cell2act[c];
+  double val = 0.0;
+  if (a >= 0) {
+    const int cls = g.dir_cls[d];
+    const BrickCG G = g.cgs[g.cg_of[cls * g.B + b]];
+    const int64_t pos = g.a2pos[(size_t)cls * g.n_act + a];
+    val = g.e[G.e_base + pos * G.S + (b - G.b0) * G.nd + g.dir_local[d]] + g.C[b] * g.off_scale;
+  }
+  g.dst[((size_t)bi * g.nd + di) * g.n_cells + c] = val;
+}
+
+BrickClosureArgs closure_args(nanobte_solver *h) {
+  const BrickState &bs = *h->brick;
+  BrickClosureArgs R{};
+  R.a = h->bd; R.W = h->W; R.cgs = bs.a.cgs; R.cg_of = bs.cg_of; R.dir_local = bs.dir_local; R.dir_cls = h->dir_cls;
+  R.cls_dirs = h->cls_dirs; R.max_dirs = h->max_cls_dirs; R.wall = bs.a.wall; R.inf = bs.a.inf; R.partial = h->g_partial;
+  R.bf_wrow = bs.bf_wrow;
+  for (int c = 0; c < NB_MAX_CLASSES; ++c) {
+    R.out_bf[c] = bs.out_bf[c]; R.out_row[c] = bs.out_row[c]; R.out_ord[c] = bs.out_ord[c]; R.n_out[c] = bs.n_out[c];
+    R.in_row[c] = bs.in_row[c]; R.in_bf[c] = bs.in_bf[c]; R.n_in[c] = bs.n_in[c];
+  }
+  return R;
+}
+
+int launch_gsum(nanobte_solver *h, const int32_t *faces, int n_faces, int therm) {
+  if (n_faces == 0) return 0;
+  BrickClosureArgs R = closure_args(h);
+  R.therm = therm;
+  int64_t nmax = 0;
+  for (int c = 0; c < h->n_cls; ++c) nmax = std::max<int64_t>(nmax, (int64_t)R.n_out[c] * h->B);
+  if (nmax > 0) {
+    dim3 grid((unsigned)((nmax + 127) / 128), h->n_cls);
+    brick_gsum_kernel<<<grid, 128, 0, h->stream>>>(R);
+    h->launches++;
+    NB_CUDA(h, cudaGetLastError());
+  }
+  return nb_launch_gcomb(h, faces, n_faces, h->brick->bf_nord);
+}
+
+int launch_inflow(nanobte_solver *h, int init) {
+  BrickClosureArgs R = closure_args(h);
+  R.init = init;
+  int nmax = 0;
+  for (int c = 0; c < h->n_cls; ++c) nmax = std::max(nmax, R.n_in[c]);
+  if (nmax == 0) return 0;
+  dim3 grid(nmax, h->brick->n_cg);
+  brick_inflow_kernel<<<grid, kBrickMaxS, 0, h->stream>>>(R);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+BrickUpdateArgs update_args(nanobte_solver *h, int mode) {
+  const BrickState &bs = *h->brick;
+  BrickUpdateArgs u{};
+  u.n_act = h->n_act; u.n_cls = h->n_cls; u.n_cg = bs.n_cg; u.mode = mode; u.cgs = bs.a.cgs; u.part = bs.a.part;
+  for (int c = 0; c < NB_MAX_CLASSES; ++c) { u.npos[c] = bs.a.npos[c]; u.th[c] = bs.th[c]; }
+  u.a2pos = bs.a2pos;
+  u.theta = h->theta; u.theta_prev = h->theta_prev; u.theta_SI = h->theta_SI; u.theta_en = h->theta_en; u.q = h->q;
+  u.x = h->cg_x; u.beta = h->beta; u.Csum = h->Csum; u.maxdT = h->d_maxdT;
+  return u;
+}
+
+}  // namespace
+
+int nb_brick_closures(nanobte_solver *h, int init) {
+  if (h->n_bf == 0) return 0;
+  h->therm_stale = true;
+  if (init) return launch_inflow(h, 1);
+  if (h->n_refl == 0) return 0;
+  int rc = launch_gsum(h, h->refl_faces, h->n_refl, 0);
+  if (rc < 0) return rc;
+  return launch_inflow(h, 0);
+}
+
+int nb_brick_refresh_thermalizing(nanobte_solver *h) {
+  if (!h->therm_stale) return 0;
+  int rc = launch_gsum(h, h->therm_faces, h->n_therm, 1);
+  if (rc < 0) return rc;
+  h->therm_stale = false;
+  return 0;
+}
+
+int nb_brick_update(nanobte_solver *h, int mode) {
+  BrickUpdateArgs u = update_args(h, mode);
+  brick_update_kernel<<<(h->n_act + 255) / 256, 256, 0, h->stream>>>(u);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+int nb_brick_set_theta(nanobte_solver *h, const double *T_cells_dev) {
+  BrickUpdateArgs u = update_args(h, 0);
+  brick_set_theta_kernel<<<(h->n_act + 255) / 256, 256, 0, h->stream>>>(h->n_act, h->n_cls, h->act2cell, T_cells_dev, h->T_ref,
+                                                                         h->theta, h->brick->a2pos, u);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+int nb_brick_get_e(nanobte_solver *h, int b0, int nb, int d0, int nd, double *dst_dev, int deviational) {
+  if (nb == 0 || nd == 0) return 0;
+  const BrickState &bs = *h->brick;
+  BrickGetEArgs g{};
+  g.n_cells = h->n_cells; g.n_act = h->n_act; g.B = h->B; g.b0 = b0; g.nb = nb; g.d0 = d0; g.nd = nd;
+  g.cell2act = h->cell2act; g.a2pos = bs.a2pos; g.dir_cls = h->dir_cls; g.dir_local = bs.dir_local; g.cg_of = bs.cg_of;
+  g.cgs = bs.a.cgs; g.e = bs.a.e; g.C = h->bd.C; g.off_scale = deviational ? 0.0 : h->T_ref / h->W; g.dst = dst_dev;
+  dim3 grid((h->n_cells + 255) / 256, nb * nd);
+  brick_get_e_kernel<<<grid, 256, 0, h->stream>>>(g);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}
+
+void nb_free_brick(nanobte_solver *h) {
+  delete h->brick;
+  h->brick = nullptr;
+}

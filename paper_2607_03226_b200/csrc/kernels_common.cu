@@ -5,7 +5,7 @@
 
 #include <algorithm>
 
-#include "internal.h"
+#include "brick.h"
 namespace cg = cooperative_groups;
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -88,6 +88,7 @@ static int launch_closure_inflow(nanobte_solver *h, int init);
 
 int nb_launch_boundary(nanobte_solver *h, int init) {
   if (h->n_bf == 0) return 0;
+  if (h->brick) return nb_brick_closures(h, init);
   if (h->split_closures) {
     h->therm_stale = true;
     if (init) return launch_closure_inflow(h, 1);
@@ -262,8 +263,14 @@ static int launch_closure_G(nanobte_solver *h, const int32_t *faces, int n_faces
   closure_gsum_kernel<<<grid, 128, 0, h->stream>>>(S);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
+  return nb_launch_gcomb(h, faces, n_faces, h->bf_nord);
+}
+
+// G_bf and the face flux of the listed faces from the per-class shares in g_partial (nord[f] shares of face f).
+int nb_launch_gcomb(nanobte_solver *h, const int32_t *faces, int n_faces, const uint8_t *nord) {
+  if (n_faces == 0) return 0;
   GcombArgs R;
-  R.a = h->bd; R.W = h->W; R.faces = faces; R.nord = h->bf_nord; R.partial = h->g_partial; R.n_faces = n_faces;
+  R.a = h->bd; R.W = h->W; R.faces = faces; R.nord = nord; R.partial = h->g_partial; R.n_faces = n_faces;
   const int64_t n = (int64_t)n_faces * h->B;
   closure_gcomb_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(R);
   h->launches++;
@@ -291,6 +298,7 @@ static int launch_closure_inflow(nanobte_solver *h, int init) {
 
 // Diagnostics of the thermalizing faces (G, face flux) from the current eps; called by the getters that expose them.
 int nb_refresh_thermalizing(nanobte_solver *h) {
+  if (h->brick) return nb_brick_refresh_thermalizing(h);
   if (!h->split_closures || !h->therm_stale) return 0;
   int rc = launch_closure_G(h, h->therm_faces, h->n_therm, 1);
   if (rc < 0) return rc;
@@ -357,6 +365,7 @@ __global__ void __launch_bounds__(256) moments_structured_kernel(MomentsArgs a) 
 int nb_launch_moments_unstructured(nanobte_solver *h);
 
 int nb_launch_moments(nanobte_solver *h) {
+  if (h->brick) return 0;  // the partial moments came out of the sweep itself
   if (h->kind == 1) return nb_launch_moments_unstructured(h);
   MomentsArgs a;
   a.e = h->sw.e;
@@ -441,6 +450,7 @@ int nb_launch_update_unstructured(nanobte_solver *h, int mode);
 int nb_launch_update(nanobte_solver *h, int mode) {
   NB_CUDA(h, cudaMemsetAsync(h->d_maxdT, 0, sizeof(unsigned long long), h->stream));
   if (h->kind == 1) return nb_launch_update_unstructured(h, mode);
+  if (h->brick) return nb_brick_update(h, mode);
   UpdateArgs u;
   u.n_act = h->n_act; u.n_cls = h->n_cls; u.mode = mode; u.dim = h->dim;
   u.part = h->part; u.e_stride = h->e_stride; u.a2pos = h->a2pos;
@@ -464,6 +474,7 @@ __global__ void set_theta_kernel(int n_act, int n_cls, const int32_t *act2cell, 
 }
 
 int nb_launch_set_theta(nanobte_solver *h, const double *T_cells_dev) {
+  if (h->brick) return nb_brick_set_theta(h, T_cells_dev);
   UpdateArgs u{};
   for (int c = 0; c < NB_MAX_CLASSES; ++c) u.tq[c] = h->tq[c];
   const int ncls = h->kind == 0 ? h->n_cls : 0;
@@ -518,6 +529,7 @@ __global__ void get_e_kernel(GetEArgs g) {
 
 int nb_launch_get_e(nanobte_solver *h, int b0, int nb, int d0, int nd, double *dst_dev, int deviational) {
   if (nb == 0 || nd == 0) return 0;
+  if (h->brick) return nb_brick_get_e(h, b0, nb, d0, nd, dst_dev, deviational);
   GetEArgs g;
   g.n_cells = h->n_cells; g.n_act = h->n_act; g.B = h->B; g.b0 = b0; g.nb = nb; g.d0 = d0; g.nd = nd;
   g.unstructured = h->kind;

@@ -1,0 +1,319 @@
+// setup_brick.cu -- (a1) one-time setup of the tile-dataflow sweep (brick.h): tiles that follow the mask, segments,
+// tasks in topological order with their up/downstream links, per-class cell tables and flags, the inflow / wall row
+// spaces, the closure tables in those row spaces, and the per-(class, group) coefficient blocks.
+#include <algorithm>
+#include <numeric>
+
+#include "brick_host.h"
+
+namespace {
+
+// Cuts of one cross-section axis: at every change of the axis' activity signature (so that walls of box-shaped masks
+// fall on tile edges and the tiles have no walls inside), then every interval longer than 8 in near-equal pieces.
+// A mask whose signature changes almost everywhere would shred the axis: then plain 8-wide tiles (walls inside the
+// tiles go through the IRR stream).
+std::vector<int> axis_cuts(int n, const std::vector<std::vector<uint8_t>> &sig) {
+  std::vector<int> marks{0};
+  for (int x = 1; x < n; ++x)
+    if (sig[x] != sig[x - 1]) marks.push_back(x);
+  marks.push_back(n);
+  if ((int)marks.size() - 1 > 2 * ((n + kBrickTile - 1) / kBrickTile) + 2) marks = {0, n};
+  std::vector<int> cuts{0};
+  for (size_t k = 0; k + 1 < marks.size(); ++k) {
+    const int len = marks[k + 1] - marks[k], pieces = (len + kBrickTile - 1) / kBrickTile;
+    for (int p = 1; p <= pieces; ++p) cuts.push_back(marks[k] + (int)((int64_t)len * p / pieces));
+  }
+  return cuts;
+}
+
+}  // namespace
+
+int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
+  const int nu = x.n[x.pa], nv = x.n[x.va], nw = x.n[x.wa];
+  const int B = x.cm->B, D = x.cm->D, ncls = x.ncls, nbf = (int)x.G->bf_act.size(), na = (int)x.G->act2cell.size();
+  auto cell_phys = [&](int u, int v, int w) { int c[3]; c[x.pa] = u; c[x.va] = v; c[x.wa] = w; return c[0] + x.n[0] * (c[1] + x.n[1] * c[2]); };
+  auto active = [&](int u, int v, int w) { return u >= 0 && u < nu && v >= 0 && v < nv && w >= 0 && w < nw && x.act[cell_phys(u, v, w)]; };
+
+  // ---- tiles and segments (physical coordinates; the same lattice for every class) --------------------------------------------
+  std::vector<std::vector<uint8_t>> sigv(nv, std::vector<uint8_t>(nw, 0)), sigw(nw, std::vector<uint8_t>(nv, 0));
+  for (int w = 0; w < nw; ++w)
+    for (int v = 0; v < nv; ++v) {
+      uint8_t any = 0;
+      for (int u = 0; u < nu && !any; ++u) any = x.act[cell_phys(u, v, w)];
+      sigv[v][w] = any;
+      sigw[w][v] = any;
+    }
+  const std::vector<int> vcut = axis_cuts(nv, sigv), wcut = axis_cuts(nw, sigw);
+  const int NTv = (int)vcut.size() - 1, NTw = (int)wcut.size() - 1;
+  const int nseg = std::max(1, (nu + 16) / 32);
+  std::vector<int> ucut(nseg + 1);
+  for (int k = 0; k <= nseg; ++k) ucut[k] = (int)((int64_t)nu * k / nseg);
+  // which (tile, segment) boxes hold an active cell
+  std::vector<uint8_t> box_on((size_t)NTv * NTw * nseg, 0);
+  auto box = [&](int J, int K, int sg) { return ((size_t)sg * NTw + K) * NTv + J; };
+  for (int sg = 0; sg < nseg; ++sg)
+    for (int K = 0; K < NTw; ++K)
+      for (int J = 0; J < NTv; ++J) {
+        uint8_t any = 0;
+        for (int u = ucut[sg]; u < ucut[sg + 1] && !any; ++u)
+          for (int w = wcut[K]; w < wcut[K + 1] && !any; ++w)
+            for (int v = vcut[J]; v < vcut[J + 1] && !any; ++v) any = x.act[cell_phys(u, v, w)];
+        box_on[box(J, K, sg)] = any;
+      }
+
+  // ---- band groups per class ------------------------------------------------------------------------------------------------------
+  bh.ncls = ncls;
+  bh.cg_of.assign((size_t)ncls * B, -1);
+  bh.dir_local.assign(D, 0);
+  std::vector<int> cls_cg0(ncls), cls_ng(ncls);
+  for (int c = 0; c < ncls; ++c) {
+    const int nd = (int)x.dirs[c].size();
+    if (nd > kBrickMaxS || nd > 32) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "brick sweep: %d directions in one octant (at most 32)", nd);
+    for (int k = 0; k < nd; ++k) bh.dir_local[x.dirs[c][k]] = k;
+    const int ng = (B * nd + kBrickMaxS - 1) / kBrickMaxS;
+    int per = (B + ng - 1) / ng;
+    while (per * nd > kBrickMaxS) --per;
+    if (per > 64) per = 64;
+    cls_cg0[c] = (int)bh.cgs.size();
+    int ngc = 0;
+    for (int b0 = 0; b0 < B; b0 += per, ++ngc) {
+      BrickCG g{};
+      g.cls = c; g.nd = nd; g.b0 = b0; g.nb = std::min(per, B - b0); g.S = g.nb * nd;
+      for (int b = b0; b < b0 + g.nb; ++b) bh.cg_of[(size_t)c * B + b] = (int)bh.cgs.size();
+      bh.cgs.push_back(g);
+    }
+    cls_ng[c] = ngc;
+  }
+
+  // ---- per class: positions, flags, rows, closure tables; tasks --------------------------------------------------------------------
+  bh.cls.resize(ncls);
+  bh.bf_wrow.assign((size_t)ncls * nbf, -1);
+  bh.a2pos.assign((size_t)ncls * na, -1);
+  std::vector<uint8_t> bf_nord(nbf, 0);
+  struct ProtoTask { BrickTask t; int key, cls, J, K, sg; };
+  std::vector<ProtoTask> protos;
+  for (int c = 0; c < ncls; ++c) {
+    BrickHost::Cls &C = bh.cls[c];
+    const int *sg3 = x.sign[c];
+    auto ph = [&](int axis, int n, int xp) { return sg3[axis] > 0 ? xp : n - 1 - xp; };  // primed -> physical
+    // primed tile / segment intervals
+    auto primed_cuts = [&](const std::vector<int> &cut, int n, int axis) {
+      std::vector<int> out(cut.size());
+      for (size_t k = 0; k < cut.size(); ++k) out[k] = sg3[axis] > 0 ? cut[k] : n - cut[cut.size() - 1 - k];
+      return out;
+    };
+    const std::vector<int> vc = primed_cuts(vcut, nv, x.va), wc = primed_cuts(wcut, nw, x.wa), uc = primed_cuts(ucut, nu, x.pa);
+    auto phys_box = [&](int Jp, int Kp, int sp) {
+      return box(sg3[x.va] > 0 ? Jp : NTv - 1 - Jp, sg3[x.wa] > 0 ? Kp : NTw - 1 - Kp, sg3[x.pa] > 0 ? sp : nseg - 1 - sp);
+    };
+    auto actp = [&](int up, int vp, int wp) {  // activity in primed coordinates (outside = inactive)
+      if (up < 0 || up >= nu || vp < 0 || vp >= nv || wp < 0 || wp >= nw) return false;
+      return x.act[cell_phys(ph(x.pa, nu, up), ph(x.va, nv, vp), ph(x.wa, nw, wp))] != 0;
+    };
+    const int side_in[3] = {2 * x.pa + (sg3[x.pa] > 0 ? 0 : 1), 2 * x.va + (sg3[x.va] > 0 ? 0 : 1), 2 * x.wa + (sg3[x.wa] > 0 ? 0 : 1)};
+    const int side_out[3] = {side_in[0] ^ 1, side_in[1] ^ 1, side_in[2] ^ 1};
+    // first pass: which boxes are tasks, their local index
+    std::vector<int> task_of((size_t)NTv * NTw * nseg, -1);
+    auto pbox = [&](int Jp, int Kp, int sp) { return ((size_t)sp * NTw + Kp) * NTv + Jp; };
+    int npos = 0, nrow = 0, nwall = 0;
+    const int first_proto = (int)protos.size();
+    for (int sp = 0; sp < nseg; ++sp)
+      for (int Kp = 0; Kp < NTw; ++Kp)
+        for (int Jp = 0; Jp < NTv; ++Jp) {
+          if (!box_on[phys_box(Jp, Kp, sp)]) continue;
+          ProtoTask P{};
+          P.cls = c; P.J = Jp; P.K = Kp; P.sg = sp; P.key = Jp + Kp + sp;
+          BrickTask &T = P.t;
+          T.nu = uc[sp + 1] - uc[sp]; T.tv = vc[Jp + 1] - vc[Jp]; T.tw = wc[Kp + 1] - wc[Kp];
+          T.pos0 = npos; npos += T.nu * kBrickCells;
+          T.fu0 = nrow; nrow += kBrickCells;
+          T.fv0 = nrow; nrow += T.nu * kBrickTile;
+          T.fw0 = nrow; nrow += T.nu * kBrickTile;
+          T.ir0 = nrow;  // IRR rows counted below
+          T.wo0 = nwall;
+          // cells in sweep order
+          C.th.resize((size_t)npos, 0.0);
+          C.qd.resize((size_t)npos, 0.0);
+          C.flg.resize((size_t)npos, 0);
+          for (int ul = 0; ul < T.nu; ++ul)
+            for (int wl = 0; wl < T.tw; ++wl)
+              for (int vl = 0; vl < T.tv; ++vl) {
+                const int up = uc[sp] + ul, vp = vc[Jp] + vl, wp = wc[Kp] + wl;
+                if (!actp(up, vp, wp)) continue;
+                const int cphys = cell_phys(ph(x.pa, nu, up), ph(x.va, nv, vp), ph(x.wa, nw, wp));
+                const int pos = T.pos0 + ul * kBrickCells + wl * kBrickTile + vl;
+                bh.a2pos[(size_t)c * na + x.G->cell2act[cphys]] = pos;
+                uint8_t f = BRK_ACT;
+                const bool upact[3] = {actp(up - 1, vp, wp), actp(up, vp - 1, wp), actp(up, vp, wp - 1)};
+                const int loc[3] = {ul, vl, wl};
+                const uint8_t inj[3] = {BRK_INJ_U, BRK_INJ_V, BRK_INJ_W};
+                for (int k = 0; k < 3; ++k) {
+                  if (upact[k] && loc[k] > 0) continue;  // interior neighbour inside the task: plane buffer / registers
+                  int row;
+                  if (loc[k] == 0) row = k == 0 ? T.fu0 + wl * kBrickTile + vl : k == 1 ? T.fv0 + ul * kBrickTile + wl : T.fw0 + ul * kBrickTile + vl;
+                  else { row = nrow++; f |= inj[k]; }
+                  if (!upact[k]) {  // a wall: the closure kernel owns this row
+                    const int bf = x.facebf[(size_t)cphys * 6 + side_in[k]];
+                    if (bf < 0) return nb_fail(h, NANOBTE_E_INVALID, "internal: brick inflow face of cell %d missing", cphys);
+                    C.in_row.push_back(row);
+                    C.in_bf.push_back(bf);
+                  }
+                }
+                bool wallout = false;
+                const bool dnact[3] = {actp(up + 1, vp, wp), actp(up, vp + 1, wp), actp(up, vp, wp + 1)};
+                for (int k = 0; k < 3; ++k)
+                  if (!dnact[k]) {
+                    const int bf = x.facebf[(size_t)cphys * 6 + side_out[k]];
+                    if (bf < 0) return nb_fail(h, NANOBTE_E_INVALID, "internal: brick outflow face of cell %d missing", cphys);
+                    wallout = true;
+                    C.out_bf.push_back(bf);
+                    C.out_row.push_back(nwall);
+                    C.out_ord.push_back(bf_nord[bf]++);
+                    bh.bf_wrow[(size_t)c * nbf + bf] = nwall;
+                  }
+                if (wallout) { f |= BRK_WALL; ++nwall; }
+                const double q = x.Qdot ? x.Qdot[cphys] : 0.0;
+                if (q != 0.0) f |= BRK_SRC;
+                C.flg[pos] = f;
+                C.th[pos] = x.T_init ? x.T_init[cphys] - x.T_ref : 0.0;
+                C.qd[pos] = q;
+              }
+          task_of[pbox(Jp, Kp, sp)] = (int)protos.size();
+          protos.push_back(P);
+        }
+    // links (indices into protos for now)
+    for (int k = first_proto; k < (int)protos.size(); ++k) {
+      ProtoTask &P = protos[k];
+      auto at = [&](int Jp, int Kp, int sp) {
+        if (Jp < 0 || Jp >= NTv || Kp < 0 || Kp >= NTw || sp < 0 || sp >= nseg) return -1;
+        return task_of[pbox(Jp, Kp, sp)];
+      };
+      P.t.up_u = at(P.J, P.K, P.sg - 1);
+      P.t.up_v = at(P.J - 1, P.K, P.sg);
+      P.t.up_w = at(P.J, P.K - 1, P.sg);
+      const int du = at(P.J, P.K, P.sg + 1), dv = at(P.J + 1, P.K, P.sg), dw = at(P.J, P.K + 1, P.sg);
+      P.t.dn_fu0 = du >= 0 ? protos[du].t.fu0 : -1;
+      P.t.dn_fv0 = dv >= 0 ? protos[dv].t.fv0 : -1;
+      P.t.dn_fw0 = dw >= 0 ? protos[dw].t.fw0 : -1;
+    }
+    C.npos = npos; C.nrow = nrow; C.nwall = std::max(1, nwall);
+    C.th.resize((size_t)npos + 64, 0.0);
+    C.qd.resize((size_t)npos + 64, 0.0);
+    C.flg.resize((size_t)npos + 64, 0);
+  }
+  bh.bf_nord = bf_nord;
+
+  // ---- tasks: one per (proto, group), topological launch order ----------------------------------------------------------------------
+  // key = primed tile/segment diagonal: every upstream task has a smaller key.  Within a key the classes and groups
+  // are interleaved so that all octants advance together.
+  std::vector<int> order(protos.size());
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int p, int q) { return protos[p].key < protos[q].key; });
+  std::vector<int> first_task(protos.size(), -1);
+  int ng_max = 0;
+  for (int c = 0; c < ncls; ++c) ng_max = std::max(ng_max, cls_ng[c]);
+  // tasks of one proto are consecutive per group ROUND: (key, group, proto) order keeps the groups of a class abreast
+  std::vector<std::vector<int>> task_id(ng_max, std::vector<int>(protos.size(), -1));
+  {
+    size_t lo = 0;
+    while (lo < order.size()) {
+      size_t hi = lo;
+      while (hi < order.size() && protos[order[hi]].key == protos[order[lo]].key) ++hi;
+      for (int g = 0; g < ng_max; ++g)
+        for (size_t k = lo; k < hi; ++k) {
+          const ProtoTask &P = protos[order[k]];
+          if (g >= cls_ng[P.cls]) continue;
+          BrickTask T = P.t;
+          T.cg = cls_cg0[P.cls] + g;
+          task_id[g][order[k]] = (int)bh.tasks.size();
+          bh.tasks.push_back(T);
+        }
+      lo = hi;
+    }
+  }
+  for (BrickTask &T : bh.tasks) {  // proto indices -> task ids of the same group
+    const int g = T.cg - cls_cg0[bh.cgs[T.cg].cls];
+    if (T.up_u >= 0) T.up_u = task_id[g][T.up_u];
+    if (T.up_v >= 0) T.up_v = task_id[g][T.up_v];
+    if (T.up_w >= 0) T.up_w = task_id[g][T.up_w];
+  }
+  for (size_t k = 0; k < bh.tasks.size(); ++k) {
+    const BrickTask &T = bh.tasks[k];
+    if (T.up_u >= (int)k || T.up_v >= (int)k || T.up_w >= (int)k) return nb_fail(h, NANOBTE_E_INVALID, "internal: brick task order is not topological");
+  }
+
+  // ---- blocks of every (class, group) and the coefficient blocks ---------------------------------------------------------------------
+  int64_t inf = 0, wall = 0, part = 0, e = 0, cf = 0;
+  for (BrickCG &g : bh.cgs) {
+    const BrickHost::Cls &C = bh.cls[g.cls];
+    auto pad = [](int64_t v) { return (v + 31) / 32 * 32; };
+    g.inf_base = inf; inf = pad(inf + (int64_t)C.nrow * g.S);
+    g.wall_base = wall; wall = pad(wall + (int64_t)C.nwall * g.S);
+    g.part_base = part; part = pad(part + (int64_t)5 * C.npos);
+    g.e_base = e; e = pad(e + (int64_t)C.npos * g.S);
+    g.coef_base = cf;
+    for (int bl = 0; bl < g.nb; ++bl)
+      for (int dl = 0; dl < g.nd; ++dl) {
+        const size_t row = (size_t)x.cls_row0[g.cls] + (size_t)dl * B + (g.b0 + bl);
+        for (int k = 0; k < 5; ++k) bh.coef.push_back(x.coef[row * 8 + k]);
+      }
+    // the loop above is band-major: system = band_local * nd + dir_local
+    for (int dl = 0; dl < g.nd; ++dl) {
+      const int d = x.dirs[g.cls][dl];
+      bh.coef.push_back(x.cm->w[d]);
+      for (int k = 0; k < 3; ++k) bh.coef.push_back(x.cm->w[d] * x.cm->s[3 * (size_t)d + k]);
+    }
+    for (int bl = 0; bl < g.nb; ++bl) {
+      bh.coef.push_back(1.0 / x.cm->tau[g.b0 + bl]);
+      bh.coef.push_back(x.cm->v[g.b0 + bl]);
+    }
+    while (bh.coef.size() & 3) bh.coef.push_back(0.0);
+    cf = (int64_t)bh.coef.size();
+  }
+  bh.inf_total = inf; bh.wall_total = wall; bh.part_total = part; bh.e_total = e;
+  return 0;
+}
+
+int nb_brick_upload(nanobte_solver *h, Arena &A, BrickHost &bh) {
+  if (!h->brick) h->brick = new BrickState();
+  BrickState &bs = *h->brick;
+  BrickArgs &a = bs.a;
+  a.tasks = A.put(bh.tasks);
+  a.cgs = A.put(bh.cgs);
+  a.n_tasks = (int)bh.tasks.size();
+  for (int c = 0; c < bh.ncls; ++c) {
+    BrickHost::Cls &C = bh.cls[c];
+    bs.th[c] = A.put(C.th);
+    a.th[c] = bs.th[c];
+    a.qd[c] = A.put(C.qd);
+    a.flg[c] = A.put(C.flg);
+    a.npos[c] = C.npos;
+    bs.in_row[c] = A.put(C.in_row);
+    bs.in_bf[c] = A.put(C.in_bf);
+    bs.n_in[c] = (int32_t)C.in_row.size();
+    bs.out_bf[c] = A.put(C.out_bf);
+    bs.out_row[c] = A.put(C.out_row);
+    bs.out_ord[c] = A.put(C.out_ord);
+    bs.n_out[c] = (int32_t)C.out_bf.size();
+  }
+  a.inf = A.zeros<double>((size_t)bh.inf_total);
+  a.wall = A.zeros<double>((size_t)bh.wall_total);
+  a.part = A.zeros<double>((size_t)bh.part_total);
+  a.e = A.zeros<double>((size_t)bh.e_total);
+  a.coef = A.put(bh.coef);
+  unsigned int *sync = A.zeros<unsigned int>((size_t)a.n_tasks + 1);
+  a.ticket = sync;
+  a.prog = sync + 1;
+  bs.bf_wrow = A.put(bh.bf_wrow);
+  bs.dir_local = A.put(bh.dir_local);
+  bs.cg_of = A.put(bh.cg_of);
+  bs.a2pos = A.put(bh.a2pos);
+  bs.bf_nord = A.put(bh.bf_nord);
+  bs.n_cg = (int)bh.cgs.size();
+  bs.smem = nb_brick_smem_bytes();
+  bs.grid = std::max(1, std::min(a.n_tasks, 3 * h->n_sm));
+  bs.inf_total = bh.inf_total; bs.wall_total = bh.wall_total; bs.part_total = bh.part_total; bs.e_total = bh.e_total;
+  bs.s_max = 0;
+  for (const BrickCG &g : bh.cgs) bs.s_max = std::max(bs.s_max, g.S);
+  return A.rc;
+}

@@ -4,6 +4,9 @@
 #include <algorithm>
 #include <numeric>
 
+#include <cstdlib>
+
+#include "brick_host.h"
 #include "host_util.h"
 
 namespace {
@@ -162,6 +165,14 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   bool uniform = true;
   for (int a = 0; a < dim; ++a)
     for (double v : g.hsz[a]) uniform &= (v == g.hsz[a][0]);
+
+  // ---- which sweep: the tile-dataflow sweep with fused moments (brick.h) on uniform 3-D grids unless the caller asks for a
+  // launch shape of the hyperplane kernels (sweep_G / sweep_threads / sweep_variant 3, 4) -------------------------------------
+  const bool brick_ok = dim == 3 && uniform;
+  if (opt->sweep_variant == 5 && !brick_ok)
+    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "the tile-dataflow sweep (sweep_variant 5) needs a 3-D grid with uniform spacing");
+  const bool use_brick = brick_ok && (opt->sweep_variant == 5 || (opt->sweep_variant == 0 && opt->sweep_G == 0 && opt->sweep_threads == 0 &&
+                                                                  std::getenv("NANOBTE_NO_BRICK") == nullptr));
 
   // ---- pencils (physical coordinates): which exist, which touch a +-v / +-w boundary face ---------------------------------------
   std::vector<uint8_t> pen_any((size_t)nv * nw, 0), pen_wall((size_t)nv * nw, 0);
@@ -454,9 +465,25 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   int nsys_min = 1 << 30;
   for (auto &o : oct) nsys_min = std::min<int>(nsys_min, (int)o.dirs.size() * B);
   h->uniform = uniform;
-  rc = nb_sweep_structured_config(h, n_pen_max, p_max, g_max, q_max, H, opt->sweep_G, opt->sweep_threads, nsys_min, opt->sweep_variant, B * D);
-  if (rc) return rc;
-  const int per_task = h->sweep_G;
+  BrickHost bh;
+  if (use_brick) {
+    BrickCtx bx;
+    for (int a = 0; a < 3; ++a) bx.n[a] = g.n[a];
+    bx.act = g.act.data(); bx.pa = pa; bx.va = va; bx.wa = wa; bx.ncls = ncls;
+    for (int ci = 0; ci < ncls; ++ci) {
+      for (int a = 0; a < 3; ++a) bx.sign[ci][a] = oct[ci].sign[a];
+      bx.dirs.push_back(oct[ci].dirs);
+    }
+    bx.facebf = facebf.data(); bx.cm = &cm; bx.G = &G; bx.coef = coef.data(); bx.cls_row0 = cls_row0.data();
+    bx.Qdot = Qdot; bx.T_init = opt->T_init; bx.T_ref = opt->T_ref;
+    rc = nb_brick_build(h, bx, bh);
+    if (rc) return rc;
+    h->sweep_variant = 5; h->sweep_G = 0; h->sweep_threads = kBrickMaxS; h->sweep_rmax = 0; h->sweep_smem = nb_brick_smem_bytes();
+  } else {
+    rc = nb_sweep_structured_config(h, n_pen_max, p_max, g_max, q_max, H, opt->sweep_G, opt->sweep_threads, nsys_min, opt->sweep_variant, B * D);
+    if (rc) return rc;
+  }
+  const int per_task = std::max(1, h->sweep_G);
   std::vector<int32_t> task_oct, task_row;
   for (int ci = 0; ci < ncls; ++ci) {
     h->cls_row0[ci] = cls_row0[ci];
@@ -467,7 +494,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
       task_row.push_back(r0);
     }
   }
-  h->n_tasks = (int)task_oct.size();
+  h->n_tasks = use_brick ? (int)bh.tasks.size() : (int)task_oct.size();
   h->n_cls = ncls; h->bd.n_cls = ncls;
   h->n_cells = nc; h->kind = 0; h->pencil_axis = pa; h->n_planes = H;
   h->uniform = uniform;
@@ -525,9 +552,14 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     h->sw.coef = A.put(coef);
     h->a2pos = A.put(a2pos);
     h->dir_cls = A.put(dir_cls);
-    const size_t part_n = std::max<size_t>((size_t)ncls * 5 * e_stride, (size_t)3 * nc + 64);
+    // the tile-dataflow sweep has its own partials and (on request) eps blocks; part[] stays as the getters' scratch
+    const size_t part_n = std::max<size_t>(use_brick ? 0 : (size_t)ncls * 5 * e_stride, (size_t)3 * nc + 64);
     h->part = A.zeros<double>(part_n);
-    double *e = A.zeros<double>((size_t)D * B * e_stride);
+    double *e = use_brick ? nullptr : A.zeros<double>((size_t)D * B * e_stride);
+    if (use_brick) {
+      rc = nb_brick_upload(h, A, bh);
+      if (rc) return nb_fail(h, rc, "device upload failed");
+    }
     h->sw.e = e; h->bd.e = e; h->bd.e_stride = e_stride;
     h->sw.bin = h->bd.bin;
     h->sw.e_stride = e_stride; h->sw.nu = nu;
