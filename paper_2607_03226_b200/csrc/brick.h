@@ -46,8 +46,11 @@ struct BrickTask {
   int32_t wo0;                 // first wall row of this task
   int32_t up_u, up_v, up_w;    // tasks whose outflow this task consumes (-1: none -- the rows are boundary values)
   int32_t dn_fu0, dn_fv0, dn_fw0;  // inflow rows of the downstream tasks this task feeds (-1: none)
-  int32_t pad;
+  int32_t plain;               // 1: every cell of the tv x tw x nu box is active (no wall inside the box): straight-line path
+  uint32_t src_lo, src_hi;     // bit u: plane u of the task holds a cell with Qdot != 0 (nu <= 64)
+  int32_t wall_any;            // the task has cells with an outgoing boundary face
 };
+static_assert(sizeof(BrickTask) == 80, "BrickTask layout");
 
 struct BrickCG {
   int32_t cls, S, nb, nd;      // class, systems (= nb * nd), bands, directions of the class; system = band_local * nd + dir_local

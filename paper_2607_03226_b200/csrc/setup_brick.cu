@@ -122,7 +122,9 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
         for (int Jp = 0; Jp < NTv; ++Jp) {
           if (!box_on[phys_box(Jp, Kp, sp)]) continue;
           ProtoTask P{};
-          P.cls = c; P.J = Jp; P.K = Kp; P.sg = sp; P.key = Jp + Kp + sp;
+          // earliest start in plane-times: a v- or w-downstream tile runs one plane behind its upstream tile, a u-downstream
+          // segment starts when the previous segment has finished
+          P.cls = c; P.J = Jp; P.K = Kp; P.sg = sp; P.key = Jp + Kp + uc[sp];
           BrickTask &T = P.t;
           T.nu = uc[sp + 1] - uc[sp]; T.tv = vc[Jp + 1] - vc[Jp]; T.tw = wc[Kp + 1] - wc[Kp];
           T.pos0 = npos; npos += T.nu * kBrickCells;
@@ -131,6 +133,9 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
           T.fw0 = nrow; nrow += T.nu * kBrickTile;
           T.ir0 = nrow;  // IRR rows counted below
           T.wo0 = nwall;
+          if (T.nu > 64) return nb_fail(h, NANOBTE_E_INVALID, "internal: brick segment of %d planes", T.nu);
+          int n_active = 0;
+          uint64_t src_planes = 0;
           // cells in sweep order
           C.th.resize((size_t)npos, 0.0);
           C.qd.resize((size_t)npos, 0.0);
@@ -144,6 +149,7 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
                 const int pos = T.pos0 + ul * kBrickCells + wl * kBrickTile + vl;
                 bh.a2pos[(size_t)c * na + x.G->cell2act[cphys]] = pos;
                 uint8_t f = BRK_ACT;
+                ++n_active;
                 const bool upact[3] = {actp(up - 1, vp, wp), actp(up, vp - 1, wp), actp(up, vp, wp - 1)};
                 const int loc[3] = {ul, vl, wl};
                 const uint8_t inj[3] = {BRK_INJ_U, BRK_INJ_V, BRK_INJ_W};
@@ -173,11 +179,14 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
                   }
                 if (wallout) { f |= BRK_WALL; ++nwall; }
                 const double q = x.Qdot ? x.Qdot[cphys] : 0.0;
-                if (q != 0.0) f |= BRK_SRC;
+                if (q != 0.0) { f |= BRK_SRC; src_planes |= 1ull << ul; }
                 C.flg[pos] = f;
                 C.th[pos] = x.T_init ? x.T_init[cphys] - x.T_ref : 0.0;
                 C.qd[pos] = q;
               }
+          T.plain = n_active == T.nu * T.tv * T.tw;
+          T.src_lo = (uint32_t)src_planes; T.src_hi = (uint32_t)(src_planes >> 32);
+          T.wall_any = nwall > T.wo0;
           task_of[pbox(Jp, Kp, sp)] = (int)protos.size();
           protos.push_back(P);
         }

@@ -6,6 +6,17 @@
 //   1/tau_b + v_b sum_a |s_a|/h_a, as in sweep_structured.cu)
 // and per cell and u-plane the partial moments of the task's systems (Eq. 5, R13, Eq. 7):
 //   part0 = sum w/tau eps, part1 = sum w eps, part2..4 = sum v w s eps.
+//
+// One u-plane of a task in two roles:
+//   substitution  thread = system.  Tasks whose box is fully active (BrickTask::plain; with tile cuts that follow the
+//                 mask that is every task of a box-shaped geometry) run straight-line code with the tile width as a
+//                 template constant: per cell one LDS (u-upwind), one STS, 4 fp64 operations.  Other tasks run the
+//                 per-cell path that reads the flag bytes (walls inside the tile).
+//   moments       thread = two cells (lane, lane + 32) x the bands of the thread's warp; per value one LDS and four
+//                 DFMA, the direction coefficients shared by the two cells.  Warps 0..2 leave their band partials in
+//                 shared memory, warp 3 adds its own in fixed order and writes the five partial moments of the plane.
+// Shared memory is the scarce resource (128 B/clk per SM against 64 DFMA/clk): per update the substitution moves
+// 16 B + 2 B (theta broadcast) and the moments 8 B + 8 B (coefficient broadcast shared by two cells).
 #include <algorithm>
 
 #include "brick.h"
@@ -35,7 +46,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 __device__ __forceinline__ void wait_progress(const unsigned int *prog, int up, unsigned int need) {
   if (up >= 0) {
     if ((threadIdx.x & 31) == 0) {
-      while (ld_relaxed(prog + up) < need) __nanosleep(100);  // cheap polls; one acquire once the value is there
+      while (ld_relaxed(prog + up) < need) __nanosleep(40);  // cheap polls; one acquire once the value is there
       (void)ld_acquire(prog + up);
     }
     __syncwarp();
@@ -55,15 +66,68 @@ __device__ __forceinline__ bool progress_ready(const unsigned int *prog, int up,
   return ok != 0;
 }
 
+constexpr int kP = kBrickPitch;
+
 struct BrickSmem {
-  double plane[kBrickCells * kBrickPitch];  // [cell][system]: eps of the previous u-plane (u-upwind values)
-  double th[2][kBrickCells];                // theta of the plane's cells, two stages
-  double qd[2][kBrickCells];                // Qdot
-  unsigned long long flg[2][kBrickCells / 8];  // flag bytes, one 64-bit word per row of 8 cells
-  double dcoef[32 * 4];                     // [nd][4]  w, w sx, w sy, w sz
-  double bcoef[64 * 2];                     // [nb][2]  1/tau, v
+  double plane[kBrickCells * kBrickPitch];     // [cell][system]: eps of the previous u-plane (u-upwind values)
+  double red[3][5][kBrickCells];               // band partials of warps 0..2 (moments)
+  double th[kBrickCells];                      // theta of the plane's cells
+  double qd[kBrickCells];                      // Qdot
+  unsigned long long flg[2][kBrickCells / 8];  // flag bytes, one 64-bit word per row of 8 cells, two stages
+  double dcoef[16 * 4];                        // [nd][4]  w, w sx, w sy, w sz
+  double bcoef[32 * 2];                        // [nb][2]  1/tau, v
   int task;
 };
+static_assert(3 * (sizeof(BrickSmem) + 1024) <= 228 * 1024, "three CTAs per SM");
+
+struct Sys {           // what a substitution thread keeps for its system
+  double k_th, k_Q, c_u, c_v, c_w;
+};
+
+// ---- one u-plane of a fully active box, TV cells per row: straight-line code ---------------------------------------------------------
+// pl = plane buffer + system; ew[v] = w-upwind values (in: tile-face inflow, out: last row); inv[w] = v-face inflow of row w.
+template <int TV>
+__device__ __forceinline__ void plain_plane(double *__restrict__ pl, const double *__restrict__ th, const double *__restrict__ qd,
+                                            const Sys &c, const int tw, const bool src, double (&ew)[kBrickTile],
+                                            const double (&inv)[kBrickTile], double *dn_fv_u, const int64_t S, double *eout_u) {
+#pragma unroll
+  for (int w = 0; w < kBrickTile; ++w) {
+    if (w < tw) {
+      double *row = pl + w * kBrickTile * kP;
+      double r[TV], eu[TV];
+#pragma unroll
+      for (int v = 0; v < TV; ++v) eu[v] = row[v * kP];
+#pragma unroll
+      for (int v = 0; v < TV; v += 2) {
+        const double2 t2 = *reinterpret_cast<const double2 *>(th + w * kBrickTile + v);
+        r[v] = c.k_th * t2.x;
+        if (v + 1 < TV) r[v + 1] = c.k_th * t2.y;
+      }
+      if (src) {
+#pragma unroll
+        for (int v = 0; v < TV; v += 2) {
+          const double2 q2 = *reinterpret_cast<const double2 *>(qd + w * kBrickTile + v);
+          r[v] = fma(c.k_Q, q2.x, r[v]);
+          if (v + 1 < TV) r[v + 1] = fma(c.k_Q, q2.y, r[v + 1]);
+        }
+      }
+#pragma unroll
+      for (int v = 0; v < TV; ++v) r[v] = fma(c.c_u, eu[v], fma(c.c_w, ew[v], r[v]));
+      double ev = inv[w];
+#pragma unroll
+      for (int v = 0; v < TV; ++v) {
+        ev = fma(c.c_v, ev, r[v]);  // the v-chain is the only dependency between the cells of a row
+        ew[v] = ev;
+        row[v * kP] = ev;
+      }
+      if (dn_fv_u) dn_fv_u[(int64_t)w * S] = ev;
+      if (eout_u) {
+#pragma unroll
+        for (int v = 0; v < TV; ++v) __stcs(eout_u + (int64_t)(w * kBrickTile + v) * S, ew[v]);
+      }
+    }
+  }
+}
 
 __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -93,27 +157,29 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     double *dn_fu = T.dn_fu0 >= 0 ? inf + (int64_t)T.dn_fu0 * S + s : nullptr;
     double *dn_fv = T.dn_fv0 >= 0 ? inf + (int64_t)T.dn_fv0 * S + s : nullptr;
     double *dn_fw = T.dn_fw0 >= 0 ? inf + (int64_t)T.dn_fw0 * S + s : nullptr;
+    const unsigned long long src_planes = ((unsigned long long)T.src_hi << 32) | T.src_lo;
 
     // coefficients of this thread's system; moment tables of the group
     const double *cf = a.coef + G.coef_base;
-    const double k_th = cf[s * 5 + 0], k_Q = cf[s * 5 + 1], c_u = cf[s * 5 + 2], c_v = cf[s * 5 + 3], c_w = cf[s * 5 + 4];
-    for (int k = t; k < G.nd * 4; k += kBrickMaxS) sm.dcoef[k] = cf[S * 5 + k];
-    for (int k = t; k < G.nb * 2; k += kBrickMaxS) sm.bcoef[k] = cf[S * 5 + G.nd * 4 + k];
+    Sys c;
+    c.k_th = cf[s * 5 + 0]; c.k_Q = cf[s * 5 + 1]; c.c_u = cf[s * 5 + 2]; c.c_v = cf[s * 5 + 3]; c.c_w = cf[s * 5 + 4];
+    if (t < G.nd * 4) sm.dcoef[t] = cf[S * 5 + t];
+    if (t < G.nb * 2) sm.bcoef[t] = cf[S * 5 + G.nd * 4 + t];
 
     // stage the cell tables of a plane: theta 32 x 16 B, Qdot 32 x 16 B, flags 4 x 16 B
-    auto stage = [&](int un, int stg) {
+    auto stage = [&](int un) {
       const int64_t off = (int64_t)un * kBrickCells;
-      if (t < 32) cp_async16(&sm.th[stg][2 * t], th_g + off + 2 * t);
-      else if (t < 64) cp_async16(&sm.qd[stg][2 * (t - 32)], qd_g + off + 2 * (t - 32));
-      else if (t < 68) cp_async16(reinterpret_cast<unsigned char *>(sm.flg[stg]) + 16 * (t - 64), flg_g + off + 16 * (t - 64));
+      if (t < 32) cp_async16(&sm.th[2 * t], th_g + off + 2 * t);
+      else if (t < 64) cp_async16(&sm.qd[2 * (t - 32)], qd_g + off + 2 * (t - 32));
+      else if (t < 68) cp_async16(reinterpret_cast<unsigned char *>(sm.flg[un & 1]) + 16 * (t - 64), flg_g + off + 16 * (t - 64));
     };
-    stage(0, 0);
+    stage(0);
     // u-face inflow -> plane buffer (the previous segment of the pencils, or boundary values)
     wait_progress(a.prog, T.up_u, 0x7fffffffu);
     if (on) {
       const double *fu = inf + (int64_t)T.fu0 * S + s;
 #pragma unroll 8
-      for (int c = 0; c < kBrickCells; ++c) sm.plane[c * kBrickPitch + s] = __ldcg(fu + (int64_t)c * S);
+      for (int cc = 0; cc < kBrickCells; ++cc) sm.plane[cc * kP + s] = __ldcg(fu + (int64_t)cc * S);
     }
     // v- and w-face inflow of plane 0
     double ew[kBrickTile], inv[kBrickTile];
@@ -127,113 +193,80 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     cp_async_wait_all();
     __syncthreads();
 
+    // bands of this warp in the moment role
+    const int b_lo = (G.nb * wid) >> 2, b_hi = (G.nb * (wid + 1)) >> 2;
+
     int ip = 0, wp = 0;  // next row of the IRR stream / of the wall rows (same value in every thread)
     for (int u = 0; u < T.nu; ++u) {
       const int st = u & 1;
-      // stage the next plane's cell tables
-      if (u + 1 < T.nu) stage(u + 1, st ^ 1);
+      const bool last_u = u + 1 == T.nu;
       // ------------------------------------------ substitution: thread = system ------------------------------------------
       if (on) {
-        const bool last_u = u + 1 == T.nu;
-        const unsigned long long full_act = 0x0101010101010101ull >> (8 * (kBrickTile - T.tv));
         double *pl = sm.plane + s;
-        for (int w = 0; w < T.tw; ++w) {
-          const unsigned long long frow = sm.flg[st][w];
-          double ev = inv[0];
-#pragma unroll
-          for (int k = 0; k + 1 < kBrickTile; ++k) inv[k] = inv[k + 1];  // inv[0] is always the current row's v-face value
-          if (frow == 0ull) continue;
-          const int c0 = w * kBrickTile;
-          if ((frow & 0x0f0f0f0f0f0f0f0full) == full_act) {
-            // ---- plain row: all tv cells active, no wall inside the tile: straight-line code, loads first ------------------
-            double eu[kBrickTile], r[kBrickTile];
-#pragma unroll
-            for (int v = 0; v < kBrickTile; ++v) eu[v] = v < T.tv ? pl[(c0 + v) * kBrickPitch] : 0.0;
-#pragma unroll
-            for (int v = 0; v < kBrickTile; v += 2) {
-              const double2 th2 = *reinterpret_cast<const double2 *>(&sm.th[st][c0 + v]);
-              r[v] = k_th * th2.x;
-              r[v + 1] = k_th * th2.y;
-            }
-            if (frow & 0x1010101010101010ull) {  // a source cell in the row (Qdot = 0 elsewhere)
-#pragma unroll
-              for (int v = 0; v < kBrickTile; v += 2) {
-                const double2 q2 = *reinterpret_cast<const double2 *>(&sm.qd[st][c0 + v]);
-                r[v] = fma(k_Q, q2.x, r[v]);
-                r[v + 1] = fma(k_Q, q2.y, r[v + 1]);
-              }
-            }
-#pragma unroll
-            for (int v = 0; v < kBrickTile; ++v) r[v] = fma(c_u, eu[v], fma(c_w, ew[v], r[v]));
-            double elast = 0.0;
-#pragma unroll
-            for (int v = 0; v < kBrickTile; ++v) {
-              if (v < T.tv) {
-                ev = fma(c_v, ev, r[v]);  // the v-chain is the only dependency between the cells of a row
-                ew[v] = ev;
-                pl[(c0 + v) * kBrickPitch] = ev;
-                if (v + 1 == T.tv) elast = ev;
-              }
-            }
-            if (dn_fv) dn_fv[(int64_t)(u * kBrickTile + w) * S] = elast;
-            if (w + 1 == T.tw && dn_fw) {
-#pragma unroll
-              for (int v = 0; v < kBrickTile; ++v)
-                if (v < T.tv) dn_fw[(int64_t)(u * kBrickTile + v) * S] = ew[v];
-            }
-            if (last_u && dn_fu) {
-#pragma unroll
-              for (int v = 0; v < kBrickTile; ++v)
-                if (v < T.tv) dn_fu[(int64_t)(c0 + v) * S] = ew[v];
-            }
-            if (frow & 0x2020202020202020ull) {  // cells with an outgoing boundary face: eps for the closures
-#pragma unroll
-              for (int v = 0; v < kBrickTile; ++v)
-                if ((frow >> (8 * v)) & BRK_WALL) wall[(int64_t)(wp++) * S] = ew[v];
-            }
-            if (a.store_e) {
-#pragma unroll
-              for (int v = 0; v < kBrickTile; ++v)
-                if (v < T.tv) __stcs(eout + ((int64_t)u * kBrickCells + c0 + v) * S, ew[v]);
-            }
-            continue;
+        if (T.plain) {
+          const bool src = (src_planes >> u) & 1ull;
+          double *dfv = dn_fv ? dn_fv + (int64_t)u * kBrickTile * S : nullptr;
+          double *eo = a.store_e ? eout + (int64_t)u * kBrickCells * S : nullptr;
+          switch (T.tv) {
+            case 8: plain_plane<8>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
+            case 7: plain_plane<7>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
+            case 6: plain_plane<6>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
+            case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
+            case 4: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
+            case 3: plain_plane<3>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
+            case 2: plain_plane<2>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
+            default: plain_plane<1>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
           }
-          // ---- general row: holes and walls inside the tile (values straight from L2; rare) ----------------------------------
+          if (dn_fw) {  // ew holds the last row
+#pragma unroll
+            for (int v = 0; v < kBrickTile; ++v)
+              if (v < T.tv) dn_fw[(int64_t)(u * kBrickTile + v) * S] = ew[v];
+          }
+        } else {
+          // ---- per-cell path: holes and walls inside the tile (wall values straight from L2) ----------------------------------
+          for (int w = 0; w < T.tw; ++w) {
+            const unsigned long long frow = sm.flg[st][w];
+            double ev = inv[0];
+#pragma unroll
+            for (int k = 0; k + 1 < kBrickTile; ++k) inv[k] = inv[k + 1];  // inv[0] is always the current row's v-face value
+            if (frow == 0ull) continue;
+            const int c0 = w * kBrickTile;
 #pragma unroll 1
-          for (int v = 0; v < T.tv; ++v) {
-            const unsigned f = (unsigned)(frow >> (8 * v)) & 0xffu;
-            double ewv = 0.0;
+            for (int v = 0; v < T.tv; ++v) {
+              const unsigned f = (unsigned)(frow >> (8 * v)) & 0xffu;
+              double ewv = 0.0;
 #pragma unroll
-            for (int k = 0; k < kBrickTile; ++k) ewv = k == v ? ew[k] : ewv;
-            if (f & BRK_ACT) {
-              const int cell = c0 + v;
-              double eu = pl[cell * kBrickPitch];
-              if (f & BRK_INJ_U) eu = __ldcg(irr + (int64_t)(ip++) * S);
-              if (f & BRK_INJ_V) ev = __ldcg(irr + (int64_t)(ip++) * S);
-              if (f & BRK_INJ_W) ewv = __ldcg(irr + (int64_t)(ip++) * S);
-              double r = k_th * sm.th[st][cell];
-              if (f & BRK_SRC) r = fma(k_Q, sm.qd[st][cell], r);
-              r = fma(c_u, eu, fma(c_w, ewv, r));
-              const double e = fma(c_v, ev, r);
-              pl[cell * kBrickPitch] = e;
-              ev = e;
-              ewv = e;
-              if (v + 1 == T.tv && dn_fv) dn_fv[(int64_t)(u * kBrickTile + w) * S] = e;
-              if (w + 1 == T.tw && dn_fw) dn_fw[(int64_t)(u * kBrickTile + v) * S] = e;
-              if (last_u && dn_fu) dn_fu[(int64_t)cell * S] = e;
-              if (f & BRK_WALL) wall[(int64_t)(wp++) * S] = e;
-              if (a.store_e) __stcs(eout + ((int64_t)u * kBrickCells + cell) * S, e);
+              for (int k = 0; k < kBrickTile; ++k) ewv = k == v ? ew[k] : ewv;
+              if (f & BRK_ACT) {
+                const int cell = c0 + v;
+                double eu = pl[cell * kP];
+                if (f & BRK_INJ_U) eu = __ldcg(irr + (int64_t)(ip++) * S);
+                if (f & BRK_INJ_V) ev = __ldcg(irr + (int64_t)(ip++) * S);
+                if (f & BRK_INJ_W) ewv = __ldcg(irr + (int64_t)(ip++) * S);
+                double r = c.k_th * sm.th[cell];
+                if (f & BRK_SRC) r = fma(c.k_Q, sm.qd[cell], r);
+                r = fma(c.c_u, eu, fma(c.c_w, ewv, r));
+                const double e = fma(c.c_v, ev, r);
+                pl[cell * kP] = e;
+                ev = e;
+                ewv = e;
+                if (v + 1 == T.tv && dn_fv) dn_fv[(int64_t)(u * kBrickTile + w) * S] = e;
+                if (w + 1 == T.tw && dn_fw) dn_fw[(int64_t)(u * kBrickTile + v) * S] = e;
+                if (a.store_e) __stcs(eout + ((int64_t)u * kBrickCells + cell) * S, e);
+              }
+#pragma unroll
+              for (int k = 0; k < kBrickTile; ++k) ew[k] = k == v ? ewv : ew[k];
             }
-#pragma unroll
-            for (int k = 0; k < kBrickTile; ++k) ew[k] = k == v ? ewv : ew[k];
           }
         }
       }
-      cp_async_wait_all();
-      __syncthreads();  // plane u is complete in the plane buffer; the staged tables of plane u+1 have landed
-      if (t == 0) {  // publish: every store of the CTA before the barrier is ordered before this release
-        __threadfence();
-        st_release(a.prog + task, u + 1 == T.nu ? 0x7fffffffu : (unsigned)(u + 1));
+      __syncthreads();  // B1: plane u is complete in the plane buffer; theta / Qdot of plane u are dead
+      if (!last_u) {
+        stage(u + 1);
+        if (t == 0) {  // publish: every store of the CTA before the barrier is ordered before this release
+          __threadfence();
+          st_release(a.prog + task, (unsigned)(u + 1));
+        }
       }
 
       // next plane's tile-face inflow: issued before the reduction if the upstream tiles are already there (the loads
@@ -245,61 +278,84 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
           ew[k] = on ? __ldcg(fw + (int64_t)(un * kBrickTile + k) * S) : 0.0;
         }
       };
-      const bool more = u + 1 < T.nu;
       bool early = false;
-      if (more) {
+      if (!last_u) {
         early = progress_ready(a.prog, T.up_v, (unsigned)(u + 2)) && progress_ready(a.prog, T.up_w, (unsigned)(u + 2));
         if (early) load_faces(u + 1);
       }
-      // ------------------------------------------ moments: lane = cell, half-warps split the bands ------------------------
-      {
-        const int cell = wid * 16 + (lane & 15), half = lane >> 4;
-        const int nb0 = (G.nb + 1) >> 1;
-        const int b_lo = half ? nb0 : 0, b_hi = half ? G.nb : nb0;
-        const double *row = sm.plane + cell * kBrickPitch;
-        double m0 = 0.0, m1 = 0.0, m2 = 0.0, m3 = 0.0, m4 = 0.0;
-        const bool act = (reinterpret_cast<const unsigned char *>(sm.flg[st])[cell] & BRK_ACT) != 0;
-        if (act) {
-          for (int b = b_lo; b < b_hi; ++b) {
-            double E = 0.0, Fx = 0.0, Fy = 0.0, Fz = 0.0;
-            const double *rb = row + b * G.nd;
-            for (int d = 0; d < G.nd; ++d) {
-              const double e = rb[d];
-              const double2 c01 = *reinterpret_cast<const double2 *>(sm.dcoef + 4 * d);
-              const double2 c23 = *reinterpret_cast<const double2 *>(sm.dcoef + 4 * d + 2);
-              E = fma(c01.x, e, E);
-              Fx = fma(c01.y, e, Fx);
-              Fy = fma(c23.x, e, Fy);
-              Fz = fma(c23.y, e, Fz);
-            }
-            const double2 bc = *reinterpret_cast<const double2 *>(sm.bcoef + 2 * b);
-            m0 = fma(bc.x, E, m0);
-            m1 += E;
-            m2 = fma(bc.y, Fx, m2);
-            m3 = fma(bc.y, Fy, m3);
-            m4 = fma(bc.y, Fz, m4);
+      // ---- out of the plane buffer (thread = system): eps of the cells with an outgoing wall (closures), the u-face of the
+      // segment ----------------------------------------------------------------------------------------------------------------
+      if (on && T.wall_any) {
+        for (int w = 0; w < T.tw; ++w) {
+          const unsigned long long frow = sm.flg[st][w];
+          if (frow & 0x2020202020202020ull) {
+#pragma unroll
+            for (int v = 0; v < kBrickTile; ++v)
+              if ((frow >> (8 * v)) & BRK_WALL) wall[(int64_t)(wp++) * S] = sm.plane[(w * kBrickTile + v) * kP + s];
           }
         }
-        m0 += __shfl_xor_sync(0xffffffffu, m0, 16);
-        m1 += __shfl_xor_sync(0xffffffffu, m1, 16);
-        m2 += __shfl_xor_sync(0xffffffffu, m2, 16);
-        m3 += __shfl_xor_sync(0xffffffffu, m3, 16);
-        m4 += __shfl_xor_sync(0xffffffffu, m4, 16);
-        if (half == 0) {
-          double *p = part + (int64_t)u * kBrickCells + cell;
-          p[0] = m0;
-          p[npos] = m1;
-          p[2 * npos] = m2;
-          p[3 * npos] = m3;
-          p[4 * npos] = m4;
+      }
+      if (on && last_u && dn_fu) {
+        for (int w = 0; w < T.tw; ++w) {
+          const unsigned long long frow = sm.flg[st][w];
+#pragma unroll
+          for (int v = 0; v < kBrickTile; ++v)
+            if ((frow >> (8 * v)) & BRK_ACT) dn_fu[(int64_t)(w * kBrickTile + v) * S] = sm.plane[(w * kBrickTile + v) * kP + s];
         }
       }
-      if (more && !early) {
-        wait_progress(a.prog, T.up_v, (unsigned)(u + 2));
-        wait_progress(a.prog, T.up_w, (unsigned)(u + 2));
-        load_faces(u + 1);
+      // ------------------------------------------ moments: thread = cells (lane, lane + 32) x the warp's bands -------------
+      {
+        const unsigned char *fb = reinterpret_cast<const unsigned char *>(sm.flg[st]);
+        const bool act0 = (fb[lane] & BRK_ACT) != 0, act1 = (fb[lane + 32] & BRK_ACT) != 0;
+        const double *row0 = sm.plane + lane * kP, *row1 = sm.plane + (lane + 32) * kP;
+        double m[2][5] = {{0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};
+        const int nd = G.nd;
+        for (int b = b_lo; b < b_hi; ++b) {
+          double E0 = 0.0, X0 = 0.0, Y0 = 0.0, Z0 = 0.0, E1 = 0.0, X1 = 0.0, Y1 = 0.0, Z1 = 0.0;
+          const double *r0 = row0 + b * nd, *r1 = row1 + b * nd;
+#pragma unroll 4
+          for (int d = 0; d < nd; ++d) {
+            const double e0 = r0[d], e1 = r1[d];
+            const double2 c01 = *reinterpret_cast<const double2 *>(sm.dcoef + 4 * d);
+            const double2 c23 = *reinterpret_cast<const double2 *>(sm.dcoef + 4 * d + 2);
+            E0 = fma(c01.x, e0, E0); X0 = fma(c01.y, e0, X0); Y0 = fma(c23.x, e0, Y0); Z0 = fma(c23.y, e0, Z0);
+            E1 = fma(c01.x, e1, E1); X1 = fma(c01.y, e1, X1); Y1 = fma(c23.x, e1, Y1); Z1 = fma(c23.y, e1, Z1);
+          }
+          const double2 bc = *reinterpret_cast<const double2 *>(sm.bcoef + 2 * b);
+          m[0][0] = fma(bc.x, E0, m[0][0]); m[0][1] += E0;
+          m[0][2] = fma(bc.y, X0, m[0][2]); m[0][3] = fma(bc.y, Y0, m[0][3]); m[0][4] = fma(bc.y, Z0, m[0][4]);
+          m[1][0] = fma(bc.x, E1, m[1][0]); m[1][1] += E1;
+          m[1][2] = fma(bc.y, X1, m[1][2]); m[1][3] = fma(bc.y, Y1, m[1][3]); m[1][4] = fma(bc.y, Z1, m[1][4]);
+        }
+        if (wid < 3) {
+#pragma unroll
+          for (int k = 0; k < 5; ++k) {
+            sm.red[wid][k][lane] = m[0][k];
+            sm.red[wid][k][lane + 32] = m[1][k];
+          }
+        }
+        if (!last_u && !early) {
+          wait_progress(a.prog, T.up_v, (unsigned)(u + 2));
+          wait_progress(a.prog, T.up_w, (unsigned)(u + 2));
+          load_faces(u + 1);
+        }
+        cp_async_wait_all();
+        __syncthreads();  // B2: the plane buffer is free again; the band partials are in place; theta of plane u+1 has landed
+        if (last_u && t == 0) {
+          __threadfence();
+          st_release(a.prog + task, 0x7fffffffu);
+        }
+        if (wid == 3) {  // fixed order: warp 0 + warp 1 + warp 2 + warp 3
+          double *p = part + (int64_t)u * kBrickCells + lane;
+#pragma unroll
+          for (int k = 0; k < 5; ++k) {
+            const double v0 = ((sm.red[0][k][lane] + sm.red[1][k][lane]) + sm.red[2][k][lane]) + m[0][k];
+            const double v1 = ((sm.red[0][k][lane + 32] + sm.red[1][k][lane + 32]) + sm.red[2][k][lane + 32]) + m[1][k];
+            if (act0) p[k * npos] = v0;
+            if (act1) p[k * npos + 32] = v1;
+          }
+        }
       }
-      __syncthreads();  // the plane buffer and stage st are free again
     }
   }
 }

@@ -12,6 +12,11 @@ import os
 import numpy as np
 import pytest
 
+# max|dtheta| histories: the entries are differences of fields of size |theta| <= ~10 K, so two correct evaluations
+# with different summation orders differ by a few tens of ulp(10 K) ~ 2e-15 each; 1e-13 is four orders below every
+# convergence tolerance used here (R11) and far above that noise.
+HIST_ATOL = 1e-13
+
 from oracle.ref import RefSolver
 from paper_2607_03226_b200 import workloads as wl
 
@@ -194,7 +199,7 @@ def test_config1_nongray_square_full_solve():
     rr, rg = r.solve(pr["tol"], pr["max_iter"]), g.solve(pr["tol"], pr["max_iter"])
     assert rr["converged"] and rg["converged"] and rr["iters"] == rg["iters"], (rr, rg)
     assert np.abs(g.get_T(0) - r.get_T(0)).max() <= 1e-8
-    np.testing.assert_allclose(g.get_history()[0], r.get_history()[0], rtol=1e-6, atol=1e-14)
+    np.testing.assert_allclose(g.get_history()[0], r.get_history()[0], rtol=1e-6, atol=HIST_ATOL)
     g.close()
     r.close()
 
@@ -218,7 +223,7 @@ def test_fullsize_converged_against_golden(name, mode):
     act = np.ones(g.n_cells, dtype=bool) if (pr["kind"] == "unstructured" or m["active"] is None) else np.asarray(m["active"]).reshape(-1) != 0
     T = g.get_T(0)[act]
     assert np.abs(T - gold["T_active"]).max() <= 1e-8, np.abs(T - gold["T_active"]).max()
-    np.testing.assert_allclose(g.get_history()[0], gold["hist_dT"], rtol=1e-6, atol=1e-14)
+    np.testing.assert_allclose(g.get_history()[0], gold["hist_dT"], rtol=1e-6, atol=HIST_ATOL)
     g.close()
 
 
