@@ -13,7 +13,8 @@
 // u-plane (release), its two downstream tiles acquire it one plane behind.  Tasks are handed out in topological
 // order by a ticket counter, so a waiting CTA only ever waits for a CTA that is already running.
 //
-// Row spaces (all rows of group g of class c are S_g doubles long, lanes = systems: every access is coalesced):
+// Row spaces (every row holds the S_g systems of group g of class c at a pitch of kBrickRow doubles, lanes = systems:
+// every access is coalesced):
 //   inflow rows of class c   per task: FU [64] (u-face of the segment), FV [nu][8], FW [nu][8] (v- / w-face, one row per
 //                            cell of the face and u-plane), IRR [n_irr] (walls inside the tile, consumption order).
 //                            Written by the upstream task (interior tile faces) or by the closure kernel (boundary
@@ -27,6 +28,7 @@
 constexpr int kBrickTile = 8;          // tile edge (pencils)
 constexpr int kBrickCells = 64;        // cells per u-plane of a tile
 constexpr int kBrickMaxS = 128;        // systems per task = threads per CTA
+constexpr int kBrickRow = 128;         // pitch in doubles of every inflow / wall / eps row (compile-time: row addresses are immediates)
 constexpr int kBrickPitch = 129;       // plane-buffer row pitch in doubles (odd: lanes = cells is conflict-free too)
 
 enum : uint8_t {

@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(128) brick_gsum_kernel(const BrickClosureArgs 
   const int bf = R.out_bf[c][j];
   if ((a.bf_type[bf] == NANOBTE_THERMALIZING) != (R.therm != 0)) return;
   const BrickCG G = R.cgs[R.cg_of[c * a.B + b]];
-  const double *src = R.wall + G.wall_base + (int64_t)R.out_row[c][j] * G.S + (b - G.b0) * G.nd;
+  const double *src = R.wall + G.wall_base + (int64_t)R.out_row[c][j] * kBrickRow + (b - G.b0) * G.nd;
   const double *sn = a.bf_sn + (size_t)bf * a.D;
   double acc = 0.0;
   for (int dl = 0; dl < G.nd; ++dl) {
@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(kBrickMaxS) brick_inflow_kernel(const BrickClo
   if (k >= R.n_in[c] || s >= G.S) return;
   const int bf = R.in_bf[c][k];
   const int type = a.bf_type[bf];
-  double *dst = R.inf + G.inf_base + (int64_t)R.in_row[c][k] * G.S + s;
+  double *dst = R.inf + G.inf_base + (int64_t)R.in_row[c][k] * kBrickRow + s;
   const int b = G.b0 + s / G.nd;
   if (type == NANOBTE_THERMALIZING) {
     if (R.init) *dst = a.C[b] * a.bf_eps_w[bf] / R.W;  // R6; never changes afterwards
@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(kBrickMaxS) brick_inflow_kernel(const BrickClo
   }
   const int cm = R.dir_cls[md];
   const BrickCG Gm = R.cgs[R.cg_of[cm * a.B + b]];
-  const double spec = R.wall[Gm.wall_base + (int64_t)R.bf_wrow[(size_t)cm * a.n_bf + bf] * Gm.S + (b - Gm.b0) * Gm.nd + R.dir_local[md]];
+  const double spec = R.wall[Gm.wall_base + (int64_t)R.bf_wrow[(size_t)cm * a.n_bf + bf] * kBrickRow + (b - Gm.b0) * Gm.nd + R.dir_local[md]];
   *dst = type == NANOBTE_SPECULAR ? spec : a.bf_p[bf] * spec + (1.0 - a.bf_p[bf]) * Gf;  // R8
 }
 
@@ -171,7 +171,7 @@ __global__ void brick_get_e_kernel(const BrickGetEArgs g) {
     const int cls = g.dir_cls[d];
     const BrickCG G = g.cgs[g.cg_of[cls * g.B + b]];
     const int64_t pos = g.a2pos[(size_t)cls * g.n_act + a];
-    val = g.e[G.e_base + pos * G.S + (b - G.b0) * G.nd + g.dir_local[d]] + g.C[b] * g.off_scale;
+    val = g.e[G.e_base + pos * kBrickRow + (b - G.b0) * G.nd + g.dir_local[d]] + g.C[b] * g.off_scale;
   }
   g.dst[((size_t)bi * g.nd + di) * g.n_cells + c] = val;
 }

@@ -256,10 +256,10 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
   for (BrickCG &g : bh.cgs) {
     const BrickHost::Cls &C = bh.cls[g.cls];
     auto pad = [](int64_t v) { return (v + 31) / 32 * 32; };
-    g.inf_base = inf; inf = pad(inf + (int64_t)C.nrow * g.S);
-    g.wall_base = wall; wall = pad(wall + (int64_t)C.nwall * g.S);
+    g.inf_base = inf; inf = pad(inf + (int64_t)C.nrow * kBrickRow);
+    g.wall_base = wall; wall = pad(wall + (int64_t)C.nwall * kBrickRow);
     g.part_base = part; part = pad(part + (int64_t)5 * C.npos);
-    g.e_base = e; e = pad(e + (int64_t)C.npos * g.S);
+    g.e_base = e; e = pad(e + (int64_t)C.npos * kBrickRow);
     g.coef_base = cf;
     for (int bl = 0; bl < g.nb; ++bl)
       for (int dl = 0; dl < g.nd; ++dl) {

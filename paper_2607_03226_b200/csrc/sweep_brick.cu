@@ -28,11 +28,6 @@ __device__ __forceinline__ unsigned int ld_acquire(const unsigned int *p) {
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-__device__ __forceinline__ unsigned int ld_relaxed(const unsigned int *p) {
-  unsigned int v;
-  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
 __device__ __forceinline__ void st_release(unsigned int *p, unsigned int v) {
   asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -41,29 +36,40 @@ __device__ __forceinline__ void cp_async16(void *dst_smem, const void *src) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// One lane per warp waits until task `up` has published at least `need` planes; the rest of the warp follows through
-// __syncwarp (memory ordering among the participating lanes), and reads the published rows with L2 loads (ld.cg).
+// Progress of the two upstream tiles (v: lane 0, w: lane 1 of every warp), polled with ONE acquire load for both and
+// remembered: an upstream tile that started earlier is usually many planes ahead, and then no poll is needed at all.
+// The published rows are read with L2 loads (ld.cg); __syncwarp orders the other lanes behind the polling lanes.
+struct Upstream {
+  const unsigned int *pv, *pw;  // progress words (nullptr: no upstream task -- boundary rows, always there)
+  unsigned int seen_v, seen_w;
+  __device__ __forceinline__ void init(const unsigned int *prog, int up_v, int up_w) {
+    pv = up_v >= 0 ? prog + up_v : nullptr;
+    pw = up_w >= 0 ? prog + up_w : nullptr;
+    seen_v = pv ? 0u : 0x7fffffffu;
+    seen_w = pw ? 0u : 0x7fffffffu;
+  }
+  __device__ __forceinline__ bool poll(unsigned int need) {  // true in every lane if both have published `need` planes
+    if (seen_v >= need && seen_w >= need) return true;
+    const int lane = threadIdx.x & 31;
+    const unsigned int *p = lane == 0 ? pv : pw;
+    unsigned int v = 0x7fffffffu;
+    if (lane < 2 && p) v = ld_acquire(p);
+    seen_v = __shfl_sync(0xffffffffu, v, 0);
+    seen_w = __shfl_sync(0xffffffffu, v, 1);
+    return seen_v >= need && seen_w >= need;
+  }
+  __device__ __forceinline__ void wait(unsigned int need) {
+    while (!poll(need)) __nanosleep(20);
+  }
+};
+
 __device__ __forceinline__ void wait_progress(const unsigned int *prog, int up, unsigned int need) {
   if (up >= 0) {
     if ((threadIdx.x & 31) == 0) {
-      while (ld_relaxed(prog + up) < need) __nanosleep(40);  // cheap polls; one acquire once the value is there
-      (void)ld_acquire(prog + up);
+      while (ld_acquire(prog + up) < need) __nanosleep(40);
     }
     __syncwarp();
   }
-}
-
-// Non-blocking form: true (in every lane) if the rows are already published.
-__device__ __forceinline__ bool progress_ready(const unsigned int *prog, int up, unsigned int need) {
-  if (up < 0) return true;
-  int ok = 0;
-  if ((threadIdx.x & 31) == 0) {
-    ok = ld_relaxed(prog + up) >= need;
-    if (ok) (void)ld_acquire(prog + up);
-  }
-  ok = __shfl_sync(0xffffffffu, ok, 0);
-  __syncwarp();
-  return ok != 0;
 }
 
 constexpr int kP = kBrickPitch;
@@ -85,11 +91,12 @@ struct Sys {           // what a substitution thread keeps for its system
 };
 
 // ---- one u-plane of a fully active box, TV cells per row: straight-line code ---------------------------------------------------------
-// pl = plane buffer + system; ew[v] = w-upwind values (in: tile-face inflow, out: last row); inv[w] = v-face inflow of row w.
+// pl = plane buffer + system; ew[v] = w-upwind values (in: tile-face inflow, out: last row); inv[w] = v-face inflow of row w;
+// dn_fv_u / eout_u = this plane's rows of the v-downstream tile / of the stored distribution (nullptr: none).
 template <int TV>
 __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const double *__restrict__ th, const double *__restrict__ qd,
                                             const Sys &c, const int tw, const bool src, double (&ew)[kBrickTile],
-                                            const double (&inv)[kBrickTile], double *dn_fv_u, const int64_t S, double *eout_u) {
+                                            const double (&inv)[kBrickTile], double *dn_fv_u, double *eout_u) {
 #pragma unroll
   for (int w = 0; w < kBrickTile; ++w) {
     if (w < tw) {
@@ -120,10 +127,10 @@ __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const doubl
         ew[v] = ev;
         row[v * kP] = ev;
       }
-      if (dn_fv_u) dn_fv_u[(int64_t)w * S] = ev;
+      if (dn_fv_u) dn_fv_u[w * kBrickRow] = ev;
       if (eout_u) {
 #pragma unroll
-        for (int v = 0; v < TV; ++v) __stcs(eout_u + (int64_t)(w * kBrickTile + v) * S, ew[v]);
+        for (int v = 0; v < TV; ++v) __stcs(eout_u + (w * kBrickTile + v) * kBrickRow, ew[v]);
       }
     }
   }
@@ -147,17 +154,18 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     const int s = on ? t : 0;
     const double *th_g = a.th[G.cls] + T.pos0, *qd_g = a.qd[G.cls] + T.pos0;
     const uint8_t *flg_g = a.flg[G.cls] + T.pos0;
-    double *inf = a.inf + G.inf_base;
-    double *wall = a.wall + G.wall_base + (int64_t)T.wo0 * S + s;
+    double *inf = a.inf + G.inf_base + s;
+    double *wall = a.wall + G.wall_base + (int64_t)T.wo0 * kBrickRow + s;
     double *part = a.part + G.part_base + T.pos0;
     const int64_t npos = a.npos[G.cls];
-    double *eout = a.e + G.e_base + (int64_t)T.pos0 * S + s;
-    const double *irr = inf + (int64_t)T.ir0 * S + s;
-    const double *fv = inf + (int64_t)T.fv0 * S + s, *fw = inf + (int64_t)T.fw0 * S + s;
-    double *dn_fu = T.dn_fu0 >= 0 ? inf + (int64_t)T.dn_fu0 * S + s : nullptr;
-    double *dn_fv = T.dn_fv0 >= 0 ? inf + (int64_t)T.dn_fv0 * S + s : nullptr;
-    double *dn_fw = T.dn_fw0 >= 0 ? inf + (int64_t)T.dn_fw0 * S + s : nullptr;
+    double *eout = a.store_e ? a.e + G.e_base + (int64_t)T.pos0 * kBrickRow + s : nullptr;
+    const double *irr = inf + (int64_t)T.ir0 * kBrickRow;
+    const double *fv = inf + (int64_t)T.fv0 * kBrickRow, *fw = inf + (int64_t)T.fw0 * kBrickRow;
+    double *dn_fu = T.dn_fu0 >= 0 ? inf + (int64_t)T.dn_fu0 * kBrickRow : nullptr;
+    double *dn_fv = T.dn_fv0 >= 0 ? inf + (int64_t)T.dn_fv0 * kBrickRow : nullptr;
+    double *dn_fw = T.dn_fw0 >= 0 ? inf + (int64_t)T.dn_fw0 * kBrickRow : nullptr;
     const unsigned long long src_planes = ((unsigned long long)T.src_hi << 32) | T.src_lo;
+    const bool plain = T.plain && T.tv >= 4;
 
     // coefficients of this thread's system; moment tables of the group
     const double *cf = a.coef + G.coef_base;
@@ -177,50 +185,53 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     // u-face inflow -> plane buffer (the previous segment of the pencils, or boundary values)
     wait_progress(a.prog, T.up_u, 0x7fffffffu);
     if (on) {
-      const double *fu = inf + (int64_t)T.fu0 * S + s;
+      const double *fu = inf + (int64_t)T.fu0 * kBrickRow;
 #pragma unroll 8
-      for (int cc = 0; cc < kBrickCells; ++cc) sm.plane[cc * kP + s] = __ldcg(fu + (int64_t)cc * S);
+      for (int cc = 0; cc < kBrickCells; ++cc) sm.plane[cc * kP + s] = __ldcg(fu + cc * kBrickRow);
     }
     // v- and w-face inflow of plane 0
+    Upstream ups;
+    ups.init(a.prog, T.up_v, T.up_w);
     double ew[kBrickTile], inv[kBrickTile];
-    wait_progress(a.prog, T.up_v, 1u);
-    wait_progress(a.prog, T.up_w, 1u);
+    auto load_faces = [&]() {  // fv / fw point at the rows of the plane to come
 #pragma unroll
-    for (int k = 0; k < kBrickTile; ++k) {
-      inv[k] = on ? __ldcg(fv + (int64_t)k * S) : 0.0;
-      ew[k] = on ? __ldcg(fw + (int64_t)k * S) : 0.0;
-    }
+      for (int k = 0; k < kBrickTile; ++k) {
+        inv[k] = on ? __ldcg(fv + k * kBrickRow) : 0.0;
+        ew[k] = on ? __ldcg(fw + k * kBrickRow) : 0.0;
+      }
+      fv += kBrickTile * kBrickRow;
+      fw += kBrickTile * kBrickRow;
+    };
+    ups.wait(1u);
+    load_faces();
     cp_async_wait_all();
     __syncthreads();
 
-    // bands of this warp in the moment role
-    const int b_lo = (G.nb * wid) >> 2, b_hi = (G.nb * (wid + 1)) >> 2;
+    // The warp's share of the moment work in half-band units (a band's directions split in two): whole bands except where
+    // a share boundary falls inside a band.  Equal shares whatever the band count.
+    const int h_lo = (2 * G.nb * wid) >> 2, h_hi = (2 * G.nb * (wid + 1)) >> 2;
+    const int nd = G.nd, nd_half = nd >> 1;
 
-    int ip = 0, wp = 0;  // next row of the IRR stream / of the wall rows (same value in every thread)
+    int ip = 0;  // next row of the IRR stream (same value in every thread)
     for (int u = 0; u < T.nu; ++u) {
       const int st = u & 1;
       const bool last_u = u + 1 == T.nu;
       // ------------------------------------------ substitution: thread = system ------------------------------------------
       if (on) {
         double *pl = sm.plane + s;
-        if (T.plain) {
+        if (plain) {
           const bool src = (src_planes >> u) & 1ull;
-          double *dfv = dn_fv ? dn_fv + (int64_t)u * kBrickTile * S : nullptr;
-          double *eo = a.store_e ? eout + (int64_t)u * kBrickCells * S : nullptr;
           switch (T.tv) {
-            case 8: plain_plane<8>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
-            case 7: plain_plane<7>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
-            case 6: plain_plane<6>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
-            case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
-            case 4: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
-            case 3: plain_plane<3>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
-            case 2: plain_plane<2>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
-            default: plain_plane<1>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dfv, S, eo); break;
+            case 8: plain_plane<8>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
+            case 7: plain_plane<7>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
+            case 6: plain_plane<6>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
+            case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
+            default: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
           }
           if (dn_fw) {  // ew holds the last row
 #pragma unroll
             for (int v = 0; v < kBrickTile; ++v)
-              if (v < T.tv) dn_fw[(int64_t)(u * kBrickTile + v) * S] = ew[v];
+              if (v < T.tv) dn_fw[v * kBrickRow] = ew[v];
           }
         } else {
           // ---- per-cell path: holes and walls inside the tile (wall values straight from L2) ----------------------------------
@@ -240,9 +251,9 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
               if (f & BRK_ACT) {
                 const int cell = c0 + v;
                 double eu = pl[cell * kP];
-                if (f & BRK_INJ_U) eu = __ldcg(irr + (int64_t)(ip++) * S);
-                if (f & BRK_INJ_V) ev = __ldcg(irr + (int64_t)(ip++) * S);
-                if (f & BRK_INJ_W) ewv = __ldcg(irr + (int64_t)(ip++) * S);
+                if (f & BRK_INJ_U) eu = __ldcg(irr + (int64_t)(ip++) * kBrickRow);
+                if (f & BRK_INJ_V) ev = __ldcg(irr + (int64_t)(ip++) * kBrickRow);
+                if (f & BRK_INJ_W) ewv = __ldcg(irr + (int64_t)(ip++) * kBrickRow);
                 double r = c.k_th * sm.th[cell];
                 if (f & BRK_SRC) r = fma(c.k_Q, sm.qd[cell], r);
                 r = fma(c.c_u, eu, fma(c.c_w, ewv, r));
@@ -250,38 +261,29 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
                 pl[cell * kP] = e;
                 ev = e;
                 ewv = e;
-                if (v + 1 == T.tv && dn_fv) dn_fv[(int64_t)(u * kBrickTile + w) * S] = e;
-                if (w + 1 == T.tw && dn_fw) dn_fw[(int64_t)(u * kBrickTile + v) * S] = e;
-                if (a.store_e) __stcs(eout + ((int64_t)u * kBrickCells + cell) * S, e);
+                if (v + 1 == T.tv && dn_fv) dn_fv[w * kBrickRow] = e;
+                if (w + 1 == T.tw && dn_fw) dn_fw[v * kBrickRow] = e;
+                if (eout) __stcs(eout + cell * kBrickRow, e);
               }
 #pragma unroll
               for (int k = 0; k < kBrickTile; ++k) ew[k] = k == v ? ewv : ew[k];
             }
           }
         }
+        if (dn_fv) dn_fv += kBrickTile * kBrickRow;
+        if (dn_fw) dn_fw += kBrickTile * kBrickRow;
+        if (eout) eout += kBrickCells * kBrickRow;
       }
       __syncthreads();  // B1: plane u is complete in the plane buffer; theta / Qdot of plane u are dead
-      if (!last_u) {
-        stage(u + 1);
-        if (t == 0) {  // publish: every store of the CTA before the barrier is ordered before this release
-          __threadfence();
-          st_release(a.prog + task, (unsigned)(u + 1));
-        }
-      }
-
-      // next plane's tile-face inflow: issued before the reduction if the upstream tiles are already there (the loads
-      // then fly during the reduction), otherwise after it
-      auto load_faces = [&](int un) {
-#pragma unroll
-        for (int k = 0; k < kBrickTile; ++k) {
-          inv[k] = on ? __ldcg(fv + (int64_t)(un * kBrickTile + k) * S) : 0.0;
-          ew[k] = on ? __ldcg(fw + (int64_t)(un * kBrickTile + k) * S) : 0.0;
-        }
-      };
       bool early = false;
       if (!last_u) {
-        early = progress_ready(a.prog, T.up_v, (unsigned)(u + 2)) && progress_ready(a.prog, T.up_w, (unsigned)(u + 2));
-        if (early) load_faces(u + 1);
+        stage(u + 1);
+        // publish: the barrier orders every store of the CTA before this release (cumulativity)
+        if (t == 0) st_release(a.prog + task, (unsigned)(u + 1));
+        // next plane's tile-face inflow: issued before the reduction if the upstream tiles are already there (the loads
+        // then fly during the reduction), otherwise after it
+        early = ups.poll((unsigned)(u + 2));
+        if (early) load_faces();
       }
       // ---- out of the plane buffer (thread = system): eps of the cells with an outgoing wall (closures), the u-face of the
       // segment ----------------------------------------------------------------------------------------------------------------
@@ -289,9 +291,13 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         for (int w = 0; w < T.tw; ++w) {
           const unsigned long long frow = sm.flg[st][w];
           if (frow & 0x2020202020202020ull) {
+            const double *prow = sm.plane + w * kBrickTile * kP + s;
 #pragma unroll
             for (int v = 0; v < kBrickTile; ++v)
-              if ((frow >> (8 * v)) & BRK_WALL) wall[(int64_t)(wp++) * S] = sm.plane[(w * kBrickTile + v) * kP + s];
+              if ((frow >> (8 * v)) & BRK_WALL) {
+                *wall = prow[v * kP];
+                wall += kBrickRow;
+              }
           }
         }
       }
@@ -300,22 +306,25 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
           const unsigned long long frow = sm.flg[st][w];
 #pragma unroll
           for (int v = 0; v < kBrickTile; ++v)
-            if ((frow >> (8 * v)) & BRK_ACT) dn_fu[(int64_t)(w * kBrickTile + v) * S] = sm.plane[(w * kBrickTile + v) * kP + s];
+            if ((frow >> (8 * v)) & BRK_ACT) dn_fu[(w * kBrickTile + v) * kBrickRow] = sm.plane[(w * kBrickTile + v) * kP + s];
         }
       }
-      // ------------------------------------------ moments: thread = cells (lane, lane + 32) x the warp's bands -------------
+      // ------------------------------------------ moments: thread = cells (lane, lane + 32) x the warp's share of bands ----
       {
         const unsigned char *fb = reinterpret_cast<const unsigned char *>(sm.flg[st]);
         const bool act0 = (fb[lane] & BRK_ACT) != 0, act1 = (fb[lane + 32] & BRK_ACT) != 0;
-        const double *row0 = sm.plane + lane * kP, *row1 = sm.plane + (lane + 32) * kP;
+        const double *row0 = sm.plane + lane * kP;
         double m[2][5] = {{0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};
-        const int nd = G.nd;
-        for (int b = b_lo; b < b_hi; ++b) {
+        for (int hh = h_lo; hh < h_hi;) {
+          const int b = hh >> 1;
+          const int d_lo = (hh & 1) ? nd_half : 0;
+          const int d_hi = (hh + 1 < h_hi || (hh & 1)) ? nd : nd_half;   // the whole band unless the share ends inside it
+          hh = 2 * b + (d_hi == nd ? 2 : 1);
           double E0 = 0.0, X0 = 0.0, Y0 = 0.0, Z0 = 0.0, E1 = 0.0, X1 = 0.0, Y1 = 0.0, Z1 = 0.0;
-          const double *r0 = row0 + b * nd, *r1 = row1 + b * nd;
+          const double *r0 = row0 + b * nd;
 #pragma unroll 4
-          for (int d = 0; d < nd; ++d) {
-            const double e0 = r0[d], e1 = r1[d];
+          for (int d = d_lo; d < d_hi; ++d) {
+            const double e0 = r0[d], e1 = r0[d + 32 * kP];
             const double2 c01 = *reinterpret_cast<const double2 *>(sm.dcoef + 4 * d);
             const double2 c23 = *reinterpret_cast<const double2 *>(sm.dcoef + 4 * d + 2);
             E0 = fma(c01.x, e0, E0); X0 = fma(c01.y, e0, X0); Y0 = fma(c23.x, e0, Y0); Z0 = fma(c23.y, e0, Z0);
@@ -335,16 +344,12 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
           }
         }
         if (!last_u && !early) {
-          wait_progress(a.prog, T.up_v, (unsigned)(u + 2));
-          wait_progress(a.prog, T.up_w, (unsigned)(u + 2));
-          load_faces(u + 1);
+          ups.wait((unsigned)(u + 2));
+          load_faces();
         }
         cp_async_wait_all();
         __syncthreads();  // B2: the plane buffer is free again; the band partials are in place; theta of plane u+1 has landed
-        if (last_u && t == 0) {
-          __threadfence();
-          st_release(a.prog + task, 0x7fffffffu);
-        }
+        if (last_u && t == 0) st_release(a.prog + task, 0x7fffffffu);
         if (wid == 3) {  // fixed order: warp 0 + warp 1 + warp 2 + warp 3
           double *p = part + (int64_t)u * kBrickCells + lane;
 #pragma unroll
