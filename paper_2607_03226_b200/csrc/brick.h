@@ -69,6 +69,7 @@ struct BrickArgs {
   const double *qd[NB_MAX_CLASSES];     // per class [npos] Qdot
   const uint8_t *flg[NB_MAX_CLASSES];   // per class [npos]
   int32_t npos[NB_MAX_CLASSES];         // positions per class (partials are [5][npos] per (class, group))
+  int32_t scratch_row[NB_MAX_CLASSES];  // per class: first of 8 inflow rows that no task reads (v-face rows of boundary tiles)
   double *inf, *wall, *part, *e;
   const double *coef;
   unsigned int *ticket;        // [1] next task

@@ -205,6 +205,7 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
       P.t.dn_fv0 = dv >= 0 ? protos[dv].t.fv0 : -1;
       P.t.dn_fw0 = dw >= 0 ? protos[dw].t.fw0 : -1;
     }
+    C.scratch_row = nrow; nrow += kBrickTile;
     C.npos = npos; C.nrow = nrow; C.nwall = std::max(1, nwall);
     C.th.resize((size_t)npos + 64, 0.0);
     C.qd.resize((size_t)npos + 64, 0.0);
@@ -297,6 +298,7 @@ int nb_brick_upload(nanobte_solver *h, Arena &A, BrickHost &bh) {
     a.qd[c] = A.put(C.qd);
     a.flg[c] = A.put(C.flg);
     a.npos[c] = C.npos;
+    a.scratch_row[c] = C.scratch_row;
     bs.in_row[c] = A.put(C.in_row);
     bs.in_bf[c] = A.put(C.in_bf);
     bs.n_in[c] = (int32_t)C.in_row.size();

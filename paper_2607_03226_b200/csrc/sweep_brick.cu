@@ -119,7 +119,7 @@ __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const doubl
         }
       }
 #pragma unroll
-      for (int v = 0; v < TV; ++v) r[v] = fma(c.c_u, eu[v], fma(c.c_w, ew[v], r[v]));
+      for (int v = 0; v < TV; ++v) r[v] = fma(c.c_w, ew[v], fma(c.c_u, eu[v], r[v]));  // same association as fast_plane
       double ev = inv[w];
 #pragma unroll
       for (int v = 0; v < TV; ++v) {
@@ -133,6 +133,53 @@ __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const doubl
         for (int v = 0; v < TV; ++v) __stcs(eout_u + (w * kBrickTile + v) * kBrickRow, ew[v]);
       }
     }
+  }
+}
+
+// ---- the same without a branch: no source in the plane, the distribution not stored, the v-face rows always written (tiles on
+// the boundary write a scratch row), all 8 rows computed (rows >= tw of a shorter tile work on values nobody reads).  Written
+// software-pipelined: the loads and the chain-independent half of row w+1 sit between the chain steps of row w, so that a warp
+// has work of its own during the 8-cycle DFMA latency of the v-chain.
+template <int TV>
+__device__ __forceinline__ void fast_plane(double *__restrict__ pl, const double *__restrict__ th, const Sys &c,
+                                           double (&ew)[kBrickTile], const double (&inv)[kBrickTile], double *__restrict__ dn_fv_u) {
+  double rp[TV], rn[TV];
+  {
+    double eu[TV];
+#pragma unroll
+    for (int v = 0; v < TV; ++v) eu[v] = pl[v * kP];
+#pragma unroll
+    for (int v = 0; v < TV; v += 2) {
+      const double2 t2 = *reinterpret_cast<const double2 *>(th + v);
+      rp[v] = fma(c.c_u, eu[v], c.k_th * t2.x);
+      if (v + 1 < TV) rp[v + 1] = fma(c.c_u, eu[v + 1], c.k_th * t2.y);
+    }
+  }
+#pragma unroll
+  for (int w = 0; w < kBrickTile; ++w) {
+    double *row = pl + w * kBrickTile * kP;
+    double eu[TV], tn[TV];
+    if (w + 1 < kBrickTile) {
+#pragma unroll
+      for (int v = 0; v < TV; ++v) eu[v] = row[(kBrickTile + v) * kP];
+#pragma unroll
+      for (int v = 0; v < TV; v += 2) {
+        const double2 t2 = *reinterpret_cast<const double2 *>(th + (w + 1) * kBrickTile + v);
+        tn[v] = t2.x;
+        if (v + 1 < TV) tn[v + 1] = t2.y;
+      }
+    }
+    double ev = inv[w];
+#pragma unroll
+    for (int v = 0; v < TV; ++v) {
+      ev = fma(c.c_v, ev, fma(c.c_w, ew[v], rp[v]));  // the v-chain is the only dependency between the cells of a row
+      ew[v] = ev;
+      row[v * kP] = ev;
+      if (w + 1 < kBrickTile) rn[v] = fma(c.c_u, eu[v], c.k_th * tn[v]);
+    }
+    dn_fv_u[w * kBrickRow] = ev;
+#pragma unroll
+    for (int v = 0; v < TV; ++v) rp[v] = rn[v];
   }
 }
 
@@ -166,6 +213,7 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     double *dn_fw = T.dn_fw0 >= 0 ? inf + (int64_t)T.dn_fw0 * kBrickRow : nullptr;
     const unsigned long long src_planes = ((unsigned long long)T.src_hi << 32) | T.src_lo;
     const bool plain = T.plain && T.tv >= 4;
+    double *scratch = a.inf + G.inf_base + (int64_t)a.scratch_row[G.cls] * kBrickRow + s;  // 8 rows nobody reads
 
     // coefficients of this thread's system; moment tables of the group
     const double *cf = a.coef + G.coef_base;
@@ -221,6 +269,16 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         double *pl = sm.plane + s;
         if (plain) {
           const bool src = (src_planes >> u) & 1ull;
+          if (!src && !eout) {
+            double *dfv = dn_fv ? dn_fv : scratch;
+            switch (T.tv) {
+              case 8: fast_plane<8>(pl, sm.th, c, ew, inv, dfv); break;
+              case 7: fast_plane<7>(pl, sm.th, c, ew, inv, dfv); break;
+              case 6: fast_plane<6>(pl, sm.th, c, ew, inv, dfv); break;
+              case 5: fast_plane<5>(pl, sm.th, c, ew, inv, dfv); break;
+              default: fast_plane<4>(pl, sm.th, c, ew, inv, dfv); break;
+            }
+          } else
           switch (T.tv) {
             case 8: plain_plane<8>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
             case 7: plain_plane<7>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
@@ -228,10 +286,11 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
             case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
             default: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
           }
-          if (dn_fw) {  // ew holds the last row
+          if (dn_fw) {  // the last row of the tile, out of the plane buffer (the thread's own stores)
+            const double *lrow = pl + (T.tw - 1) * kBrickTile * kP;
 #pragma unroll
             for (int v = 0; v < kBrickTile; ++v)
-              if (v < T.tv) dn_fw[v * kBrickRow] = ew[v];
+              if (v < T.tv) dn_fw[v * kBrickRow] = lrow[v * kP];
           }
         } else {
           // ---- per-cell path: holes and walls inside the tile (wall values straight from L2) ----------------------------------
@@ -256,7 +315,7 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
                 if (f & BRK_INJ_W) ewv = __ldcg(irr + (int64_t)(ip++) * kBrickRow);
                 double r = c.k_th * sm.th[cell];
                 if (f & BRK_SRC) r = fma(c.k_Q, sm.qd[cell], r);
-                r = fma(c.c_u, eu, fma(c.c_w, ewv, r));
+                r = fma(c.c_w, ewv, fma(c.c_u, eu, r));
                 const double e = fma(c.c_v, ev, r);
                 pl[cell * kP] = e;
                 ev = e;
