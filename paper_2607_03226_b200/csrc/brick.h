@@ -40,6 +40,17 @@ enum : uint8_t {
   BRK_WALL = 32     // has an outgoing boundary face for this class: eps goes to the next wall row
 };
 
+// How a task learns that the rows of an inflow face are there.
+//   BOUNDARY  no upstream task: closure rows, written before the launch.
+//   TAGGED    every row of the face is written by the upstream task.  The least significant mantissa bit of a value that
+//             crosses a tile face carries the parity of the sweep (a relative perturbation of at most 2.2e-16, below the
+//             rounding of the substitution itself), so the value is its own ready flag: no fence, no counter, no poll
+//             separate from the load; a stale row (last sweep's) has the other parity and is simply loaded again.
+//   COUNTER   the face mixes rows of the upstream task with closure rows (walls inside a tile face): the upstream task
+//             publishes a progress counter with release semantics after every plane (BrickTask::publish), this task
+//             acquires it.
+enum : int32_t { BRK_FACE_BOUNDARY = 0, BRK_FACE_TAGGED = 1, BRK_FACE_COUNTER = 2 };
+
 struct BrickTask {
   int32_t cg;                  // (class, group) index
   int32_t nu, tv, tw;          // planes, tile width (v), tile height (w)
@@ -51,8 +62,11 @@ struct BrickTask {
   int32_t plain;               // 1: every cell of the tv x tw x nu box is active (no wall inside the box): straight-line path
   uint32_t src_lo, src_hi;     // bit u: plane u of the task holds a cell with Qdot != 0 (nu <= 64)
   int32_t wall_any;            // the task has cells with an outgoing boundary face
+  int32_t fv_mode, fw_mode;    // how the v- / w-face inflow rows become valid: BRK_FACE_*
+  int32_t publish;             // a downstream task follows this one through the progress counter: publish every plane
+  int32_t pad;
 };
-static_assert(sizeof(BrickTask) == 80, "BrickTask layout");
+static_assert(sizeof(BrickTask) == 96, "BrickTask layout");
 
 struct BrickCG {
   int32_t cls, S, nb, nd;      // class, systems (= nb * nd), bands, directions of the class; system = band_local * nd + dir_local
@@ -65,6 +79,7 @@ struct BrickArgs {
   const BrickTask *tasks;      // in launch (topological) order
   const BrickCG *cgs;
   int32_t n_tasks, store_e;
+  uint32_t parity;             // of this sweep (alternates; the rows start as zeros, so the first sweep has parity 1)
   const double *th[NB_MAX_CLASSES];     // per class [npos] theta (sweep order; refreshed by the update kernel)
   const double *qd[NB_MAX_CLASSES];     // per class [npos] Qdot
   const uint8_t *flg[NB_MAX_CLASSES];   // per class [npos]
@@ -83,6 +98,7 @@ struct BrickState {
   size_t smem = 0;
   int64_t inf_total = 0, wall_total = 0, part_total = 0, e_total = 0;
   bool e_valid = false;        // the last sweep stored eps
+  uint32_t parity = 0;         // of the last sweep
   // closures
   const int32_t *in_row[NB_MAX_CLASSES] = {nullptr}, *in_bf[NB_MAX_CLASSES] = {nullptr};  // boundary-inflow rows of a class
   int32_t n_in[NB_MAX_CLASSES] = {0};

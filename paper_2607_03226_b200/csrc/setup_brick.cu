@@ -68,12 +68,12 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
   std::vector<int> cls_cg0(ncls), cls_ng(ncls);
   for (int c = 0; c < ncls; ++c) {
     const int nd = (int)x.dirs[c].size();
-    if (nd > kBrickMaxS || nd > 32) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "brick sweep: %d directions in one octant (at most 32)", nd);
+    if (nd > 16) return nb_fail(h, NANOBTE_E_UNSUPPORTED, "brick sweep: %d directions in one octant (at most 16)", nd);
     for (int k = 0; k < nd; ++k) bh.dir_local[x.dirs[c][k]] = k;
     const int ng = (B * nd + kBrickMaxS - 1) / kBrickMaxS;
     int per = (B + ng - 1) / ng;
     while (per * nd > kBrickMaxS) --per;
-    if (per > 64) per = 64;
+    if (per > 32) per = 32;
     cls_cg0[c] = (int)bh.cgs.size();
     int ngc = 0;
     for (int b0 = 0; b0 < B; b0 += per, ++ngc) {
@@ -200,6 +200,22 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
       P.t.up_u = at(P.J, P.K, P.sg - 1);
       P.t.up_v = at(P.J - 1, P.K, P.sg);
       P.t.up_w = at(P.J, P.K - 1, P.sg);
+      // face modes: TAGGED if every upstream cell across the face is active (then every row of the face is the upstream
+      // task's), COUNTER if the face mixes task rows and closure rows
+      auto face_mode = [&](int up, bool vface) {
+        if (up < 0) return (int32_t)BRK_FACE_BOUNDARY;
+        const int n2 = vface ? P.t.tw : P.t.tv;
+        for (int ul = 0; ul < P.t.nu; ++ul)
+          for (int k = 0; k < n2; ++k) {
+            const int upp = uc[P.sg] + ul, vp = vface ? vc[P.J] - 1 : vc[P.J] + k, wp = vface ? wc[P.K] + k : wc[P.K] - 1;
+            if (!actp(upp, vp, wp)) return (int32_t)BRK_FACE_COUNTER;
+          }
+        return (int32_t)BRK_FACE_TAGGED;
+      };
+      P.t.fv_mode = face_mode(P.t.up_v, true);
+      P.t.fw_mode = face_mode(P.t.up_w, false);
+      if (P.t.fv_mode == BRK_FACE_COUNTER) protos[P.t.up_v].t.publish = 1;
+      if (P.t.fw_mode == BRK_FACE_COUNTER) protos[P.t.up_w].t.publish = 1;
       const int du = at(P.J, P.K, P.sg + 1), dv = at(P.J + 1, P.K, P.sg), dw = at(P.J, P.K + 1, P.sg);
       P.t.dn_fu0 = du >= 0 ? protos[du].t.fu0 : -1;
       P.t.dn_fv0 = dv >= 0 ? protos[dv].t.fv0 : -1;

@@ -168,9 +168,11 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
 
   // ---- which sweep: the tile-dataflow sweep with fused moments (brick.h) on uniform 3-D grids unless the caller asks for a
   // launch shape of the hyperplane kernels (sweep_G / sweep_threads / sweep_variant 3, 4) -------------------------------------
-  const bool brick_ok = dim == 3 && uniform;
+  size_t brick_max_dirs = 0;
+  for (const OctHost &o : oct) brick_max_dirs = std::max(brick_max_dirs, o.dirs.size());
+  const bool brick_ok = dim == 3 && uniform && brick_max_dirs <= 16;
   if (opt->sweep_variant == 5 && !brick_ok)
-    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "the tile-dataflow sweep (sweep_variant 5) needs a 3-D grid with uniform spacing");
+    return nb_fail(h, NANOBTE_E_UNSUPPORTED, "the tile-dataflow sweep (sweep_variant 5) needs a 3-D grid with uniform spacing and at most 16 directions per octant");
   const bool use_brick = brick_ok && (opt->sweep_variant == 5 || (opt->sweep_variant == 0 && opt->sweep_G == 0 && opt->sweep_threads == 0 &&
                                                                   std::getenv("NANOBTE_NO_BRICK") == nullptr));
 

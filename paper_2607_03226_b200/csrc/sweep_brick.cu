@@ -42,7 +42,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 struct Upstream {
   const unsigned int *pv, *pw;  // progress words (nullptr: no upstream task -- boundary rows, always there)
   unsigned int seen_v, seen_w;
-  __device__ __forceinline__ void init(const unsigned int *prog, int up_v, int up_w) {
+  __device__ __forceinline__ void init(const unsigned int *prog, int up_v, int up_w) {  // < 0: nothing to wait for
     pv = up_v >= 0 ? prog + up_v : nullptr;
     pw = up_w >= 0 ? prog + up_w : nullptr;
     seen_v = pv ? 0u : 0x7fffffffu;
@@ -74,6 +74,27 @@ __device__ __forceinline__ void wait_progress(const unsigned int *prog, int up, 
 
 constexpr int kP = kBrickPitch;
 
+// A value that crosses a tile face: its least significant mantissa bit is the sweep parity (brick.h, BRK_FACE_TAGGED).
+__device__ __forceinline__ double tag(double x, unsigned par) {
+  return __hiloint2double(__double2hiint(x), (int)(((unsigned)__double2loint(x) & ~1u) | par));
+}
+// Face rows are read at the L2 (the point of coherence), and every time the code says so (the settle loop re-reads them).
+__device__ __forceinline__ double ld_face(const double *p) {
+  double v;
+  asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ unsigned stale_bit(double x, unsigned par) { return ((unsigned)__double2loint(x) ^ par) & 1u; }
+
+#ifdef BRICK_PROF
+__device__ unsigned long long g_brick_prof[16];
+#define PROF_T(var) const long long var = clock64()
+#define PROF_ADD(k, a, b) if (t == 0) prof[k] += (unsigned long long)((b) - (a))
+#else
+#define PROF_T(var)
+#define PROF_ADD(k, a, b)
+#endif
+
 struct BrickSmem {
   double plane[kBrickCells * kBrickPitch];     // [cell][system]: eps of the previous u-plane (u-upwind values)
   double red[3][5][kBrickCells];               // band partials of warps 0..2 (moments)
@@ -96,7 +117,7 @@ struct Sys {           // what a substitution thread keeps for its system
 template <int TV>
 __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const double *__restrict__ th, const double *__restrict__ qd,
                                             const Sys &c, const int tw, const bool src, double (&ew)[kBrickTile],
-                                            const double (&inv)[kBrickTile], double *dn_fv_u, double *eout_u) {
+                                            const double (&inv)[kBrickTile], double *dn_fv_u, double *eout_u, const unsigned par) {
 #pragma unroll
   for (int w = 0; w < kBrickTile; ++w) {
     if (w < tw) {
@@ -127,7 +148,7 @@ __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const doubl
         ew[v] = ev;
         row[v * kP] = ev;
       }
-      if (dn_fv_u) dn_fv_u[w * kBrickRow] = ev;
+      if (dn_fv_u) dn_fv_u[w * kBrickRow] = tag(ev, par);
       if (eout_u) {
 #pragma unroll
         for (int v = 0; v < TV; ++v) __stcs(eout_u + (w * kBrickTile + v) * kBrickRow, ew[v]);
@@ -142,7 +163,8 @@ __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const doubl
 // has work of its own during the 8-cycle DFMA latency of the v-chain.
 template <int TV>
 __device__ __forceinline__ void fast_plane(double *__restrict__ pl, const double *__restrict__ th, const Sys &c,
-                                           double (&ew)[kBrickTile], const double (&inv)[kBrickTile], double *__restrict__ dn_fv_u) {
+                                           double (&ew)[kBrickTile], const double (&inv)[kBrickTile], double *__restrict__ dn_fv_u,
+                                           const unsigned par) {
   double rp[TV], rn[TV];
   {
     double eu[TV];
@@ -177,9 +199,47 @@ __device__ __forceinline__ void fast_plane(double *__restrict__ pl, const double
       row[v * kP] = ev;
       if (w + 1 < kBrickTile) rn[v] = fma(c.c_u, eu[v], c.k_th * tn[v]);
     }
-    dn_fv_u[w * kBrickRow] = ev;
+    dn_fv_u[w * kBrickRow] = tag(ev, par);
 #pragma unroll
     for (int v = 0; v < TV; ++v) rp[v] = rn[v];
+  }
+}
+
+// ---- moments of one u-plane, one thread: cells (lane, lane + 32), ND consecutive directions, all bands --------------------------------
+// The band sums come first (three weights: 1/tau_b, 1, v_b -- 3 fp64 operations per value), the direction weights once per
+// plane:  m0 = sum_d w_d sum_b eps/tau_b,  m1 = sum_d w_d sum_b eps,  m2..4 = sum_d w_d s_d sum_b v_b eps.
+// row = plane buffer + cell * pitch + first direction; bcoef = [nb][2] (1/tau, v); dcoef = [ND][4] (w, w sx, w sy, w sz).
+template <int ND>
+__device__ __forceinline__ void moments_dirs(const double *__restrict__ row, const double *__restrict__ bcoef,
+                                             const double *__restrict__ dcoef, const int nb, const int nd, double (&m)[2][5]) {
+  double A[ND][2], Bs[ND][2], Cv[ND][2];
+#pragma unroll
+  for (int j = 0; j < ND; ++j) A[j][0] = A[j][1] = Bs[j][0] = Bs[j][1] = Cv[j][0] = Cv[j][1] = 0.0;
+#pragma unroll 2
+  for (int b = 0; b < nb; ++b) {
+    const double2 bc = *reinterpret_cast<const double2 *>(bcoef + 2 * b);
+#pragma unroll
+    for (int j = 0; j < ND; ++j) {
+      const double e0 = row[j], e1 = row[j + 32 * kP];
+      A[j][0] = fma(bc.x, e0, A[j][0]); Bs[j][0] += e0; Cv[j][0] = fma(bc.y, e0, Cv[j][0]);
+      A[j][1] = fma(bc.x, e1, A[j][1]); Bs[j][1] += e1; Cv[j][1] = fma(bc.y, e1, Cv[j][1]);
+    }
+    row += nd;
+  }
+#pragma unroll
+  for (int k = 0; k < 5; ++k) m[0][k] = m[1][k] = 0.0;
+#pragma unroll
+  for (int j = 0; j < ND; ++j) {
+    const double2 c01 = *reinterpret_cast<const double2 *>(dcoef + 4 * j);
+    const double2 c23 = *reinterpret_cast<const double2 *>(dcoef + 4 * j + 2);
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      m[q][0] = fma(c01.x, A[j][q], m[q][0]);
+      m[q][1] = fma(c01.x, Bs[j][q], m[q][1]);
+      m[q][2] = fma(c01.y, Cv[j][q], m[q][2]);
+      m[q][3] = fma(c23.x, Cv[j][q], m[q][3]);
+      m[q][4] = fma(c23.y, Cv[j][q], m[q][4]);
+    }
   }
 }
 
@@ -238,30 +298,54 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
       for (int cc = 0; cc < kBrickCells; ++cc) sm.plane[cc * kP + s] = __ldcg(fu + cc * kBrickRow);
     }
     // v- and w-face inflow of plane 0
-    Upstream ups;
-    ups.init(a.prog, T.up_v, T.up_w);
+    const unsigned par = a.parity;
+    Upstream ups;  // only the faces that mix task rows and closure rows are followed through counters
+    ups.init(a.prog, T.fv_mode == BRK_FACE_COUNTER ? T.up_v : -1, T.fw_mode == BRK_FACE_COUNTER ? T.up_w : -1);
+    const bool counters = T.fv_mode == BRK_FACE_COUNTER || T.fw_mode == BRK_FACE_COUNTER;
+    const int chk_v = T.fv_mode == BRK_FACE_TAGGED ? T.tw : 0, chk_w = T.fw_mode == BRK_FACE_TAGGED ? T.tv : 0;
     double ew[kBrickTile], inv[kBrickTile];
     auto load_faces = [&]() {  // fv / fw point at the rows of the plane to come
 #pragma unroll
       for (int k = 0; k < kBrickTile; ++k) {
-        inv[k] = on ? __ldcg(fv + k * kBrickRow) : 0.0;
-        ew[k] = on ? __ldcg(fw + k * kBrickRow) : 0.0;
+        inv[k] = on ? ld_face(fv + k * kBrickRow) : 0.0;
+        ew[k] = on ? ld_face(fw + k * kBrickRow) : 0.0;
+      }
+    };
+    // tagged faces: rows that still carry the other parity are last sweep's -- load again until the upstream tile has
+    // written them (every thread follows its own system; nobody else's values are involved)
+    auto settle_faces = [&]() {
+      if (on && (chk_v | chk_w)) {
+        for (;;) {
+          unsigned bad = 0;
+#pragma unroll
+          for (int k = 0; k < kBrickTile; ++k) {
+            if (k < chk_v) bad |= stale_bit(inv[k], par);
+            if (k < chk_w) bad |= stale_bit(ew[k], par);
+          }
+          if (!bad) break;
+          __nanosleep(20);
+          load_faces();
+        }
       }
       fv += kBrickTile * kBrickRow;
       fw += kBrickTile * kBrickRow;
     };
-    ups.wait(1u);
+    if (counters) ups.wait(1u);
     load_faces();
+    settle_faces();
     cp_async_wait_all();
     __syncthreads();
 
-    // The warp's share of the moment work in half-band units (a band's directions split in two): whole bands except where
-    // a share boundary falls inside a band.  Equal shares whatever the band count.
-    const int h_lo = (2 * G.nb * wid) >> 2, h_hi = (2 * G.nb * (wid + 1)) >> 2;
-    const int nd = G.nd, nd_half = nd >> 1;
+    // The warp's share of the moment work: a quarter of the class's directions (at most 4: nd <= 16), all bands.
+    const int nd = G.nd;
+    const int dw0 = (nd * wid) >> 2, dw1 = (nd * (wid + 1)) >> 2;
 
+#ifdef BRICK_PROF
+    unsigned long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
     int ip = 0;  // next row of the IRR stream (same value in every thread)
     for (int u = 0; u < T.nu; ++u) {
+      PROF_T(p0);
       const int st = u & 1;
       const bool last_u = u + 1 == T.nu;
       // ------------------------------------------ substitution: thread = system ------------------------------------------
@@ -272,25 +356,25 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
           if (!src && !eout) {
             double *dfv = dn_fv ? dn_fv : scratch;
             switch (T.tv) {
-              case 8: fast_plane<8>(pl, sm.th, c, ew, inv, dfv); break;
-              case 7: fast_plane<7>(pl, sm.th, c, ew, inv, dfv); break;
-              case 6: fast_plane<6>(pl, sm.th, c, ew, inv, dfv); break;
-              case 5: fast_plane<5>(pl, sm.th, c, ew, inv, dfv); break;
-              default: fast_plane<4>(pl, sm.th, c, ew, inv, dfv); break;
+              case 8: fast_plane<8>(pl, sm.th, c, ew, inv, dfv, par); break;
+              case 7: fast_plane<7>(pl, sm.th, c, ew, inv, dfv, par); break;
+              case 6: fast_plane<6>(pl, sm.th, c, ew, inv, dfv, par); break;
+              case 5: fast_plane<5>(pl, sm.th, c, ew, inv, dfv, par); break;
+              default: fast_plane<4>(pl, sm.th, c, ew, inv, dfv, par); break;
             }
           } else
           switch (T.tv) {
-            case 8: plain_plane<8>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
-            case 7: plain_plane<7>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
-            case 6: plain_plane<6>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
-            case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
-            default: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout); break;
+            case 8: plain_plane<8>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
+            case 7: plain_plane<7>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
+            case 6: plain_plane<6>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
+            case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
+            default: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
           }
           if (dn_fw) {  // the last row of the tile, out of the plane buffer (the thread's own stores)
             const double *lrow = pl + (T.tw - 1) * kBrickTile * kP;
 #pragma unroll
             for (int v = 0; v < kBrickTile; ++v)
-              if (v < T.tv) dn_fw[v * kBrickRow] = lrow[v * kP];
+              if (v < T.tv) dn_fw[v * kBrickRow] = tag(lrow[v * kP], par);
           }
         } else {
           // ---- per-cell path: holes and walls inside the tile (wall values straight from L2) ----------------------------------
@@ -320,8 +404,8 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
                 pl[cell * kP] = e;
                 ev = e;
                 ewv = e;
-                if (v + 1 == T.tv && dn_fv) dn_fv[w * kBrickRow] = e;
-                if (w + 1 == T.tw && dn_fw) dn_fw[v * kBrickRow] = e;
+                if (v + 1 == T.tv && dn_fv) dn_fv[w * kBrickRow] = tag(e, par);
+                if (w + 1 == T.tw && dn_fw) dn_fw[v * kBrickRow] = tag(e, par);
                 if (eout) __stcs(eout + cell * kBrickRow, e);
               }
 #pragma unroll
@@ -333,15 +417,17 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         if (dn_fw) dn_fw += kBrickTile * kBrickRow;
         if (eout) eout += kBrickCells * kBrickRow;
       }
+      PROF_T(p1);
       __syncthreads();  // B1: plane u is complete in the plane buffer; theta / Qdot of plane u are dead
+      PROF_T(p2);
       bool early = false;
       if (!last_u) {
         stage(u + 1);
-        // publish: the barrier orders every store of the CTA before this release (cumulativity)
-        if (t == 0) st_release(a.prog + task, (unsigned)(u + 1));
-        // next plane's tile-face inflow: issued before the reduction if the upstream tiles are already there (the loads
-        // then fly during the reduction), otherwise after it
-        early = ups.poll((unsigned)(u + 2));
+        // counter protocol only: the barrier orders every store of the CTA before this release (cumulativity)
+        if (T.publish && t == 0) st_release(a.prog + task, (unsigned)(u + 1));
+        // next plane's tile-face inflow: the loads fly during the reduction (counter faces: only if the upstream tile is
+        // already there, otherwise after the reduction)
+        early = !counters || ups.poll((unsigned)(u + 2));
         if (early) load_faces();
       }
       // ---- out of the plane buffer (thread = system): eps of the cells with an outgoing wall (closures), the u-face of the
@@ -368,32 +454,20 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
             if ((frow >> (8 * v)) & BRK_ACT) dn_fu[(w * kBrickTile + v) * kBrickRow] = sm.plane[(w * kBrickTile + v) * kP + s];
         }
       }
-      // ------------------------------------------ moments: thread = cells (lane, lane + 32) x the warp's share of bands ----
+      PROF_T(p3);
+      // ------------------------------------------ moments: thread = cells (lane, lane + 32) x the warp's directions -------
       {
         const unsigned char *fb = reinterpret_cast<const unsigned char *>(sm.flg[st]);
         const bool act0 = (fb[lane] & BRK_ACT) != 0, act1 = (fb[lane + 32] & BRK_ACT) != 0;
-        const double *row0 = sm.plane + lane * kP;
-        double m[2][5] = {{0, 0, 0, 0, 0}, {0, 0, 0, 0, 0}};
-        for (int hh = h_lo; hh < h_hi;) {
-          const int b = hh >> 1;
-          const int d_lo = (hh & 1) ? nd_half : 0;
-          const int d_hi = (hh + 1 < h_hi || (hh & 1)) ? nd : nd_half;   // the whole band unless the share ends inside it
-          hh = 2 * b + (d_hi == nd ? 2 : 1);
-          double E0 = 0.0, X0 = 0.0, Y0 = 0.0, Z0 = 0.0, E1 = 0.0, X1 = 0.0, Y1 = 0.0, Z1 = 0.0;
-          const double *r0 = row0 + b * nd;
-#pragma unroll 4
-          for (int d = d_lo; d < d_hi; ++d) {
-            const double e0 = r0[d], e1 = r0[d + 32 * kP];
-            const double2 c01 = *reinterpret_cast<const double2 *>(sm.dcoef + 4 * d);
-            const double2 c23 = *reinterpret_cast<const double2 *>(sm.dcoef + 4 * d + 2);
-            E0 = fma(c01.x, e0, E0); X0 = fma(c01.y, e0, X0); Y0 = fma(c23.x, e0, Y0); Z0 = fma(c23.y, e0, Z0);
-            E1 = fma(c01.x, e1, E1); X1 = fma(c01.y, e1, X1); Y1 = fma(c23.x, e1, Y1); Z1 = fma(c23.y, e1, Z1);
-          }
-          const double2 bc = *reinterpret_cast<const double2 *>(sm.bcoef + 2 * b);
-          m[0][0] = fma(bc.x, E0, m[0][0]); m[0][1] += E0;
-          m[0][2] = fma(bc.y, X0, m[0][2]); m[0][3] = fma(bc.y, Y0, m[0][3]); m[0][4] = fma(bc.y, Z0, m[0][4]);
-          m[1][0] = fma(bc.x, E1, m[1][0]); m[1][1] += E1;
-          m[1][2] = fma(bc.y, X1, m[1][2]); m[1][3] = fma(bc.y, Y1, m[1][3]); m[1][4] = fma(bc.y, Z1, m[1][4]);
+        double m[2][5];
+        switch (dw1 - dw0) {
+          case 4: moments_dirs<4>(sm.plane + lane * kP + dw0, sm.bcoef, sm.dcoef + 4 * dw0, G.nb, nd, m); break;
+          case 3: moments_dirs<3>(sm.plane + lane * kP + dw0, sm.bcoef, sm.dcoef + 4 * dw0, G.nb, nd, m); break;
+          case 2: moments_dirs<2>(sm.plane + lane * kP + dw0, sm.bcoef, sm.dcoef + 4 * dw0, G.nb, nd, m); break;
+          case 1: moments_dirs<1>(sm.plane + lane * kP + dw0, sm.bcoef, sm.dcoef + 4 * dw0, G.nb, nd, m); break;
+          default:
+#pragma unroll
+            for (int k = 0; k < 5; ++k) m[0][k] = m[1][k] = 0.0;
         }
         if (wid < 3) {
 #pragma unroll
@@ -402,12 +476,23 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
             sm.red[wid][k][lane + 32] = m[1][k];
           }
         }
-        if (!last_u && !early) {
-          ups.wait((unsigned)(u + 2));
-          load_faces();
+        PROF_T(p4);
+        if (!last_u) {
+          if (!early) {
+            ups.wait((unsigned)(u + 2));
+            load_faces();
+          }
+          settle_faces();
         }
+        PROF_T(p5);
         cp_async_wait_all();
         __syncthreads();  // B2: the plane buffer is free again; the band partials are in place; theta of plane u+1 has landed
+        PROF_T(p6);
+        PROF_ADD(0, p0, p1); PROF_ADD(1, p1, p2); PROF_ADD(2, p2, p3); PROF_ADD(3, p3, p4); PROF_ADD(4, p4, p5); PROF_ADD(5, p5, p6);
+#ifdef BRICK_PROF
+        if (t == 0) prof[6] += 1;
+        if (t == 0 && early) prof[7] += 1;
+#endif
         if (last_u && t == 0) st_release(a.prog + task, 0x7fffffffu);
         if (wid == 3) {  // fixed order: warp 0 + warp 1 + warp 2 + warp 3
           double *p = part + (int64_t)u * kBrickCells + lane;
@@ -421,6 +506,10 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         }
       }
     }
+#ifdef BRICK_PROF
+    if (t == 0)
+      for (int k = 0; k < 8; ++k) atomicAdd(&g_brick_prof[k], prof[k]);
+#endif
   }
 }
 
@@ -430,6 +519,8 @@ int nb_launch_sweep_brick(nanobte_solver *h, int store_e) {
   BrickState &bs = *h->brick;
   BrickArgs a = bs.a;
   a.store_e = store_e;
+  bs.parity ^= 1u;
+  a.parity = bs.parity;
   NB_CUDA(h, cudaMemsetAsync(a.ticket, 0, sizeof(unsigned int) * (size_t)(a.n_tasks + 1), h->stream));  // ticket + progress
   NB_CUDA(h, cudaFuncSetAttribute(sweep_brick_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BrickSmem)));
   sweep_brick_kernel<<<bs.grid, kBrickMaxS, sizeof(BrickSmem), h->stream>>>(a);
@@ -440,3 +531,12 @@ int nb_launch_sweep_brick(nanobte_solver *h, int store_e) {
 }
 
 size_t nb_brick_smem_bytes() { return sizeof(BrickSmem); }
+
+#ifdef BRICK_PROF
+extern "C" int nanobte_debug_brick_prof(unsigned long long *out, int reset) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, g_brick_prof, sizeof(unsigned long long) * 16);
+  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_brick_prof, z, sizeof(z)); }
+  return 0;
+}
+#endif
