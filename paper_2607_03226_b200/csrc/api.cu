@@ -5,6 +5,7 @@
 #include <cstdlib>
 
 #include "brick.h"
+#include "cg_mg.h"
 #include "host_util.h"
 
 int nb_fail(nanobte_solver *h, int code, const char *fmt, ...) {
@@ -323,6 +324,15 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
     h->cgf_xprev = A.zeros<double>(2 * na);
     h->cgf_gpart = A.zeros<double>((size_t)8 * nblk + 8);
     h->cgf_recycle = std::getenv("NANOBTE_CG_NO_RECYCLE") == nullptr;
+    // uniform 3-D structured grids: multigrid-preconditioned CG (cg_mg.cu) unless a test hook asks for a plain-CG kernel
+    if (uni && nf == 6 && c.dim == 3 && g.cg_grid[0] > 0 && !h->cg_force_generic && std::getenv("NANOBTE_CG_NO_MG") == nullptr &&
+        std::getenv("NANOBTE_CG_NO_UNI") == nullptr && std::getenv("NANOBTE_CG_NO_RECYCLE") == nullptr) {
+      // the coefficients in the order of the faces, before the CG renumbering
+      double cfu0[6] = {0, 0, 0, 0, 0, 0};
+      for (int f = 0; f < 6; ++f) cfu0[f] = cfu[f];
+      const int rc_mg = nb_mg_build(h, A, g, cfu0, g.cg_grid);
+      if (rc_mg < 0) return rc_mg;
+    }
   }
   h->tagface_ptr = A.put(g.tagface_ptr);
   h->tagface = A.put(g.tagface);
@@ -336,6 +346,7 @@ extern "C" void nanobte_destroy(nanobte_solver *h) {
   if (h->stream || h->arena) cudaStreamSynchronize(h->stream);
   nb_free_unstructured(h);
   nb_free_brick(h);
+  nb_free_mg(h);
   if (h->arena && h->arena_owned) cudaFree(h->arena);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;

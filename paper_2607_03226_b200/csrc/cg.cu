@@ -9,6 +9,7 @@
 //   CG from delta = 0, stop at ||r||^2 <= rtol^2 ||rhs||^2                               (R14e)
 #include <cooperative_groups.h>
 
+#include "cg_mg.h"
 #include "internal.h"
 namespace cg = cooperative_groups;
 
@@ -509,6 +510,7 @@ int nb_cg_blocks(nanobte_solver *h) {
 
 int nb_cg_solve(nanobte_solver *h, int *iters) {
   if (iters) *iters = -1;  // read back by the caller together with max|dT|
+  if (h->mg && !h->cg_force_generic) return nb_mg_solve(h);
   if (h->cgf_ok && !h->cg_force_generic) return cg_solve_fused(h);
   CgArgs a;
   a.n = h->n_act; a.nf = h->cg_nf; a.max_iter = h->cg_max_iter; a.B = h->B;

@@ -81,6 +81,7 @@ struct GenericTables {
   std::vector<double> cg_coef, cg_diag;
   std::vector<int32_t> cellbf_ptr, cellbf;
   std::vector<double> cg_xyz;      // [n][3] cell centres in any consistent unit (partitioning of the CG only)
+  int cg_grid[3] = {0, 0, 0};      // structured grids: lattice dimensions, cg_xyz holds the integer lattice coordinates
   std::vector<int32_t> tagface_ptr, tagface;
   int64_t bin_total = 0;
 };

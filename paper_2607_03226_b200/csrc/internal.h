@@ -98,6 +98,8 @@ struct nanobte_solver {
 
   // tile-dataflow sweep with fused moments (brick.h); non-null = this path is the solver's sweep
   struct BrickState *brick = nullptr;
+  // multigrid-preconditioned CG (cg_mg.h); non-null = the synthetic correction uses it
+  struct MgPlan *mg = nullptr;
   bool keep_e = true;  // nanobte_sweep stores the distribution (nanobte_set_keep_e)
 
   // unstructured sweep (see sweep_unstructured.cu)

@@ -422,6 +422,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   G.vol.resize(na); G.Qdot_act.resize(na); G.theta0.resize(na);
   G.cg_nf = nside;
   G.cg_xyz.assign((size_t)3 * na, 0.0);
+  for (int k = 0; k < 3; ++k) G.cg_grid[k] = g.n[k];
   G.cg_nbr.assign((size_t)nside * na, 0);
   G.cg_coef.assign((size_t)nside * na, 0.0);
   G.cg_diag.assign(na, 0.0);
