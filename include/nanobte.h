@@ -150,6 +150,9 @@ typedef struct {
   int32_t cg_face_uniform;      /* fused kernel: face-uniform stencil (uniform structured grids)   */
   int32_t cg_recycle;           /* fused kernel: recycled initial guess on                         */
   int32_t sweep_variant;        /* 3 / 4: hyperplane kernels, 5: tile-dataflow sweep with fused moments, 1: unstructured level sweep */
+  int32_t cg_multigrid;         /* 1: nanobte_diffusion_correct runs the multigrid-preconditioned CG (uniform 3-D structured
+                                   grids; cg_mg.cu); the cg_* fields above then describe the plain-CG plan kept as fallback */
+  int32_t cg_mg_levels;         /* levels of its hierarchy (0 without it)                                             */
 } nanobte_info;
 
 /* Bytes of device workspace create_* would need for this problem (same validation as create). */

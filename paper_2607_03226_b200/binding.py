@@ -67,7 +67,8 @@ class Info(C.Structure):
                 ("sweep_rmax", C.c_int32), ("pencil_axis", C.c_int32), ("n_pos", C.c_int64), ("n_inflow", C.c_int64),
                 ("device_bytes", C.c_size_t), ("sweep_smem_bytes", C.c_size_t), ("cg_fused", C.c_int32),
                 ("cg_cells_per_thread", C.c_int32), ("cg_ctas", C.c_int32), ("cg_face_uniform", C.c_int32),
-                ("cg_recycle", C.c_int32), ("sweep_variant", C.c_int32)]
+                ("cg_recycle", C.c_int32), ("sweep_variant", C.c_int32), ("cg_multigrid", C.c_int32),
+                ("cg_mg_levels", C.c_int32)]
 
 
 class NanoBTEError(RuntimeError):

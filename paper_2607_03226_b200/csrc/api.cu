@@ -569,6 +569,8 @@ extern "C" int nanobte_get_info(const nanobte_solver *h, nanobte_info *o) {
   const bool fused = h->cgf_ok && !h->cg_force_generic;
   o->cg_fused = fused; o->cg_cells_per_thread = fused ? h->cgf_cpt : 0; o->cg_ctas = fused ? h->cgf_nblk : h->cg_blocks;
   o->cg_face_uniform = fused && h->cgf_uni; o->cg_recycle = fused && h->cgf_recycle;
+  o->cg_multigrid = h->mg && !h->cg_force_generic ? 1 : 0;
+  o->cg_mg_levels = o->cg_multigrid ? h->mg->levels : 0;
   o->sweep_variant = h->kind == 1 ? 1 : h->sweep_variant;
   return 0;
 }

@@ -110,6 +110,7 @@ struct BrickState {
   const int32_t *dir_local = nullptr;                  // [D] index of a direction inside its class
   const int32_t *cg_of = nullptr;                      // [n_cls][B] (class, band) -> cg
   const int32_t *a2pos = nullptr;                      // [n_cls][n_act]
+  const int32_t *pos2a = nullptr;                      // [npos of class 0]
   double *th[NB_MAX_CLASSES] = {nullptr};
 };
 

@@ -95,6 +95,8 @@ struct BrickUpdateArgs {
   const double *part;
   int32_t npos[NB_MAX_CLASSES];
   const int32_t *a2pos;  // [n_cls][n_act]
+  const int32_t *pos2a;  // [npos[0]] cell at a position of class 0 (-1: none): threads follow the positions, so that the loads of
+                         // the partial moments are coalesced (the tiles are the same lattice in every class)
   double *th[NB_MAX_CLASSES];
   double *theta, *theta_prev, *theta_SI, *theta_en, *q;
   const double *x;
@@ -104,9 +106,10 @@ struct BrickUpdateArgs {
 
 __global__ void __launch_bounds__(256) brick_update_kernel(const BrickUpdateArgs u) {
   __shared__ double red[8];
-  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p0 = blockIdx.x * blockDim.x + threadIdx.x;
+  const int a = p0 < u.npos[0] ? u.pos2a[p0] : -1;
   double d = 0.0;
-  if (a < u.n_act) {
+  if (a >= 0) {
     double th;
     if (u.mode == 0) {
       double m[5] = {0, 0, 0, 0, 0};
@@ -171,7 +174,7 @@ __global__ void brick_get_e_kernel(const BrickGetEArgs g) {
     const int cls = g.dir_cls[d];
     const BrickCG G = g.cgs[g.cg_of[cls * g.B + b]];
     const int64_t pos = g.a2pos[(size_t)cls * g.n_act + a];
-    val = g.e[G.e_base + pos * kBrickRow + (b - G.b0) * G.nd + g.dir_local[d]] + g.C[b] * g.off_scale;
+    val = g.e[G.e_base + pos * G.S + (b - G.b0) * G.nd + g.dir_local[d]] + g.C[b] * g.off_scale;
   }
   g.dst[((size_t)bi * g.nd + di) * g.n_cells + c] = val;
 }
@@ -223,6 +226,7 @@ BrickUpdateArgs update_args(nanobte_solver *h, int mode) {
   u.n_act = h->n_act; u.n_cls = h->n_cls; u.n_cg = bs.n_cg; u.mode = mode; u.cgs = bs.a.cgs; u.part = bs.a.part;
   for (int c = 0; c < NB_MAX_CLASSES; ++c) { u.npos[c] = bs.a.npos[c]; u.th[c] = bs.th[c]; }
   u.a2pos = bs.a2pos;
+  u.pos2a = bs.pos2a;
   u.theta = h->theta; u.theta_prev = h->theta_prev; u.theta_SI = h->theta_SI; u.theta_en = h->theta_en; u.q = h->q;
   u.x = h->cg_x; u.beta = h->beta; u.Csum = h->Csum; u.maxdT = h->d_maxdT;
   return u;
@@ -250,7 +254,7 @@ int nb_brick_refresh_thermalizing(nanobte_solver *h) {
 
 int nb_brick_update(nanobte_solver *h, int mode) {
   BrickUpdateArgs u = update_args(h, mode);
-  brick_update_kernel<<<(h->n_act + 255) / 256, 256, 0, h->stream>>>(u);
+  brick_update_kernel<<<(u.npos[0] + 255) / 256, 256, 0, h->stream>>>(u);
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
   return 0;

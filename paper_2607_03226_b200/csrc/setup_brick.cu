@@ -276,7 +276,7 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
     g.inf_base = inf; inf = pad(inf + (int64_t)C.nrow * kBrickRow);
     g.wall_base = wall; wall = pad(wall + (int64_t)C.nwall * kBrickRow);
     g.part_base = part; part = pad(part + (int64_t)5 * C.npos);
-    g.e_base = e; e = pad(e + (int64_t)C.npos * kBrickRow);
+    g.e_base = e; e = pad(e + (int64_t)C.npos * g.S);  // the stored distribution: pitch S (it is the big array)
     g.coef_base = cf;
     for (int bl = 0; bl < g.nb; ++bl)
       for (int dl = 0; dl < g.nd; ++dl) {
@@ -335,6 +335,12 @@ int nb_brick_upload(nanobte_solver *h, Arena &A, BrickHost &bh) {
   bs.dir_local = A.put(bh.dir_local);
   bs.cg_of = A.put(bh.cg_of);
   bs.a2pos = A.put(bh.a2pos);
+  {
+    const int na = (int)(bh.a2pos.size() / bh.ncls);
+    std::vector<int32_t> pos2a((size_t)bh.cls[0].npos + 64, -1);
+    for (int a = 0; a < na; ++a) pos2a[bh.a2pos[a]] = a;
+    bs.pos2a = A.put(pos2a);
+  }
   bs.bf_nord = A.put(bh.bf_nord);
   bs.n_cg = (int)bh.cgs.size();
   bs.smem = nb_brick_smem_bytes();

@@ -113,11 +113,12 @@ struct Sys {           // what a substitution thread keeps for its system
 
 // ---- one u-plane of a fully active box, TV cells per row: straight-line code ---------------------------------------------------------
 // pl = plane buffer + system; ew[v] = w-upwind values (in: tile-face inflow, out: last row); inv[w] = v-face inflow of row w;
-// dn_fv_u / eout_u = this plane's rows of the v-downstream tile / of the stored distribution (nullptr: none).
+// dn_fv_u / eout_u = this plane's rows of the v-downstream tile / of the stored distribution (pitch S; nullptr: none).
 template <int TV>
 __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const double *__restrict__ th, const double *__restrict__ qd,
                                             const Sys &c, const int tw, const bool src, double (&ew)[kBrickTile],
-                                            const double (&inv)[kBrickTile], double *dn_fv_u, double *eout_u, const unsigned par) {
+                                            const double (&inv)[kBrickTile], double *dn_fv_u, double *eout_u, const int S,
+                                            const unsigned par) {
 #pragma unroll
   for (int w = 0; w < kBrickTile; ++w) {
     if (w < tw) {
@@ -151,7 +152,7 @@ __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const doubl
       if (dn_fv_u) dn_fv_u[w * kBrickRow] = tag(ev, par);
       if (eout_u) {
 #pragma unroll
-        for (int v = 0; v < TV; ++v) __stcs(eout_u + (w * kBrickTile + v) * kBrickRow, ew[v]);
+        for (int v = 0; v < TV; ++v) __stcs(eout_u + (w * kBrickTile + v) * S, ew[v]);
       }
     }
   }
@@ -265,7 +266,7 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     double *wall = a.wall + G.wall_base + (int64_t)T.wo0 * kBrickRow + s;
     double *part = a.part + G.part_base + T.pos0;
     const int64_t npos = a.npos[G.cls];
-    double *eout = a.store_e ? a.e + G.e_base + (int64_t)T.pos0 * kBrickRow + s : nullptr;
+    double *eout = a.store_e ? a.e + G.e_base + (int64_t)T.pos0 * S + s : nullptr;  // pitch S
     const double *irr = inf + (int64_t)T.ir0 * kBrickRow;
     const double *fv = inf + (int64_t)T.fv0 * kBrickRow, *fw = inf + (int64_t)T.fw0 * kBrickRow;
     double *dn_fu = T.dn_fu0 >= 0 ? inf + (int64_t)T.dn_fu0 * kBrickRow : nullptr;
@@ -364,11 +365,11 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
             }
           } else
           switch (T.tv) {
-            case 8: plain_plane<8>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
-            case 7: plain_plane<7>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
-            case 6: plain_plane<6>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
-            case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
-            default: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, par); break;
+            case 8: plain_plane<8>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, S, par); break;
+            case 7: plain_plane<7>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, S, par); break;
+            case 6: plain_plane<6>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, S, par); break;
+            case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, S, par); break;
+            default: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, S, par); break;
           }
           if (dn_fw) {  // the last row of the tile, out of the plane buffer (the thread's own stores)
             const double *lrow = pl + (T.tw - 1) * kBrickTile * kP;
@@ -406,7 +407,7 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
                 ewv = e;
                 if (v + 1 == T.tv && dn_fv) dn_fv[w * kBrickRow] = tag(e, par);
                 if (w + 1 == T.tw && dn_fw) dn_fw[v * kBrickRow] = tag(e, par);
-                if (eout) __stcs(eout + cell * kBrickRow, e);
+                if (eout) __stcs(eout + cell * S, e);
               }
 #pragma unroll
               for (int k = 0; k < kBrickTile; ++k) ew[k] = k == v ? ewv : ew[k];
@@ -415,7 +416,7 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         }
         if (dn_fv) dn_fv += kBrickTile * kBrickRow;
         if (dn_fw) dn_fw += kBrickTile * kBrickRow;
-        if (eout) eout += kBrickCells * kBrickRow;
+        if (eout) eout += kBrickCells * S;
       }
       PROF_T(p1);
       __syncthreads();  // B1: plane u is complete in the plane buffer; theta / Qdot of plane u are dead

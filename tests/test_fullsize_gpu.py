@@ -142,21 +142,27 @@ FULLMESH = {
     "finfet_96x48x48": (lambda: wl.config_finfet(nx=96, ny=48, nz=48, B=2, n_polar=2, n_azim=8), "synthetic", 2),
     "cube_72": (lambda: wl.config_cube(n=72, B=2, n_polar=2, n_azim=8, mode="synthetic"), "synthetic", 8),
     "triangles": (lambda: wl.config_triangles(B=3, D=16), "plain", None),
+    # the plain fused CG (cg_fused_kernel<6,4,uni>, 148 CTAs), which the multigrid CG replaces on these grids by default
+    "finfet-plaincg": (lambda: wl.config_finfet(B=2, n_polar=2, n_azim=8), "synthetic", 4),
 }
 
 
 @pytest.mark.parametrize("name", list(FULLMESH))
-def test_fullmesh_few_bands_steps(name):
+def test_fullmesh_few_bands_steps(name, monkeypatch):
     """The FULL mesh of configs 2-4 (and two meshes that put 2 and 8 cells on a CG thread) with a 2-3-band table on both
     sides: eps, theta_SI, theta_en, q, G, boundary heat and theta after diffusion_correct, element by element against
-    the oracle for 3 steps.  Runs cg_fused_kernel<6,4,uni> with 148 CTAs, its halo batches and tail, update_kernel's class
-    combine and the closures at the mesh size of the bench."""
+    the oracle for 3 steps.  Runs the CG kernel of the bench (cg_mg_kernel, 148 CTAs; cg_fused_kernel<6,4,uni> with its halo
+    batches and tail in the -plaincg case), the combine of the partial moments and the closures at the mesh size of the
+    bench."""
     from paper_2607_03226_b200.binding import Solver
     make, mode, cpt = FULLMESH[name]
     pr = make()
+    if name.endswith("-plaincg"):
+        monkeypatch.setenv("NANOBTE_CG_NO_MG", "1")
     g, r = Solver(pr), RefSolver(pr)
     if cpt is not None:
         assert g.info["cg_fused"] == 1 and g.info["cg_cells_per_thread"] == cpt, g.info
+        assert g.info["cg_multigrid"] == (0 if name.endswith("-plaincg") else 1), g.info
         if cpt >= 4:
             assert g.info["cg_ctas"] == 148
     rng = np.random.default_rng(11)

@@ -375,14 +375,41 @@ def test_fused_cg_cells_per_thread_on_cuts(monkeypatch, nblk, cpt, hook):
     configs use (4 cells per thread on configs 2-4; 2 and 8 on meshes around them), with the face-uniform and the
     general stencil, with and without the recycled guess: element-wise against the oracle for 3 synthetic steps."""
     monkeypatch.setenv("NANOBTE_CG_NBLK", str(nblk))
+    monkeypatch.setenv("NANOBTE_CG_NO_MG", "1")
     if hook:
         monkeypatch.setenv(hook, "1")
     pr = wl.config_finfet(nx=32, ny=16, nz=16, B=3, n_polar=2, n_azim=8)
     g = gpu_solver(pr)
+    assert g.info["cg_multigrid"] == 0
     assert g.info["cg_fused"] == 1 and g.info["cg_cells_per_thread"] == cpt and g.info["cg_ctas"] <= nblk, g.info
     assert g.info["cg_face_uniform"] == (0 if hook == "NANOBTE_CG_NO_UNI" else 1)
     g.close()
     step_parity(pr, 3, T_init=random_T(pr, 10), mode="synthetic")
+
+
+@pytest.mark.parametrize("which,nblk", [("finfet", 0), ("finfet", 2), ("finfet", 5), ("cube20", 0), ("cube20", 4), ("cube33", 0),
+                                        ("cube33", 40)])
+def test_multigrid_cg_on_cuts(monkeypatch, which, nblk):
+    """cg_mg_kernel (the synthetic correction's default on uniform 3-D grids) with 1, 3-4 and 7-8 level-3 aggregates per CTA
+    (its slots-per-thread instantiations), on a masked grid and on lattices whose edge is not a multiple of 8 (partly
+    empty aggregates, empty slots): theta after the correction element-wise against the oracle for 3 synthetic steps, and
+    far fewer iterations than the oracle's unpreconditioned CG (same system, same ||r|| <= rtol ||rhs||: reading R14e')."""
+    if nblk:
+        monkeypatch.setenv("NANOBTE_CG_NBLK", str(nblk))
+    pr = {"finfet": lambda: wl.config_finfet(nx=32, ny=16, nz=16, B=3, n_polar=2, n_azim=8),
+          "cube20": lambda: wl.config_cube(n=20, B=3, n_polar=2, n_azim=8, mode="synthetic"),
+          "cube33": lambda: wl.config_cube(n=33, B=2, n_polar=2, n_azim=8, mode="synthetic")}[which]()
+    g, r = gpu_solver(pr), RefSolver(pr)
+    assert g.info["cg_multigrid"] == 1 and g.info["cg_mg_levels"] >= 4, g.info
+    T0 = random_T(pr, 21)
+    g.set_T(T0); r.set_T(T0)
+    for _ in range(3):
+        g.sweep(); r.sweep()
+        g.update_temperature(); r.update_temperature()
+        (ig, _), (ir, _) = g.diffusion_correct(), r.diffusion_correct()
+        assert rel(g.get_T(0) - pr["T_ref"], r.get_T(0) - pr["T_ref"]) <= 1e-9
+        assert 0 < ig <= 40 and ig < ir // 3, (ig, ir)
+    g.close(); r.close()
 
 
 def test_cg_not_converged_is_reported():
