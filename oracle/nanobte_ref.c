@@ -649,6 +649,66 @@ int nanobte_ref_diffusion_correct(nanobte_ref *h, int *cg_iters, double *max_dT)
 }
 
 /* ------------------------------------------------------------------------------------------ */
+/* O9: Fourier initial guess                                                                     */
+/* ------------------------------------------------------------------------------------------ */
+/* PAPER.md:228 (section IV): "A Fourier diffusion solve provides the initial temperature guess".  Reading R21: theta^0
+ * solves the steady heat-conduction problem  -div(kappa grad theta) = Qdot  with theta = T_w - T_ref on thermalizing
+ * faces and zero flux through every other boundary face, discretised with the same two-point-flux operator as the
+ * synthetic correction (diffusion_apply, R14d-e: kappa from the discrete quadrature, wall distance = cell centre to face):
+ *     sum_{f interior} kappa A_f (theta_c - theta_N)/d_f + sum_{f thermalizing} kappa A_f (theta_c - theta_w,f)/d_cf = V_c Qdot_c
+ * solved by the same unpreconditioned CG from zero to ||r|| <= cg_rtol ||rhs||.  The distribution is not touched
+ * (eps^0 stays what it is, R12); only theta is set. */
+int nanobte_ref_init_fourier(nanobte_ref *h, int *cg_iters) {
+  const int na = h->n_act;
+  int any_therm = 0;
+  for (int bf = 0; bf < h->n_bf; ++bf)
+    if (h->tag_type[h->bf_tag[bf]] == 0) any_therm = 1;
+  if (!any_therm) FAIL(h, NBR_E_SINGULAR, "the Fourier guess needs at least one thermalizing face");
+  double *rhs = malloc(sizeof(double) * na), *x = calloc(na, sizeof(double)), *r = malloc(sizeof(double) * na);
+  double *p = malloc(sizeof(double) * na), *Ap = malloc(sizeof(double) * na);
+  if (!rhs || !x || !r || !p || !Ap) FAIL(h, NBR_E_ALLOC, "alloc in CG");
+  for (int a = 0; a < na; ++a) {
+    double acc = h->vol[a] * h->Qdot[a];
+    for (int f = h->fptr[a]; f < h->fptr[a + 1]; ++f)
+      if (h->fnbr[f] < 0 && h->tag_type[h->bf_tag[h->fbf[f]]] == 0)
+        acc += h->kappa * h->farea[f] * (h->tag_T[h->bf_tag[h->fbf[f]]] - h->T_ref) / h->fdist[f];
+    rhs[a] = acc;
+  }
+  double bb = 0.0;
+  for (int a = 0; a < na; ++a) {
+    r[a] = p[a] = rhs[a];
+    bb += rhs[a] * rhs[a];
+  }
+  int it = 0;
+  double rr = bb;
+  const double stop2 = h->cg_rtol * h->cg_rtol * bb;
+  while (rr > stop2 && it < h->cg_max_iter) {
+    diffusion_apply(h, p, Ap);
+    double pAp = 0.0;
+    for (int a = 0; a < na; ++a) pAp += p[a] * Ap[a];
+    double alpha = rr / pAp;
+    double rr_new = 0.0;
+    for (int a = 0; a < na; ++a) {
+      x[a] += alpha * p[a];
+      r[a] -= alpha * Ap[a];
+      rr_new += r[a] * r[a];
+    }
+    double bet = rr_new / rr;
+    for (int a = 0; a < na; ++a) p[a] = r[a] + bet * p[a];
+    rr = rr_new;
+    ++it;
+  }
+  int ok = 1;
+  for (int a = 0; a < na; ++a) {
+    h->theta[a] = x[a];
+    ok &= isfinite(x[a]) != 0;
+  }
+  free(rhs); free(x); free(r); free(p); free(Ap);
+  if (cg_iters) *cg_iters = it;
+  return ok ? NBR_OK : NBR_E_NONFINITE;
+}
+
+/* ------------------------------------------------------------------------------------------ */
 /* O7: outer loop                                                                               */
 /* ------------------------------------------------------------------------------------------ */
 static int push_history(nanobte_ref *h, double dT, int cg) {

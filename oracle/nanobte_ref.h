@@ -86,6 +86,7 @@ int nanobte_ref_set_threads(nanobte_ref *h, int n); /* OpenMP threads for sweep/
 int nanobte_ref_sweep(nanobte_ref *h);                                   /* O3 then O2 */
 int nanobte_ref_update_temperature(nanobte_ref *h, double *max_dT);      /* O4, G refresh, O5 */
 int nanobte_ref_diffusion_correct(nanobte_ref *h, int *cg_iters, double *max_dT); /* O6 */
+int nanobte_ref_init_fourier(nanobte_ref *h, int *cg_iters);               /* O9: theta <- Fourier solution (R21) */
 int nanobte_ref_solve(nanobte_ref *h, double tol, int max_iter, int mode /*0 plain,1 synthetic*/,
                       int *iters_out, double *last_dT_out);              /* O7 */
 

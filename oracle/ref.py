@@ -62,6 +62,7 @@ def _load():
     lib.nanobte_ref_sweep.argtypes = [vp]
     lib.nanobte_ref_update_temperature.argtypes = [vp, _dp]
     lib.nanobte_ref_diffusion_correct.argtypes = [vp, _ip, _dp]
+    lib.nanobte_ref_init_fourier.argtypes = [vp, _ip]
     lib.nanobte_ref_solve.argtypes = [vp, C.c_double, C.c_int, C.c_int, _ip, _dp]
     lib.nanobte_ref_set_T.argtypes = [vp, _dp]
     lib.nanobte_ref_get_T.argtypes = [vp, C.c_int, _dp]
@@ -175,6 +176,12 @@ class RefSolver:
         it, d = C.c_int32(), C.c_double()
         self._chk(self._lib.nanobte_ref_diffusion_correct(self._h, C.byref(it), C.byref(d)))
         return it.value, d.value
+
+    def init_fourier(self):
+        """O9 / R21: theta <- solution of the steady heat-conduction problem; returns the CG iterations."""
+        it = C.c_int32()
+        self._chk(self._lib.nanobte_ref_init_fourier(self._h, C.byref(it)))
+        return it.value
 
     def solve(self, tol, max_iter, mode="plain"):
         it, d = C.c_int32(), C.c_double()

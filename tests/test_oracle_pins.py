@@ -294,6 +294,84 @@ def test_P6_diffusion_correction_is_dense_solve(name):
     assert 0 < it <= g.n_act + 5
 
 
+# ------------------------------------------------------------------------------------------------
+# P9: Fourier initial guess (O9, reading R21)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", list(TINY))
+def test_P9_fourier_guess_is_dense_conduction_solve(name):
+    """theta^0 against a dense LAPACK solve of the conduction problem assembled here from the raw face geometry
+    (fvgeom): interior two-point fluxes, Dirichlet T_w at thermalizing faces at the centre-to-face distance, zero flux
+    elsewhere, source V Qdot -- and the integral balance: what leaves through the thermalizing faces is what is generated."""
+    pr = TINY[name]
+    g = fvgeom.Geom(pr)
+    if not (g.bf_type == 0).any():
+        pytest.skip("no thermalizing face")
+    kappa = (pr["bands"]["C"] * pr["bands"]["v"] ** 2 * pr["bands"]["tau"]).sum() / g.dim
+    M = g.diffusion_matrix(kappa)
+    Q = np.zeros(g.n_act) if pr.get("Qdot") is None else g.to_active(np.asarray(pr["Qdot"], dtype=float))
+    rhs = g.vol * Q
+    out = 0.0
+    for (a, nbr, bf, A, n, d) in g.faces:
+        if bf >= 0 and g.bf_type[bf] == 0:
+            rhs[a] += kappa * A / d * (g.bf_Tw[bf] - pr["T_ref"])
+    th = np.linalg.solve(M, rhs)
+    r = RefSolver(pr, T_init=random_T(pr, 4))  # whatever theta was before, the guess replaces it
+    it = r.init_fourier()
+    got = g.to_active(r.get_T(0)) - pr["T_ref"]
+    scale = max(np.abs(th).max(), 1e-300)
+    assert np.abs(got - th).max() <= 1e-9 * scale
+    assert 0 < it <= g.n_act + 5
+    for (a, nbr, bf, A, n, d) in g.faces:
+        if bf >= 0 and g.bf_type[bf] == 0:
+            out += kappa * A / d * (got[a] - (g.bf_Tw[bf] - pr["T_ref"]))
+    gen = (g.vol * Q).sum()
+    assert out == pytest.approx(gen, rel=1e-8, abs=1e-9 * kappa * np.abs(got).max() * g.bf_area.max() / max(np.sqrt(g.vol.max()), 1e-300))
+
+
+def test_P9_fourier_guess_closed_forms():
+    """Slab between thermalizing walls at x = 0 and x = L, reflecting elsewhere, uniform cells of size h.
+    (a) no source: the two-point-flux solution is the straight line through the wall temperatures, exactly, at the cell
+    centres.  (b) uniform source, both walls at T_ref: theta_i = Q/(2 kappa) x_i (L - x_i) + Q h^2/(8 kappa): the second
+    difference of a quadratic is exact, and the half-cell wall distance shifts the parabola by a constant
+    (both checked to rounding)."""
+    n, L = 16, 200e-9
+    pr = wl.config_gray_square(n=n, D=8)
+    h = L / n
+    xc = (np.arange(n) + 0.5) * h
+    kappa = (pr["bands"]["C"] * pr["bands"]["v"] ** 2 * pr["bands"]["tau"]).sum() / 2
+    r = RefSolver(pr)
+    r.init_fourier()
+    th = (r.get_T(0) - pr["T_ref"]).reshape(n, n)
+    line = 1.0 + (-1.0 - 1.0) * xc / L       # walls at 301 K and 299 K, T_ref 300 K
+    assert np.abs(th - line[None, :]).max() <= 1e-12
+    pr2 = dict(pr)
+    m2 = dict(pr["mesh"])
+    m2["tags"] = [(t[0], 300.0) if t[0] == 0 else t for t in pr["mesh"]["tags"]]
+    pr2["mesh"] = m2
+    Q = 1e17
+    pr2["Qdot"] = np.full(n * n, Q)
+    r2 = RefSolver(pr2)
+    r2.init_fourier()
+    th2 = (r2.get_T(0) - pr2["T_ref"]).reshape(n, n)
+    para = Q / (2 * kappa) * xc * (L - xc) + Q * h * h / (8 * kappa)
+    assert np.abs(th2 - para[None, :]).max() <= 1e-10 * para.max()
+
+
+def test_P9_fourier_start_reaches_the_same_fixed_point():
+    """The guess changes the iterate path, not the fixed point: solve() from theta^0 ends at the converged field of the
+    run from T_ref (to the tolerance of the two runs), in fewer iterations on a diffusive case."""
+    pr = wl.config_gray_square(n=12, D=8)
+    pr["bands"] = dict(pr["bands"])
+    pr["bands"]["tau"] = pr["bands"]["tau"] * 0.05  # Kn = 0.025: diffusive, where the Fourier field is close
+    a, b = RefSolver(pr), RefSolver(pr)
+    ra = a.solve(1e-10, 20000)
+    b.init_fourier()
+    rb = b.solve(1e-10, 20000)
+    assert ra["converged"] and rb["converged"]
+    assert np.abs(a.get_T(0) - b.get_T(0)).max() <= 1e-7
+    assert rb["iters"] < ra["iters"]
+
+
 def test_P6_plain_equals_synthetic_config0_family():
     # the paper's use case is the diffusive side (PAPER.md:69); cells stay optically thin (R14f)
     for n, kn_scale in ((12, 1.0), (24, 0.1)):
