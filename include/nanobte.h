@@ -194,6 +194,14 @@ int nanobte_update_temperature(nanobte_solver *, double *max_dT);
  * options.cg_max_iter with ||r|| > cg_rtol ||rhs||. */
 int nanobte_diffusion_correct(nanobte_solver *, int32_t *cg_iters, double *max_dT);
 
+/* Fourier initial guess (section IV: "A Fourier diffusion solve provides the initial temperature guess";
+ * reading R21): T <- the solution of the steady heat-conduction problem -div(kappa grad T) = Qdot with T = T_w on
+ * thermalizing faces and zero flux through every other face, on the two-point-flux operator of the synthetic correction
+ * (same kappa, same CG, same cg_rtol / cg_max_iter).  Replaces the lattice temperature only (as nanobte_set_T does); the
+ * distribution and the wall caches keep their state, so call it before the first sweep.  cg_iters: host pointer or NULL;
+ * synchronises.  NANOBTE_E_SINGULAR without a thermalizing face, NANOBTE_NOT_CONVERGED as nanobte_diffusion_correct. */
+int nanobte_init_fourier(nanobte_solver *, int32_t *cg_iters);
+
 /* One source iteration as nanobte_solve runs it: sweep, closures + moments + update and, in synthetic mode, the CG
  * correction.  On grids swept by the tile-dataflow kernel the sweep of a step keeps the
  * distribution on chip (the moments are reduced inside the sweep; only wall-cell values and tile faces

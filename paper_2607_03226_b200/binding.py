@@ -21,7 +21,7 @@ ERRORS = {0: "OK", 1: "NOT_CONVERGED", -1: "INVALID", -2: "ALLOC", -3: "CUDA", -
 EXPORTS = [
     "nanobte_workspace_bytes_structured", "nanobte_workspace_bytes_unstructured", "nanobte_create_structured",
     "nanobte_create_unstructured", "nanobte_destroy", "nanobte_sweep", "nanobte_update_temperature",
-    "nanobte_diffusion_correct", "nanobte_step", "nanobte_set_keep_e", "nanobte_solve", "nanobte_set_T", "nanobte_get_T", "nanobte_get_q", "nanobte_get_e",
+    "nanobte_diffusion_correct", "nanobte_init_fourier", "nanobte_step", "nanobte_set_keep_e", "nanobte_solve", "nanobte_set_T", "nanobte_get_T", "nanobte_get_q", "nanobte_get_e",
     "nanobte_get_G", "nanobte_get_boundary_heat", "nanobte_get_history", "nanobte_get_info", "nanobte_launch_count",
     "nanobte_kappa", "nanobte_strerror", "nanobte_last_error",
 ]
@@ -101,6 +101,7 @@ def load():
     lib.nanobte_sweep.argtypes = [vp]
     lib.nanobte_update_temperature.argtypes = [vp, _dp]
     lib.nanobte_diffusion_correct.argtypes = [vp, _ip, _dp]
+    lib.nanobte_init_fourier.argtypes = [vp, _ip]
     lib.nanobte_step.argtypes = [vp, C.c_int32, _dp, _ip]
     lib.nanobte_set_keep_e.argtypes = [vp, C.c_int32]
     lib.nanobte_solve.argtypes = [vp, C.c_double, C.c_int32, C.c_int32, _ip, _dp]
@@ -275,6 +276,12 @@ class Solver:
         it, d = C.c_int32(), C.c_double()
         self._chk(self._lib.nanobte_diffusion_correct(self._h, C.byref(it), C.byref(d)))
         return it.value, d.value
+
+    def init_fourier(self):
+        """nanobte_init_fourier: T <- Fourier (steady conduction) solution, PAPER.md:228 / R21; returns the CG iterations."""
+        it = C.c_int32()
+        self._chk(self._lib.nanobte_init_fourier(self._h, C.byref(it)))
+        return it.value
 
     def step(self, mode="plain"):
         """One source iteration as solve() runs it; returns (max|dT|, CG iterations)."""

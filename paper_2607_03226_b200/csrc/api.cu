@@ -208,6 +208,7 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
   h->cg_diag = A.put(g.cg_diag);
   h->cellbf_ptr = A.put(g.cellbf_ptr);
   h->cellbf = A.put(g.cellbf);
+  h->fourier_rhs = A.put(g.fourier_rhs);
   h->cg_x = A.zeros<double>(na);
   h->cg_r = A.zeros<double>(na);
   h->cg_p0 = A.zeros<double>(na);
@@ -408,6 +409,31 @@ extern "C" int nanobte_diffusion_correct(nanobte_solver *h, int32_t *cg_iters, d
   if (max_dT) *max_dT = d;
   if (cg_failed) {
     h->cgf_nprev = 0;  // do not recycle a solution that is not one
+    nb_fail(h, NANOBTE_NOT_CONVERGED, "CG stopped at cg_max_iter = %d above rtol = %g", h->cg_max_iter, h->cg_rtol);
+    return NANOBTE_NOT_CONVERGED;
+  }
+  return 0;
+}
+
+extern "C" int nanobte_init_fourier(nanobte_solver *h, int32_t *cg_iters) {
+  if (!h || !h->arena) return NANOBTE_E_INVALID;
+  if (!h->any_therm) return nb_fail(h, NANOBTE_E_SINGULAR, "the Fourier guess needs at least one thermalizing face");
+  // R21: A theta = V Qdot + sum_thermalizing kappa A_f (T_w - T_ref) / d_cf with the operator of the synthetic
+  // correction; the right-hand side is a table built at create, the solver is the CG of nanobte_diffusion_correct
+  h->cgf_nprev = 0;
+  h->cg_rhs_direct = h->fourier_rhs;
+  int rc = nb_cg_solve(h, nullptr);
+  h->cg_rhs_direct = nullptr;
+  h->cgf_nprev = 0;  // this solution says nothing about the corrections to come
+  if (rc < 0) return rc;
+  if ((rc = nb_launch_scatter_cells(h, h->cg_x, h->part, 1, h->T_ref)) < 0) return rc;
+  if ((rc = nb_launch_set_theta(h, h->part)) < 0) return rc;
+  NB_CUDA(h, cudaMemcpyAsync(h->h_pinned, h->d_maxdT, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  NB_CUDA(h, cudaStreamSynchronize(h->stream));
+  unsigned long long it;
+  memcpy(&it, h->h_pinned + 1, sizeof(it));
+  if (cg_iters) *cg_iters = (int32_t)(it & 0xffffffffull);
+  if ((it >> 40) & 1ull) {
     nb_fail(h, NANOBTE_NOT_CONVERGED, "CG stopped at cg_max_iter = %d above rtol = %g", h->cg_max_iter, h->cg_rtol);
     return NANOBTE_NOT_CONVERGED;
   }

@@ -22,6 +22,7 @@ struct CgArgs {
   const double *coef;    // [nf][n]  kappa A_f / d_f for interior faces, 0 otherwise
   const double *diag;    // [n]      sum of interior + thermalizing face coefficients
   const double *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
+  const double *rhs_direct;  // non-null: the right-hand side itself (Fourier initial guess, R21)
   const int32_t *cellbf_ptr, *cellbf;
   double *x, *r, *p0, *p1, *ap, *partial;
   unsigned long long *iters_out;
@@ -65,12 +66,17 @@ __global__ void __launch_bounds__(256) cg_kernel(CgArgs a) {
   // right-hand side, x = 0, r = rhs, p_old = rhs
   double loc = 0.0;
   for (int i = tid; i < a.n; i += nth) {
-    double rhs = a.vol[i] * a.beta * (a.theta_SI[i] - a.theta_prev[i]);
-    for (int k = a.cellbf_ptr[i]; k < a.cellbf_ptr[i + 1]; ++k) {
-      const int bf = a.cellbf[k];
-      double F = 0.0;
-      for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
-      rhs += a.bf_area[bf] * F;
+    double rhs;
+    if (a.rhs_direct) {
+      rhs = a.rhs_direct[i];
+    } else {
+      rhs = a.vol[i] * a.beta * (a.theta_SI[i] - a.theta_prev[i]);
+      for (int k = a.cellbf_ptr[i]; k < a.cellbf_ptr[i + 1]; ++k) {
+        const int bf = a.cellbf[k];
+        double F = 0.0;
+        for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
+        rhs += a.bf_area[bf] * F;
+      }
     }
     a.x[i] = 0.0;
     a.r[i] = rhs;
@@ -142,6 +148,7 @@ struct CgfArgs {
   int32_t n, nf, nblk, chunk, nh_cap, max_iter, B;
   const int32_t *nloc, *perm;
   const double *coef, *diag, *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
+  const double *rhs_direct;  // non-null: the right-hand side itself (Fourier initial guess, R21)
   const int32_t *cellbf_ptr, *cellbf, *hptr, *hidx;
   double *x, *w, *part;
   unsigned int *bar;
@@ -213,12 +220,17 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
       }
       dg[c] = a.diag[i];
       const int io = a.perm[i];  // the cell in the solver's own (active) numbering
-      double rhs = a.vol[io] * a.beta * (a.theta_SI[io] - a.theta_prev[io]);  // R14c
-      for (int q = a.cellbf_ptr[io]; q < a.cellbf_ptr[io + 1]; ++q) {        // R14c'
-        const int bf = a.cellbf[q];
-        double F = 0.0;
-        for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
-        rhs += a.bf_area[bf] * F;
+      double rhs;
+      if (a.rhs_direct) {
+        rhs = a.rhs_direct[io];
+      } else {
+        rhs = a.vol[io] * a.beta * (a.theta_SI[io] - a.theta_prev[io]);  // R14c
+        for (int q = a.cellbf_ptr[io]; q < a.cellbf_ptr[io + 1]; ++q) {  // R14c'
+          const int bf = a.cellbf[q];
+          double F = 0.0;
+          for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
+          rhs += a.bf_area[bf] * F;
+        }
       }
       r[c] = rhs;
       r_loc[li] = rhs;
@@ -486,6 +498,7 @@ static int cg_solve_fused(nanobte_solver *h) {
   a.nloc = h->cgf_nloc; a.perm = h->cgf_perm; a.coef = h->cgf_coef; a.diag = h->cgf_diag; a.vol = h->vol;
   a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev; a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area;
   a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf; a.hptr = h->cgf_hptr; a.hidx = h->cgf_hidx;
+  a.rhs_direct = h->cg_rhs_direct;
   a.x = h->cg_x; a.w = h->cgf_w; a.part = h->cgf_part; a.bar = h->cgf_bar;
   a.iters_out = h->d_maxdT + 1;
   a.beta = h->beta; a.rtol = h->cg_rtol;
@@ -517,6 +530,7 @@ int nb_cg_solve(nanobte_solver *h, int *iters) {
   a.nbr = h->cg_nbr; a.coef = h->cg_coef; a.diag = h->cg_diag;
   a.vol = h->vol; a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev;
   a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area; a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf;
+  a.rhs_direct = h->cg_rhs_direct;
   a.x = h->cg_x; a.r = h->cg_r; a.p0 = h->cg_p0; a.p1 = h->cg_p1; a.ap = h->cg_rhs; a.partial = h->cg_partial;
   a.iters_out = h->d_maxdT + 1;
   a.beta = h->beta; a.rtol = h->cg_rtol;

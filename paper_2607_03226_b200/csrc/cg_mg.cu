@@ -183,12 +183,17 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
       for (int f = 0; f < 6; ++f) nl[c][f] = a.nbr0[(int64_t)f * nslot0 + base0 + li];
       const int io = cell[c];
       if (io >= 0) {
-        double rhs = a.vol[io] * a.beta * (a.theta_SI[io] - a.theta_prev[io]);  // R14c
-        for (int q = a.cellbf_ptr[io]; q < a.cellbf_ptr[io + 1]; ++q) {        // R14c'
-          const int bf = a.cellbf[q];
-          double F = 0.0;
-          for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
-          rhs += a.bf_area[bf] * F;
+        double rhs;
+        if (a.rhs_direct) {
+          rhs = a.rhs_direct[io];
+        } else {
+          rhs = a.vol[io] * a.beta * (a.theta_SI[io] - a.theta_prev[io]);  // R14c
+          for (int q = a.cellbf_ptr[io]; q < a.cellbf_ptr[io + 1]; ++q) {  // R14c'
+            const int bf = a.cellbf[q];
+            double F = 0.0;
+            for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
+            rhs += a.bf_area[bf] * F;
+          }
         }
         r[c] = rhs;
       }
@@ -797,6 +802,7 @@ int nb_mg_solve(nanobte_solver *h) {
   MgArgs a = P.a;
   a.max_iter = h->cg_max_iter; a.B = h->B; a.rtol = h->cg_rtol; a.beta = h->beta;
   a.vol = h->vol; a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev; a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area;
+  a.rhs_direct = h->cg_rhs_direct;
   a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf; a.x = h->cg_x; a.iters_out = h->d_maxdT + 1;
   mg_fn fn = mg_pick(P.cpt);
   if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "internal: no multigrid CG variant for %d slots per thread", P.cpt);

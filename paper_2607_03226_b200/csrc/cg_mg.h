@@ -48,6 +48,7 @@ struct MgArgs {
   double *g3;                      // [n3] published level-3 right-hand side
   // right-hand side, result, reductions
   const double *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
+  const double *rhs_direct;        // non-null: the right-hand side itself (Fourier initial guess, R21)
   const int32_t *cellbf_ptr, *cellbf;
   double *x;                       // [n_act] solution, active-cell order
   double *part;                    // [2][nblk][4]

@@ -80,6 +80,7 @@ struct GenericTables {
   std::vector<int32_t> cg_nbr;
   std::vector<double> cg_coef, cg_diag;
   std::vector<int32_t> cellbf_ptr, cellbf;
+  std::vector<double> fourier_rhs;  // [n] right-hand side of the Fourier initial guess (R21): V Qdot + sum_thermalizing kappa A_f (T_w - T_ref) / d_cf
   std::vector<double> cg_xyz;      // [n][3] cell centres in any consistent unit (partitioning of the CG only)
   int cg_grid[3] = {0, 0, 0};      // structured grids: lattice dimensions, cg_xyz holds the integer lattice coordinates
   std::vector<int32_t> tagface_ptr, tagface;

@@ -141,6 +141,8 @@ struct nanobte_solver {
   const double *cg_coef = nullptr;       // [nf][n_act]
   const double *cg_diag = nullptr, *vol = nullptr;
   const int32_t *cellbf_ptr = nullptr, *cellbf = nullptr;  // CSR: reflecting boundary faces of each active cell
+  const double *fourier_rhs = nullptr;   // [n_act] right-hand side of the Fourier initial guess (R21)
+  const double *cg_rhs_direct = nullptr; // non-null: the CG kernels take this right-hand side instead of R14c/R14c'
   int cg_nf = 0;
   double *cg_x = nullptr, *cg_r = nullptr, *cg_p0 = nullptr, *cg_p1 = nullptr, *cg_rhs = nullptr, *cg_scal = nullptr;
   double *cg_partial = nullptr;

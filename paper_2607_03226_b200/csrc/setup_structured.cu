@@ -426,6 +426,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   G.cg_nbr.assign((size_t)nside * na, 0);
   G.cg_coef.assign((size_t)nside * na, 0.0);
   G.cg_diag.assign(na, 0.0);
+  G.fourier_rhs.assign(na, 0.0);
   G.cellbf_ptr.assign(na + 1, 0);
   for (int a = 0; a < na; ++a) {
     const int c = G.act2cell[a];
@@ -434,6 +435,7 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
     G.vol[a] = hh[0] * hh[1] * hh[2];
     for (int k = 0; k < 3; ++k) G.cg_xyz[3 * (size_t)a + k] = ijk[k];
     G.Qdot_act[a] = Qdot ? Qdot[c] : 0.0;
+    G.fourier_rhs[a] = G.vol[a] * G.Qdot_act[a];
     G.theta0[a] = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
     for (int side = 0; side < nside; ++side) {
       const int axis = side / 2, sgn = (side & 1) ? 1 : -1;
@@ -449,7 +451,10 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
         G.cg_diag[a] += cf;
       } else {
         const int f = facebf[(size_t)c * 6 + side];
-        if (G.bf_type[f] == NANOBTE_THERMALIZING) G.cg_diag[a] += cm.kappa * area / (0.5 * hh[axis]);  // delta = 0 on the wall (R14e)
+        if (G.bf_type[f] == NANOBTE_THERMALIZING) {
+          G.cg_diag[a] += cm.kappa * area / (0.5 * hh[axis]);  // delta = 0 on the wall (R14e)
+          G.fourier_rhs[a] += cm.kappa * area / (0.5 * hh[axis]) * G.bf_eps_w[f];  // theta = T_w - T_ref on the wall (R21)
+        }
         else G.cellbf.push_back(f);
       }
     }

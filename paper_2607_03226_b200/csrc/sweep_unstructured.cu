@@ -713,12 +713,14 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
   G.cg_nbr.assign((size_t)maxf * nc, 0);
   G.cg_coef.assign((size_t)maxf * nc, 0.0);
   G.cg_diag.assign(nc, 0.0);
+  G.fourier_rhs.assign(nc, 0.0);
   G.cellbf_ptr.assign(nc + 1, 0);
   G.cg_xyz.assign((size_t)3 * nc, 0.0);
   for (int c = 0; c < nc; ++c) {
     G.cg_xyz[3 * (size_t)c] = cen[2 * c];
     G.cg_xyz[3 * (size_t)c + 1] = cen[2 * c + 1];
     G.Qdot_act[c] = Qdot ? Qdot[c] : 0.0;
+    G.fourier_rhs[c] = G.vol[c] * G.Qdot_act[c];
     G.theta0[c] = opt->T_init ? opt->T_init[c] - opt->T_ref : 0.0;
     for (int k = 0; k < maxf; ++k) G.cg_nbr[(size_t)k * nc + c] = c;
     int k = 0;
@@ -730,6 +732,7 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
         G.cg_diag[c] += cf;
       } else if (G.bf_type[fbf[f]] == NANOBTE_THERMALIZING) {
         G.cg_diag[c] += cm.kappa * flen[f] / fdist[f];  // delta = 0 on the wall
+        G.fourier_rhs[c] += cm.kappa * flen[f] / fdist[f] * G.bf_eps_w[fbf[f]];  // theta = T_w - T_ref on the wall (R21)
       } else {
         G.cellbf.push_back(fbf[f]);
       }

@@ -412,6 +412,53 @@ def test_multigrid_cg_on_cuts(monkeypatch, which, nblk):
     g.close(); r.close()
 
 
+# ---- Fourier initial guess (reading R21) --------------------------------------------------------------
+FOURIER_CASES = {
+    "tiny": lambda name: TINY[name],
+    "cube20": lambda _: wl.config_cube(n=20, B=3, n_polar=2, n_azim=8, mode="synthetic"),
+    "finfet": lambda _: wl.config_finfet(nx=32, ny=16, nz=16, B=3, n_polar=2, n_azim=8),
+    "square": lambda _: wl.config_nongray_square(n=24, B=3, D=8),
+    "triangles": lambda _: wl.config_triangles(n=24, side=1e-7, B=3, D=8, hole_radius=1.5e-8),
+}
+
+
+@pytest.mark.parametrize("case", [("tiny", k) for k in TINY] + [(k, None) for k in FOURIER_CASES if k != "tiny"])
+def test_fourier_guess_matches_oracle(case):
+    """nanobte_init_fourier against the oracle's O9 (every CG kernel: multigrid on the 3-D uniform grids, fused elsewhere):
+    the field element by element (CG to rtol 1e-12 on both sides: compared at 1e-9 like the correction), then the
+    first sweep and update from it at the sweep tolerance."""
+    kind, name = case
+    pr = FOURIER_CASES[kind](name)
+    g, r = gpu_solver(pr, T_init=random_T(pr, 31)), RefSolver(pr, T_init=random_T(pr, 31))
+    if not any(t[0] == 0 for t in pr["mesh"]["tags"]):
+        with pytest.raises(Exception):
+            g.init_fourier()
+        g.close(); r.close()
+        return
+    ig, ir = g.init_fourier(), r.init_fourier()
+    a, b = g.get_T(0) - pr["T_ref"], r.get_T(0) - pr["T_ref"]
+    assert rel(a, b) <= 1e-9, rel(a, b)
+    assert 0 < ig <= ir + max(2, ir // 20)
+    r.set_T(g.get_T(0))  # the same start on both sides: the sweep is compared at its own tolerance
+    g.sweep(); r.sweep()
+    compare_state(g, r, pr, "sweep after the Fourier guess")
+    dg, dr = g.update_temperature(), r.update_temperature()
+    compare_fields(g, r, pr, "update after the Fourier guess")
+    assert abs(dg - dr) <= 1e-9 * abs(dr) + 1e-13
+    g.close(); r.close()
+
+
+def test_fourier_guess_then_solve_counts():
+    """solve() from the Fourier field: the same iteration count and converged field as the oracle started the same way."""
+    pr = wl.config_finfet(nx=24, ny=12, nz=12, B=4, n_polar=2, n_azim=8)
+    g, r = gpu_solver(pr), RefSolver(pr)
+    g.init_fourier(); r.init_fourier()
+    rg, rr = g.solve(1e-9, 3000, "synthetic"), r.solve(1e-9, 3000, "synthetic")
+    assert rg["converged"] and rr["converged"] and rg["iters"] == rr["iters"], (rg, rr)
+    assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
+    g.close(); r.close()
+
+
 def test_cg_not_converged_is_reported():
     """cg_max_iter too small: diffusion_correct and solve say NOT_CONVERGED (1) instead of OK."""
     pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
