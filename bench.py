@@ -329,18 +329,37 @@ def main():
                    "barrier + synchronize"}
     g.close()
 
-    # ---- roofline of the dominant kernel (the sweep): 8 algorithmic bytes per update ----------
+    # ---- roofline of the dominant kernel (the sweep): 8 algorithmic bytes per update (the eps store of the sweep;
+    # DESIGN.md section 6).  The tile-dataflow kernel also does the moments (SURVEY: 8 B/update more, the eps load) and moves
+    # neither through HBM, so for it the HBM figure is an equivalent rate, not traffic: the measured DRAM bytes are in
+    # "traffic", and what bounds the kernel itself is in "on_chip" (fp64 pipe and shared-memory crossbar).
     peak, peak_src = measured_peaks()
     alg_bytes = 8.0 * upd
     achieved = alg_bytes / (sweep_ms * 1e-3) / 1e9
-    kernel = ("sweep_structured_kernel" if pr["kind"] == "structured" else
+    brick = pr["kind"] == "structured" and info.get("sweep_variant") == 5
+    kernel = (("sweep_brick_kernel" if brick else "sweep_structured_kernel") if pr["kind"] == "structured" else
               ("sweep_unstructured_staged_kernel" if info.get("sweep_rmax", 0) == 0 else "sweep_unstructured_kernel"))
     roofline = {"bound": "hbm", "kernel": kernel,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                 "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
-                "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": sweep_ms,
-                "moments_pass": {"achieved": alg_bytes / (update_ms * 1e-3) / 1e9, "launch_ms": update_ms,
-                                 "note": "closures + moments + update; 8 B/update read"}}
+                "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": sweep_ms}
+    if brick:
+        # fp64 operations per update: 4 (substitution) + 3 (band sums of the moments) + 5/B per direction weight ~ 7.2;
+        # peak = 64 DFMA/clk/SM x SMs x clock (B300_MICROARCH.md unit counts; 58/clk measured with a DFMA-only kernel)
+        sm_clock = (clocks.get("sm_mhz") or 1965.0) * 1e6
+        ops = (7.0 + 5.0 / max(1, len(pr["bands"]["C"]))) * upd
+        alu_peak = 64.0 * 148 * sm_clock
+        smem_bytes = 26.0 * upd   # STS 8 + LDS 8 (u-upwind) + LDS 8 (moments) + theta broadcast 2 per update
+        roofline["fused"] = {"note": "sweep + moments in one kernel: nothing of eps goes to HBM unless asked for",
+                             "algorithmic_bytes_sweep_plus_moments": 16.0 * upd,
+                             "equivalent_GBs_sweep_plus_moments": 16.0 * upd / (sweep_ms * 1e-3) / 1e9}
+        roofline["on_chip"] = {"alu": {"bound": "alu", "achieved": ops / (sweep_ms * 1e-3) / 1e12, "peak": alu_peak / 1e12,
+                                       "unit": "T fp64 op/s", "frac": ops / (sweep_ms * 1e-3) / alu_peak},
+                               "smem": {"achieved": smem_bytes / (sweep_ms * 1e-3) / 1e12, "peak": 128.0 * 148 * sm_clock / 1e12,
+                                        "unit": "TB/s", "frac": smem_bytes / (sweep_ms * 1e-3) / (128.0 * 148 * sm_clock)}}
+    else:
+        roofline["moments_pass"] = {"achieved": alg_bytes / (update_ms * 1e-3) / 1e9, "launch_ms": update_ms,
+                                    "note": "closures + moments + update; 8 B/update read"}
     tr = os.path.join(ROOT, "profiles", "traffic.json")  # copied from ncu --set full captures; each entry names its capture
     if os.path.exists(tr):
         try:
@@ -356,8 +375,8 @@ def main():
            "config": workload_config(pr, mode, {"parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                                                 "sweep": {k: info[k] for k in ("sweep_G", "sweep_threads", "sweep_rmax", "n_tasks", "n_planes",
                                                                                "sweep_smem_bytes", "pencil_axis")},
-                                                "cg": {k: info[k] for k in ("cg_fused", "cg_cells_per_thread", "cg_ctas", "cg_face_uniform",
-                                                                            "cg_recycle")},
+                                                "cg": {k: info[k] for k in ("cg_multigrid", "cg_mg_levels", "cg_fused", "cg_cells_per_thread",
+                                                                            "cg_ctas", "cg_face_uniform", "cg_recycle")},
                                                 "device_bytes": info["device_bytes"]}),
            "sweep_updates_per_s": world * upd / (sweep_ms * 1e-3), "s_per_iteration": ms_per_step * 1e-3,
            "breakdown_ms": {"sweep": sweep_ms, "closures_moments_update": update_ms, "cg": cg_ms},
@@ -375,6 +394,18 @@ def main():
                                       "converged": res["converged"], "tol_K": pr["tol"], "last_dT_K": res["last_dT"],
                                       "cg_iters_total": int(g2.get_history()[1].sum())}
         g2.close()
+        if pr["mode"] == "synthetic" or any(t[0] == 0 for t in pr["mesh"]["tags"]):
+            # the same solve started from the Fourier field (nanobte_init_fourier), the guess inside the clock
+            g3 = Solver(pr, **skw)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            cg0 = g3.init_fourier()
+            res = g3.solve(pr["tol"], pr["max_iter"], mode)
+            torch.cuda.synchronize()
+            out["time_to_convergence"]["fourier_start"] = {"seconds": time.perf_counter() - t0, "iterations": res["iters"],
+                                                           "converged": res["converged"], "guess_cg_iters": cg0,
+                                                           "cg_iters_total": int(g3.get_history()[1].sum())}
+            g3.close()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         # the oracle as it stands on this box's host cores: all cores and one core, per phase
         cores = len(os.sched_getaffinity(0))

@@ -224,6 +224,80 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
   };
 
   unsigned int epoch = 1;
+  // ---- recycled initial guess: x_0 = Galerkin projection of the right-hand side on the span of the last two solutions (the operator
+  // never changes and successive corrections become collinear; cg.cu has the same step).  Their halo values were written by
+  // earlier launches and are simply read; one reduction of six scalars.  The stopping rule keeps ||rhs||.
+  double bb_total = -1.0;
+  if (a.nprev > 0) {
+    double X[2][CPT], AX[2][CPT];
+#pragma unroll
+    for (int v = 0; v < 2; ++v) {
+      const double *xp = a.xprev + (size_t)v * nslot0;
+      const bool have = v < a.nprev;
+      __syncthreads();
+#pragma unroll
+      for (int c = 0; c < CPT; ++c) {
+        const int li = tid + c * kMgThreads;
+        X[v][c] = (have && li < n0) ? xp[base0 + li] : 0.0;
+        if (li < n0) x0[li] = X[v][c];
+      }
+      for (int j = tid; j < nh0; j += kMgThreads) x0[n0 + j] = have ? xp[hidx0[j]] : 0.0;
+      __syncthreads();
+#pragma unroll
+      for (int c = 0; c < CPT; ++c) AX[v][c] = A0(c, x0, X[v][c]);
+    }
+    double sums[6] = {0, 0, 0, 0, 0, 0};  // X1.b, X2.b, X1.AX1, X1.AX2, X2.AX2, b.b
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+      sums[0] += X[0][c] * r[c];
+      sums[1] += X[1][c] * r[c];
+      sums[2] += X[0][c] * AX[0][c];
+      sums[3] += X[0][c] * AX[1][c];
+      sums[4] += X[1][c] * AX[1][c];
+      sums[5] += r[c] * r[c];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) sums[q] += __shfl_xor_sync(0xffffffffu, sums[q], o);
+      if (lane == 0) y0[q * (kMgThreads / 32) + wid] = sums[q];
+    }
+    __syncthreads();
+    if (tid < 6) {
+      double t = 0.0;
+      for (int w2 = 0; w2 < kMgThreads / 32; ++w2) t += y0[tid * (kMgThreads / 32) + w2];
+      a.gpart[(size_t)k * 8 + tid] = t;
+    }
+    grid_barrier(a.bar, epoch++ * a.nblk);
+    double tot[6];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+      double t = 0.0;
+      for (int c2 = lane; c2 < a.nblk; c2 += 32) t += __ldcg(a.gpart + (size_t)c2 * 8 + q);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+      tot[q] = t;
+    }
+    bb_total = tot[5];
+    double c1 = 0.0, c2 = 0.0;
+    const double det = tot[2] * tot[4] - tot[3] * tot[3];
+    if (a.nprev > 1 && det > 1e-8 * tot[2] * tot[4]) {  // two independent directions
+      c1 = (tot[0] * tot[4] - tot[1] * tot[3]) / det;
+      c2 = (tot[1] * tot[2] - tot[0] * tot[3]) / det;
+    } else if (tot[2] > 0.0) {
+      c1 = tot[0] / tot[2];
+    }
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+      const int li = tid + c * kMgThreads;
+      if (li < n0) {
+        xs[li] = c1 * X[0][c] + c2 * X[1][c];
+        r[c] -= c1 * AX[0][c] + c2 * AX[1][c];
+      }
+    }
+    __syncthreads();
+  }
   double g_prev = 1.0, alpha_prev = 1.0, stop2 = 0.0;
   int it = 0;
   bool not_converged = false;
@@ -406,7 +480,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     __syncthreads();
     gam = red[60]; del = red[61]; rho = red[62];
     __syncthreads();
-    if (it == 0) stop2 = a.rtol * a.rtol * rho;  // x_0 = 0: r_0 = rhs
+    if (it == 0) stop2 = a.rtol * a.rtol * (bb_total >= 0.0 ? bb_total : rho);  // without a guess x_0 = 0: r_0 = rhs
     if (!(rho > stop2)) break;
     if (it >= a.max_iter) { not_converged = true; break; }
     const double bet = it ? gam / g_prev : 0.0;
@@ -428,7 +502,11 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
 #pragma unroll
   for (int c = 0; c < CPT; ++c) {
     const int li = tid + c * kMgThreads;
-    if (li < n0 && cell[c] >= 0) a.x[cell[c]] = xs[li];
+    if (li < n0) {
+      if (cell[c] >= 0) a.x[cell[c]] = xs[li];
+      a.xprev[nslot0 + base0 + li] = a.xprev[base0 + li];  // history of the recycled initial guess
+      a.xprev[base0 + li] = xs[li];
+    }
   }
   if (k == 0 && tid == 0) *a.iters_out = (unsigned long long)it | (not_converged ? kCgNotConverged : 0ull);
 }
@@ -788,6 +866,8 @@ int nb_mg_build(nanobte_solver *h, Arena &A, const GenericTables &g, const doubl
   a.gnbr = A.put(gnbr); a.gcnt = A.put(gcnt); a.gchild = A.put(gchild); a.gpar = A.put(gpar);
   a.gdinv = A.put(gdinv); a.gdiag = A.put(gdiag); a.ginv = A.put(ginv);
   a.g3 = A.zeros<double>((size_t)n3 + 8);
+  a.xprev = A.zeros<double>((size_t)2 * nslot[0]);
+  a.gpart = A.zeros<double>((size_t)8 * nblk + 8);
   a.part = A.zeros<double>((size_t)8 * nblk + 8);
   a.bar = A.zeros<unsigned int>(4);
   a.cap0 = cap[0]; a.caph0 = caph[0]; a.cap1 = cap[1]; a.caph1 = caph[1]; a.cap2 = cap[2]; a.caph2 = caph[2];
@@ -803,6 +883,8 @@ int nb_mg_solve(nanobte_solver *h) {
   a.max_iter = h->cg_max_iter; a.B = h->B; a.rtol = h->cg_rtol; a.beta = h->beta;
   a.vol = h->vol; a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev; a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area;
   a.rhs_direct = h->cg_rhs_direct;
+  a.nprev = h->cgf_nprev;  // the history counter of the handle (reset by solve / set_T / a failed or foreign solve)
+  h->cgf_nprev = std::min(2, h->cgf_nprev + 1);
   a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf; a.x = h->cg_x; a.iters_out = h->d_maxdT + 1;
   mg_fn fn = mg_pick(P.cpt);
   if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "internal: no multigrid CG variant for %d slots per thread", P.cpt);

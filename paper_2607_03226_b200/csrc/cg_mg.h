@@ -46,6 +46,10 @@ struct MgArgs {
   const double *gdinv, *gdiag;     // [ntot]
   const double *ginv;              // [nc][nc] inverse of the coarsest operator
   double *g3;                      // [n3] published level-3 right-hand side
+  // recycled initial guess (as in cg.cu): the last two solutions per level-0 slot, and a reduction buffer
+  int32_t nprev;
+  double *xprev;                   // [2][nslot0]
+  double *gpart;                   // [nblk][8]
   // right-hand side, result, reductions
   const double *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
   const double *rhs_direct;        // non-null: the right-hand side itself (Fourier initial guess, R21)
