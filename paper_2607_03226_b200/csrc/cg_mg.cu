@@ -44,6 +44,30 @@ __device__ __forceinline__ void grid_barrier(unsigned int *bar, unsigned int tar
   __syncthreads();
 }
 
+// Values that cross CTA borders carry a sequence bit in their last mantissa bit (a relative perturbation of at most
+// 2.2e-16, deterministic): the value is its own ready flag.  Buffers are double-buffered by iteration parity and zeroed
+// before the launch; iteration `it` writes buffer it & 1 with bit ((it >> 1) & 1) ^ 1, so what is left in that buffer from
+// iteration it - 2 (or the zeros of the launch) has the other bit.  A CTA cannot be two iterations ahead of a CTA it
+// exchanges with (every iteration ends in an all-to-all of the dot products), which is what makes two buffers enough.
+__device__ __forceinline__ double mg_tag(double x, unsigned bit) {
+  return __hiloint2double(__double2hiint(x), (int)(((unsigned)__double2loint(x) & ~1u) | bit));
+}
+__device__ __forceinline__ double mg_load(const double *p, unsigned bit) {
+  double v;
+  for (;;) {
+    asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    if ((((unsigned)__double2loint(v)) & 1u) == bit) return v;
+    __nanosleep(20);
+  }
+}
+
+#ifdef MG_PROF
+__device__ unsigned long long g_mg_prof[16];
+#define MGP(k) do { if (tid == 0 && blockIdx.x == 0) { const long long t_ = clock64(); g_mg_prof[k] += (unsigned long long)(t_ - tprof); tprof = t_; } } while (0)
+#else
+#define MGP(k)
+#endif
+
 // A level held in shared memory (levels 1.. ; level 0 keeps its stencil in registers).
 struct Lv {
   int n;                 // own unknowns
@@ -216,10 +240,13 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     }
     return acc;
   };
-  auto exchange = [&](double *xg, int64_t base, const double *xv, int n, double *halo, const int32_t *hidx, int nh, unsigned int &epoch) {
-    for (int i = tid; i < n; i += kMgThreads) xg[base + i] = xv[i];
-    grid_barrier(a.bar, epoch++ * a.nblk);
-    for (int j = tid; j < nh; j += kMgThreads) halo[j] = __ldcg(xg + hidx[j]);
+  int it = 0;
+  // publish the own part of an iterate, then read the halo: no barrier (see mg_tag)
+  auto exchange = [&](double *xg2, int64_t nslot, int64_t base, const double *xv, int n, double *halo, const int32_t *hidx, int nh) {
+    double *buf = xg2 + (size_t)(it & 1) * nslot;
+    const unsigned bit = ((unsigned)(it >> 1) & 1u) ^ 1u;
+    for (int i = tid; i < n; i += kMgThreads) __stcg(buf + base + i, mg_tag(xv[i], bit));
+    for (int j = tid; j < nh; j += kMgThreads) halo[j] = mg_load(buf + hidx[j], bit);
     __syncthreads();
   };
 
@@ -299,9 +326,14 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     __syncthreads();
   }
   double g_prev = 1.0, alpha_prev = 1.0, stop2 = 0.0;
-  int it = 0;
   bool not_converged = false;
+  const int64_t nslot1 = (int64_t)a.a3ptr[a.nblk] * 64, nslot2 = (int64_t)a.a3ptr[a.nblk] * 8;
+#ifdef MG_PROF
+  long long tprof = clock64();
+#endif
   for (;; ++it) {
+    const unsigned bit = ((unsigned)(it >> 1) & 1u) ^ 1u;
+    MGP(9);
     // =================================== u = M^-1 r : one V-cycle ===================================================================
     // ---- level 0 down: x = B r, exchange, residual, restriction
     double xv[CPT];
@@ -321,7 +353,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
       if (li < n0) x0[li] = xv[c];
     }
     __syncthreads();
-    exchange(a.xg[0], base0, x0, n0, x0 + n0, hidx0, nh0, epoch);
+    exchange(a.xg[0], nslot0, base0, x0, n0, x0 + n0, hidx0, nh0);
 #pragma unroll
     for (int c = 0; c < CPT; ++c) {
       const int li = tid + c * kMgThreads;
@@ -333,26 +365,31 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
       L1.g[i] = ((q[0] + q[1]) + (q[2] + q[3])) + ((q[4] + q[5]) + (q[6] + q[7]));
     }
     __syncthreads();
+    MGP(0);
     // ---- level 1 down
     presmooth(L1, cfu);
-    exchange(a.xg[1], base1, L1.x, n1, L1.x + n1, hidx1, nh1, epoch);
+    exchange(a.xg[1], nslot1, base1, L1.x, n1, L1.x + n1, hidx1, nh1);
     residual(L1, cfu);
     for (int i = tid; i < n2; i += kMgThreads) {
       const double *q = L1.res + 8 * i;
       L2.g[i] = ((q[0] + q[1]) + (q[2] + q[3])) + ((q[4] + q[5]) + (q[6] + q[7]));
     }
     __syncthreads();
+    MGP(1);
     // ---- level 2 down; the level-3 right-hand side is published
     presmooth(L2, cfu);
-    exchange(a.xg[2], base2, L2.x, n2, L2.x + n2, hidx2, nh2, epoch);
+    exchange(a.xg[2], nslot2, base2, L2.x, n2, L2.x + n2, hidx2, nh2);
     residual(L2, cfu);
-    for (int i = tid; i < na3; i += kMgThreads) {
-      const double *q = L2.res + 8 * i;
-      a.g3[a3lo + i] = ((q[0] + q[1]) + (q[2] + q[3])) + ((q[4] + q[5]) + (q[6] + q[7]));
+    {
+      double *g3b = a.g3 + (size_t)(it & 1) * a.n_l[3];
+      for (int i = tid; i < na3; i += kMgThreads) {
+        const double *q = L2.res + 8 * i;
+        __stcg(g3b + a3lo + i, mg_tag(((q[0] + q[1]) + (q[2] + q[3])) + ((q[4] + q[5]) + (q[6] + q[7])), bit));
+      }
+      for (int i = tid; i < a.n_l[3]; i += kMgThreads) gg[i] = mg_load(g3b + i, bit);
+      __syncthreads();
     }
-    grid_barrier(a.bar, epoch++ * a.nblk);
-    for (int i = tid; i < a.n_l[3]; i += kMgThreads) gg[i] = __ldcg(a.g3 + i);
-    __syncthreads();
+    MGP(2);
     // ---- levels 3.. : the same arithmetic in every CTA
     for (int l = 3; l < a.nlev; ++l) {
       const int o = a.off_l[l], n = a.n_l[l];
@@ -390,20 +427,23 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
       __syncthreads();
       postsmooth(G, cfu);
     }
+    MGP(3);
     // ---- level 2 up: correction of own and halo entries from level 3 (every CTA has all of it), post-smoothing, publish
     for (int i = tid; i < n2; i += kMgThreads)
       if (dinv2[i] != 0.0) L2.x[i] += a.tau * gx[a3lo + (i >> 3)];  // empty slots stay zero
     for (int j = tid; j < nh2; j += kMgThreads) L2.x[n2 + j] += a.tau * gx[hpar2[j]];
     __syncthreads();
     postsmooth(L2, cfu);
-    exchange(a.xg[2], base2, L2.x, n2, L2.x + n2, hidx2, nh2, epoch);
+    exchange(a.xu[2], nslot2, base2, L2.x, n2, L2.x + n2, hidx2, nh2);
+    MGP(4);
     // ---- level 1 up
     for (int i = tid; i < n1; i += kMgThreads)
       if (dinv1[i] != 0.0) L1.x[i] += a.tau * L2.x[i >> 3];
     for (int j = tid; j < nh1; j += kMgThreads) L1.x[n1 + j] += a.tau * L2.x[hpar1[j]];
     __syncthreads();
     postsmooth(L1, cfu);
-    exchange(a.xg[1], base1, L1.x, n1, L1.x + n1, hidx1, nh1, epoch);
+    exchange(a.xu[1], nslot1, base1, L1.x, n1, L1.x + n1, hidx1, nh1);
+    MGP(5);
     // ---- level 0 up: correction, x += B (r - A x); the result is u
     for (int j = tid; j < nh0; j += kMgThreads) x0[n0 + j] += a.tau * L1.x[hpar0[j]];
 #pragma unroll
@@ -431,8 +471,9 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
       if (li < n0) x0[li] = xv[c];
     }
     __syncthreads();
+    MGP(6);
     // =================================== w = A u, the three dot products =============================================================
-    exchange(a.xg[0], base0, x0, n0, x0 + n0, hidx0, nh0, epoch);
+    exchange(a.xu[0], nslot0, base0, x0, n0, x0 + n0, hidx0, nh0);
     double gam = 0.0, del = 0.0, rho = 0.0;
 #pragma unroll
     for (int c = 0; c < CPT; ++c) {
@@ -459,15 +500,13 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
         D += __shfl_xor_sync(0xffffffffu, D, o);
         R += __shfl_xor_sync(0xffffffffu, R, o);
       }
-      if (lane == 0) { pp[4 * k] = G; pp[4 * k + 1] = D; pp[4 * k + 2] = R; }
-    }
-    grid_barrier(a.bar, epoch++ * a.nblk);
-    if (wid == 0) {  // fixed summation order -> the same bits in every CTA
-      double G = 0.0, D = 0.0, R = 0.0;
+      if (lane == 0) { __stcg(pp + 4 * k, mg_tag(G, bit)); __stcg(pp + 4 * k + 1, mg_tag(D, bit)); __stcg(pp + 4 * k + 2, mg_tag(R, bit)); }
+      // every CTA reads the tagged partials of every CTA (the same values, bit for bit) and sums them in a fixed order
+      G = 0.0; D = 0.0; R = 0.0;
       for (int q = lane; q < a.nblk; q += 32) {
-        G += __ldcg(pp + 4 * q);
-        D += __ldcg(pp + 4 * q + 1);
-        R += __ldcg(pp + 4 * q + 2);
+        G += mg_load(pp + 4 * q, bit);
+        D += mg_load(pp + 4 * q + 1, bit);
+        R += mg_load(pp + 4 * q + 2, bit);
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
@@ -480,6 +519,10 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     __syncthreads();
     gam = red[60]; del = red[61]; rho = red[62];
     __syncthreads();
+    MGP(7);
+#ifdef MG_PROF
+    if (tid == 0 && blockIdx.x == 0) g_mg_prof[10] += 1;
+#endif
     if (it == 0) stop2 = a.rtol * a.rtol * (bb_total >= 0.0 ? bb_total : rho);  // without a guess x_0 = 0: r_0 = rhs
     if (!(rho > stop2)) break;
     if (it >= a.max_iter) { not_converged = true; break; }
@@ -856,7 +899,16 @@ int nb_mg_build(nanobte_solver *h, Arena &A, const GenericTables &g, const doubl
     a.hptr[l] = A.put(hptr[l]);
     if (hidx[l].empty()) { hidx[l].push_back(0); hpar[l].push_back(0); }
     a.hidx[l] = A.put(hidx[l]); a.hpar[l] = A.put(hpar[l]);
-    a.xg[l] = A.zeros<double>((size_t)nslot[l]);
+  }
+  {  // everything that crosses CTA borders in one block (zeroed before every launch)
+    size_t nd = 0;
+    for (int l = 0; l < 3; ++l) nd += (size_t)4 * nslot[l];
+    nd += (size_t)2 * n3 + (size_t)8 * nblk + 64;
+    double *blk = A.zeros<double>(nd);
+    a.xbuf = blk; a.xbuf_bytes = nd * sizeof(double);
+    for (int l = 0; l < 3; ++l) { a.xg[l] = blk; blk += (size_t)2 * nslot[l]; a.xu[l] = blk; blk += (size_t)2 * nslot[l]; }
+    a.g3 = blk; blk += (size_t)2 * n3;
+    a.part = blk;
   }
   a.cell0 = A.put(cell0); a.nbr0 = A.put(nbr_h[0]); a.dinv0 = A.put(dinv_h[0]); a.diag0 = A.put(diag_h[0]);
   for (int l = 1; l < 3; ++l) { a.nbr[l] = A.put(nbr_h[l]); a.cnt[l] = A.put(cnt_h[l]); a.dinv[l] = A.put(dinv_h[l]); a.diag[l] = A.put(diag_h[l]); }
@@ -865,10 +917,8 @@ int nb_mg_build(nanobte_solver *h, Arena &A, const GenericTables &g, const doubl
   for (int l = 0; l < kMgMaxLevels; ++l) { a.n_l[l] = l < nlev ? n_l[l] : 0; a.off_l[l] = l < nlev ? off_l[l] : 0; }
   a.gnbr = A.put(gnbr); a.gcnt = A.put(gcnt); a.gchild = A.put(gchild); a.gpar = A.put(gpar);
   a.gdinv = A.put(gdinv); a.gdiag = A.put(gdiag); a.ginv = A.put(ginv);
-  a.g3 = A.zeros<double>((size_t)n3 + 8);
   a.xprev = A.zeros<double>((size_t)2 * nslot[0]);
   a.gpart = A.zeros<double>((size_t)8 * nblk + 8);
-  a.part = A.zeros<double>((size_t)8 * nblk + 8);
   a.bar = A.zeros<unsigned int>(4);
   a.cap0 = cap[0]; a.caph0 = caph[0]; a.cap1 = cap[1]; a.caph1 = caph[1]; a.cap2 = cap[2]; a.caph2 = caph[2];
   P->cpt = cpt; P->smem = smem; P->levels = nlev;
@@ -890,11 +940,21 @@ int nb_mg_solve(nanobte_solver *h) {
   if (!fn) return nb_fail(h, NANOBTE_E_INVALID, "internal: no multigrid CG variant for %d slots per thread", P.cpt);
   NB_CUDA(h, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem));
   NB_CUDA(h, cudaMemsetAsync(a.bar, 0, sizeof(unsigned int), h->stream));
+  NB_CUDA(h, cudaMemsetAsync(a.xbuf, 0, a.xbuf_bytes, h->stream));  // sequence bits start from zero (see mg_tag)
   void *args[] = {&a};
   NB_CUDA(h, cudaLaunchCooperativeKernel((void *)fn, dim3(a.nblk), dim3(kMgThreads), args, P.smem, h->stream));
   h->launches++;
   return 0;
 }
+
+#ifdef MG_PROF
+extern "C" int nanobte_debug_mg_prof(unsigned long long *out, int reset) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, g_mg_prof, sizeof(unsigned long long) * 16);
+  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_mg_prof, z, sizeof(z)); }
+  return 0;
+}
+#endif
 
 void nb_free_mg(nanobte_solver *h) {
   delete h->mg;

@@ -37,7 +37,11 @@ struct MgArgs {
   // (levels 0, 1: own slot or own count + halo position; level 2: global level-3 unknown)
   const int32_t *hidx[kMgDist];
   const int32_t *hpar[kMgDist];
-  double *xg[kMgDist];             // published iterates, per global slot
+  // published iterates per global slot, [2][nslot_l] each (double-buffered by iteration parity): xg = on the way down,
+  // xu = on the way up (level 0: u).  Every published value carries a sequence bit in its last mantissa bit (see
+  // exchange() in cg_mg.cu), so a reader needs no barrier: it re-reads until the bit is the current one.
+  double *xg[kMgDist], *xu[kMgDist];
+  void *xbuf; size_t xbuf_bytes;   // all of them, g3 and part: zeroed before every launch
   // levels 3 .. nlev-1, the same in every CTA
   int32_t nlev, n_l[kMgMaxLevels], off_l[kMgMaxLevels];  // unknowns per level, offset of the level in the arrays below
   const uint16_t *gnbr, *gcnt;     // [6][ntot]   (index inside the level)
@@ -45,7 +49,7 @@ struct MgArgs {
   const uint16_t *gpar;            // [ntot]      parent in the level above
   const double *gdinv, *gdiag;     // [ntot]
   const double *ginv;              // [nc][nc] inverse of the coarsest operator
-  double *g3;                      // [n3] published level-3 right-hand side
+  double *g3;                      // [2][n3] published level-3 right-hand side (tagged like the iterates)
   // recycled initial guess (as in cg.cu): the last two solutions per level-0 slot, and a reduction buffer
   int32_t nprev;
   double *xprev;                   // [2][nslot0]
@@ -55,7 +59,7 @@ struct MgArgs {
   const double *rhs_direct;        // non-null: the right-hand side itself (Fourier initial guess, R21)
   const int32_t *cellbf_ptr, *cellbf;
   double *x;                       // [n_act] solution, active-cell order
-  double *part;                    // [2][nblk][4]
+  double *part;                    // [2][nblk][4] tagged partial dot products
   unsigned int *bar;
   unsigned long long *iters_out;
   // shared-memory carve-up (element counts, the same for every CTA: maxima over the CTAs)
