@@ -95,14 +95,12 @@ __device__ __forceinline__ double apply_own(const Lv &L, const double *v, int i,
   return acc;
 }
 
-// x = B g with x = 0 before (two Jacobi steps on the own block); leaves x[0..n)
+// x = B g with x = 0 before (two Jacobi steps on the own block); leaves x[0..n).  Two block-synchronised phases.
 __device__ __forceinline__ void presmooth(const Lv &L, const double *cfu) {
   const int tid = threadIdx.x;
-  for (int i = tid; i < L.n; i += kMgThreads) L.x[i] = L.dinv[i] * L.g[i];
+  for (int i = tid; i < L.n; i += kMgThreads) L.tmp[i] = L.dinv[i] * L.g[i];
   __syncthreads();
-  for (int i = tid; i < L.n; i += kMgThreads) L.tmp[i] = L.x[i] + L.dinv[i] * (L.g[i] - apply_own(L, L.x, i, cfu));
-  __syncthreads();
-  for (int i = tid; i < L.n; i += kMgThreads) L.x[i] = L.tmp[i];
+  for (int i = tid; i < L.n; i += kMgThreads) L.x[i] = L.tmp[i] + L.dinv[i] * (L.g[i] - apply_own(L, L.tmp, i, cfu));
   __syncthreads();
 }
 // res = g - A x (halo of x valid)
@@ -110,11 +108,14 @@ __device__ __forceinline__ void residual(const Lv &L, const double *cfu) {
   for (int i = threadIdx.x; i < L.n; i += kMgThreads) L.res[i] = L.g[i] - apply_full(L, L.x, i, cfu);
   __syncthreads();
 }
-// x += B (g - A x)   (halo of x valid; the halo is not updated)
+// x += B (g - A x)   (halo of x valid; the halo is not updated).  Two block-synchronised phases.
 __device__ __forceinline__ void postsmooth(const Lv &L, const double *cfu) {
   const int tid = threadIdx.x;
-  residual(L, cfu);
-  for (int i = tid; i < L.n; i += kMgThreads) L.tmp[i] = L.dinv[i] * L.res[i];
+  for (int i = tid; i < L.n; i += kMgThreads) {
+    const double r = L.g[i] - apply_full(L, L.x, i, cfu);
+    L.res[i] = r;
+    L.tmp[i] = L.dinv[i] * r;
+  }
   __syncthreads();
   for (int i = tid; i < L.n; i += kMgThreads)
     L.x[i] += L.tmp[i] + L.dinv[i] * (L.res[i] - apply_own(L, L.tmp, i, cfu));
@@ -341,15 +342,13 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     for (int c = 0; c < CPT; ++c) {
       const int li = tid + c * kMgThreads;
       xv[c] = dv[c] * r[c];
-      if (li < n0) x0[li] = xv[c];
+      if (li < n0) y0[li] = xv[c];
     }
-    __syncthreads();
-#pragma unroll
-    for (int c = 0; c < CPT; ++c) xv[c] += dv[c] * (r[c] - A0own(c, x0, xv[c]));
     __syncthreads();
 #pragma unroll
     for (int c = 0; c < CPT; ++c) {
       const int li = tid + c * kMgThreads;
+      xv[c] += dv[c] * (r[c] - A0own(c, y0, xv[c]));
       if (li < n0) x0[li] = xv[c];
     }
     __syncthreads();
