@@ -130,6 +130,12 @@ typedef struct {
   int32_t sweep_variant;        /* 0 = auto; 3 = hyperplane sweep, single-buffered state (any spacing); 4 = hyperplane sweep,
                                    double-buffered (uniform); 5 = tile-dataflow sweep with fused moments (3-D, uniform;
                                    what auto picks there unless sweep_G / sweep_threads are given)              */
+  /* Band shards (the (direction, band) tasks are distributed, the mesh is replicated, the contributions are
+   * merged by one all-reduce per iteration).  A solver created on a SUBSET of the band table takes the sums over the
+   * WHOLE table here (> 0; 0 = computed from the bands given): beta = sum_b C_b/tau_b (Eq. 5), sum_b C_b (R13) and
+   * kappa (R14d); bands.src_share then carries the source shares of the subset in the whole table.  Its moments are the
+   * subset's terms of the global sums: nanobte_export_moments / nanobte_import_moments. */
+  double beta_total, Csum_total, kappa_total;
 } nanobte_options;
 
 /* Layout / schedule facts of a created solver (for reporting and roofline arithmetic). */
@@ -193,6 +199,20 @@ int nanobte_update_temperature(nanobte_solver *, double *max_dT);
  * Returns NANOBTE_NOT_CONVERGED (state valid, T updated with the last CG iterate) when the CG stopped on
  * options.cg_max_iter with ||r|| > cg_rtol ||rhs||. */
 int nanobte_diffusion_correct(nanobte_solver *, int32_t *cg_iters, double *max_dT);
+
+/* Band-sharded runs (Eq. 14), see nanobte_options.beta_total.  After nanobte_update_temperature on every
+ * shard, nanobte_export_moments writes this shard's terms of the update, [n_active] T_SI - T_ref (Eq. 5), [n_active]
+ * T_energy - T_ref (R13), [n_active][3] q (Eq. 7), [n_bfaces] the heat flux leaking through reflecting faces summed over the
+ * shard's bands (R14c'), nanobte_moments_len doubles in all; the caller sums the buffers of all shards element-wise (one
+ * all-reduce) and hands the result to nanobte_import_moments on every shard, which sets the three fields and the leak,
+ * T <- T_SI (Eq. 6) and returns max|T_new - T_old| (host pointer or NULL; synchronises iff != NULL).  A synthetic
+ * correction (nanobte_diffusion_correct) after the import uses the imported leak; every shard then solves the same
+ * system and ends with the same T.  dst / src: device pointers if *_is_device != 0, else host. */
+int nanobte_band_totals(const nanobte_bands *whole_table, const nanobte_quadrature *, int32_t dim,
+                        double *out /* [3] host: beta, sum C, kappa of the whole table */);
+int64_t nanobte_moments_len(const nanobte_solver *);
+int nanobte_export_moments(nanobte_solver *, double *dst, int32_t dst_is_device);
+int nanobte_import_moments(nanobte_solver *, const double *src, int32_t src_is_device, double *max_dT);
 
 /* Fourier initial guess (section IV: "A Fourier diffusion solve provides the initial temperature guess";
  * reading R21): T <- the solution of the steady heat-conduction problem -div(kappa grad T) = Qdot with T = T_w on

@@ -21,7 +21,8 @@ ERRORS = {0: "OK", 1: "NOT_CONVERGED", -1: "INVALID", -2: "ALLOC", -3: "CUDA", -
 EXPORTS = [
     "nanobte_workspace_bytes_structured", "nanobte_workspace_bytes_unstructured", "nanobte_create_structured",
     "nanobte_create_unstructured", "nanobte_destroy", "nanobte_sweep", "nanobte_update_temperature",
-    "nanobte_diffusion_correct", "nanobte_init_fourier", "nanobte_step", "nanobte_set_keep_e", "nanobte_solve", "nanobte_set_T", "nanobte_get_T", "nanobte_get_q", "nanobte_get_e",
+    "nanobte_diffusion_correct", "nanobte_init_fourier", "nanobte_band_totals", "nanobte_moments_len", "nanobte_export_moments",
+    "nanobte_import_moments", "nanobte_step", "nanobte_set_keep_e", "nanobte_solve", "nanobte_set_T", "nanobte_get_T", "nanobte_get_q", "nanobte_get_e",
     "nanobte_get_G", "nanobte_get_boundary_heat", "nanobte_get_history", "nanobte_get_info", "nanobte_launch_count",
     "nanobte_kappa", "nanobte_strerror", "nanobte_last_error",
 ]
@@ -57,7 +58,8 @@ class UnstructuredMesh(C.Structure):
 class Options(C.Structure):
     _fields_ = [("T_ref", C.c_double), ("T_init", _dp), ("stream", C.c_void_p), ("workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("cg_rtol", C.c_double), ("cg_max_iter", C.c_int32),
-                ("sweep_G", C.c_int32), ("sweep_threads", C.c_int32), ("sweep_variant", C.c_int32)]
+                ("sweep_G", C.c_int32), ("sweep_threads", C.c_int32), ("sweep_variant", C.c_int32),
+                ("beta_total", C.c_double), ("Csum_total", C.c_double), ("kappa_total", C.c_double)]
 
 
 class Info(C.Structure):
@@ -102,6 +104,10 @@ def load():
     lib.nanobte_update_temperature.argtypes = [vp, _dp]
     lib.nanobte_diffusion_correct.argtypes = [vp, _ip, _dp]
     lib.nanobte_init_fourier.argtypes = [vp, _ip]
+    lib.nanobte_moments_len.argtypes = [vp]
+    lib.nanobte_moments_len.restype = C.c_int64
+    lib.nanobte_export_moments.argtypes = [vp, C.c_void_p, C.c_int32]
+    lib.nanobte_import_moments.argtypes = [vp, C.c_void_p, C.c_int32, _dp]
     lib.nanobte_step.argtypes = [vp, C.c_int32, _dp, _ip]
     lib.nanobte_set_keep_e.argtypes = [vp, C.c_int32]
     lib.nanobte_solve.argtypes = [vp, C.c_double, C.c_int32, C.c_int32, _ip, _dp]
@@ -182,7 +188,7 @@ def workspace_bytes(problem, sweep_G=0, sweep_threads=0, sweep_variant=0):
     """Device bytes a Solver for this problem needs (host-only call; also validates the problem)."""
     lib = load()
     ms = _Marshalled(problem)
-    opt = Options(float(problem["T_ref"]), None, None, None, 0, 0.0, 0, sweep_G, sweep_threads, sweep_variant)
+    opt = Options(float(problem["T_ref"]), None, None, None, 0, 0.0, 0, sweep_G, sweep_threads, sweep_variant, 0.0, 0.0, 0.0)
     out = C.c_size_t()
     fn = lib.nanobte_workspace_bytes_structured if ms.kind == "structured" else lib.nanobte_workspace_bytes_unstructured
     rc = fn(C.byref(ms.mesh), C.byref(ms.bands), C.byref(ms.quad), ms.tags, ms.n_tags, C.byref(opt), C.byref(out))
@@ -195,7 +201,8 @@ class Solver:
     """One problem instance on the current CUDA device (same call shapes as the C ABI)."""
 
     def __init__(self, problem, T_init=None, cg_rtol=1e-12, cg_max_iter=100000, share=None, sweep_G=0,
-                 sweep_threads=0, sweep_variant=0, own_workspace=True):
+                 sweep_threads=0, sweep_variant=0, own_workspace=True, totals=None):
+        """totals = (beta, Csum, kappa) of the whole band table when `problem` carries a band shard (nanobte_options)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("nanobte needs a CUDA device (sm_100); there is no CPU fallback")
@@ -206,7 +213,8 @@ class Solver:
         self.B, self.D = ms.bands.B, ms.quad.D
         self.stream = torch.cuda.current_stream()
         opt = Options(float(problem["T_ref"]), _p(ms.keep["Ti"], _dp), C.c_void_p(self.stream.cuda_stream), None, 0,
-                      float(cg_rtol), int(cg_max_iter), int(sweep_G), int(sweep_threads), int(sweep_variant))
+                      float(cg_rtol), int(cg_max_iter), int(sweep_G), int(sweep_threads), int(sweep_variant),
+                      *(tuple(float(x) for x in totals) if totals is not None else (0.0, 0.0, 0.0)))
         structured = ms.kind == "structured"
         self._ws = None
         if own_workspace:  # device memory is a torch tensor (PyTorch: buffers and streams only)
@@ -276,6 +284,22 @@ class Solver:
         it, d = C.c_int32(), C.c_double()
         self._chk(self._lib.nanobte_diffusion_correct(self._h, C.byref(it), C.byref(d)))
         return it.value, d.value
+
+    def export_moments(self, out=None):
+        """nanobte_export_moments into a device tensor (torch, float64, nanobte_moments_len long): this shard's terms."""
+        n = int(self._lib.nanobte_moments_len(self._h))
+        if out is None:
+            out = self._torch.empty(n, dtype=self._torch.float64, device="cuda")
+        assert out.is_cuda and out.dtype == self._torch.float64 and out.numel() == n and out.is_contiguous()
+        self._chk(self._lib.nanobte_export_moments(self._h, C.c_void_p(out.data_ptr()), 1))
+        return out
+
+    def import_moments(self, buf, sync=True):
+        """nanobte_import_moments from a device tensor holding the element-wise sum over all shards; returns max|dT|."""
+        assert buf.is_cuda and buf.dtype == self._torch.float64 and buf.is_contiguous()
+        d = C.c_double()
+        self._chk(self._lib.nanobte_import_moments(self._h, C.c_void_p(buf.data_ptr()), 1, C.byref(d) if sync else None))
+        return d.value if sync else None
 
     def init_fourier(self):
         """nanobte_init_fourier: T <- Fourier (steady conduction) solution, PAPER.md:228 / R21; returns the CG iterations."""

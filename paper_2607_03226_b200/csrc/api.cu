@@ -209,6 +209,7 @@ int nb_upload_generic(nanobte_solver *h, Arena &A, const Common &c, GenericTable
   h->cellbf_ptr = A.put(g.cellbf_ptr);
   h->cellbf = A.put(g.cellbf);
   h->fourier_rhs = A.put(g.fourier_rhs);
+  h->leak_sum = A.zeros<double>(nbf + 8);
   h->cg_x = A.zeros<double>(na);
   h->cg_r = A.zeros<double>(na);
   h->cg_p0 = A.zeros<double>(na);
@@ -390,6 +391,7 @@ extern "C" int nanobte_update_temperature(nanobte_solver *h, double *max_dT) {
   }
   if ((rc = nb_launch_moments(h)) < 0) return rc;   // O4
   if ((rc = nb_launch_update(h, 0)) < 0) return rc; // O5
+  h->leak_imported = false;  // a correction after this update sums its own bands' face fluxes unless moments are imported
   if (max_dT) return read_maxdT(h, max_dT);
   return 0;
 }
@@ -412,6 +414,53 @@ extern "C" int nanobte_diffusion_correct(nanobte_solver *h, int32_t *cg_iters, d
     nb_fail(h, NANOBTE_NOT_CONVERGED, "CG stopped at cg_max_iter = %d above rtol = %g", h->cg_max_iter, h->cg_rtol);
     return NANOBTE_NOT_CONVERGED;
   }
+  return 0;
+}
+
+// ---- band shards (Eq. 14): this shard's terms of the update out, the sums over all shards in ---------------------------
+// The sums a shard needs about the WHOLE band table: out[0] = beta, out[1] = sum C, out[2] = kappa (same code as create).
+extern "C" int nanobte_band_totals(const nanobte_bands *bands, const nanobte_quadrature *quad, int32_t dim, double *out) {
+  if (!out || (dim != 2 && dim != 3)) return NANOBTE_E_INVALID;
+  nanobte_solver tmp;
+  Common c;
+  const int rc = nb_validate_common(&tmp, dim, bands, quad, nullptr, 0, c);
+  if (rc < 0) return rc;
+  out[0] = c.beta; out[1] = c.Csum; out[2] = c.kappa;
+  return 0;
+}
+
+extern "C" int64_t nanobte_moments_len(const nanobte_solver *h) { return h ? (int64_t)5 * h->n_act + h->n_bf : 0; }
+
+extern "C" int nanobte_export_moments(nanobte_solver *h, double *dst, int32_t dst_is_device) {
+  if (!h || !h->arena || !dst) return NANOBTE_E_INVALID;
+  const size_t na = (size_t)h->n_act;
+  double *stage = dst_is_device ? dst : h->part;  // part holds >= 3 n_cells + 64 doubles; the leak goes through leak_sum
+  const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  int rc = nb_launch_leak_sum(h);  // leak_sum[bf] = sum over this shard's bands of the face flux (R14c')
+  if (rc < 0) return rc;
+  (void)stage;
+  NB_CUDA(h, cudaMemcpyAsync(dst, h->theta_SI, na * sizeof(double), kind, h->stream));
+  NB_CUDA(h, cudaMemcpyAsync(dst + na, h->theta_en, na * sizeof(double), kind, h->stream));
+  NB_CUDA(h, cudaMemcpyAsync(dst + 2 * na, h->q, 3 * na * sizeof(double), kind, h->stream));
+  if (h->n_bf) NB_CUDA(h, cudaMemcpyAsync(dst + 5 * na, h->leak_sum, (size_t)h->n_bf * sizeof(double), kind, h->stream));
+  if (!dst_is_device) NB_CUDA(h, cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+extern "C" int nanobte_import_moments(nanobte_solver *h, const double *src, int32_t src_is_device, double *max_dT) {
+  if (!h || !h->arena || !src) return NANOBTE_E_INVALID;
+  const size_t na = (size_t)h->n_act;
+  const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  NB_CUDA(h, cudaMemcpyAsync(h->theta_SI, src, na * sizeof(double), kind, h->stream));
+  NB_CUDA(h, cudaMemcpyAsync(h->theta_en, src + na, na * sizeof(double), kind, h->stream));
+  NB_CUDA(h, cudaMemcpyAsync(h->q, src + 2 * na, 3 * na * sizeof(double), kind, h->stream));
+  if (h->n_bf) NB_CUDA(h, cudaMemcpyAsync(h->leak_sum, src + 5 * na, (size_t)h->n_bf * sizeof(double), kind, h->stream));
+  h->leak_imported = true;
+  // T <- T_SI (Eq. 6) and max|T_new - T_old| through the update kernel's "T_SI + delta" form with delta = 0
+  NB_CUDA(h, cudaMemsetAsync(h->cg_x, 0, na * sizeof(double), h->stream));
+  int rc = nb_launch_update(h, 1);
+  if (rc < 0) return rc;
+  if (max_dT) return read_maxdT(h, max_dT);
   return 0;
 }
 

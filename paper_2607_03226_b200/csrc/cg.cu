@@ -23,6 +23,7 @@ struct CgArgs {
   const double *diag;    // [n]      sum of interior + thermalizing face coefficients
   const double *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
   const double *rhs_direct;  // non-null: the right-hand side itself (Fourier initial guess, R21)
+  const double *leak_sum;    // non-null: [n_bf] the face leak summed over all bands (band shards)
   const int32_t *cellbf_ptr, *cellbf;
   double *x, *r, *p0, *p1, *ap, *partial;
   unsigned long long *iters_out;
@@ -74,7 +75,8 @@ __global__ void __launch_bounds__(256) cg_kernel(CgArgs a) {
       for (int k = a.cellbf_ptr[i]; k < a.cellbf_ptr[i + 1]; ++k) {
         const int bf = a.cellbf[k];
         double F = 0.0;
-        for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
+        if (a.leak_sum) F = a.leak_sum[bf];
+        else for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
         rhs += a.bf_area[bf] * F;
       }
     }
@@ -149,6 +151,7 @@ struct CgfArgs {
   const int32_t *nloc, *perm;
   const double *coef, *diag, *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
   const double *rhs_direct;  // non-null: the right-hand side itself (Fourier initial guess, R21)
+  const double *leak_sum;    // non-null: [n_bf] the face leak summed over all bands (band shards)
   const int32_t *cellbf_ptr, *cellbf, *hptr, *hidx;
   double *x, *w, *part;
   unsigned int *bar;
@@ -228,7 +231,8 @@ __global__ void __launch_bounds__(kCgfThreads, 1) cg_fused_kernel(CgfArgs a) {
         for (int q = a.cellbf_ptr[io]; q < a.cellbf_ptr[io + 1]; ++q) {  // R14c'
           const int bf = a.cellbf[q];
           double F = 0.0;
-          for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
+          if (a.leak_sum) F = a.leak_sum[bf];
+          else for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
           rhs += a.bf_area[bf] * F;
         }
       }
@@ -499,6 +503,7 @@ static int cg_solve_fused(nanobte_solver *h) {
   a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev; a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area;
   a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf; a.hptr = h->cgf_hptr; a.hidx = h->cgf_hidx;
   a.rhs_direct = h->cg_rhs_direct;
+  a.leak_sum = h->leak_imported ? h->leak_sum : nullptr;
   a.x = h->cg_x; a.w = h->cgf_w; a.part = h->cgf_part; a.bar = h->cgf_bar;
   a.iters_out = h->d_maxdT + 1;
   a.beta = h->beta; a.rtol = h->cg_rtol;
@@ -531,6 +536,7 @@ int nb_cg_solve(nanobte_solver *h, int *iters) {
   a.vol = h->vol; a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev;
   a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area; a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf;
   a.rhs_direct = h->cg_rhs_direct;
+  a.leak_sum = h->leak_imported ? h->leak_sum : nullptr;
   a.x = h->cg_x; a.r = h->cg_r; a.p0 = h->cg_p0; a.p1 = h->cg_p1; a.ap = h->cg_rhs; a.partial = h->cg_partial;
   a.iters_out = h->d_maxdT + 1;
   a.beta = h->beta; a.rtol = h->cg_rtol;

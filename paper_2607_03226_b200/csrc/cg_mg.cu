@@ -216,7 +216,8 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
           for (int q = a.cellbf_ptr[io]; q < a.cellbf_ptr[io + 1]; ++q) {  // R14c'
             const int bf = a.cellbf[q];
             double F = 0.0;
-            for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
+            if (a.leak_sum) F = a.leak_sum[bf];
+            else for (int b = 0; b < a.B; ++b) F += a.faceflux[(size_t)bf * a.B + b];
             rhs += a.bf_area[bf] * F;
           }
         }
@@ -932,6 +933,7 @@ int nb_mg_solve(nanobte_solver *h) {
   a.max_iter = h->cg_max_iter; a.B = h->B; a.rtol = h->cg_rtol; a.beta = h->beta;
   a.vol = h->vol; a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev; a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area;
   a.rhs_direct = h->cg_rhs_direct;
+  a.leak_sum = h->leak_imported ? h->leak_sum : nullptr;
   a.nprev = h->cgf_nprev;  // the history counter of the handle (reset by solve / set_T / a failed or foreign solve)
   h->cgf_nprev = std::min(2, h->cgf_nprev + 1);
   a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf; a.x = h->cg_x; a.iters_out = h->d_maxdT + 1;

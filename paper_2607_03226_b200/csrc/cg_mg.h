@@ -57,6 +57,7 @@ struct MgArgs {
   // right-hand side, result, reductions
   const double *vol, *theta_SI, *theta_prev, *faceflux, *bf_area;
   const double *rhs_direct;        // non-null: the right-hand side itself (Fourier initial guess, R21)
+  const double *leak_sum;          // non-null: [n_bf] the face leak summed over all bands (band shards)
   const int32_t *cellbf_ptr, *cellbf;
   double *x;                       // [n_act] solution, active-cell order
   double *part;                    // [2][nblk][4] tagged partial dot products

@@ -143,6 +143,8 @@ struct nanobte_solver {
   const int32_t *cellbf_ptr = nullptr, *cellbf = nullptr;  // CSR: reflecting boundary faces of each active cell
   const double *fourier_rhs = nullptr;   // [n_act] right-hand side of the Fourier initial guess (R21)
   const double *cg_rhs_direct = nullptr; // non-null: the CG kernels take this right-hand side instead of R14c/R14c'
+  double *leak_sum = nullptr;            // [n_bf] band shards: the R14c' leak summed over ALL bands (nanobte_import_moments)
+  bool leak_imported = false;            // the CG takes leak_sum instead of summing its own bands' face fluxes
   int cg_nf = 0;
   double *cg_x = nullptr, *cg_r = nullptr, *cg_p0 = nullptr, *cg_p1 = nullptr, *cg_rhs = nullptr, *cg_scal = nullptr;
   double *cg_partial = nullptr;
@@ -192,6 +194,7 @@ int nb_launch_get_e(nanobte_solver *h, int b0, int nb, int d0, int nd, double *d
 int nb_launch_scatter_cells(nanobte_solver *h, const double *src_act, double *dst_cells, int ncomp, double add);
 int nb_launch_set_theta(nanobte_solver *h, const double *T_cells_dev);
 int nb_launch_tagheat(nanobte_solver *h);
+int nb_launch_leak_sum(nanobte_solver *h);
 int nb_cg_solve(nanobte_solver *h, int *iters);
 int nb_cg_blocks(nanobte_solver *h);
 // sweep_structured.cu

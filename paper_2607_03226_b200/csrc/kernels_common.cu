@@ -569,3 +569,20 @@ int nb_launch_tagheat(nanobte_solver *h) {
   NB_CUDA(h, cudaGetLastError());
   return 0;
 }
+
+// ---- band shards: the reflecting-face leak of R14c' summed over this solver's bands (nanobte_export_moments) -----------------------------
+__global__ void leak_sum_kernel(int n_bf, int B, const double *faceflux, double *leak) {
+  const int bf = blockIdx.x * blockDim.x + threadIdx.x;
+  if (bf >= n_bf) return;
+  double F = 0.0;
+  for (int b = 0; b < B; ++b) F += faceflux[(size_t)bf * B + b];
+  leak[bf] = F;
+}
+
+int nb_launch_leak_sum(nanobte_solver *h) {
+  if (h->n_bf == 0) return 0;
+  leak_sum_kernel<<<(h->n_bf + 255) / 256, 256, 0, h->stream>>>(h->n_bf, h->B, h->bd.faceflux, h->leak_sum);
+  h->launches++;
+  NB_CUDA(h, cudaGetLastError());
+  return 0;
+}

@@ -65,6 +65,14 @@ int build(nanobte_solver *h, const nanobte_structured_mesh *m, const nanobte_ban
   Common cm;
   int rc = nb_validate_common(h, dim, bands, quad, tags, n_tags, cm);
   if (rc) return rc;
+  // band shard: the sums over the whole band table come from the caller (nanobte_options)
+  if (opt->beta_total > 0.0) cm.beta = opt->beta_total;
+  if (opt->Csum_total > 0.0) {
+    cm.Csum = opt->Csum_total;
+    if (bands->src_share == nullptr)  // source shares of the shard's bands in the whole table (R5)
+      for (int b = 0; b < cm.B; ++b) cm.share[b] = cm.C[b] / cm.Csum;
+  }
+  if (opt->kappa_total > 0.0) cm.kappa = opt->kappa_total;
   const int B = cm.B, D = cm.D;
 
   GenericTables G;

@@ -497,6 +497,14 @@ int build_uns(nanobte_solver *h, const nanobte_unstructured_mesh *m, const nanob
   Common cm;
   int rc = nb_validate_common(h, 2, bands, quad, tags, n_tags, cm);
   if (rc) return rc;
+  // band shard: the sums over the whole band table come from the caller (nanobte_options)
+  if (opt->beta_total > 0.0) cm.beta = opt->beta_total;
+  if (opt->Csum_total > 0.0) {
+    cm.Csum = opt->Csum_total;
+    if (bands->src_share == nullptr)  // source shares of the shard's bands in the whole table (R5)
+      for (int b = 0; b < cm.B; ++b) cm.share[b] = cm.C[b] / cm.Csum;
+  }
+  if (opt->kappa_total > 0.0) cm.kappa = opt->kappa_total;
   const int B = cm.B, D = cm.D;
   const int nf = m->cell_ptr[nc];
   if (m->cell_ptr[0] != 0 || nf < 3 * nc) return nb_fail(h, NANOBTE_E_INVALID, "bad cell_ptr");

@@ -459,6 +459,64 @@ def test_fourier_guess_then_solve_counts():
     g.close(); r.close()
 
 
+# ---- band shards (Eq. 14) -------------------------------------------------------------------------------
+@pytest.mark.parametrize("which,mode,world", [("cube", "plain", 2), ("finfet", "synthetic", 2), ("finfet", "synthetic", 3),
+                                              ("triangles", "plain", 2), ("square", "plain", 4)])
+def test_band_shards_on_one_gpu_match_the_unsharded_solver(which, mode, world):
+    """`world` shards of the band table side by side on one GPU (they never wait for one another: the test sums their
+    exported buffers where a process group would all-reduce them): after every step every shard holds the lattice
+    temperature of the unsharded solver and of the oracle, the CG counts agree, and a converged run takes the same number
+    of iterations."""
+    from paper_2607_03226_b200.sharded import ShardedSolver
+    pr = {"cube": lambda: wl.config_cube(n=12, B=5, n_polar=2, n_azim=8, mode="synthetic"),
+          "finfet": lambda: wl.config_finfet(nx=24, ny=12, nz=12, B=6, n_polar=2, n_azim=8),
+          "triangles": lambda: wl.config_triangles(n=16, side=1e-7, B=5, D=8, hole_radius=1.5e-8),
+          "square": lambda: wl.config_nongray_square(n=24, B=6, D=8)}[which]()
+    shards = [ShardedSolver(pr, r, world) for r in range(world)]
+    g, r = gpu_solver(pr), RefSolver(pr)
+    assert sorted(b for s in shards for b in s.bands) == list(range(len(pr["bands"]["C"])))
+    for n in range(3):
+        bufs = [s.local_update() for s in shards]
+        tot = bufs[0].clone()
+        for b in bufs[1:]:
+            tot += b
+        outs = [s.finish(tot, mode) for s in shards]
+        g.sweep(); r.sweep()
+        dg, dr = g.update_temperature(), r.update_temperature()
+        ig = ir = 0
+        if mode == "synthetic":
+            (ig, dg), (ir, dr) = g.diffusion_correct(), r.diffusion_correct()
+        Tg, Tr = g.get_T(0) - pr["T_ref"], r.get_T(0) - pr["T_ref"]
+        for s, (dT, it) in zip(shards, outs):
+            Ts = s.local.get_T(0) - pr["T_ref"]
+            assert rel(Ts, Tg) <= 1e-9 and rel(Ts, Tr) <= 1e-9, (n, rel(Ts, Tg), rel(Ts, Tr))
+            assert abs(dT - dg) <= 1e-8 * abs(dg) + 1e-13
+            assert abs(it - ig) <= max(2, ig // 10)
+            for which_T in (1, 2):
+                assert rel(s.local.get_T(which_T) - pr["T_ref"], r.get_T(which_T) - pr["T_ref"]) <= 1e-9
+            assert rel(s.local.get_q(), r.get_q()) <= 1e-9
+        assert np.array_equal(shards[0].local.get_T(0), shards[-1].local.get_T(0))  # bitwise the same on every shard
+    for s in shards:
+        s.close()
+    # converged: same count as the unsharded oracle
+    shards = [ShardedSolver(pr, k, world) for k in range(world)]
+    r2 = RefSolver(pr)
+    rr = r2.solve(1e-9, 3000, mode)
+    n, dT = 0, 1.0
+    while dT >= 1e-9 and n < 3000:
+        bufs = [s.local_update() for s in shards]
+        tot = bufs[0].clone()
+        for b in bufs[1:]:
+            tot += b
+        dT = max(s.finish(tot, mode)[0] for s in shards)
+        n += 1
+    assert rr["converged"] and n == rr["iters"], (n, rr)
+    assert np.abs(shards[0].local.get_T(0) - r2.get_T(0)).max() <= TOL_T_CONVERGED
+    for s in shards:
+        s.close()
+    g.close(); r.close(); r2.close()
+
+
 def test_cg_not_converged_is_reported():
     """cg_max_iter too small: diffusion_correct and solve say NOT_CONVERGED (1) instead of OK."""
     pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
