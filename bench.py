@@ -47,6 +47,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-convergence", action="store_true", help="skip the time-to-convergence run")
     ap.add_argument("--cpu-sample-bands", type=int, default=0, help="bands in the oracle's sample (0 = auto)")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "bands"],
+                    help="N > 1: independent replicas (default; the north_star keeps the path on one GPU) or ONE problem with the band "
+                         "table split over the ranks and one all-reduce per iteration (PAPER.md:115-121; strong scaling)")
     ap.add_argument("--sweep-G", type=int, default=0)
     ap.add_argument("--sweep-threads", type=int, default=0)
     ap.add_argument("--sweep-variant", type=int, default=0)
@@ -202,6 +205,44 @@ def run_oracle(pr, mode, steps, warmup, n_bands, threads):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
+def bench_band_shards(args, pr, mode, rank, world, local, dist, skw):
+    """--shard bands: ONE problem, the band table split over the ranks (paper_2607_03226_b200/sharded.py), one NCCL all-reduce
+    of the update tensor per source iteration.  Strong scaling: value = updates of the whole problem / time."""
+    import torch
+    from paper_2607_03226_b200 import replicas, sharded
+    from paper_2607_03226_b200 import workloads as wl
+    s = sharded.ShardedSolver(pr, rank, world, dist=dist, **skw)
+    upd = wl.n_updates(pr)
+    for _ in range(args.warmup):
+        s.step(mode)
+    replicas.barrier(dist, torch.cuda.synchronize)
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.local.launches
+    sampler.start()
+    e0.record()
+    cg = [s.step(mode)[1] for _ in range(args.steps)]
+    e1.record()
+    replicas.barrier(dist, torch.cuda.synchronize)
+    clocks = sampler.stop()
+    ms = replicas.max_over_ranks(e0.elapsed_time(e1), dist, "cuda") / args.steps
+    n_len = 5 * s.local.n_active + s.local.n_bf
+    out = {"metric": METRIC, "value": upd / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_config(pr, mode, {"parallelism": f"band shards x{world}, one all-reduce of {n_len} doubles per iteration",
+                                                "bands_of_rank0": len(s.bands)}),
+           "cg_iters_per_step": float(np.mean(cg)) if cg else 0.0, "gpu_launches": int(s.local.launches - l0), "clocks": clocks,
+           "e2e": {"value": upd / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 16,
+                   "note": "band-shard arm: device-resident state, one 16-byte read per step (max|dT|, CG count)"}}
+    s.close()
+    if rank == 0:
+        print(json.dumps(out))
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     args = parse_args()
     from paper_2607_03226_b200 import replicas
@@ -243,6 +284,8 @@ def main():
     from paper_2607_03226_b200.binding import Solver
 
     skw = dict(sweep_G=args.sweep_G, sweep_threads=args.sweep_threads, sweep_variant=args.sweep_variant)
+    if args.shard == "bands":
+        return bench_band_shards(args, pr, mode, rank, world, local, dist, skw)
     t_c0 = time.perf_counter()
     g = Solver(pr, **skw)
     g.set_keep_e(False)  # the sweeps of an iteration leave eps where solve() leaves it (on chip where the kernel can)

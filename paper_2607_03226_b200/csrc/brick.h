@@ -75,6 +75,14 @@ struct BrickCG {
   int64_t coef_base;           // [S][5] sweep coefficients, then [nd][4] (w, w s), then [nb][2] (1/tau, v)
 };
 
+// One boundary-inflow row of a class, everything the closure kernel needs about it in one 16-byte load.
+struct BrickInRow {
+  int32_t bf;          // boundary face
+  int32_t row;         // inflow row (of every group of the class)
+  int32_t msrc;        // wall row, in the mirror class, of the cell the specular part comes from (-1: none)
+  uint8_t type, cm, perm, pad;  // face type; mirror class; which direction permutation of the class (BrickState::in_perm)
+};
+
 struct BrickArgs {
   const BrickTask *tasks;      // in launch (topological) order
   const BrickCG *cgs;
@@ -111,6 +119,10 @@ struct BrickState {
   const int32_t *cg_of = nullptr;                      // [n_cls][B] (class, band) -> cg
   const int32_t *a2pos = nullptr;                      // [n_cls][n_act]
   const int32_t *pos2a = nullptr;                      // [npos of class 0]
+  const BrickInRow *in_rec[NB_MAX_CLASSES] = {nullptr};  // per class [n_in]: records of the fast inflow kernel
+  const uint8_t *in_perm = nullptr;                    // [n_cls][8][16] direction -> mirrored direction (local indices; 255: none)
+  int32_t cg0[NB_MAX_CLASSES] = {0};                   // first (class, group) of a class
+  bool in_fast = false;                                // the records are valid (same band groups in every class, <= 8 permutations)
   double *th[NB_MAX_CLASSES] = {nullptr};
 };
 

@@ -29,6 +29,7 @@ struct BrickHost {
     std::vector<int32_t> in_row, in_bf;             // boundary-inflow rows and their faces
     std::vector<int32_t> out_bf, out_row;           // outgoing faces and the wall row of their cell, wall-row order
     std::vector<uint8_t> out_ord;                   // rank of the class among the face's outgoing classes
+    std::vector<BrickInRow> in_rec;                 // records of the fast inflow kernel
     int npos = 0, nrow = 0, nwall = 0, scratch_row = 0;
   };
   int ncls = 0;
@@ -37,7 +38,9 @@ struct BrickHost {
   std::vector<BrickCG> cgs;
   std::vector<double> coef;
   std::vector<int32_t> cg_of, dir_local, bf_wrow, a2pos;
-  std::vector<uint8_t> bf_nord;
+  std::vector<uint8_t> bf_nord, in_perm;
+  std::vector<int32_t> cg0;
+  bool in_fast = false;
   int64_t inf_total = 0, wall_total = 0, part_total = 0, e_total = 0;
 };
 

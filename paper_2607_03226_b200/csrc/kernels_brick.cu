@@ -32,6 +32,10 @@ struct BrickClosureArgs {
   int32_t n_in[NB_MAX_CLASSES];
   const int32_t *bf_wrow;    // [n_cls][n_bf]
   int32_t init;
+  // fast inflow kernel
+  const BrickInRow *in_rec[NB_MAX_CLASSES];
+  const uint8_t *in_perm;    // [n_cls][8][16]
+  int32_t cg0[NB_MAX_CLASSES];
 };
 
 // gnum share of one class: sum over the class's directions of w (s.n) eps at the wall cell (R7).  One thread per
@@ -85,6 +89,60 @@ __global__ void __launch_bounds__(kBrickMaxS) brick_inflow_kernel(const BrickClo
   const BrickCG Gm = R.cgs[R.cg_of[cm * a.B + b]];
   const double spec = R.wall[Gm.wall_base + (int64_t)R.bf_wrow[(size_t)cm * a.n_bf + bf] * kBrickRow + (b - Gm.b0) * Gm.nd + R.dir_local[md]];
   *dst = type == NANOBTE_SPECULAR ? spec : a.bf_p[bf] * spec + (1.0 - a.bf_p[bf]) * Gf;  // R8
+}
+
+// The same from the per-row records built at create (BrickInRow): a CTA takes kInRows consecutive rows of one (class, group),
+// lanes = systems.  Per row one 16-byte record (uniform), then G / p / the mirror group's base (independent loads), then the
+// wall value: three dependent loads instead of eight, four rows in flight.
+constexpr int kInRows = 4;
+__global__ void __launch_bounds__(kBrickMaxS) brick_inflow_fast_kernel(const BrickClosureArgs R) {
+  const BoundaryArgs &a = R.a;
+  const BrickCG G = R.cgs[blockIdx.y];
+  const int c = G.cls, s = threadIdx.x;
+  if (s >= G.S) return;
+  const int k0 = blockIdx.x * kInRows, n_in = R.n_in[c];
+  if (k0 >= n_in) return;
+  const int bl = s / G.nd, dl = s - bl * G.nd, b = G.b0 + bl;
+  const int g = blockIdx.y - R.cg0[c];           // band group index: the same in the mirror class
+  const double Cb = a.C[b] / R.W;
+  double *inf = R.inf + G.inf_base + s;
+  BrickInRow rec[kInRows];
+#pragma unroll
+  for (int q = 0; q < kInRows; ++q) {
+    rec[q].bf = -1;
+    if (k0 + q < n_in) rec[q] = R.in_rec[c][k0 + q];
+  }
+  double Gf[kInRows], p[kInRows], spec[kInRows];
+  bool has[kInRows];
+#pragma unroll
+  for (int q = 0; q < kInRows; ++q) {
+    Gf[q] = p[q] = spec[q] = 0.0;
+    has[q] = false;
+    if (rec[q].bf < 0 || rec[q].type == NANOBTE_THERMALIZING || R.init) continue;
+    if (rec[q].type != NANOBTE_SPECULAR) Gf[q] = a.G[(size_t)rec[q].bf * a.B + b];
+    if (rec[q].type == NANOBTE_MIXED) p[q] = a.bf_p[rec[q].bf];
+    if (rec[q].type != NANOBTE_DIFFUSE && rec[q].msrc >= 0) {
+      const int dlm = R.in_perm[((size_t)c * 8 + rec[q].perm) * 16 + dl];
+      if (dlm != 255) {
+        const BrickCG &Gm = R.cgs[R.cg0[rec[q].cm] + g];
+        spec[q] = R.wall[Gm.wall_base + (int64_t)rec[q].msrc * kBrickRow + bl * Gm.nd + dlm];
+        has[q] = true;
+      }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < kInRows; ++q) {
+    if (rec[q].bf < 0) continue;
+    double *dst = inf + (int64_t)rec[q].row * kBrickRow;
+    if (rec[q].type == NANOBTE_THERMALIZING) {
+      if (R.init) *dst = Cb * a.bf_eps_w[rec[q].bf];  // R6; never changes afterwards
+      continue;
+    }
+    if (R.init) continue;  // eps^0 = 0 (R12)
+    if (rec[q].type == NANOBTE_DIFFUSE) *dst = Gf[q];                                                   // R7
+    else if (rec[q].type == NANOBTE_SPECULAR) *dst = spec[q];                                           // mirror (0 if s.n == 0, R15)
+    else *dst = has[q] ? p[q] * spec[q] + (1.0 - p[q]) * Gf[q] : 0.0;                                   // R8
+  }
 }
 
 // Combine the partials of every (class, group) per cell in fixed order, update T, track max |dT|, refresh the
@@ -185,7 +243,9 @@ BrickClosureArgs closure_args(nanobte_solver *h) {
   R.a = h->bd; R.W = h->W; R.cgs = bs.a.cgs; R.cg_of = bs.cg_of; R.dir_local = bs.dir_local; R.dir_cls = h->dir_cls;
   R.cls_dirs = h->cls_dirs; R.max_dirs = h->max_cls_dirs; R.wall = bs.a.wall; R.inf = bs.a.inf; R.partial = h->g_partial;
   R.bf_wrow = bs.bf_wrow;
+  R.in_perm = bs.in_perm;
   for (int c = 0; c < NB_MAX_CLASSES; ++c) {
+    R.in_rec[c] = bs.in_rec[c]; R.cg0[c] = bs.cg0[c];
     R.out_bf[c] = bs.out_bf[c]; R.out_row[c] = bs.out_row[c]; R.out_ord[c] = bs.out_ord[c]; R.n_out[c] = bs.n_out[c];
     R.in_row[c] = bs.in_row[c]; R.in_bf[c] = bs.in_bf[c]; R.n_in[c] = bs.n_in[c];
   }
@@ -213,8 +273,13 @@ int launch_inflow(nanobte_solver *h, int init) {
   int nmax = 0;
   for (int c = 0; c < h->n_cls; ++c) nmax = std::max(nmax, R.n_in[c]);
   if (nmax == 0) return 0;
-  dim3 grid(nmax, h->brick->n_cg);
-  brick_inflow_kernel<<<grid, kBrickMaxS, 0, h->stream>>>(R);
+  if (h->brick->in_fast) {
+    dim3 grid((nmax + kInRows - 1) / kInRows, h->brick->n_cg);
+    brick_inflow_fast_kernel<<<grid, kBrickMaxS, 0, h->stream>>>(R);
+  } else {
+    dim3 grid(nmax, h->brick->n_cg);
+    brick_inflow_kernel<<<grid, kBrickMaxS, 0, h->stream>>>(R);
+  }
   h->launches++;
   NB_CUDA(h, cudaGetLastError());
   return 0;

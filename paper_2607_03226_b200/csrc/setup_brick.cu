@@ -2,6 +2,7 @@
 // tasks in topological order with their up/downstream links, per-class cell tables and flags, the inflow / wall row
 // spaces, the closure tables in those row spaces, and the per-(class, group) coefficient blocks.
 #include <algorithm>
+#include <cstdlib>
 #include <numeric>
 
 #include "brick_host.h"
@@ -229,6 +230,56 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
   }
   bh.bf_nord = bf_nord;
 
+  // ---- records of the fast inflow kernel: per inflow row its face, type, the mirror class and the wall row the specular part
+  // comes from; per class the (at most 8) permutations "direction -> mirrored direction" that occur ---------------------------------
+  {
+    std::vector<int> dcls(D, 0);
+    for (int c = 0; c < ncls; ++c)
+      for (int d : x.dirs[c]) dcls[d] = c;
+    bh.in_perm.assign((size_t)ncls * 8 * 16, 255);
+    bh.in_fast = true;
+    for (int c = 0; c < ncls && bh.in_fast; ++c) {
+      BrickHost::Cls &C = bh.cls[c];
+      const int nd = (int)x.dirs[c].size();
+      int nperm = 0;
+      C.in_rec.resize(C.in_row.size());
+      for (size_t k = 0; k < C.in_row.size() && bh.in_fast; ++k) {
+        BrickInRow R{};
+        R.bf = C.in_bf[k]; R.row = C.in_row[k]; R.msrc = -1; R.type = (uint8_t)x.G->bf_type[R.bf]; R.cm = 0; R.perm = 0;
+        if (R.type == NANOBTE_SPECULAR || R.type == NANOBTE_MIXED) {
+          uint8_t pm[16];
+          int cm = -1;
+          for (int dl = 0; dl < 16; ++dl) pm[dl] = 255;
+          for (int dl = 0; dl < nd; ++dl) {
+            const int md = x.G->bf_mirror[(size_t)R.bf * D + x.dirs[c][dl]];
+            if (md < 0) continue;
+            if (cm >= 0 && dcls[md] != cm) bh.in_fast = false;  // the mirror images of one class in two classes: general kernel
+            cm = dcls[md];
+            pm[dl] = (uint8_t)bh.dir_local[md];
+          }
+          if (cm >= 0) {
+            R.cm = (uint8_t)cm;
+            R.msrc = bh.bf_wrow[(size_t)cm * nbf + R.bf];
+            if (R.msrc < 0) bh.in_fast = false;
+            int id = -1;
+            for (int q = 0; q < nperm && id < 0; ++q)
+              if (std::equal(pm, pm + 16, &bh.in_perm[((size_t)c * 8 + q) * 16])) id = q;
+            if (id < 0) {
+              if (nperm == 8) { bh.in_fast = false; break; }
+              id = nperm++;
+              std::copy(pm, pm + 16, &bh.in_perm[((size_t)c * 8 + id) * 16]);
+            }
+            R.perm = (uint8_t)id;
+          }
+        }
+        C.in_rec[k] = R;
+      }
+    }
+    bh.cg0.assign(cls_cg0.begin(), cls_cg0.end());
+    for (int c = 1; c < ncls; ++c)  // the same band groups in every class (then the mirror group is the same group index)
+      if (cls_ng[c] != cls_ng[0] || x.dirs[c].size() != x.dirs[0].size()) bh.in_fast = false;
+  }
+
   // ---- tasks: one per (proto, group), topological launch order ----------------------------------------------------------------------
   // key = primed tile/segment diagonal: every upstream task has a smaller key.  Within a key the classes and groups
   // are interleaved so that all octants advance together.
@@ -322,6 +373,8 @@ int nb_brick_upload(nanobte_solver *h, Arena &A, BrickHost &bh) {
     bs.out_row[c] = A.put(C.out_row);
     bs.out_ord[c] = A.put(C.out_ord);
     bs.n_out[c] = (int32_t)C.out_bf.size();
+    if (bh.in_fast) bs.in_rec[c] = A.put(C.in_rec);
+    bs.cg0[c] = bh.cg0[c];
   }
   a.inf = A.zeros<double>((size_t)bh.inf_total);
   a.wall = A.zeros<double>((size_t)bh.wall_total);
@@ -342,6 +395,8 @@ int nb_brick_upload(nanobte_solver *h, Arena &A, BrickHost &bh) {
     bs.pos2a = A.put(pos2a);
   }
   bs.bf_nord = A.put(bh.bf_nord);
+  bs.in_perm = A.put(bh.in_perm);
+  bs.in_fast = bh.in_fast && std::getenv("NANOBTE_BRICK_SLOW_INFLOW") == nullptr;
   bs.n_cg = (int)bh.cgs.size();
   bs.smem = nb_brick_smem_bytes();
   bs.grid = std::max(1, std::min(a.n_tasks, 3 * h->n_sm));

@@ -233,6 +233,30 @@ def test_fullsize_converged_against_golden(name, mode):
     g.close()
 
 
+def test_grid_128_cubed():
+    """A 128^3 grid (2.1 M cells, a cross-section of 16,384 pencils): refused as UNSUPPORTED by the hyperplane kernels of
+    round 1 (shape limits), swept by the tile-dataflow kernel (no cross-section limit).  One plain source
+    iteration element by element against the oracle."""
+    from paper_2607_03226_b200.binding import Solver
+    pr = wl.config_cube(n=128, B=2, n_polar=2, n_azim=8)
+    g, r = Solver(pr), RefSolver(pr)
+    assert g.info["sweep_variant"] == 5
+    rng = np.random.default_rng(5)
+    T0 = pr["T_ref"] + rng.uniform(-2.0, 2.0, n_cells_of(pr))
+    g.set_T(T0); r.set_T(T0)
+    g.sweep(); r.sweep()
+    for b in range(2):
+        eg, er = g.get_e(b, 1)[0], r.get_e(b, 1)[0]
+        assert rel(eg, er) <= TOL_SWEEP
+        del eg, er
+    dg, dr = g.update_temperature(), r.update_temperature()
+    assert abs(dg - dr) <= 1e-9 * abs(dr) + 1e-13
+    for which in (0, 1, 2):
+        assert rel(g.get_T(which) - pr["T_ref"], r.get_T(which) - pr["T_ref"]) <= TOL_SWEEP
+    assert rel(g.get_q(), r.get_q()) <= TOL_SWEEP
+    g.close(); r.close()
+
+
 def test_config0_against_golden_file():
     """tests/golden/config0_oracle.txt (written by make_config0_golden.py from oracle/ only)."""
     from paper_2607_03226_b200.binding import Solver

@@ -517,6 +517,14 @@ def test_band_shards_on_one_gpu_match_the_unsharded_solver(which, mode, world):
     g.close(); r.close(); r2.close()
 
 
+def test_brick_general_inflow_kernel(monkeypatch):
+    """NANOBTE_BRICK_SLOW_INFLOW=1: the closure kernel of the tile-dataflow path that looks the mirror direction up per thread
+    (the fallback when the per-row records do not apply) instead of the record-based one."""
+    monkeypatch.setenv("NANOBTE_BRICK_SLOW_INFLOW", "1")
+    step_parity(wl.config_finfet(nx=16, ny=8, nz=8, B=3, n_polar=2, n_azim=8), 3, mode="synthetic")
+    step_parity(wl.config_cube(n=12, B=3, n_polar=2, n_azim=8), 3)
+
+
 def test_cg_not_converged_is_reported():
     """cg_max_iter too small: diffusion_correct and solve say NOT_CONVERGED (1) instead of OK."""
     pr = wl.config_finfet(nx=24, ny=12, nz=12, B=3, n_polar=2, n_azim=8)
