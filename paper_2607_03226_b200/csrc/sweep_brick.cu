@@ -159,10 +159,10 @@ __device__ __forceinline__ void plain_plane(double *__restrict__ pl, const doubl
 }
 
 // ---- the same without a branch: no source in the plane, the distribution not stored, the v-face rows always written (tiles on
-// the boundary write a scratch row), all 8 rows computed (rows >= tw of a shorter tile work on values nobody reads).  Written
+// the boundary write a scratch row), ROWS = 7 or 8 rows computed (rows >= tw of a shorter tile work on values nobody reads).  Written
 // software-pipelined: the loads and the chain-independent half of row w+1 sit between the chain steps of row w, so that a warp
 // has work of its own during the 8-cycle DFMA latency of the v-chain.
-template <int TV>
+template <int TV, int ROWS>
 __device__ __forceinline__ void fast_plane(double *__restrict__ pl, const double *__restrict__ th, const Sys &c,
                                            double (&ew)[kBrickTile], const double (&inv)[kBrickTile], double *__restrict__ dn_fv_u,
                                            const unsigned par) {
@@ -179,10 +179,10 @@ __device__ __forceinline__ void fast_plane(double *__restrict__ pl, const double
     }
   }
 #pragma unroll
-  for (int w = 0; w < kBrickTile; ++w) {
+  for (int w = 0; w < ROWS; ++w) {
     double *row = pl + w * kBrickTile * kP;
     double eu[TV], tn[TV];
-    if (w + 1 < kBrickTile) {
+    if (w + 1 < ROWS) {
 #pragma unroll
       for (int v = 0; v < TV; ++v) eu[v] = row[(kBrickTile + v) * kP];
 #pragma unroll
@@ -198,7 +198,7 @@ __device__ __forceinline__ void fast_plane(double *__restrict__ pl, const double
       ev = fma(c.c_v, ev, fma(c.c_w, ew[v], rp[v]));  // the v-chain is the only dependency between the cells of a row
       ew[v] = ev;
       row[v * kP] = ev;
-      if (w + 1 < kBrickTile) rn[v] = fma(c.c_u, eu[v], c.k_th * tn[v]);
+      if (w + 1 < ROWS) rn[v] = fma(c.c_u, eu[v], c.k_th * tn[v]);
     }
     dn_fv_u[w * kBrickRow] = tag(ev, par);
 #pragma unroll
@@ -274,6 +274,7 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     double *dn_fw = T.dn_fw0 >= 0 ? inf + (int64_t)T.dn_fw0 * kBrickRow : nullptr;
     const unsigned long long src_planes = ((unsigned long long)T.src_hi << 32) | T.src_lo;
     const bool plain = T.plain && T.tv >= 4;
+    const bool rows7 = T.tw <= 7;  // the branch-free substitution computes 7 or 8 rows
     double *scratch = a.inf + G.inf_base + (int64_t)a.scratch_row[G.cls] * kBrickRow + s;  // 8 rows nobody reads
 
     // coefficients of this thread's system; moment tables of the group
@@ -357,11 +358,11 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
           if (!src && !eout) {
             double *dfv = dn_fv ? dn_fv : scratch;
             switch (T.tv) {
-              case 8: fast_plane<8>(pl, sm.th, c, ew, inv, dfv, par); break;
-              case 7: fast_plane<7>(pl, sm.th, c, ew, inv, dfv, par); break;
-              case 6: fast_plane<6>(pl, sm.th, c, ew, inv, dfv, par); break;
-              case 5: fast_plane<5>(pl, sm.th, c, ew, inv, dfv, par); break;
-              default: fast_plane<4>(pl, sm.th, c, ew, inv, dfv, par); break;
+              case 8: if (rows7) fast_plane<8, 7>(pl, sm.th, c, ew, inv, dfv, par); else fast_plane<8, 8>(pl, sm.th, c, ew, inv, dfv, par); break;
+              case 7: if (rows7) fast_plane<7, 7>(pl, sm.th, c, ew, inv, dfv, par); else fast_plane<7, 8>(pl, sm.th, c, ew, inv, dfv, par); break;
+              case 6: if (rows7) fast_plane<6, 7>(pl, sm.th, c, ew, inv, dfv, par); else fast_plane<6, 8>(pl, sm.th, c, ew, inv, dfv, par); break;
+              case 5: if (rows7) fast_plane<5, 7>(pl, sm.th, c, ew, inv, dfv, par); else fast_plane<5, 8>(pl, sm.th, c, ew, inv, dfv, par); break;
+              default: if (rows7) fast_plane<4, 7>(pl, sm.th, c, ew, inv, dfv, par); else fast_plane<4, 8>(pl, sm.th, c, ew, inv, dfv, par); break;
             }
           } else
           switch (T.tv) {
