@@ -392,7 +392,9 @@ def main():
         sm_clock = (clocks.get("sm_mhz") or 1965.0) * 1e6
         ops = (7.0 + 5.0 / max(1, len(pr["bands"]["C"]))) * upd
         alu_peak = 64.0 * 148 * sm_clock
-        smem_bytes = 26.0 * upd   # STS 8 + LDS 8 (u-upwind) + LDS 8 (moments) + theta broadcast 2 per update
+        # shared-memory bytes per update: STS 8 + LDS 8 (u-upwind) + 8 (theta: a broadcast still returns 8 B per lane) + LDS 8
+        # (moments) + ~3 (band coefficients, 16 B per 6 values) = 35; ncu counts 48 B/update (rows of a 7-row tile padded to 8, conflicts)
+        smem_bytes = 35.0 * upd
         roofline["fused"] = {"note": "sweep + moments in one kernel: nothing of eps goes to HBM unless asked for",
                              "algorithmic_bytes_sweep_plus_moments": 16.0 * upd,
                              "equivalent_GBs_sweep_plus_moments": 16.0 * upd / (sweep_ms * 1e-3) / 1e9}

@@ -9,14 +9,16 @@
 //
 // One u-plane of a task in two roles:
 //   substitution  thread = system.  Tasks whose box is fully active (BrickTask::plain; with tile cuts that follow the
-//                 mask that is every task of a box-shaped geometry) run straight-line code with the tile width as a
-//                 template constant: per cell one LDS (u-upwind), one STS, 4 fp64 operations.  Other tasks run the
+//                 mask that is every task of a box-shaped geometry) run branch-free, software-pipelined code with the tile
+//                 width and the row count as template constants (fast_plane): per cell one LDS (u-upwind), one STS,
+//                 4 fp64 operations.  Planes with a source or a stored distribution take plain_plane, other tasks the
 //                 per-cell path that reads the flag bytes (walls inside the tile).
-//   moments       thread = two cells (lane, lane + 32) x the bands of the thread's warp; per value one LDS and four
-//                 DFMA, the direction coefficients shared by the two cells.  Warps 0..2 leave their band partials in
-//                 shared memory, warp 3 adds its own in fixed order and writes the five partial moments of the plane.
-// Shared memory is the scarce resource (128 B/clk per SM against 64 DFMA/clk): per update the substitution moves
-// 16 B + 2 B (theta broadcast) and the moments 8 B + 8 B (coefficient broadcast shared by two cells).
+//   moments       thread = two cells (lane, lane + 32) x a quarter of the class's directions, all bands: the band sums
+//                 first (3 fp64 operations per value), the direction weights once per plane.  Warps 0..2 leave their
+//                 partials in shared memory, warp 3 adds its own in fixed order and writes the five partial moments.
+// Tile faces cross CTAs through L2 tagged with the sweep parity (brick.h, BRK_FACE_TAGGED): no fence, no counter.
+// Shared memory is the scarce resource (128 B/clk per SM against 64 DFMA/clk; a broadcast load still returns 8 B per
+// lane): per update STS 8 B + u-upwind 8 B + theta 8 B + moments 8 B + band coefficients ~3 B = 35 B.
 #include <algorithm>
 
 #include "brick.h"
