@@ -39,10 +39,13 @@
  * flux of reflecting walls is evaluated in closed form and relies on that symmetry.
  *
  * Environment hooks, read at create, for tests and tuning only (each selects another of the library's own CUDA
- * paths; none of them leaves the GPU): NANOBTE_CG_GENERIC=1 (multi-pass CG kernel), NANOBTE_CG_NO_UNI=1 (per-cell CG
- * stencil on uniform grids), NANOBTE_CG_NO_RECYCLE=1 (CG from zero instead of the recycled initial guess), NANOBTE_UNS_PLAIN=1 (non-staged unstructured sweep), NANOBTE_SWEEP_RP=0 (run-time row
- * pitch in the structured sweep), NANOBTE_CG_NBLK=k (at most k CTAs in the fused CG: more cells per thread on small
- * meshes).
+ * paths; none of them leaves the GPU): NANOBTE_NO_BRICK=1 (hyperplane sweep + separate moment pass instead of the
+ * tile-dataflow sweep on uniform 3-D grids), NANOBTE_BRICK_SLOW_INFLOW=1 (general closure kernel of that path),
+ * NANOBTE_CG_NO_MG=1 (plain fused CG instead of the multigrid-preconditioned one), NANOBTE_CG_GENERIC=1 (multi-pass
+ * CG kernel), NANOBTE_CG_NO_UNI=1 (per-cell CG stencil on uniform grids; implies NO_MG), NANOBTE_CG_NO_RECYCLE=1 (plain CG
+ * from zero instead of the recycled initial guess; implies NO_MG: the oracle's iterate sequence), NANOBTE_UNS_PLAIN=1
+ * (non-staged unstructured sweep), NANOBTE_SWEEP_RP=0 (run-time row pitch in the hyperplane sweep), NANOBTE_CG_NBLK=k
+ * (at most k CTAs in the CG kernels: more cells per thread on small meshes).
  */
 #ifndef NANOBTE_H
 #define NANOBTE_H
