@@ -114,3 +114,18 @@ def test_no_cpu_fallback(lib):
     assert rc == -4
     assert b"no CPU fallback" in lib.nanobte_last_error(h) or b"CUDA" in lib.nanobte_last_error(h)
     lib.nanobte_destroy(h)
+
+
+def test_band_totals_closed_forms(lib):
+    """nanobte_band_totals (host only): beta = sum C/tau (Eq. 5), sum C (R13), kappa = (1/dim) sum C v^2 tau
+    (R14d: kinetic-theory value for unit directions spanning the mesh dimension) for the tables of configs 2 and 4."""
+    from paper_2607_03226_b200 import sharded
+    for pr, dim in ((wl.config_nongray_square(n=8), 2), (wl.config_finfet(nx=8, ny=4, nz=4), 3)):
+        beta, Csum, kappa = sharded.band_totals(pr)
+        b = pr["bands"]
+        assert beta == pytest.approx((b["C"] / b["tau"]).sum(), rel=1e-14)
+        assert Csum == pytest.approx(b["C"].sum(), rel=1e-14)
+        assert kappa == pytest.approx((b["C"] * b["v"] ** 2 * b["tau"]).sum() / dim, rel=1e-12)
+        # a shard's rows are the rank's round-robin share of the table
+        sub = sharded.shard_problem(pr, 1, 3)
+        assert np.array_equal(sub["bands"]["C"], b["C"][1::3]) and sub["mesh"] is pr["mesh"]
