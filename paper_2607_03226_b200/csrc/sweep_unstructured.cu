@@ -348,22 +348,30 @@ __global__ void __launch_bounds__(256) moments_unstructured_kernel(const UnsArgs
       dd[u] = d0 + 4 * u + dl;
       base[u] = dd[u] < a.D ? ((int64_t)dd[u] * a.e_stride + __ldg(a.a2pos + (int64_t)dd[u] * a.n_act + c)) * a.B : -1;
     }
-    for (int b0 = 0; b0 < a.B; b0 += 8) {
-      const int b = b0 + b8;
-      if (b < a.B) {
-        double v[4];
+    constexpr int KB = 3;  // band chunks of 8 in flight on top of the 4 direction groups: 12 loads per lane before the first use (5: slower)
+    for (int b0 = 0; b0 < a.B; b0 += 8 * KB) {
+      double v[KB][4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) v[u] = base[u] >= 0 ? __ldcs(a.e + base[u] + b) : 0.0;
-        const double it = its[b], vb = vbs[b];
+      for (int k = 0; k < KB; ++k) {
+        const int b = b0 + 8 * k + b8;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          if (base[u] >= 0) {
-            const double wv = wsm[dd[u]] * v[u];
-            A1 += it * wv;                         // Eq. 5 numerator
-            A2 += wv;                              // R13
-            qx += vb * (wss[3 * dd[u]] * v[u]);    // Eq. 7
-            qy += vb * (wss[3 * dd[u] + 1] * v[u]);
-            qz += vb * (wss[3 * dd[u] + 2] * v[u]);
+        for (int u = 0; u < 4; ++u) v[k][u] = (b < a.B && base[u] >= 0) ? __ldcs(a.e + base[u] + b) : 0.0;
+      }
+#pragma unroll
+      for (int k = 0; k < KB; ++k) {
+        const int b = b0 + 8 * k + b8;
+        if (b < a.B) {
+          const double it = its[b], vb = vbs[b];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            if (base[u] >= 0) {
+              const double wv = wsm[dd[u]] * v[k][u];
+              A1 += it * wv;                            // Eq. 5 numerator
+              A2 += wv;                                 // R13
+              qx += vb * (wss[3 * dd[u]] * v[k][u]);    // Eq. 7
+              qy += vb * (wss[3 * dd[u] + 1] * v[k][u]);
+              qz += vb * (wss[3 * dd[u] + 2] * v[k][u]);
+            }
           }
         }
       }
