@@ -15,8 +15,8 @@
 //                prolongation never leave the CTA; iterates cross CTA borders through global memory + one grid barrier.
 //   levels 3..   a few hundred unknowns: every CTA holds them in shared memory and repeats the same arithmetic
 //                (bitwise identical, no communication); the coarsest level (<= 32 unknowns) is a dense inverse.
-// Smoother: x <- x + B (g - A x) with B = two damped-Jacobi steps on the CTA's own diagonal block (no communication,
-// symmetric), once before and once after the coarse correction, which is scaled by tau (over-correction for the
+// Smoother: x <- x + B (g - A x) with B = two damped-Jacobi steps (omega = 0.9) on the CTA's own diagonal block (no communication,
+// symmetric), once before and once after the coarse correction, which is scaled by tau = 2 (over-correction for the
 // piecewise-constant prolongation).  The V-cycle is a fixed symmetric positive definite operator, as CG requires.
 // CG in the Chronopoulos-Gear form (one reduction per iteration): u = M^-1 r, w = A u, gamma = (r,u), delta = (w,u).
 // All reductions are fixed trees over per-CTA partials: bitwise reproducible, identical scalars in every CTA.
@@ -611,7 +611,11 @@ bool dense_inverse(std::vector<double> &M, int n) {
 int nb_mg_build(nanobte_solver *h, Arena &A, const GenericTables &g, const double *cfu, const int grid[3]) {
   const int na = (int)g.act2cell.size();
   if (g.cg_nf != 6 || na < 64) return 0;
-  const double omega = 0.8, tau = 1.6;
+  // damping and over-correction: scanned on configs 3 and 4 (omega 0.7 .. 0.95 x tau 1.4 .. 3.0: 16 iterations per solve here,
+  // 20 at 0.8 / 1.6, 35 at 0.95 / 3.0); omega < 1 keeps the two-step Jacobi smoother positive definite
+  double omega = 0.9, tau = 2.0;
+  if (const char *env = std::getenv("NANOBTE_MG_OMEGA")) omega = std::atof(env);  // tuning hooks
+  if (const char *env = std::getenv("NANOBTE_MG_TAU")) tau = std::atof(env);
   // ---- lattices -------------------------------------------------------------------------------------------------------------------------------
   std::vector<Lat> lat(1);
   {
