@@ -434,11 +434,9 @@ extern "C" int64_t nanobte_moments_len(const nanobte_solver *h) { return h ? (in
 extern "C" int nanobte_export_moments(nanobte_solver *h, double *dst, int32_t dst_is_device) {
   if (!h || !h->arena || !dst) return NANOBTE_E_INVALID;
   const size_t na = (size_t)h->n_act;
-  double *stage = dst_is_device ? dst : h->part;  // part holds >= 3 n_cells + 64 doubles; the leak goes through leak_sum
   const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
   int rc = nb_launch_leak_sum(h);  // leak_sum[bf] = sum over this shard's bands of the face flux (R14c')
   if (rc < 0) return rc;
-  (void)stage;
   NB_CUDA(h, cudaMemcpyAsync(dst, h->theta_SI, na * sizeof(double), kind, h->stream));
   NB_CUDA(h, cudaMemcpyAsync(dst + na, h->theta_en, na * sizeof(double), kind, h->stream));
   NB_CUDA(h, cudaMemcpyAsync(dst + 2 * na, h->q, 3 * na * sizeof(double), kind, h->stream));
