@@ -28,7 +28,10 @@
  * Device memory: if options.workspace is non-NULL it must be a device allocation of at least
  * nanobte_workspace_bytes_*() bytes, 256-byte aligned, owned by the caller (e.g. a torch tensor) and
  * alive until nanobte_destroy; otherwise the library allocates with cudaMalloc and frees at destroy.
- * All kernels are enqueued on options.stream (a cudaStream_t; NULL = legacy default stream).
+ * All kernels are enqueued on options.stream (a cudaStream_t; NULL = legacy default stream), or on a second stream of the
+ * library's own that is forked from and joined back into options.stream with events inside one call (the moment combine
+ * runs beside the closure kernels on the tile-dataflow path; NANOBTE_NO_AUX_STREAM=1 keeps everything on one stream): towards
+ * the caller every call is ordered on options.stream.
  *
  * Errors: int return; 0 OK; NANOBTE_NOT_CONVERGED (1) = state valid, max_iter reached; < 0 error.  No
  * exceptions cross the ABI, no global state; nanobte_last_error(h) gives the message.  There is NO CPU

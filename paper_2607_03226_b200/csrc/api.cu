@@ -349,6 +349,9 @@ extern "C" void nanobte_destroy(nanobte_solver *h) {
   nb_free_unstructured(h);
   nb_free_brick(h);
   nb_free_mg(h);
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
+  if (h->aux_stream) cudaStreamDestroy(h->aux_stream);
   if (h->arena && h->arena_owned) cudaFree(h->arena);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   delete h;
@@ -385,12 +388,28 @@ static int read_maxdT(nanobte_solver *h, double *out) {
 extern "C" int nanobte_update_temperature(nanobte_solver *h, double *max_dT) {
   if (!h || !h->arena) return NANOBTE_E_INVALID;
   int rc;
+  const bool fork = h->brick && h->swept_since_closure && h->aux_stream;
+  if (fork) {  // O4 + O5 beside the closures (disjoint data: partial moments / theta here, wall rows / G / inflow rows there)
+    NB_CUDA(h, cudaEventRecord(h->ev_fork, h->stream));
+    NB_CUDA(h, cudaStreamWaitEvent(h->aux_stream, h->ev_fork, 0));
+    cudaStream_t main = h->stream;
+    h->stream = h->aux_stream;
+    rc = nb_launch_moments(h);
+    if (rc >= 0) rc = nb_launch_update(h, 0);
+    h->stream = main;
+    if (rc < 0) return rc;
+    NB_CUDA(h, cudaEventRecord(h->ev_join, h->aux_stream));
+  }
   if (h->swept_since_closure) {  // G, face fluxes, inflow cache for the next sweep (O3); once per sweep
     if ((rc = nb_launch_boundary(h)) < 0) return rc;
     h->swept_since_closure = false;
   }
-  if ((rc = nb_launch_moments(h)) < 0) return rc;   // O4
-  if ((rc = nb_launch_update(h, 0)) < 0) return rc; // O5
+  if (fork) {
+    NB_CUDA(h, cudaStreamWaitEvent(h->stream, h->ev_join, 0));
+  } else {
+    if ((rc = nb_launch_moments(h)) < 0) return rc;   // O4
+    if ((rc = nb_launch_update(h, 0)) < 0) return rc; // O5
+  }
   h->leak_imported = false;  // a correction after this update sums its own bands' face fluxes unless moments are imported
   if (max_dT) return read_maxdT(h, max_dT);
   return 0;

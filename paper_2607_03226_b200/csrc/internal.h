@@ -77,6 +77,10 @@ struct nanobte_solver {
   int cg_max_iter = 100000;
   bool any_therm = false;
   cudaStream_t stream = nullptr;
+  // second stream of the library's own (tile-dataflow path): the moment combine + update runs beside the closure kernels of the
+  // same iteration (they touch disjoint data); forked and joined with the two events inside nanobte_update_temperature
+  cudaStream_t aux_stream = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   int n_sm = 148;
 
   // device arena

@@ -397,6 +397,12 @@ int nb_brick_upload(nanobte_solver *h, Arena &A, BrickHost &bh) {
   bs.bf_nord = A.put(bh.bf_nord);
   bs.in_perm = A.put(bh.in_perm);
   bs.in_fast = bh.in_fast && std::getenv("NANOBTE_BRICK_SLOW_INFLOW") == nullptr;
+  if (!A.dry && !h->aux_stream && std::getenv("NANOBTE_NO_AUX_STREAM") == nullptr) {
+    if (cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess)
+      return nb_fail(h, NANOBTE_E_CUDA, "second stream of the tile-dataflow path");
+  }
   bs.n_cg = (int)bh.cgs.size();
   bs.smem = nb_brick_smem_bytes();
   bs.grid = std::max(1, std::min(a.n_tasks, 3 * h->n_sm));
