@@ -64,9 +64,11 @@ struct BrickTask {
   int32_t wall_any;            // the task has cells with an outgoing boundary face
   int32_t fv_mode, fw_mode;    // how the v- / w-face inflow rows become valid: BRK_FACE_*
   int32_t publish;             // a downstream task follows this one through the progress counter: publish every plane
-  int32_t pad;
+  int32_t wu0, wv0, ww0;       // wall rows as face blocks (first row or -1): what the u- / v- / w-face stores go to where there
+                               // is no downstream tile but a wall (tasks whose faces are each all wall or all interior)
+  int32_t pad[2];
 };
-static_assert(sizeof(BrickTask) == 96, "BrickTask layout");
+static_assert(sizeof(BrickTask) == 112, "BrickTask layout");
 
 struct BrickCG {
   int32_t cls, S, nb, nd;      // class, systems (= nb * nd), bands, directions of the class; system = band_local * nd + dir_local

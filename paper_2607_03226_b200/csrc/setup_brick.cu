@@ -91,7 +91,8 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
   bh.bf_wrow.assign((size_t)ncls * nbf, -1);
   bh.a2pos.assign((size_t)ncls * na, -1);
   std::vector<uint8_t> bf_nord(nbf, 0);
-  struct ProtoTask { BrickTask t; int key, cls, J, K, sg; };
+  struct OutEnt { int j, k, ul, vl, wl; };   // an outgoing wall face of a task: entry in Cls::out_*, side, cell
+  struct ProtoTask { BrickTask t; int key, cls, J, K, sg; std::vector<OutEnt> outs; int wall_cnt[3]; bool pure; };
   std::vector<ProtoTask> protos;
   for (int c = 0; c < ncls; ++c) {
     BrickHost::Cls &C = bh.cls[c];
@@ -137,6 +138,9 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
           if (T.nu > 64) return nb_fail(h, NANOBTE_E_INVALID, "internal: brick segment of %d planes", T.nu);
           int n_active = 0;
           uint64_t src_planes = 0;
+          std::vector<OutEnt> &outs = P.outs;
+          int (&wall_cnt)[3] = P.wall_cnt;
+          wall_cnt[0] = wall_cnt[1] = wall_cnt[2] = 0;
           // cells in sweep order
           C.th.resize((size_t)npos, 0.0);
           C.qd.resize((size_t)npos, 0.0);
@@ -173,6 +177,8 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
                     const int bf = x.facebf[(size_t)cphys * 6 + side_out[k]];
                     if (bf < 0) return nb_fail(h, NANOBTE_E_INVALID, "internal: brick outflow face of cell %d missing", cphys);
                     wallout = true;
+                    outs.push_back({(int)C.out_bf.size(), k, ul, vl, wl});
+                    ++wall_cnt[k];
                     C.out_bf.push_back(bf);
                     C.out_row.push_back(nwall);
                     C.out_ord.push_back(bf_nord[bf]++);
@@ -188,6 +194,10 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
           T.plain = n_active == T.nu * T.tv * T.tw;
           T.src_lo = (uint32_t)src_planes; T.src_hi = (uint32_t)(src_planes >> 32);
           T.wall_any = nwall > T.wo0;
+          T.wu0 = T.wv0 = T.ww0 = -1;
+          const int face_n[3] = {T.tv * T.tw, T.nu * T.tw, T.nu * T.tv};
+          P.pure = T.plain && T.wall_any && (wall_cnt[0] == 0 || wall_cnt[0] == face_n[0]) &&
+                   (wall_cnt[1] == 0 || wall_cnt[1] == face_n[1]) && (wall_cnt[2] == 0 || wall_cnt[2] == face_n[2]);
           task_of[pbox(Jp, Kp, sp)] = (int)protos.size();
           protos.push_back(P);
         }
@@ -221,6 +231,24 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
       P.t.dn_fu0 = du >= 0 ? protos[du].t.fu0 : -1;
       P.t.dn_fv0 = dv >= 0 ? protos[dv].t.fv0 : -1;
       P.t.dn_fw0 = dw >= 0 ? protos[dw].t.fw0 : -1;
+      // A fully active box whose downstream faces are each all wall (and then without a downstream tile) or all interior: its
+      // wall rows become face blocks with the addressing of the inflow faces (u-face [w][v], v-face [u][w], w-face [u][v]), so
+      // that the sweep stores wall values where it would store the face of a downstream tile -- no pass over the wall cells
+      // afterwards.  (The rows given out cell by cell above stay unused.)
+      if (P.pure && !(P.wall_cnt[0] && du >= 0) && !(P.wall_cnt[1] && dv >= 0) && !(P.wall_cnt[2] && dw >= 0)) {
+        BrickTask &T = P.t;
+        if (P.wall_cnt[0]) { T.wu0 = nwall; nwall += kBrickCells; }
+        if (P.wall_cnt[1]) { T.wv0 = nwall; nwall += T.nu * kBrickTile; }
+        if (P.wall_cnt[2]) { T.ww0 = nwall; nwall += T.nu * kBrickTile; }
+        for (const OutEnt &e : P.outs) {
+          const int row = e.k == 0 ? T.wu0 + e.wl * kBrickTile + e.vl : e.k == 1 ? T.wv0 + e.ul * kBrickTile + e.wl : T.ww0 + e.ul * kBrickTile + e.vl;
+          C.out_row[e.j] = row;
+          bh.bf_wrow[(size_t)c * nbf + C.out_bf[e.j]] = row;
+        }
+        T.wall_any = 0;  // nothing left for the pass over the wall cells
+      }
+      P.outs.clear();
+      P.outs.shrink_to_fit();
     }
     C.scratch_row = nrow; nrow += kBrickTile;
     C.npos = npos; C.nrow = nrow; C.nwall = std::max(1, nwall);

@@ -274,6 +274,11 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     double *dn_fu = T.dn_fu0 >= 0 ? inf + (int64_t)T.dn_fu0 * kBrickRow : nullptr;
     double *dn_fv = T.dn_fv0 >= 0 ? inf + (int64_t)T.dn_fv0 * kBrickRow : nullptr;
     double *dn_fw = T.dn_fw0 >= 0 ? inf + (int64_t)T.dn_fw0 * kBrickRow : nullptr;
+    // a face that is all wall (and has no downstream tile): its values go to the task's wall rows, which have the same
+    // addressing as a downstream tile's face rows (setup_brick.cu) -- the closures read them there
+    if (T.wu0 >= 0) dn_fu = a.wall + G.wall_base + (int64_t)T.wu0 * kBrickRow + s;
+    if (T.wv0 >= 0) dn_fv = a.wall + G.wall_base + (int64_t)T.wv0 * kBrickRow + s;
+    if (T.ww0 >= 0) dn_fw = a.wall + G.wall_base + (int64_t)T.ww0 * kBrickRow + s;
     const unsigned long long src_planes = ((unsigned long long)T.src_hi << 32) | T.src_lo;
     const bool plain = T.plain && T.tv >= 4;
     const bool rows7 = T.tw <= 7;  // the branch-free substitution computes 7 or 8 rows
