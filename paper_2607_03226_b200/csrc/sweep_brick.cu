@@ -379,11 +379,17 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
             case 5: plain_plane<5>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, S, par); break;
             default: plain_plane<4>(pl, sm.th, sm.qd, c, T.tw, src, ew, inv, dn_fv, eout, S, par); break;
           }
-          if (dn_fw) {  // the last row of the tile, out of the plane buffer (the thread's own stores)
-            const double *lrow = pl + (T.tw - 1) * kBrickTile * kP;
+          if (dn_fw) {  // the last row of the tile: still in ew unless the branch-free path computed rows beyond tw
+            if ((src || eout) || T.tw == (rows7 ? 7 : 8)) {
 #pragma unroll
-            for (int v = 0; v < kBrickTile; ++v)
-              if (v < T.tv) dn_fw[v * kBrickRow] = tag(lrow[v * kP], par);
+              for (int v = 0; v < kBrickTile; ++v)
+                if (v < T.tv) dn_fw[v * kBrickRow] = tag(ew[v], par);
+            } else {  // out of the plane buffer (the thread's own stores)
+              const double *lrow = pl + (T.tw - 1) * kBrickTile * kP;
+#pragma unroll
+              for (int v = 0; v < kBrickTile; ++v)
+                if (v < T.tv) dn_fw[v * kBrickRow] = tag(lrow[v * kP], par);
+            }
           }
         } else {
           // ---- per-cell path: holes and walls inside the tile (wall values straight from L2) ----------------------------------
