@@ -13,9 +13,8 @@
 //                 width and the row count as template constants (fast_plane): per cell one LDS (u-upwind), one STS,
 //                 4 fp64 operations.  Planes with a source or a stored distribution take plain_plane, other tasks the
 //                 per-cell path that reads the flag bytes (walls inside the tile).
-//   moments       thread = two cells (lane, lane + 32) x a quarter of the class's directions, all bands: the band sums
-//                 first (3 fp64 operations per value), the direction weights once per plane.  Warps 0..2 leave their
-//                 partials in shared memory, warp 3 adds its own in fixed order and writes the five partial moments.
+//   moments       thread = one cell x half of the class's directions, all bands: the band sums first (3 fp64 operations
+//                 per value), the direction weights once per plane; a warp owns 16 cells, one shuffle joins the halves.
 // Tile faces cross CTAs through L2 tagged with the sweep parity (brick.h, BRK_FACE_TAGGED): no fence, no counter.
 // Shared memory is the scarce resource (128 B/clk per SM against 64 DFMA/clk; a broadcast load still returns 8 B per
 // lane): per update STS 8 B + u-upwind 8 B + theta 8 B + moments 8 B + band coefficients ~3 B = 35 B.
@@ -99,7 +98,6 @@ __device__ unsigned long long g_brick_prof[16];
 
 struct BrickSmem {
   double plane[kBrickCells * kBrickPitch];     // [cell][system]: eps of the previous u-plane (u-upwind values)
-  double red[3][5][kBrickCells];               // band partials of warps 0..2 (moments)
   double th[kBrickCells];                      // theta of the plane's cells
   double qd[kBrickCells];                      // Qdot
   unsigned long long flg[2][kBrickCells / 8];  // flag bytes, one 64-bit word per row of 8 cells, two stages
@@ -208,41 +206,39 @@ __device__ __forceinline__ void fast_plane(double *__restrict__ pl, const double
   }
 }
 
-// ---- moments of one u-plane, one thread: cells (lane, lane + 32), ND consecutive directions, all bands --------------------------------
+// ---- moments of one u-plane, one thread: one cell, ND consecutive directions, all bands ---------------------------------------------------
 // The band sums come first (three weights: 1/tau_b, 1, v_b -- 3 fp64 operations per value), the direction weights once per
 // plane:  m0 = sum_d w_d sum_b eps/tau_b,  m1 = sum_d w_d sum_b eps,  m2..4 = sum_d w_d s_d sum_b v_b eps.
 // row = plane buffer + cell * pitch + first direction; bcoef = [nb][2] (1/tau, v); dcoef = [ND][4] (w, w sx, w sy, w sz).
 template <int ND>
-__device__ __forceinline__ void moments_dirs(const double *__restrict__ row, const double *__restrict__ bcoef,
-                                             const double *__restrict__ dcoef, const int nb, const int nd, double (&m)[2][5]) {
-  double A[ND][2], Bs[ND][2], Cv[ND][2];
+__device__ __forceinline__ void moments_cell(const double *__restrict__ row, const double *__restrict__ bcoef,
+                                             const double *__restrict__ dcoef, const int nb, const int nd, double (&m)[5]) {
+  double A[ND], Bs[ND], Cv[ND];
 #pragma unroll
-  for (int j = 0; j < ND; ++j) A[j][0] = A[j][1] = Bs[j][0] = Bs[j][1] = Cv[j][0] = Cv[j][1] = 0.0;
+  for (int j = 0; j < ND; ++j) A[j] = Bs[j] = Cv[j] = 0.0;
 #pragma unroll 2
   for (int b = 0; b < nb; ++b) {
     const double2 bc = *reinterpret_cast<const double2 *>(bcoef + 2 * b);
 #pragma unroll
     for (int j = 0; j < ND; ++j) {
-      const double e0 = row[j], e1 = row[j + 32 * kP];
-      A[j][0] = fma(bc.x, e0, A[j][0]); Bs[j][0] += e0; Cv[j][0] = fma(bc.y, e0, Cv[j][0]);
-      A[j][1] = fma(bc.x, e1, A[j][1]); Bs[j][1] += e1; Cv[j][1] = fma(bc.y, e1, Cv[j][1]);
+      const double e = row[j];
+      A[j] = fma(bc.x, e, A[j]);
+      Bs[j] += e;
+      Cv[j] = fma(bc.y, e, Cv[j]);
     }
     row += nd;
   }
 #pragma unroll
-  for (int k = 0; k < 5; ++k) m[0][k] = m[1][k] = 0.0;
+  for (int k = 0; k < 5; ++k) m[k] = 0.0;
 #pragma unroll
   for (int j = 0; j < ND; ++j) {
     const double2 c01 = *reinterpret_cast<const double2 *>(dcoef + 4 * j);
     const double2 c23 = *reinterpret_cast<const double2 *>(dcoef + 4 * j + 2);
-#pragma unroll
-    for (int q = 0; q < 2; ++q) {
-      m[q][0] = fma(c01.x, A[j][q], m[q][0]);
-      m[q][1] = fma(c01.x, Bs[j][q], m[q][1]);
-      m[q][2] = fma(c01.y, Cv[j][q], m[q][2]);
-      m[q][3] = fma(c23.x, Cv[j][q], m[q][3]);
-      m[q][4] = fma(c23.y, Cv[j][q], m[q][4]);
-    }
+    m[0] = fma(c01.x, A[j], m[0]);
+    m[1] = fma(c01.x, Bs[j], m[1]);
+    m[2] = fma(c01.y, Cv[j], m[2]);
+    m[3] = fma(c23.x, Cv[j], m[3]);
+    m[4] = fma(c23.y, Cv[j], m[4]);
   }
 }
 
@@ -345,9 +341,7 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     cp_async_wait_all();
     __syncthreads();
 
-    // The warp's share of the moment work: a quarter of the class's directions (at most 4: nd <= 16), all bands.
     const int nd = G.nd;
-    const int dw0 = (nd * wid) >> 2, dw1 = (nd * (wid + 1)) >> 2;
 
 #ifdef BRICK_PROF
     unsigned long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -470,26 +464,34 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         }
       }
       PROF_T(p3);
-      // ------------------------------------------ moments: thread = cells (lane, lane + 32) x the warp's directions -------
+      // ------------------------------------------ moments: thread = one cell x half of the class's directions ------------------
+      // a warp owns 16 cells (lanes 0-15 and 16-31 the two halves of the directions): one shuffle completes the sums, no
+      // exchange between warps
       {
-        const unsigned char *fb = reinterpret_cast<const unsigned char *>(sm.flg[st]);
-        const bool act0 = (fb[lane] & BRK_ACT) != 0, act1 = (fb[lane + 32] & BRK_ACT) != 0;
-        double m[2][5];
-        switch (dw1 - dw0) {
-          case 4: moments_dirs<4>(sm.plane + lane * kP + dw0, sm.bcoef, sm.dcoef + 4 * dw0, G.nb, nd, m); break;
-          case 3: moments_dirs<3>(sm.plane + lane * kP + dw0, sm.bcoef, sm.dcoef + 4 * dw0, G.nb, nd, m); break;
-          case 2: moments_dirs<2>(sm.plane + lane * kP + dw0, sm.bcoef, sm.dcoef + 4 * dw0, G.nb, nd, m); break;
-          case 1: moments_dirs<1>(sm.plane + lane * kP + dw0, sm.bcoef, sm.dcoef + 4 * dw0, G.nb, nd, m); break;
+        const int mh = lane >> 4, cell = wid * 16 + (lane & 15);
+        const int dh0 = (nd * mh) >> 1, dh1 = (nd * (mh + 1)) >> 1;
+        const bool act = (reinterpret_cast<const unsigned char *>(sm.flg[st])[cell] & BRK_ACT) != 0;
+        const double *mrow = sm.plane + cell * kP + dh0, *mdc = sm.dcoef + 4 * dh0;
+        double m[5];
+        switch (dh1 - dh0) {
+          case 8: moments_cell<8>(mrow, sm.bcoef, mdc, G.nb, nd, m); break;
+          case 7: moments_cell<7>(mrow, sm.bcoef, mdc, G.nb, nd, m); break;
+          case 6: moments_cell<6>(mrow, sm.bcoef, mdc, G.nb, nd, m); break;
+          case 5: moments_cell<5>(mrow, sm.bcoef, mdc, G.nb, nd, m); break;
+          case 4: moments_cell<4>(mrow, sm.bcoef, mdc, G.nb, nd, m); break;
+          case 3: moments_cell<3>(mrow, sm.bcoef, mdc, G.nb, nd, m); break;
+          case 2: moments_cell<2>(mrow, sm.bcoef, mdc, G.nb, nd, m); break;
+          case 1: moments_cell<1>(mrow, sm.bcoef, mdc, G.nb, nd, m); break;
           default:
 #pragma unroll
-            for (int k = 0; k < 5; ++k) m[0][k] = m[1][k] = 0.0;
+            for (int k = 0; k < 5; ++k) m[k] = 0.0;
         }
-        if (wid < 3) {
 #pragma unroll
-          for (int k = 0; k < 5; ++k) {
-            sm.red[wid][k][lane] = m[0][k];
-            sm.red[wid][k][lane + 32] = m[1][k];
-          }
+        for (int k = 0; k < 5; ++k) m[k] += __shfl_xor_sync(0xffffffffu, m[k], 16);  // a + b on both sides: the same bits
+        if (mh == 0 && act) {
+          double *p = part + (int64_t)u * kBrickCells + cell;
+#pragma unroll
+          for (int k = 0; k < 5; ++k) p[k * npos] = m[k];
         }
         PROF_T(p4);
         if (!last_u) {
@@ -501,7 +503,7 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         }
         PROF_T(p5);
         cp_async_wait_all();
-        __syncthreads();  // B2: the plane buffer is free again; the band partials are in place; theta of plane u+1 has landed
+        __syncthreads();  // B2: the plane buffer is free again; theta of plane u+1 has landed
         PROF_T(p6);
         PROF_ADD(0, p0, p1); PROF_ADD(1, p1, p2); PROF_ADD(2, p2, p3); PROF_ADD(3, p3, p4); PROF_ADD(4, p4, p5); PROF_ADD(5, p5, p6);
 #ifdef BRICK_PROF
@@ -509,16 +511,6 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         if (t == 0 && early) prof[7] += 1;
 #endif
         if (last_u && t == 0) st_release(a.prog + task, 0x7fffffffu);
-        if (wid == 3) {  // fixed order: warp 0 + warp 1 + warp 2 + warp 3
-          double *p = part + (int64_t)u * kBrickCells + lane;
-#pragma unroll
-          for (int k = 0; k < 5; ++k) {
-            const double v0 = ((sm.red[0][k][lane] + sm.red[1][k][lane]) + sm.red[2][k][lane]) + m[0][k];
-            const double v1 = ((sm.red[0][k][lane + 32] + sm.red[1][k][lane + 32]) + sm.red[2][k][lane + 32]) + m[1][k];
-            if (act0) p[k * npos] = v0;
-            if (act1) p[k * npos + 32] = v1;
-          }
-        }
       }
     }
 #ifdef BRICK_PROF
