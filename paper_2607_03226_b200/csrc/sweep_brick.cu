@@ -304,6 +304,9 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     }
     // v- and w-face inflow of plane 0
     const unsigned par = a.parity;
+#ifdef BRICK_PROF
+    unsigned long long prof[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+#endif
     Upstream ups;  // only the faces that mix task rows and closure rows are followed through counters
     ups.init(a.prog, T.fv_mode == BRK_FACE_COUNTER ? T.up_v : -1, T.fw_mode == BRK_FACE_COUNTER ? T.up_w : -1);
     const bool counters = T.fv_mode == BRK_FACE_COUNTER || T.fw_mode == BRK_FACE_COUNTER;
@@ -328,6 +331,9 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
             if (k < chk_w) bad |= stale_bit(ew[k], par);
           }
           if (!bad) break;
+#ifdef BRICK_PROF
+          if (t == 0) prof[7] += 1;
+#endif
           __nanosleep(20);
           load_faces();
         }
@@ -343,9 +349,6 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
 
     const int nd = G.nd;
 
-#ifdef BRICK_PROF
-    unsigned long long prof[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
     int ip = 0;  // next row of the IRR stream (same value in every thread)
     for (int u = 0; u < T.nu; ++u) {
       PROF_T(p0);
@@ -508,7 +511,6 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
         PROF_ADD(0, p0, p1); PROF_ADD(1, p1, p2); PROF_ADD(2, p2, p3); PROF_ADD(3, p3, p4); PROF_ADD(4, p4, p5); PROF_ADD(5, p5, p6);
 #ifdef BRICK_PROF
         if (t == 0) prof[6] += 1;
-        if (t == 0 && early) prof[7] += 1;
 #endif
         if (last_u && t == 0) st_release(a.prog + task, 0x7fffffffu);
       }
