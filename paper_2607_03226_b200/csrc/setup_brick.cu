@@ -92,7 +92,7 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
   bh.a2pos.assign((size_t)ncls * na, -1);
   std::vector<uint8_t> bf_nord(nbf, 0);
   struct OutEnt { int j, k, ul, vl, wl; };   // an outgoing wall face of a task: entry in Cls::out_*, side, cell
-  struct ProtoTask { BrickTask t; int key, cls, J, K, sg; std::vector<OutEnt> outs; int wall_cnt[3]; bool pure; };
+  struct ProtoTask { BrickTask t; int key, cls, J, K, sg; std::vector<OutEnt> outs; int wall_cnt[3]; };
   std::vector<ProtoTask> protos;
   for (int c = 0; c < ncls; ++c) {
     BrickHost::Cls &C = bh.cls[c];
@@ -195,9 +195,31 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
           T.src_lo = (uint32_t)src_planes; T.src_hi = (uint32_t)(src_planes >> 32);
           T.wall_any = nwall > T.wo0;
           T.wu0 = T.wv0 = T.ww0 = -1;
+          // A fully active box whose downstream faces are each all wall (and then without a downstream tile) or all interior:
+          // its wall rows become face blocks with the addressing of the inflow faces (u-face [w][v], v-face [u][w], w-face
+          // [u][v]), so that the sweep stores wall values where it would store the face of a downstream tile -- no pass over
+          // the wall cells afterwards.
+          auto box_exists = [&](int Jq, int Kq, int sq) {
+            return Jq >= 0 && Jq < NTv && Kq >= 0 && Kq < NTw && sq >= 0 && sq < nseg && box_on[phys_box(Jq, Kq, sq)] != 0;
+          };
           const int face_n[3] = {T.tv * T.tw, T.nu * T.tw, T.nu * T.tv};
-          P.pure = T.plain && T.wall_any && (wall_cnt[0] == 0 || wall_cnt[0] == face_n[0]) &&
-                   (wall_cnt[1] == 0 || wall_cnt[1] == face_n[1]) && (wall_cnt[2] == 0 || wall_cnt[2] == face_n[2]);
+          const bool dn_exists[3] = {box_exists(Jp, Kp, sp + 1), box_exists(Jp + 1, Kp, sp), box_exists(Jp, Kp + 1, sp)};
+          bool pure = T.plain && T.wall_any;
+          for (int k = 0; k < 3; ++k) pure = pure && (wall_cnt[k] == 0 || (wall_cnt[k] == face_n[k] && !dn_exists[k]));
+          if (pure) {
+            nwall = T.wo0;  // the rows given out cell by cell above are taken back
+            if (wall_cnt[0]) { T.wu0 = nwall; nwall += kBrickCells; }
+            if (wall_cnt[1]) { T.wv0 = nwall; nwall += T.nu * kBrickTile; }
+            if (wall_cnt[2]) { T.ww0 = nwall; nwall += T.nu * kBrickTile; }
+            for (const OutEnt &e : outs) {
+              const int row = e.k == 0 ? T.wu0 + e.wl * kBrickTile + e.vl : e.k == 1 ? T.wv0 + e.ul * kBrickTile + e.wl : T.ww0 + e.ul * kBrickTile + e.vl;
+              C.out_row[e.j] = row;
+              bh.bf_wrow[(size_t)c * nbf + C.out_bf[e.j]] = row;
+            }
+            T.wall_any = 0;  // nothing left for the pass over the wall cells
+          }
+          outs.clear();
+          outs.shrink_to_fit();
           task_of[pbox(Jp, Kp, sp)] = (int)protos.size();
           protos.push_back(P);
         }
@@ -231,24 +253,7 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
       P.t.dn_fu0 = du >= 0 ? protos[du].t.fu0 : -1;
       P.t.dn_fv0 = dv >= 0 ? protos[dv].t.fv0 : -1;
       P.t.dn_fw0 = dw >= 0 ? protos[dw].t.fw0 : -1;
-      // A fully active box whose downstream faces are each all wall (and then without a downstream tile) or all interior: its
-      // wall rows become face blocks with the addressing of the inflow faces (u-face [w][v], v-face [u][w], w-face [u][v]), so
-      // that the sweep stores wall values where it would store the face of a downstream tile -- no pass over the wall cells
-      // afterwards.  (The rows given out cell by cell above stay unused.)
-      if (P.pure && !(P.wall_cnt[0] && du >= 0) && !(P.wall_cnt[1] && dv >= 0) && !(P.wall_cnt[2] && dw >= 0)) {
-        BrickTask &T = P.t;
-        if (P.wall_cnt[0]) { T.wu0 = nwall; nwall += kBrickCells; }
-        if (P.wall_cnt[1]) { T.wv0 = nwall; nwall += T.nu * kBrickTile; }
-        if (P.wall_cnt[2]) { T.ww0 = nwall; nwall += T.nu * kBrickTile; }
-        for (const OutEnt &e : P.outs) {
-          const int row = e.k == 0 ? T.wu0 + e.wl * kBrickTile + e.vl : e.k == 1 ? T.wv0 + e.ul * kBrickTile + e.wl : T.ww0 + e.ul * kBrickTile + e.vl;
-          C.out_row[e.j] = row;
-          bh.bf_wrow[(size_t)c * nbf + C.out_bf[e.j]] = row;
-        }
-        T.wall_any = 0;  // nothing left for the pass over the wall cells
-      }
-      P.outs.clear();
-      P.outs.shrink_to_fit();
+
     }
     C.scratch_row = nrow; nrow += kBrickTile;
     C.npos = npos; C.nrow = nrow; C.nwall = std::max(1, nwall);

@@ -71,7 +71,9 @@ def test_workspace_bytes_and_host_setup(lib, name, kw, nupd):
     if nupd is not None:
         assert wl.n_updates(pr) == nupd
     assert nbytes > n_e  # the e array dominates; tables and caches come on top
-    assert nbytes < 3 * n_e + (64 << 20)
+    # tile-dataflow path: positions padded to 64 per tile plane, tile-face and wall rows at a pitch of 128 systems, partial
+    # moments, multigrid tables -- on a grid this small (tiles 4 cells wide) that is up to ~4x the distribution itself
+    assert nbytes < 4 * n_e + (64 << 20)
 
 
 def test_host_validation_errors(lib):
