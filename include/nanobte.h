@@ -256,6 +256,20 @@ int nanobte_get_G(nanobte_solver *, double *dst /* [n_bfaces][B] deviational dif
 /* Heat leaving through the faces of each tag [W, or W/m in 2-D], outward positive (O8), for the last
  * sweep + update pair.  per_tag is a host pointer [n_tags]; synchronises. */
 int nanobte_get_boundary_heat(nanobte_solver *, double *per_tag);
+/* The same quantity (O8) for callers that may not allocate -- code under CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc: no cudaMalloc/cudaFree and no allocating library routine is called, by this
+ * entry point or below it.  The faces of a tag are summed by 16 blocks whose partial sums go through a file-scope static
+ * device array (csrc/noalloc.cu; 34 KiB, held by every GPU that loads the library until the process exits) and are joined
+ * in a fixed order, so the result is reproducible run to run and equals nanobte_get_boundary_heat's up to the order of
+ * the additions.  per_tag: [n_tags], caller-owned, a device pointer (dst_is_device = 1: nothing synchronises, the result
+ * is ordered on the solver's stream) or a host pointer (0: synchronises).  The device the solver was created on must
+ * be current, as for every call.  Errors: NANOBTE_E_INVALID if n_tags > NANOBTE_NOALLOC_MAX_TAGS (message in
+ * nanobte_last_error; use nanobte_get_boundary_heat then) or a null argument; NANOBTE_E_CUDA as elsewhere.
+ * All calls on one GPU share the static array, whatever the solver: calls that overlap on the GPU (other streams,
+ * other threads' solvers) race on it; calls on one stream, or otherwise ordered, do not.  Nothing in it needs clearing
+ * between calls (every entry that is read was written by the same call). */
+#define NANOBTE_NOALLOC_MAX_TAGS 256
+int nanobte_get_boundary_heat_noalloc(nanobte_solver *, double *per_tag, int32_t dst_is_device);
 /* History of the last nanobte_solve: returns the number of iterations recorded, fills up to cap entries. */
 int nanobte_get_history(nanobte_solver *, double *dT, int32_t *cg_iters, int32_t cap);
 int nanobte_get_info(const nanobte_solver *, nanobte_info *out);

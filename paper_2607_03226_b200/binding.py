@@ -23,7 +23,7 @@ EXPORTS = [
     "nanobte_create_unstructured", "nanobte_destroy", "nanobte_sweep", "nanobte_update_temperature",
     "nanobte_diffusion_correct", "nanobte_init_fourier", "nanobte_band_totals", "nanobte_moments_len", "nanobte_export_moments",
     "nanobte_import_moments", "nanobte_step", "nanobte_set_keep_e", "nanobte_solve", "nanobte_set_T", "nanobte_get_T", "nanobte_get_q", "nanobte_get_e",
-    "nanobte_get_G", "nanobte_get_boundary_heat", "nanobte_get_history", "nanobte_get_info", "nanobte_launch_count",
+    "nanobte_get_G", "nanobte_get_boundary_heat", "nanobte_get_boundary_heat_noalloc", "nanobte_get_history", "nanobte_get_info", "nanobte_launch_count",
     "nanobte_kappa", "nanobte_strerror", "nanobte_last_error",
 ]
 
@@ -117,6 +117,7 @@ def load():
     lib.nanobte_get_e.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, C.c_int32, C.c_int32]
     lib.nanobte_get_G.argtypes = [vp, vp, C.c_int32]
     lib.nanobte_get_boundary_heat.argtypes = [vp, _dp]
+    lib.nanobte_get_boundary_heat_noalloc.argtypes = [vp, vp, C.c_int32]
     lib.nanobte_get_history.argtypes = [vp, _dp, _ip, C.c_int32]
     lib.nanobte_get_info.argtypes = [vp, C.POINTER(Info)]
     lib.nanobte_launch_count.argtypes = [vp]
@@ -368,6 +369,13 @@ class Solver:
     def get_boundary_heat(self):
         out = np.zeros(max(1, self.n_tags))
         self._chk(self._lib.nanobte_get_boundary_heat(self._h, out.ctypes.data_as(_dp)))
+        return out[:self.n_tags]
+
+    def get_boundary_heat_noalloc(self, device=False):
+        """nanobte_get_boundary_heat_noalloc: the same per-tag heat through the library's static scratch (no allocation
+        below the C-ABI; at most NANOBTE_NOALLOC_MAX_TAGS = 256 tags)."""
+        out, p = self._out((max(1, self.n_tags),), device)
+        self._chk(self._lib.nanobte_get_boundary_heat_noalloc(self._h, p, int(device)))
         return out[:self.n_tags]
 
     def get_history(self):

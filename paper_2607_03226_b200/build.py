@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libnanobte.so")
 SOURCES = ["api.cu", "setup_structured.cu", "sweep_structured.cu", "kernels_common.cu", "cg.cu", "sweep_unstructured.cu",
-           "setup_brick.cu", "sweep_brick.cu", "kernels_brick.cu", "cg_mg.cu"]
+           "setup_brick.cu", "sweep_brick.cu", "kernels_brick.cu", "cg_mg.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--fmad=true",
               "-Xcompiler", "-fPIC,-O2,-Wall,-Wno-unused-function", "-cudart", "static"]
 
