@@ -85,6 +85,13 @@ struct BrickInRow {
   uint8_t type, cm, perm, pad;  // face type; mirror class; which direction permutation of the class (BrickState::in_perm)
 };
 
+// One outgoing-face entry of a class (gsum kernel): the face, its wall row (of every group of the class), the class's rank
+// among the face's outgoing classes and the face type in one 16-byte load.
+struct BrickOutRow {
+  int32_t bf, row;
+  uint8_t ord, type, pad[6];
+};
+
 struct BrickArgs {
   const BrickTask *tasks;      // in launch (topological) order
   const BrickCG *cgs;
@@ -121,6 +128,7 @@ struct BrickState {
   const int32_t *cg_of = nullptr;                      // [n_cls][B] (class, band) -> cg
   const int32_t *a2pos = nullptr;                      // [n_cls][n_act]
   const int32_t *pos2a = nullptr;                      // [npos of class 0]
+  const BrickOutRow *out_rec[NB_MAX_CLASSES] = {nullptr};  // per class [n_out]: records of the gsum kernel
   const BrickInRow *in_rec[NB_MAX_CLASSES] = {nullptr};  // per class [n_in]: records of the fast inflow kernel
   const uint8_t *in_perm = nullptr;                    // [n_cls][8][16] direction -> mirrored direction (local indices; 255: none)
   int32_t cg0[NB_MAX_CLASSES] = {0};                   // first (class, group) of a class

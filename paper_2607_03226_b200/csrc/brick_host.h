@@ -29,6 +29,7 @@ struct BrickHost {
     std::vector<int32_t> in_row, in_bf;             // boundary-inflow rows and their faces
     std::vector<int32_t> out_bf, out_row;           // outgoing faces and the wall row of their cell, wall-row order
     std::vector<uint8_t> out_ord;                   // rank of the class among the face's outgoing classes
+    std::vector<BrickOutRow> out_rec;               // records of the gsum kernel
     std::vector<BrickInRow> in_rec;                 // records of the fast inflow kernel
     int npos = 0, nrow = 0, nwall = 0, scratch_row = 0;
   };

@@ -164,6 +164,9 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
   L1.nbr = nbr1; L1.cnt = cnt1; L1.dinv = dinv1; L1.diag = diag1;
   L2.nbr = nbr2; L2.cnt = cnt2; L2.dinv = dinv2; L2.diag = diag2;
 
+#ifdef MG_PROF
+  long long tprof = clock64();
+#endif
   // ---- load the CTA's tables ------------------------------------------------------------------------------------------------------------
   for (int i = tid; i < n1; i += kMgThreads) {
     dinv1[i] = a.dinv[1][base1 + i]; diag1[i] = a.diag[1][base1 + i];
@@ -190,6 +193,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
   for (int j = tid; j < nh2; j += kMgThreads) { hidx2[j] = a.hidx[2][h2lo + j]; hpar2[j] = a.hpar[2][h2lo + j]; }
   if (tid == 0) { x0[n0 + nh0] = 0.0; L1.x[n1 + nh1] = 0.0; L2.x[n2 + nh2] = 0.0; }
 
+  MGP(11);
   // ---- level 0: stencil, right-hand side (R14c, R14c'), CG vectors ------------------------------------------------------------------------
   const int64_t nslot0 = (int64_t)a.a3ptr[a.nblk] * 512;
   uint16_t nl[CPT][6];
@@ -226,6 +230,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     }
   }
   __syncthreads();
+  MGP(12);
 
   auto A0 = [&](int c, const double *v, double vc) {  // full operator, row of slot c of this thread
     double acc = dg[c] * vc;
@@ -330,9 +335,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
   double g_prev = 1.0, alpha_prev = 1.0, stop2 = 0.0;
   bool not_converged = false;
   const int64_t nslot1 = (int64_t)a.a3ptr[a.nblk] * 64, nslot2 = (int64_t)a.a3ptr[a.nblk] * 8;
-#ifdef MG_PROF
-  long long tprof = clock64();
-#endif
+  MGP(13);
   for (;; ++it) {
     const unsigned bit = ((unsigned)(it >> 1) & 1u) ^ 1u;
     MGP(9);

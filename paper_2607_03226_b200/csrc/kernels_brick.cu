@@ -24,6 +24,7 @@ struct BrickClosureArgs {
   // gsum
   const int32_t *out_bf[NB_MAX_CLASSES], *out_row[NB_MAX_CLASSES];
   const uint8_t *out_ord[NB_MAX_CLASSES];
+  const BrickOutRow *out_rec[NB_MAX_CLASSES];
   int32_t n_out[NB_MAX_CLASSES];
   int32_t therm;             // 1: thermalizing faces only, 0: all the others
   double *partial;           // [4][n_bf][B]
@@ -36,27 +37,94 @@ struct BrickClosureArgs {
   const BrickInRow *in_rec[NB_MAX_CLASSES];
   const uint8_t *in_perm;    // [n_cls][8][16]
   int32_t cg0[NB_MAX_CLASSES];
+  int32_t n_cls;
 };
 
-// gnum share of one class: sum over the class's directions of w (s.n) eps at the wall cell (R7).  One thread per
-// (outgoing face entry, band); the directions of a (cell, band) are contiguous in the wall row.
-__global__ void __launch_bounds__(128) brick_gsum_kernel(const BrickClosureArgs R) {
+// gnum share of one class: sum over the class's directions of w (s.n) eps at the wall cell (R7).  A warp walks over
+// outgoing face entries of its class: per entry one 16-byte record (fetched one entry ahead), then the entry's wall rows (one
+// per band group, S <= 128 contiguous doubles each) with coalesced loads, all in flight before the first use, through
+// shared memory; lanes = bands then add the nd values of their band times w (s.n) in direction order (the arithmetic of a
+// thread per (entry, band) walking its directions, bit for bit).
+constexpr int kGsumGroups = 4;  // band groups covered by one pass (a class with more takes several)
+constexpr int kGsumWarps = 4;
+__global__ void __launch_bounds__(32 * kGsumWarps) brick_gsum_kernel(const BrickClosureArgs R) {
+  __shared__ double buf[kGsumWarps][kGsumGroups * kBrickRow];
+  __shared__ double wsn[kGsumWarps][16];  // w (s.n) of the class's directions at the entry's face
   const BoundaryArgs &a = R.a;
-  const int c = blockIdx.y;
-  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= (int64_t)R.n_out[c] * a.B) return;
-  const int j = (int)(idx / a.B), b = (int)(idx % a.B);
-  const int bf = R.out_bf[c][j];
-  if ((a.bf_type[bf] == NANOBTE_THERMALIZING) != (R.therm != 0)) return;
-  const BrickCG G = R.cgs[R.cg_of[c * a.B + b]];
-  const double *src = R.wall + G.wall_base + (int64_t)R.out_row[c][j] * kBrickRow + (b - G.b0) * G.nd;
-  const double *sn = a.bf_sn + (size_t)bf * a.D;
-  double acc = 0.0;
-  for (int dl = 0; dl < G.nd; ++dl) {
-    const int d = R.cls_dirs[c * R.max_dirs + dl];
-    acc += a.w[d] * sn[d] * src[dl];
+  const int c = blockIdx.y, wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_out = R.n_out[c], stride = gridDim.x * kGsumWarps;
+  int j = blockIdx.x * kGsumWarps + wid;
+  if (j >= n_out) return;
+  const int g0 = R.cg0[c], ng = R.cg_of[c * a.B + a.B - 1] - g0 + 1;
+  const int nd = R.cgs[g0].nd;
+  double *mine = buf[wid];
+  int S[kGsumGroups];
+  int64_t wbase[kGsumGroups];
+#pragma unroll
+  for (int q = 0; q < kGsumGroups; ++q) {
+    S[q] = q < ng ? R.cgs[g0 + q].S : 0;
+    wbase[q] = q < ng ? R.cgs[g0 + q].wall_base : 0;
   }
-  R.partial[((size_t)R.out_ord[c][j] * a.n_bf + bf) * a.B + b] = acc;
+  // lane = band (the bands beyond 32 and the groups beyond kGsumGroups take the general loops below)
+  int my_q = -1, my_off = 0;
+  double wd = 0.0;
+  int dd = 0;
+  if (lane < a.B) {
+    my_q = R.cg_of[c * a.B + lane] - g0;
+    my_off = my_q * kBrickRow + (lane - R.cgs[g0 + my_q].b0) * nd;
+  }
+  if (lane < nd) {
+    dd = R.cls_dirs[c * R.max_dirs + lane];
+    wd = a.w[dd];
+  }
+  BrickOutRow nxt = R.out_rec[c][j];
+  for (; j < n_out; j += stride) {
+    const BrickOutRow rec = nxt;
+    if (j + stride < n_out) nxt = R.out_rec[c][j + stride];
+    if ((rec.type == NANOBTE_THERMALIZING) != (R.therm != 0)) continue;
+    double *out = R.partial + ((size_t)rec.ord * a.n_bf + rec.bf) * a.B;
+    double v[kGsumGroups][4];
+#pragma unroll
+    for (int q = 0; q < kGsumGroups; ++q) {
+      const double *src = R.wall + wbase[q] + (int64_t)rec.row * kBrickRow;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) v[q][k] = lane + 32 * k < S[q] ? __ldg(src + lane + 32 * k) : 0.0;
+    }
+    if (lane < nd) wsn[wid][lane] = wd * a.bf_sn[(size_t)rec.bf * a.D + dd];
+#pragma unroll
+    for (int q = 0; q < kGsumGroups; ++q) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (lane + 32 * k < S[q]) mine[q * kBrickRow + lane + 32 * k] = v[q][k];
+    }
+    __syncwarp();
+    if (my_q >= 0 && my_q < kGsumGroups) {
+      double acc = 0.0;
+      for (int dl = 0; dl < nd; ++dl) acc = fma(wsn[wid][dl], mine[my_off + dl], acc);
+      out[lane] = acc;
+    }
+    for (int b = lane + 32; b < a.B; b += 32) {  // more than 32 bands
+      const int q = R.cg_of[c * a.B + b] - g0;
+      if (q >= kGsumGroups) continue;
+      const int off = q * kBrickRow + (b - R.cgs[g0 + q].b0) * nd;
+      double acc = 0.0;
+      for (int dl = 0; dl < nd; ++dl) acc = fma(wsn[wid][dl], mine[off + dl], acc);
+      out[b] = acc;
+    }
+    for (int gb = kGsumGroups; gb < ng; ++gb) {  // more than kGsumGroups band groups: one group at a time
+      __syncwarp();
+      const BrickCG &G = R.cgs[g0 + gb];
+      const double *src = R.wall + G.wall_base + (int64_t)rec.row * kBrickRow;
+      for (int e = lane; e < G.S; e += 32) mine[e] = __ldg(src + e);
+      __syncwarp();
+      for (int bl = lane; bl < G.nb; bl += 32) {
+        double acc = 0.0;
+        for (int dl = 0; dl < nd; ++dl) acc = fma(wsn[wid][dl], mine[bl * nd + dl], acc);
+        out[G.b0 + bl] = acc;
+      }
+    }
+    __syncwarp();
+  }
 }
 
 // Inflow rows of the boundary faces (R6-R8, lagged R9): one CTA per (row, (class, group)), lanes = systems.
@@ -91,57 +159,78 @@ __global__ void __launch_bounds__(kBrickMaxS) brick_inflow_kernel(const BrickClo
   *dst = type == NANOBTE_SPECULAR ? spec : a.bf_p[bf] * spec + (1.0 - a.bf_p[bf]) * Gf;  // R8
 }
 
-// The same from the per-row records built at create (BrickInRow): a CTA takes kInRows consecutive rows of one (class, group),
-// lanes = systems.  Per row one 16-byte record (uniform), then G / p / the mirror group's base (independent loads), then the
-// wall value: three dependent loads instead of eight, four rows in flight.
+// The same from the per-row records built at create (BrickInRow): a CTA belongs to one (class, group), lanes = systems, and
+// walks over the class's rows kInRows at a time.  What does not depend on the row is set up once per CTA: the thread's band
+// and direction, its mirror direction under each of the class's (at most 8) permutations packed in one register, the wall
+// block and direction count of this band group in every class.  Per row: one 16-byte record (uniform; the next rows' records
+// are fetched while these are worked on), then G / p (independent loads), then the wall value.
 constexpr int kInRows = 4;
 __global__ void __launch_bounds__(kBrickMaxS) brick_inflow_fast_kernel(const BrickClosureArgs R) {
+  __shared__ int64_t m_base[NB_MAX_CLASSES];
+  __shared__ int32_t m_nd[NB_MAX_CLASSES];
   const BoundaryArgs &a = R.a;
   const BrickCG G = R.cgs[blockIdx.y];
   const int c = G.cls, s = threadIdx.x;
-  if (s >= G.S) return;
-  const int k0 = blockIdx.x * kInRows, n_in = R.n_in[c];
-  if (k0 >= n_in) return;
-  const int bl = s / G.nd, dl = s - bl * G.nd, b = G.b0 + bl;
   const int g = blockIdx.y - R.cg0[c];           // band group index: the same in the mirror class
-  const double Cb = a.C[b] / R.W;
-  double *inf = R.inf + G.inf_base + s;
-  BrickInRow rec[kInRows];
-#pragma unroll
-  for (int q = 0; q < kInRows; ++q) {
-    rec[q].bf = -1;
-    if (k0 + q < n_in) rec[q] = R.in_rec[c][k0 + q];
+  if (s < R.n_cls) {
+    const BrickCG &Gm = R.cgs[R.cg0[s] + g];
+    m_base[s] = Gm.wall_base;
+    m_nd[s] = Gm.nd;
   }
-  double Gf[kInRows], p[kInRows], spec[kInRows];
-  bool has[kInRows];
+  __syncthreads();
+  const int n_in = R.n_in[c];
+  if (s >= G.S) return;
+  const int bl = s / G.nd, dl = s - bl * G.nd, b = G.b0 + bl;
+  unsigned long long perms = 0;                  // byte q: mirror direction (local to its class) under permutation q, 255 = none
+#pragma unroll
+  for (int q = 0; q < 8; ++q) perms |= (unsigned long long)R.in_perm[((size_t)c * 8 + q) * 16 + dl] << (8 * q);
+  double *inf = R.inf + G.inf_base + s;
+  const double *Gb = a.G + b;
+  const int stride = gridDim.x * kInRows;
+  BrickInRow nxt[kInRows];
 #pragma unroll
   for (int q = 0; q < kInRows; ++q) {
-    Gf[q] = p[q] = spec[q] = 0.0;
-    has[q] = false;
-    if (rec[q].bf < 0 || rec[q].type == NANOBTE_THERMALIZING || R.init) continue;
-    if (rec[q].type != NANOBTE_SPECULAR) Gf[q] = a.G[(size_t)rec[q].bf * a.B + b];
-    if (rec[q].type == NANOBTE_MIXED) p[q] = a.bf_p[rec[q].bf];
-    if (rec[q].type != NANOBTE_DIFFUSE && rec[q].msrc >= 0) {
-      const int dlm = R.in_perm[((size_t)c * 8 + rec[q].perm) * 16 + dl];
-      if (dlm != 255) {
-        const BrickCG &Gm = R.cgs[R.cg0[rec[q].cm] + g];
-        spec[q] = R.wall[Gm.wall_base + (int64_t)rec[q].msrc * kBrickRow + bl * Gm.nd + dlm];
-        has[q] = true;
+    nxt[q].bf = -1;
+    if (blockIdx.x * kInRows + q < n_in) nxt[q] = R.in_rec[c][blockIdx.x * kInRows + q];
+  }
+  for (int k0 = blockIdx.x * kInRows; k0 < n_in; k0 += stride) {
+    BrickInRow rec[kInRows];
+#pragma unroll
+    for (int q = 0; q < kInRows; ++q) {
+      rec[q] = nxt[q];
+      nxt[q].bf = -1;
+      if (k0 + stride + q < n_in) nxt[q] = R.in_rec[c][k0 + stride + q];
+    }
+    double Gf[kInRows], p[kInRows], spec[kInRows];
+    bool has[kInRows];
+#pragma unroll
+    for (int q = 0; q < kInRows; ++q) {
+      Gf[q] = p[q] = spec[q] = 0.0;
+      has[q] = false;
+      if (rec[q].bf < 0 || rec[q].type == NANOBTE_THERMALIZING || R.init) continue;
+      if (rec[q].type != NANOBTE_SPECULAR) Gf[q] = Gb[(size_t)rec[q].bf * a.B];
+      if (rec[q].type == NANOBTE_MIXED) p[q] = a.bf_p[rec[q].bf];
+      if (rec[q].type != NANOBTE_DIFFUSE && rec[q].msrc >= 0) {
+        const int dlm = (int)((perms >> (8 * rec[q].perm)) & 255ull);
+        if (dlm != 255) {
+          spec[q] = R.wall[m_base[rec[q].cm] + (int64_t)rec[q].msrc * kBrickRow + bl * m_nd[rec[q].cm] + dlm];
+          has[q] = true;
+        }
       }
     }
-  }
 #pragma unroll
-  for (int q = 0; q < kInRows; ++q) {
-    if (rec[q].bf < 0) continue;
-    double *dst = inf + (int64_t)rec[q].row * kBrickRow;
-    if (rec[q].type == NANOBTE_THERMALIZING) {
-      if (R.init) *dst = Cb * a.bf_eps_w[rec[q].bf];  // R6; never changes afterwards
-      continue;
+    for (int q = 0; q < kInRows; ++q) {
+      if (rec[q].bf < 0) continue;
+      double *dst = inf + (int64_t)rec[q].row * kBrickRow;
+      if (rec[q].type == NANOBTE_THERMALIZING) {
+        if (R.init) *dst = a.C[b] / R.W * a.bf_eps_w[rec[q].bf];  // R6; never changes afterwards
+        continue;
+      }
+      if (R.init) continue;  // eps^0 = 0 (R12)
+      if (rec[q].type == NANOBTE_DIFFUSE) *dst = Gf[q];                                                   // R7
+      else if (rec[q].type == NANOBTE_SPECULAR) *dst = spec[q];                                           // mirror (0 if s.n == 0, R15)
+      else *dst = has[q] ? p[q] * spec[q] + (1.0 - p[q]) * Gf[q] : 0.0;                                   // R8
     }
-    if (R.init) continue;  // eps^0 = 0 (R12)
-    if (rec[q].type == NANOBTE_DIFFUSE) *dst = Gf[q];                                                   // R7
-    else if (rec[q].type == NANOBTE_SPECULAR) *dst = spec[q];                                           // mirror (0 if s.n == 0, R15)
-    else *dst = has[q] ? p[q] * spec[q] + (1.0 - p[q]) * Gf[q] : 0.0;                                   // R8
   }
 }
 
@@ -244,9 +333,11 @@ BrickClosureArgs closure_args(nanobte_solver *h) {
   R.cls_dirs = h->cls_dirs; R.max_dirs = h->max_cls_dirs; R.wall = bs.a.wall; R.inf = bs.a.inf; R.partial = h->g_partial;
   R.bf_wrow = bs.bf_wrow;
   R.in_perm = bs.in_perm;
+  R.n_cls = h->n_cls;
   for (int c = 0; c < NB_MAX_CLASSES; ++c) {
     R.in_rec[c] = bs.in_rec[c]; R.cg0[c] = bs.cg0[c];
     R.out_bf[c] = bs.out_bf[c]; R.out_row[c] = bs.out_row[c]; R.out_ord[c] = bs.out_ord[c]; R.n_out[c] = bs.n_out[c];
+    R.out_rec[c] = bs.out_rec[c];
     R.in_row[c] = bs.in_row[c]; R.in_bf[c] = bs.in_bf[c]; R.n_in[c] = bs.n_in[c];
   }
   return R;
@@ -257,9 +348,11 @@ int launch_gsum(nanobte_solver *h, const int32_t *faces, int n_faces, int therm)
   BrickClosureArgs R = closure_args(h);
   R.therm = therm;
   int64_t nmax = 0;
-  for (int c = 0; c < h->n_cls; ++c) nmax = std::max<int64_t>(nmax, (int64_t)R.n_out[c] * h->B);
+  for (int c = 0; c < h->n_cls; ++c) nmax = std::max<int64_t>(nmax, R.n_out[c]);
   if (nmax > 0) {
-    dim3 grid((unsigned)((nmax + 127) / 128), h->n_cls);
+    // a few waves of CTAs; each warp walks over its share of the entries
+    const int64_t want = ((int64_t)32 * h->n_sm + h->n_cls - 1) / h->n_cls;
+    dim3 grid((unsigned)std::max<int64_t>(1, std::min<int64_t>((nmax + kGsumWarps - 1) / kGsumWarps, want)), h->n_cls);
     brick_gsum_kernel<<<grid, 128, 0, h->stream>>>(R);
     h->launches++;
     NB_CUDA(h, cudaGetLastError());
@@ -274,7 +367,9 @@ int launch_inflow(nanobte_solver *h, int init) {
   for (int c = 0; c < h->n_cls; ++c) nmax = std::max(nmax, R.n_in[c]);
   if (nmax == 0) return 0;
   if (h->brick->in_fast) {
-    dim3 grid((nmax + kInRows - 1) / kInRows, h->brick->n_cg);
+    // a few waves of CTAs; each walks over its share of the rows
+    const int want = (32 * h->n_sm + h->brick->n_cg - 1) / h->brick->n_cg;
+    dim3 grid(std::max(1, std::min((nmax + kInRows - 1) / kInRows, want)), h->brick->n_cg);
     brick_inflow_fast_kernel<<<grid, kBrickMaxS, 0, h->stream>>>(R);
   } else {
     dim3 grid(nmax, h->brick->n_cg);

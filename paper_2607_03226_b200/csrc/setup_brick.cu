@@ -309,6 +309,15 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
       }
     }
     bh.cg0.assign(cls_cg0.begin(), cls_cg0.end());
+    for (int c = 0; c < ncls; ++c) {  // records of the gsum kernel (the wall rows are final here)
+      BrickHost::Cls &C = bh.cls[c];
+      C.out_rec.resize(C.out_bf.size());
+      for (size_t j = 0; j < C.out_rec.size(); ++j) {
+        BrickOutRow R{};
+        R.bf = C.out_bf[j]; R.row = C.out_row[j]; R.ord = C.out_ord[j]; R.type = (uint8_t)x.G->bf_type[R.bf];
+        C.out_rec[j] = R;
+      }
+    }
     for (int c = 1; c < ncls; ++c)  // the same band groups in every class (then the mirror group is the same group index)
       if (cls_ng[c] != cls_ng[0] || x.dirs[c].size() != x.dirs[0].size()) bh.in_fast = false;
   }
@@ -405,6 +414,7 @@ int nb_brick_upload(nanobte_solver *h, Arena &A, BrickHost &bh) {
     bs.out_bf[c] = A.put(C.out_bf);
     bs.out_row[c] = A.put(C.out_row);
     bs.out_ord[c] = A.put(C.out_ord);
+    bs.out_rec[c] = A.put(C.out_rec);
     bs.n_out[c] = (int32_t)C.out_bf.size();
     if (bh.in_fast) bs.in_rec[c] = A.put(C.in_rec);
     bs.cg0[c] = bh.cg0[c];
