@@ -77,6 +77,8 @@ struct BrickCG {
   int64_t coef_base;           // [S][5] sweep coefficients, then [nd][4] (w, w s), then [nb][2] (1/tau, v)
 };
 
+constexpr int kBrickInRows = 4;  // records per batch of the fast inflow kernel (one face type per batch)
+
 // One boundary-inflow row of a class, everything the closure kernel needs about it in one 16-byte load.
 struct BrickInRow {
   int32_t bf;          // boundary face
@@ -129,7 +131,8 @@ struct BrickState {
   const int32_t *a2pos = nullptr;                      // [n_cls][n_act]
   const int32_t *pos2a = nullptr;                      // [npos of class 0]
   const BrickOutRow *out_rec[NB_MAX_CLASSES] = {nullptr};  // per class [n_out]: records of the gsum kernel
-  const BrickInRow *in_rec[NB_MAX_CLASSES] = {nullptr};  // per class [n_in]: records of the fast inflow kernel
+  const BrickInRow *in_rec[NB_MAX_CLASSES] = {nullptr};  // per class [n_rec]: records of the fast inflow kernel, by type
+  int32_t n_rec[NB_MAX_CLASSES] = {0};
   const uint8_t *in_perm = nullptr;                    // [n_cls][8][16] direction -> mirrored direction (local indices; 255: none)
   int32_t cg0[NB_MAX_CLASSES] = {0};                   // first (class, group) of a class
   bool in_fast = false;                                // the records are valid (same band groups in every class, <= 8 permutations)

@@ -31,6 +31,7 @@ struct BrickClosureArgs {
   // inflow
   const int32_t *in_row[NB_MAX_CLASSES], *in_bf[NB_MAX_CLASSES];
   int32_t n_in[NB_MAX_CLASSES];
+  int32_t n_rec[NB_MAX_CLASSES];
   const int32_t *bf_wrow;    // [n_cls][n_bf]
   int32_t init;
   // fast inflow kernel
@@ -47,8 +48,18 @@ struct BrickClosureArgs {
 // thread per (entry, band) walking its directions, bit for bit).
 constexpr int kGsumGroups = 4;  // band groups covered by one pass (a class with more takes several)
 constexpr int kGsumWarps = 4;
+// A band's nd values sit at pitch nd + 1 (nd >= 8; fewer directions: no pad) and a group's block at pitch 146 (= 2 mod 16):
+// with nd = 12 and 10 bands per group the 30 lanes of the summation hit 30 different banks in every half-warp.
+constexpr int kGsumPitch = 146;
+static_assert(kGsumPitch >= kBrickRow + kBrickRow / 8, "a row of 128 values with one pad per band of >= 8 directions");
+__device__ __forceinline__ BrickOutRow ld_out_rec(const BrickOutRow *p) {
+  const int4 r = __ldg(reinterpret_cast<const int4 *>(p));
+  BrickOutRow o;
+  o.bf = r.x; o.row = r.y; o.ord = (uint8_t)(r.z & 255); o.type = (uint8_t)((r.z >> 8) & 255);
+  return o;
+}
 __global__ void __launch_bounds__(32 * kGsumWarps) brick_gsum_kernel(const BrickClosureArgs R) {
-  __shared__ double buf[kGsumWarps][kGsumGroups * kBrickRow];
+  __shared__ double buf[kGsumWarps][kGsumGroups * kGsumPitch];
   __shared__ double wsn[kGsumWarps][16];  // w (s.n) of the class's directions at the entry's face
   const BoundaryArgs &a = R.a;
   const int c = blockIdx.y, wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -56,7 +67,7 @@ __global__ void __launch_bounds__(32 * kGsumWarps) brick_gsum_kernel(const Brick
   int j = blockIdx.x * kGsumWarps + wid;
   if (j >= n_out) return;
   const int g0 = R.cg0[c], ng = R.cg_of[c * a.B + a.B - 1] - g0 + 1;
-  const int nd = R.cgs[g0].nd;
+  const int nd = R.cgs[g0].nd, ndp = nd >= 8 ? nd + 1 : nd;
   double *mine = buf[wid];
   int S[kGsumGroups];
   int64_t wbase[kGsumGroups];
@@ -71,16 +82,19 @@ __global__ void __launch_bounds__(32 * kGsumWarps) brick_gsum_kernel(const Brick
   int dd = 0;
   if (lane < a.B) {
     my_q = R.cg_of[c * a.B + lane] - g0;
-    my_off = my_q * kBrickRow + (lane - R.cgs[g0 + my_q].b0) * nd;
+    my_off = my_q * kGsumPitch + (lane - R.cgs[g0 + my_q].b0) * ndp;
   }
+  int pos[4];  // where value lane + 32 k of a row goes
+#pragma unroll
+  for (int k = 0; k < 4; ++k) pos[k] = lane + 32 * k + (ndp > nd ? (lane + 32 * k) / nd : 0);
   if (lane < nd) {
     dd = R.cls_dirs[c * R.max_dirs + lane];
     wd = a.w[dd];
   }
-  BrickOutRow nxt = R.out_rec[c][j];
+  BrickOutRow nxt = ld_out_rec(R.out_rec[c] + j);
   for (; j < n_out; j += stride) {
     const BrickOutRow rec = nxt;
-    if (j + stride < n_out) nxt = R.out_rec[c][j + stride];
+    if (j + stride < n_out) nxt = ld_out_rec(R.out_rec[c] + j + stride);
     if ((rec.type == NANOBTE_THERMALIZING) != (R.therm != 0)) continue;
     double *out = R.partial + ((size_t)rec.ord * a.n_bf + rec.bf) * a.B;
     double v[kGsumGroups][4];
@@ -95,7 +109,7 @@ __global__ void __launch_bounds__(32 * kGsumWarps) brick_gsum_kernel(const Brick
     for (int q = 0; q < kGsumGroups; ++q) {
 #pragma unroll
       for (int k = 0; k < 4; ++k)
-        if (lane + 32 * k < S[q]) mine[q * kBrickRow + lane + 32 * k] = v[q][k];
+        if (lane + 32 * k < S[q]) mine[q * kGsumPitch + pos[k]] = v[q][k];
     }
     __syncwarp();
     if (my_q >= 0 && my_q < kGsumGroups) {
@@ -106,7 +120,7 @@ __global__ void __launch_bounds__(32 * kGsumWarps) brick_gsum_kernel(const Brick
     for (int b = lane + 32; b < a.B; b += 32) {  // more than 32 bands
       const int q = R.cg_of[c * a.B + b] - g0;
       if (q >= kGsumGroups) continue;
-      const int off = q * kBrickRow + (b - R.cgs[g0 + q].b0) * nd;
+      const int off = q * kGsumPitch + (b - R.cgs[g0 + q].b0) * ndp;
       double acc = 0.0;
       for (int dl = 0; dl < nd; ++dl) acc = fma(wsn[wid][dl], mine[off + dl], acc);
       out[b] = acc;
@@ -159,78 +173,81 @@ __global__ void __launch_bounds__(kBrickMaxS) brick_inflow_kernel(const BrickClo
   *dst = type == NANOBTE_SPECULAR ? spec : a.bf_p[bf] * spec + (1.0 - a.bf_p[bf]) * Gf;  // R8
 }
 
-// The same from the per-row records built at create (BrickInRow): a CTA belongs to one (class, group), lanes = systems, and
-// walks over the class's rows kInRows at a time.  What does not depend on the row is set up once per CTA: the thread's band
-// and direction, its mirror direction under each of the class's (at most 8) permutations packed in one register, the wall
-// block and direction count of this band group in every class.  Per row: one 16-byte record (uniform; the next rows' records
-// are fetched while these are worked on), then G / p (independent loads), then the wall value.
-constexpr int kInRows = 4;
+// The same from the per-row records built at create (BrickInRow), for every launch but the first (R.init, general kernel):
+// a CTA belongs to one (class, group), lanes = systems, and walks over the class's records kBrickInRows at a time; the
+// records are sorted by face type and padded, so a batch has one type and takes one uniform branch into straight-line code.
+// What does not depend on the row is set up once per CTA: the thread's band and direction, its mirror direction under each
+// of the class's (at most 8) permutations packed in one register, the wall block of this band group in every class (the
+// classes have the same directions per band here, BrickState::in_fast).  Per row: one 16-byte record (uniform; the next
+// batch's records are fetched while these are worked on), then G / p / the wall value (independent loads), then
+//   diffuse G (R7)    specular: the mirror value    mixed: p spec + (1 - p) G (R8)    0 where s.n == 0 (R15).
+constexpr int kInRows = kBrickInRows;
 __global__ void __launch_bounds__(kBrickMaxS) brick_inflow_fast_kernel(const BrickClosureArgs R) {
   __shared__ int64_t m_base[NB_MAX_CLASSES];
-  __shared__ int32_t m_nd[NB_MAX_CLASSES];
   const BoundaryArgs &a = R.a;
   const BrickCG G = R.cgs[blockIdx.y];
   const int c = G.cls, s = threadIdx.x;
   const int g = blockIdx.y - R.cg0[c];           // band group index: the same in the mirror class
-  if (s < R.n_cls) {
-    const BrickCG &Gm = R.cgs[R.cg0[s] + g];
-    m_base[s] = Gm.wall_base;
-    m_nd[s] = Gm.nd;
-  }
+  if (s < R.n_cls) m_base[s] = R.cgs[R.cg0[s] + g].wall_base;
   __syncthreads();
-  const int n_in = R.n_in[c];
+  const int n_rec = R.n_rec[c];
   if (s >= G.S) return;
-  const int bl = s / G.nd, dl = s - bl * G.nd, b = G.b0 + bl;
+  const int bl = s / G.nd, dl = s - bl * G.nd;
   unsigned long long perms = 0;                  // byte q: mirror direction (local to its class) under permutation q, 255 = none
 #pragma unroll
   for (int q = 0; q < 8; ++q) perms |= (unsigned long long)R.in_perm[((size_t)c * 8 + q) * 16 + dl] << (8 * q);
   double *inf = R.inf + G.inf_base + s;
-  const double *Gb = a.G + b;
+  const double *Gb = a.G + G.b0 + bl;
+  const double *wall = R.wall + bl * G.nd;
+  const int4 *recs = reinterpret_cast<const int4 *>(R.in_rec[c]);
   const int stride = gridDim.x * kInRows;
-  BrickInRow nxt[kInRows];
+  int4 nxt[kInRows];  // x: face (-1: padding), y: inflow row, z: wall row of the mirror cell, w: type | mirror class << 8 | permutation << 16
+  if (blockIdx.x * kInRows < n_rec) {
 #pragma unroll
-  for (int q = 0; q < kInRows; ++q) {
-    nxt[q].bf = -1;
-    if (blockIdx.x * kInRows + q < n_in) nxt[q] = R.in_rec[c][blockIdx.x * kInRows + q];
+    for (int q = 0; q < kInRows; ++q) nxt[q] = __ldg(recs + blockIdx.x * kInRows + q);
   }
-  for (int k0 = blockIdx.x * kInRows; k0 < n_in; k0 += stride) {
-    BrickInRow rec[kInRows];
+  for (int k0 = blockIdx.x * kInRows; k0 < n_rec; k0 += stride) {
+    int4 rec[kInRows];
+#pragma unroll
+    for (int q = 0; q < kInRows; ++q) rec[q] = nxt[q];
+    if (k0 + stride < n_rec) {
+#pragma unroll
+      for (int q = 0; q < kInRows; ++q) nxt[q] = __ldg(recs + k0 + stride + q);
+    }
+    const int type = rec[0].w & 255;
+    if (type == NANOBTE_DIFFUSE) {
+      double Gf[kInRows];
+#pragma unroll
+      for (int q = 0; q < kInRows; ++q) Gf[q] = rec[q].x >= 0 ? Gb[(size_t)rec[q].x * a.B] : 0.0;
+#pragma unroll
+      for (int q = 0; q < kInRows; ++q)
+        if (rec[q].x >= 0) inf[(int64_t)rec[q].y * kBrickRow] = Gf[q];
+      continue;
+    }
+    bool mir[kInRows];
+    double spec[kInRows];
 #pragma unroll
     for (int q = 0; q < kInRows; ++q) {
-      rec[q] = nxt[q];
-      nxt[q].bf = -1;
-      if (k0 + stride + q < n_in) nxt[q] = R.in_rec[c][k0 + stride + q];
+      const int cm = (rec[q].w >> 8) & 255, perm = (rec[q].w >> 16) & 255;
+      const int dlm = (int)((perms >> (8 * perm)) & 255ull);
+      mir[q] = rec[q].x >= 0 && rec[q].z >= 0 && dlm != 255;
+      spec[q] = mir[q] ? wall[m_base[cm] + (int64_t)rec[q].z * kBrickRow + dlm] : 0.0;
     }
-    double Gf[kInRows], p[kInRows], spec[kInRows];
-    bool has[kInRows];
+    if (type == NANOBTE_SPECULAR) {
+#pragma unroll
+      for (int q = 0; q < kInRows; ++q)
+        if (rec[q].x >= 0) inf[(int64_t)rec[q].y * kBrickRow] = spec[q];
+      continue;
+    }
+    double Gf[kInRows], p[kInRows];
 #pragma unroll
     for (int q = 0; q < kInRows; ++q) {
-      Gf[q] = p[q] = spec[q] = 0.0;
-      has[q] = false;
-      if (rec[q].bf < 0 || rec[q].type == NANOBTE_THERMALIZING || R.init) continue;
-      if (rec[q].type != NANOBTE_SPECULAR) Gf[q] = Gb[(size_t)rec[q].bf * a.B];
-      if (rec[q].type == NANOBTE_MIXED) p[q] = a.bf_p[rec[q].bf];
-      if (rec[q].type != NANOBTE_DIFFUSE && rec[q].msrc >= 0) {
-        const int dlm = (int)((perms >> (8 * rec[q].perm)) & 255ull);
-        if (dlm != 255) {
-          spec[q] = R.wall[m_base[rec[q].cm] + (int64_t)rec[q].msrc * kBrickRow + bl * m_nd[rec[q].cm] + dlm];
-          has[q] = true;
-        }
-      }
+      Gf[q] = mir[q] ? Gb[(size_t)rec[q].x * a.B] : 0.0;
+      p[q] = rec[q].x >= 0 ? a.bf_p[rec[q].x] : 0.0;
     }
 #pragma unroll
-    for (int q = 0; q < kInRows; ++q) {
-      if (rec[q].bf < 0) continue;
-      double *dst = inf + (int64_t)rec[q].row * kBrickRow;
-      if (rec[q].type == NANOBTE_THERMALIZING) {
-        if (R.init) *dst = a.C[b] / R.W * a.bf_eps_w[rec[q].bf];  // R6; never changes afterwards
-        continue;
-      }
-      if (R.init) continue;  // eps^0 = 0 (R12)
-      if (rec[q].type == NANOBTE_DIFFUSE) *dst = Gf[q];                                                   // R7
-      else if (rec[q].type == NANOBTE_SPECULAR) *dst = spec[q];                                           // mirror (0 if s.n == 0, R15)
-      else *dst = has[q] ? p[q] * spec[q] + (1.0 - p[q]) * Gf[q] : 0.0;                                   // R8
-    }
+    for (int q = 0; q < kInRows; ++q)
+      if (rec[q].x >= 0) inf[(int64_t)rec[q].y * kBrickRow] = mir[q] ? p[q] * spec[q] + (1.0 - p[q]) * Gf[q] : 0.0;
   }
 }
 
@@ -338,7 +355,7 @@ BrickClosureArgs closure_args(nanobte_solver *h) {
     R.in_rec[c] = bs.in_rec[c]; R.cg0[c] = bs.cg0[c];
     R.out_bf[c] = bs.out_bf[c]; R.out_row[c] = bs.out_row[c]; R.out_ord[c] = bs.out_ord[c]; R.n_out[c] = bs.n_out[c];
     R.out_rec[c] = bs.out_rec[c];
-    R.in_row[c] = bs.in_row[c]; R.in_bf[c] = bs.in_bf[c]; R.n_in[c] = bs.n_in[c];
+    R.in_row[c] = bs.in_row[c]; R.in_bf[c] = bs.in_bf[c]; R.n_in[c] = bs.n_in[c]; R.n_rec[c] = bs.n_rec[c];
   }
   return R;
 }
@@ -366,10 +383,13 @@ int launch_inflow(nanobte_solver *h, int init) {
   int nmax = 0;
   for (int c = 0; c < h->n_cls; ++c) nmax = std::max(nmax, R.n_in[c]);
   if (nmax == 0) return 0;
-  if (h->brick->in_fast) {
-    // a few waves of CTAs; each walks over its share of the rows
+  if (h->brick->in_fast && !init) {
+    int rmax = 0;
+    for (int c = 0; c < h->n_cls; ++c) rmax = std::max(rmax, R.n_rec[c]);
+    if (rmax == 0) return 0;  // thermalizing faces only: nothing changes after the first launch
+    // a few waves of CTAs; each walks over its share of the records
     const int want = (32 * h->n_sm + h->brick->n_cg - 1) / h->brick->n_cg;
-    dim3 grid(std::max(1, std::min((nmax + kInRows - 1) / kInRows, want)), h->brick->n_cg);
+    dim3 grid(std::max(1, std::min(rmax / kInRows, want)), h->brick->n_cg);
     brick_inflow_fast_kernel<<<grid, kBrickMaxS, 0, h->stream>>>(R);
   } else {
     dim3 grid(nmax, h->brick->n_cg);

@@ -307,6 +307,19 @@ int nb_brick_build(nanobte_solver *h, const BrickCtx &x, BrickHost &bh) {
         }
         C.in_rec[k] = R;
       }
+      // the fast kernel takes kBrickInRows records at a time and branches once per batch: the records go by type (thermalizing
+      // rows never change after the first launch and are left out), every type padded to whole batches with empty records
+      std::vector<BrickInRow> by_type;
+      for (int ty : {NANOBTE_DIFFUSE, NANOBTE_SPECULAR, NANOBTE_MIXED}) {
+        for (const BrickInRow &R : C.in_rec)
+          if (R.type == ty) by_type.push_back(R);
+        while (by_type.size() % kBrickInRows) {
+          BrickInRow E{};
+          E.bf = -1; E.row = 0; E.msrc = -1; E.type = (uint8_t)ty;
+          by_type.push_back(E);
+        }
+      }
+      C.in_rec.swap(by_type);
     }
     bh.cg0.assign(cls_cg0.begin(), cls_cg0.end());
     for (int c = 0; c < ncls; ++c) {  // records of the gsum kernel (the wall rows are final here)
@@ -416,7 +429,7 @@ int nb_brick_upload(nanobte_solver *h, Arena &A, BrickHost &bh) {
     bs.out_ord[c] = A.put(C.out_ord);
     bs.out_rec[c] = A.put(C.out_rec);
     bs.n_out[c] = (int32_t)C.out_bf.size();
-    if (bh.in_fast) bs.in_rec[c] = A.put(C.in_rec);
+    if (bh.in_fast) { bs.in_rec[c] = A.put(C.in_rec); bs.n_rec[c] = (int32_t)C.in_rec.size(); }
     bs.cg0[c] = bh.cg0[c];
   }
   a.inf = A.zeros<double>((size_t)bh.inf_total);
