@@ -48,8 +48,9 @@
  * CG kernel), NANOBTE_CG_NO_UNI=1 (per-cell CG stencil on uniform grids; implies NO_MG), NANOBTE_CG_NO_RECYCLE=1 (plain CG
  * from zero instead of the recycled initial guess; implies NO_MG: the oracle's iterate sequence), NANOBTE_UNS_PLAIN=1
  * (non-staged unstructured sweep), NANOBTE_SWEEP_RP=0 (run-time row pitch in the hyperplane sweep), NANOBTE_CG_NBLK=k
- * (at most k CTAs in the CG kernels: more cells per thread on small meshes), NANOBTE_MG_OMEGA / NANOBTE_MG_TAU (damping and
- * over-correction of the multigrid preconditioner; defaults 0.9 and 2.0).
+ * (at most k CTAs in the CG kernels: more cells per thread on small meshes), NANOBTE_MG_OMEGA / NANOBTE_MG_OMEGA2 /
+ * NANOBTE_MG_TAU (weights of the two Jacobi steps and over-correction of the multigrid preconditioner; defaults 1.45, 0.65
+ * and 1.9; OMEGA alone sets both weights).
  */
 #ifndef NANOBTE_H
 #define NANOBTE_H

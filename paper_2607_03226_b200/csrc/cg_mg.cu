@@ -15,9 +15,14 @@
 //                prolongation never leave the CTA; iterates cross CTA borders through global memory + one grid barrier.
 //   levels 3..   a few hundred unknowns: every CTA holds them in shared memory and repeats the same arithmetic
 //                (bitwise identical, no communication); the coarsest level (<= 32 unknowns) is a dense inverse.
-// Smoother: x <- x + B (g - A x) with B = two damped-Jacobi steps (omega = 0.9) on the CTA's own diagonal block (no communication,
-// symmetric), once before and once after the coarse correction, which is scaled by tau = 2 (over-correction for the
-// piecewise-constant prolongation).  The V-cycle is a fixed symmetric positive definite operator, as CG requires.
+// Smoother: x <- x + B (g - A x) with B = two damped-Jacobi steps on the CTA's own diagonal block (no communication),
+//   B = (w1 + w2) D^-1 - w1 w2 D^-1 A_own D^-1,  w1 = 1.45, w2 = 0.65:
+// symmetric whatever the weights, and positive definite because the eigenvalues of D^-1 A_own lie in (0, 2) and
+// 1/w1 + 1/w2 = 2.23 > 2.  Two different weights put the roots of the error polynomial (1 - w1 z)(1 - w2 z) at both ends of
+// the rough part of the spectrum (a Chebyshev smoother of degree two) instead of twice in its middle: 20 % fewer CG
+// iterations than w1 = w2 = 0.9 at the same cost.  Once before and once after the coarse correction, which is scaled by
+// tau = 1.9 (over-correction for the piecewise-constant prolongation).  The V-cycle is a fixed symmetric positive definite
+// operator, as CG requires.
 // CG in the Chronopoulos-Gear form (one reduction per iteration): u = M^-1 r, w = A u, gamma = (r,u), delta = (w,u).
 // All reductions are fixed trees over per-CTA partials: bitwise reproducible, identical scalars in every CTA.
 #include <algorithm>
@@ -96,11 +101,11 @@ __device__ __forceinline__ double apply_own(const Lv &L, const double *v, int i,
 }
 
 // x = B g with x = 0 before (two Jacobi steps on the own block); leaves x[0..n).  Two block-synchronised phases.
-__device__ __forceinline__ void presmooth(const Lv &L, const double *cfu) {
+__device__ __forceinline__ void presmooth(const Lv &L, const double *cfu, const double rho) {
   const int tid = threadIdx.x;
   for (int i = tid; i < L.n; i += kMgThreads) L.tmp[i] = L.dinv[i] * L.g[i];
   __syncthreads();
-  for (int i = tid; i < L.n; i += kMgThreads) L.x[i] = L.tmp[i] + L.dinv[i] * (L.g[i] - apply_own(L, L.tmp, i, cfu));
+  for (int i = tid; i < L.n; i += kMgThreads) L.x[i] = L.tmp[i] + rho * L.dinv[i] * (L.g[i] - apply_own(L, L.tmp, i, cfu));
   __syncthreads();
 }
 // res = g - A x (halo of x valid)
@@ -109,7 +114,7 @@ __device__ __forceinline__ void residual(const Lv &L, const double *cfu) {
   __syncthreads();
 }
 // x += B (g - A x)   (halo of x valid; the halo is not updated).  Two block-synchronised phases.
-__device__ __forceinline__ void postsmooth(const Lv &L, const double *cfu) {
+__device__ __forceinline__ void postsmooth(const Lv &L, const double *cfu, const double rho) {
   const int tid = threadIdx.x;
   for (int i = tid; i < L.n; i += kMgThreads) {
     const double r = L.g[i] - apply_full(L, L.x, i, cfu);
@@ -118,7 +123,7 @@ __device__ __forceinline__ void postsmooth(const Lv &L, const double *cfu) {
   }
   __syncthreads();
   for (int i = tid; i < L.n; i += kMgThreads)
-    L.x[i] += L.tmp[i] + L.dinv[i] * (L.res[i] - apply_own(L, L.tmp, i, cfu));
+    L.x[i] += L.tmp[i] + rho * L.dinv[i] * (L.res[i] - apply_own(L, L.tmp, i, cfu));
   __syncthreads();
 }
 
@@ -352,7 +357,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
 #pragma unroll
     for (int c = 0; c < CPT; ++c) {
       const int li = tid + c * kMgThreads;
-      xv[c] += dv[c] * (r[c] - A0own(c, y0, xv[c]));
+      xv[c] += a.rho * dv[c] * (r[c] - A0own(c, y0, xv[c]));
       if (li < n0) x0[li] = xv[c];
     }
     __syncthreads();
@@ -370,7 +375,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     __syncthreads();
     MGP(0);
     // ---- level 1 down
-    presmooth(L1, cfu);
+    presmooth(L1, cfu, a.rho);
     exchange(a.xg[1], nslot1, base1, L1.x, n1, L1.x + n1, hidx1, nh1);
     residual(L1, cfu);
     for (int i = tid; i < n2; i += kMgThreads) {
@@ -380,7 +385,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     __syncthreads();
     MGP(1);
     // ---- level 2 down; the level-3 right-hand side is published
-    presmooth(L2, cfu);
+    presmooth(L2, cfu, a.rho);
     exchange(a.xg[2], nslot2, base2, L2.x, n2, L2.x + n2, hidx2, nh2);
     residual(L2, cfu);
     {
@@ -408,7 +413,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
         __syncthreads();
         break;
       }
-      presmooth(G, cfu);
+      presmooth(G, cfu, a.rho);
       residual(G, cfu);
       const int o2 = a.off_l[l + 1], n2c = a.n_l[l + 1];
       for (int i = tid; i < n2c; i += kMgThreads) {
@@ -428,7 +433,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
       G.dinv = gdinv + o; G.diag = gdiag + o; G.stride = a.ntot;
       for (int i = tid; i < n; i += kMgThreads) G.x[i] += a.tau * gx[o2 + gpar[o + i]];
       __syncthreads();
-      postsmooth(G, cfu);
+      postsmooth(G, cfu, a.rho);
     }
     MGP(3);
     // ---- level 2 up: correction of own and halo entries from level 3 (every CTA has all of it), post-smoothing, publish
@@ -436,7 +441,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
       if (dinv2[i] != 0.0) L2.x[i] += a.tau * gx[a3lo + (i >> 3)];  // empty slots stay zero
     for (int j = tid; j < nh2; j += kMgThreads) L2.x[n2 + j] += a.tau * gx[hpar2[j]];
     __syncthreads();
-    postsmooth(L2, cfu);
+    postsmooth(L2, cfu, a.rho);
     exchange(a.xu[2], nslot2, base2, L2.x, n2, L2.x + n2, hidx2, nh2);
     MGP(4);
     // ---- level 1 up
@@ -444,7 +449,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
       if (dinv1[i] != 0.0) L1.x[i] += a.tau * L2.x[i >> 3];
     for (int j = tid; j < nh1; j += kMgThreads) L1.x[n1 + j] += a.tau * L2.x[hpar1[j]];
     __syncthreads();
-    postsmooth(L1, cfu);
+    postsmooth(L1, cfu, a.rho);
     exchange(a.xu[1], nslot1, base1, L1.x, n1, L1.x + n1, hidx1, nh1);
     MGP(5);
     // ---- level 0 up: correction, x += B (r - A x); the result is u
@@ -470,7 +475,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
 #pragma unroll
     for (int c = 0; c < CPT; ++c) {
       const int li = tid + c * kMgThreads;
-      xv[c] += y1[c] + dv[c] * (rs[c] - A0own(c, y0, y1[c]));  // u
+      xv[c] += y1[c] + a.rho * dv[c] * (rs[c] - A0own(c, y0, y1[c]));  // u
       if (li < n0) x0[li] = xv[c];
     }
     __syncthreads();
@@ -614,10 +619,12 @@ bool dense_inverse(std::vector<double> &M, int n) {
 int nb_mg_build(nanobte_solver *h, Arena &A, const GenericTables &g, const double *cfu, const int grid[3]) {
   const int na = (int)g.act2cell.size();
   if (g.cg_nf != 6 || na < 64) return 0;
-  // damping and over-correction: scanned on configs 3 and 4 (omega 0.7 .. 0.95 x tau 1.4 .. 3.0: 16 iterations per solve here,
-  // 20 at 0.8 / 1.6, 35 at 0.95 / 3.0); omega < 1 keeps the two-step Jacobi smoother positive definite
-  double omega = 0.9, tau = 2.0;
-  if (const char *env = std::getenv("NANOBTE_MG_OMEGA")) omega = std::atof(env);  // tuning hooks
+  // Jacobi weights and over-correction, scanned on configs 3 and 4, on cuts and on grids with 4:2:1 spacings (CG iterations per
+  // solve on config 4 after the first few source iterations: 17.8 at 0.9 / 0.9 / 2.0, 14.2 at 1.45 / 0.65 / 1.9; the count
+  // rises steeply once 1/w1 + 1/w2 comes within 0.1 of 2, e.g. 23 at 1.4 / 0.75)
+  double omega = 1.45, omega2 = 0.65, tau = 1.9;
+  if (const char *env = std::getenv("NANOBTE_MG_OMEGA")) { omega = std::atof(env); omega2 = omega; }  // tuning hooks
+  if (const char *env = std::getenv("NANOBTE_MG_OMEGA2")) omega2 = std::atof(env);
   if (const char *env = std::getenv("NANOBTE_MG_TAU")) tau = std::atof(env);
   // ---- lattices -------------------------------------------------------------------------------------------------------------------------------
   std::vector<Lat> lat(1);
@@ -899,7 +906,7 @@ int nb_mg_build(nanobte_solver *h, Arena &A, const GenericTables &g, const doubl
 
   MgPlan *P = new MgPlan();
   MgArgs &a = P->a;
-  a.nblk = nblk; a.n_act = na; a.omega = omega; a.tau = tau;
+  a.nblk = nblk; a.n_act = na; a.omega = omega; a.tau = tau; a.rho = omega2 / omega;
   for (int f = 0; f < 6; ++f) a.cfu[f] = cfu[f];
   a.a3ptr = A.put(a3ptr);
   for (int l = 0; l < 3; ++l) {

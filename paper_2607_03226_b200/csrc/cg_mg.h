@@ -20,6 +20,7 @@ constexpr int kMgCoarsest = 32;   // the coarsest level is solved with its dense
 struct MgArgs {
   int32_t nblk, n_act, max_iter, B;
   double rtol, beta, omega, tau;
+  double rho;                      // second Jacobi step's damping over the first's (the dinv arrays carry the first's)
   double cfu[6];                   // kappa A_f / d_f of the six face directions (-x +x -y +y -z +z)
   // per CTA: [nblk + 1] prefix offsets
   const int32_t *a3ptr;            // level-3 aggregates (= global level-3 unknowns, CTA-contiguous)
