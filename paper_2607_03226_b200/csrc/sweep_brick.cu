@@ -89,6 +89,13 @@ __device__ __forceinline__ unsigned stale_bit(double x, unsigned par) { return (
 
 #ifdef BRICK_PROF
 __device__ unsigned long long g_brick_prof[16];
+constexpr int kBrickTlMax = 1 << 15;
+__device__ unsigned long long g_brick_tl[kBrickTlMax][4];  // per task: ticket taken, first plane ready, done [ns]; SM | nu << 32
+__device__ __forceinline__ unsigned long long gtime() {
+  unsigned long long v;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(v));
+  return v;
+}
 #define PROF_T(var) const long long var = clock64()
 #define PROF_ADD(k, a, b) if (t == 0) prof[k] += (unsigned long long)((b) - (a))
 #else
@@ -253,6 +260,9 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     __syncthreads();
     const int task = sm.task;
     if (task >= a.n_tasks) break;
+#ifdef BRICK_PROF
+    const unsigned long long tl0 = gtime();
+#endif
     const BrickTask T = a.tasks[task];
     const BrickCG G = a.cgs[T.cg];
     const int S = G.S;
@@ -346,6 +356,9 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
     settle_faces();
     cp_async_wait_all();
     __syncthreads();
+#ifdef BRICK_PROF
+    const unsigned long long tl1 = gtime();
+#endif
 
     const int nd = G.nd;
 
@@ -516,8 +529,15 @@ __global__ void __launch_bounds__(kBrickMaxS, 3) sweep_brick_kernel(const BrickA
       }
     }
 #ifdef BRICK_PROF
-    if (t == 0)
+    if (t == 0) {
       for (int k = 0; k < 8; ++k) atomicAdd(&g_brick_prof[k], prof[k]);
+      if (task < kBrickTlMax) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
+        g_brick_tl[task][0] = tl0; g_brick_tl[task][1] = tl1; g_brick_tl[task][2] = gtime();
+        g_brick_tl[task][3] = smid | ((unsigned long long)T.nu << 32) | ((unsigned long long)(T.tv * T.tw) << 48);
+      }
+    }
 #endif
   }
 }
@@ -546,6 +566,11 @@ extern "C" int nanobte_debug_brick_prof(unsigned long long *out, int reset) {
   cudaDeviceSynchronize();
   cudaMemcpyFromSymbol(out, g_brick_prof, sizeof(unsigned long long) * 16);
   if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_brick_prof, z, sizeof(z)); }
+  return 0;
+}
+extern "C" int nanobte_debug_brick_timeline(unsigned long long *out, int n_tasks) {  // [n_tasks][4] of the last sweep
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, g_brick_tl, sizeof(unsigned long long) * 4 * (size_t)std::min(n_tasks, kBrickTlMax));
   return 0;
 }
 #endif
