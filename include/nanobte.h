@@ -44,6 +44,7 @@
  * Environment hooks, read at create, for tests and tuning only (each selects another of the library's own CUDA
  * paths; none of them leaves the GPU): NANOBTE_NO_BRICK=1 (hyperplane sweep + separate moment pass instead of the
  * tile-dataflow sweep on uniform 3-D grids), NANOBTE_BRICK_SLOW_INFLOW=1 (general closure kernel of that path),
+ * NANOBTE_BRICK_ENDSEG=n (planes in the end segments of long pencils on that path; 0 = even segments),
  * NANOBTE_CG_NO_MG=1 (plain fused CG instead of the multigrid-preconditioned one), NANOBTE_CG_GENERIC=1 (multi-pass
  * CG kernel), NANOBTE_CG_NO_UNI=1 (per-cell CG stencil on uniform grids; implies NO_MG), NANOBTE_CG_NO_RECYCLE=1 (plain CG
  * from zero instead of the recycled initial guess; implies NO_MG: the oracle's iterate sequence), NANOBTE_UNS_PLAIN=1
