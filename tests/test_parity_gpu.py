@@ -179,6 +179,16 @@ def test_finfet_cut_solve():
         assert np.abs(g.get_T(0) - r.get_T(0)).max() <= TOL_T_CONVERGED
 
 
+@pytest.mark.parametrize("which", ["cube", "finfet"])
+def test_brick_closures_many_bands_and_groups(which):
+    """40 bands x 16 directions per octant: five band groups of eight bands per class and more bands than lanes, i.e. the
+    general loops of brick_gsum_kernel (groups beyond the four of one pass, bands beyond 32) and inflow records of every
+    face type (cube: thermalizing, diffuse, specular; finfet: mixed) with 16-direction permutations."""
+    pr = (wl.config_cube(n=12, B=40, n_polar=8, n_azim=16, mode="synthetic") if which == "cube"
+          else wl.config_finfet(nx=16, ny=8, nz=8, B=40, n_polar=8, n_azim=16))
+    step_parity(pr, 2, T_init=random_T(pr, 21), mode="synthetic")
+
+
 # ---- unstructured polygon meshes (BASELINE.json configs[4] family): level-scheduled sweep --------------------------------------
 def test_tiny_triangles_steps():
     pr = TINY["tri4x4"]
