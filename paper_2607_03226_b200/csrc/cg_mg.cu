@@ -947,7 +947,13 @@ int nb_mg_solve(nanobte_solver *h) {
   a.max_iter = h->cg_max_iter; a.B = h->B; a.rtol = h->cg_rtol; a.beta = h->beta;
   a.vol = h->vol; a.theta_SI = h->theta_SI; a.theta_prev = h->theta_prev; a.faceflux = h->bd.faceflux; a.bf_area = h->bd.bf_area;
   a.rhs_direct = h->cg_rhs_direct;
-  a.leak_sum = h->leak_imported ? h->leak_sum : nullptr;
+  // the band sum of the face fluxes (R14c') once per face by a small kernel, in band order as the in-kernel loop would add
+  // them: 30 strided loads per wall face are 15 us of the solve when the cooperative kernel does them itself
+  if (!h->leak_imported && !a.rhs_direct && h->n_bf > 0) {
+    int rc = nb_launch_leak_sum(h);
+    if (rc < 0) return rc;
+  }
+  a.leak_sum = (h->leak_imported || (!a.rhs_direct && h->n_bf > 0)) ? h->leak_sum : nullptr;
   a.nprev = h->cgf_nprev;  // the history counter of the handle (reset by solve / set_T / a failed or foreign solve)
   h->cgf_nprev = std::min(2, h->cgf_nprev + 1);
   a.cellbf_ptr = h->cellbf_ptr; a.cellbf = h->cellbf; a.x = h->cg_x; a.iters_out = h->d_maxdT + 1;
