@@ -189,6 +189,17 @@ def test_brick_closures_many_bands_and_groups(which):
     step_parity(pr, 2, T_init=random_T(pr, 21), mode="synthetic")
 
 
+@pytest.mark.parametrize("endseg", [None, "0", "20"])
+def test_brick_long_pencils_segmentations(monkeypatch, endseg):
+    """Pencils of 128 cells: the tile-dataflow sweep cuts them into 12 + 52 + 52 + 12 planes (default), evenly
+    (NANOBTE_BRICK_ENDSEG=0) or with 20-plane ends; the u-face hand-over between segments and the source-plane masks of
+    52-plane segments against the oracle."""
+    if endseg is not None:
+        monkeypatch.setenv("NANOBTE_BRICK_ENDSEG", endseg)
+    pr = wl.config_finfet(nx=128, ny=16, nz=16, B=3, n_polar=2, n_azim=8)
+    step_parity(pr, 2, T_init=random_T(pr, 22), mode="synthetic")
+
+
 # ---- unstructured polygon meshes (BASELINE.json configs[4] family): level-scheduled sweep --------------------------------------
 def test_tiny_triangles_steps():
     pr = TINY["tri4x4"]
