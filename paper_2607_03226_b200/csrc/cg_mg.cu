@@ -5,14 +5,14 @@
 //
 // The paper solves this system with a cached sparse LU; the oracle with an unpreconditioned CG from
 // zero (R14e).  Here the system and the stopping rule are the oracle's, the iterates are not (reading R14e'): on config 4
-// the plain CG needs ~660 iterations of one grid barrier each, this one ~25 iterations of 8.
+// the plain CG needs ~570 iterations of one grid barrier each, this one 11-16 iterations of ~41 us without any.
 //
 // Hierarchy (built at create, nb_mg_build): level l+1 = 2 x 2 x 2 aggregates of the level-l lattice, piecewise-constant
 // prolongation P, Galerkin operators P^T A P.  On a uniform grid every fine face of direction f has the coefficient
 // cfu[f], so a coarse face is a COUNT of fine faces and the coarse diagonal is the counts plus the summed Dirichlet terms:
 // the coarse operators are exact and cost two bytes per face.
 //   levels 0..2  distributed: a CTA owns whole level-3 aggregates (8^3 cells) and the octree below them, so restriction and
-//                prolongation never leave the CTA; iterates cross CTA borders through global memory + one grid barrier.
+//                prolongation never leave the CTA; iterates cross CTA borders through global memory, tagged (mg_tag below).
 //   levels 3..   a few hundred unknowns: every CTA holds them in shared memory and repeats the same arithmetic
 //                (bitwise identical, no communication); the coarsest level (<= 32 unknowns) is a dense inverse.
 // Smoother: x <- x + B (g - A x) with B = two damped-Jacobi steps on the CTA's own diagonal block (no communication),
