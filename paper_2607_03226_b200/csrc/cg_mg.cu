@@ -171,6 +171,7 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
 
 #ifdef MG_PROF
   long long tprof = clock64();
+  const long long tprof0 = tprof;
 #endif
   // ---- load the CTA's tables ------------------------------------------------------------------------------------------------------------
   for (int i = tid; i < n1; i += kMgThreads) {
@@ -560,6 +561,9 @@ __global__ void __launch_bounds__(kMgThreads, 1) cg_mg_kernel(const MgArgs a) {
     }
   }
   if (k == 0 && tid == 0) *a.iters_out = (unsigned long long)it | (not_converged ? kCgNotConverged : 0ull);
+#ifdef MG_PROF
+  if (tid == 0 && blockIdx.x == 0) { g_mg_prof[14] += (unsigned long long)(clock64() - tprof0); g_mg_prof[15] += 1; }
+#endif
 }
 
 typedef void (*mg_fn)(MgArgs);
