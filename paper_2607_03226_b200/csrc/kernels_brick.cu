@@ -46,7 +46,7 @@ struct BrickClosureArgs {
 // per band group, S <= 128 contiguous doubles each) with coalesced loads, all in flight before the first use, through
 // shared memory; lanes = bands then add the nd values of their band times w (s.n) in direction order (the arithmetic of a
 // thread per (entry, band) walking its directions, bit for bit).
-constexpr int kGsumGroups = 4;  // band groups covered by one pass (a class with more takes several)
+constexpr int kGsumGroups = 3;  // band groups covered by one pass (a class with more takes several)
 constexpr int kGsumWarps = 4;
 // A band's nd values sit at pitch nd + 1 (nd >= 8; fewer directions: no pad) and a group's block at pitch 146 (= 2 mod 16):
 // with nd = 12 and 10 bands per group the 30 lanes of the summation hit 30 different banks in every half-warp.
