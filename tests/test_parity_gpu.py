@@ -348,6 +348,27 @@ def test_random_masks(seed):
         step_parity(pr, 3, T_init=random_T(pr, seed), sweep_variant=variant)
 
 
+@pytest.mark.parametrize("seed", [100, 110, 121, 124, 137])
+def test_random_masks_many_systems(seed):
+    """Random masked boxes with 16 to 128 directions and up to 33 bands (more bands than lanes, 12 or 16 directions per
+    octant, five wall types on interior faces) through the default path: the tile-dataflow sweep and its record-driven
+    closure kernels, including the geometries where the mirror images of a class split and the general inflow kernel runs."""
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = int(rng.integers(3, 24)), int(rng.integers(2, 14)), int(rng.integers(2, 12))
+    active = (rng.random(nx * ny * nz) > rng.choice([0.0, 0.1, 0.3])).astype(np.uint8)
+    active[int(rng.integers(0, nx * ny * nz))] = 1
+    tags = [(wl.THERMALIZING, 303.0), (wl.THERMALIZING, 298.0), (wl.DIFFUSE, 0.0), (wl.SPECULAR, 0.0), (wl.MIXED, 0.0)]
+    side_tags = [int(t) for t in rng.permutation(5)] + [int(rng.integers(0, 5))]
+    if 0 not in side_tags and 1 not in side_tags:
+        side_tags[0] = 0
+    npol, naz = [(2, 8), (4, 8), (6, 16), (8, 16)][int(rng.integers(0, 4))]
+    B = int(rng.choice([3, 11, 33]))
+    Q = np.where(rng.random(nx * ny * nz) > 0.6, 1e17 * rng.random(nx * ny * nz), 0.0)
+    pr = wl.make_structured_problem(nx, ny, nz, 7e-9, 9e-9, 11e-9, small_bands(B, seed), wl.product_quadrature(npol, naz), tags,
+                                    side_tags, active=active, Qdot=Q, p_seed=seed)
+    step_parity(pr, 3, T_init=random_T(pr, seed), mode="synthetic" if seed % 2 else "plain")
+
+
 def test_library_owned_memory_matches_caller_owned_workspace():
     """options.workspace == NULL: the library allocates its arena itself (cudaMalloc) -- same results, bit for bit."""
     pr = wl.config_cube(n=10, B=2, n_polar=2, n_azim=8)
