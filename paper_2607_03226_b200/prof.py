@@ -51,7 +51,7 @@ def sweep(args):
     print(f"{args.workload}: {int(planes / n_steps)} (task, plane) pairs per sweep; cycles per plane and CTA")
     for k, nm in enumerate(names):
         print(f"  {nm:54s} {v[k] / planes:8.0f}")
-    print(f"  {"sum":54s} {v[:6].sum() / planes:8.0f}   settle re-loads per plane {v[7] / planes:.2f}")
+    print(f"  {'sum':54s} {v[:6].sum() / planes:8.0f}   settle re-loads per plane {v[7] / planes:.2f}")
     # timeline of the last sweep
     n = g.info["n_tasks"]
     buf = np.zeros((n, 4), dtype=np.uint64)
